@@ -1,0 +1,266 @@
+"""ctypes binding of the CPU oracle (oracle/oracle.cpp).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+reference legs import this package; the product (paper_2510_24154_b200) never
+does.  It imports nothing from the product either.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+LEDGER_NAMES = ("emitted", "dep_phantom", "dep_epid_scored", "dep_epid_other", "dep_air", "escaped",
+                "n_histories", "reserved")
+COUNTER_NAMES = ("woodcock_flights", "air_flights", "epid_flights", "n_pe", "n_compton", "n_pair",
+                 "esteps_phantom", "esteps_air", "esteps_epid", "n_secondaries", "uncollided_at_epid",
+                 "max_stack", "kn_iterations", "photon_cutoffs", "e_tracks", "zero_steps")
+
+
+def build(force=False):
+    """Compile liboracle.so with g++ (plain -O2, never tuned)."""
+    if not force and os.path.exists(_LIB) and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC):
+        return _LIB
+    subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-o", _LIB, _SRC])
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_create.restype = C.c_void_p
+        _lib.orc_last_error.restype = C.c_char_p
+        for f in ("orc_stop_pow", "orc_majorant", "orc_highland_theta0", "orc_field_size", "orc_lut_bilinear"):
+            getattr(_lib, f).restype = C.c_double
+    return _lib
+
+
+def _p(a, t):
+    return a.ctypes.data_as(C.POINTER(t)) if a is not None else None
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def _u8(a):
+    return np.ascontiguousarray(a, dtype=np.uint8)
+
+
+def philox(ctr, key):
+    c = (C.c_uint32 * 4)(*ctr); k = (C.c_uint32 * 2)(*key); o = (C.c_uint32 * 4)()
+    lib().orc_philox4x32_10(c, k, o)
+    return [int(v) for v in o]
+
+
+def sample_compton(E, seed, n):
+    eps = np.empty(n); cost = np.empty(n)
+    lib().orc_sample_compton(C.c_double(E), C.c_uint64(seed), C.c_uint64(n), _p(eps, C.c_double), _p(cost, C.c_double))
+    return eps, cost
+
+
+def compton_events(E, d0, seed, n):
+    out = np.empty((n, 8)); d = np.ascontiguousarray(d0, dtype=np.float64)
+    lib().orc_compton_events(C.c_double(E), _p(d, C.c_double), C.c_uint64(seed), C.c_uint64(n), _p(out, C.c_double))
+    return out
+
+
+def sample_deflection(d0, theta0, seed, n):
+    out = np.empty((n, 3)); d = np.ascontiguousarray(d0, dtype=np.float64)
+    lib().orc_sample_deflection(_p(d, C.c_double), C.c_double(theta0), C.c_uint64(seed), C.c_uint64(n), _p(out, C.c_double))
+    return out
+
+
+def lut_bilinear(lut, t_min, t_max, s_min, s_max, t, s):
+    a = np.ascontiguousarray(lut, dtype=np.float64)
+    return lib().orc_lut_bilinear(_p(a, C.c_double), a.shape[0], a.shape[1], C.c_double(t_min), C.c_double(t_max),
+                                  C.c_double(s_min), C.c_double(s_max), C.c_double(t), C.c_double(s))
+
+
+class Oracle:
+    """One oracle context loaded from a `gen.make_config` dictionary (or its pieces)."""
+
+    def __init__(self, cfg=None):
+        self._l = lib()
+        self._h = C.c_void_p(self._l.orc_create())
+        self.cfg = None
+        if cfg is not None:
+            self.load(cfg)
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            self._l.orc_destroy(self._h); self._h = None
+
+    def _chk(self, rc):
+        if rc != 0:
+            raise RuntimeError("oracle error %d: %s" % (rc, self._l.orc_last_error(self._h).decode()))
+
+    # ---- loading (mirrors the C-ABI of include/aepid.h, independent code)
+    def init_materials(self, t):
+        E, T = _f32(t["E_grid"]), _f32(t["T_grid"])
+        mc, mp, mpp, sp, x0 = (_f32(t[k]) for k in ("mu_compton", "mu_pe", "mu_pair", "stop_pow", "rad_len"))
+        self.n_mat = int(mc.shape[0])
+        self._chk(self._l.orc_init_materials(self._h, self.n_mat, len(E), _p(E, C.c_float), _p(mc, C.c_float), _p(mp, C.c_float),
+                                             _p(mpp, C.c_float), len(T), _p(T, C.c_float), _p(sp, C.c_float), _p(x0, C.c_float)))
+
+    def load_phantom(self, ph):
+        rho, mat = _f32(ph["density"]), _u8(ph["material"])
+        sp, org = _f32(ph["spacing"]), _f32(ph["origin"])
+        self.nvox = (int(ph["nz"]), int(ph["ny"]), int(ph["nx"]))
+        self._chk(self._l.orc_load_phantom(self._h, int(ph["nx"]), int(ph["ny"]), int(ph["nz"]), _p(sp, C.c_float), _p(org, C.c_float),
+                                           _p(rho, C.c_float), _p(mat, C.c_uint8)))
+
+    def load_epid_layers(self, ep):
+        th, rho = _f32(ep["thickness"]), _f32(ep["density"])
+        mat, sc = _u8(ep["material"]), _u8(ep["scored"])
+        self.nu, self.nv = int(ep["nu"]), int(ep["nv"])
+        self._chk(self._l.orc_load_epid_layers(self._h, len(th), _p(th, C.c_float), _p(mat, C.c_uint8), _p(rho, C.c_float), _p(sc, C.c_uint8),
+                                               C.c_float(ep["sid"]), self.nu, self.nv, C.c_float(ep["pitch"])))
+
+    def load_source(self, s):
+        src, ax = _f32(s["src_pos"]), _f32(s["beam_axes"]).reshape(9)
+        ed, pdf, fl = _f32(s["E_edges"]), _f32(s["E_pdf"]), _f32(s["fluence"])
+        self._chk(self._l.orc_load_source(self._h, _p(src, C.c_float), _p(ax, C.c_float), len(pdf), _p(ed, C.c_float), _p(pdf, C.c_float),
+                                          int(s["fu"]), int(s["fv"]), C.c_float(s["f_pitch"]), C.c_float(s["f_plane_dist"]), _p(fl, C.c_float)))
+
+    def set_physics(self, ph):
+        self._chk(self._l.orc_set_physics(self._h, int(ph["mode"]), C.c_double(ph["photon_cut"]), C.c_double(ph["electron_cut"]),
+                                          C.c_double(ph["f_E"]), C.c_double(ph["s_max"])))
+
+    def set_options(self, tracking=0, rebin=1, want_phantom_sq=True, fc_bins=0, fc_w0=0.0, fc_dw=1.0):
+        self.rebin, self.fc_bins = int(rebin), int(fc_bins)
+        self._chk(self._l.orc_set_options(self._h, int(tracking), int(rebin), int(bool(want_phantom_sq)), int(fc_bins),
+                                          C.c_double(fc_w0), C.c_double(fc_dw)))
+        self._want_sq = bool(want_phantom_sq)
+
+    def set_fixed_primary(self, ptype, E=0.0, pos=(0, 0, 0), direction=(0, 0, 1)):
+        p = (C.c_double * 3)(*pos); d = (C.c_double * 3)(*direction)
+        self._chk(self._l.orc_set_fixed_primary(self._h, int(ptype), C.c_double(E), p, d))
+
+    def load(self, cfg):
+        self.cfg = cfg
+        self.init_materials(cfg["tables"])
+        self.load_phantom(cfg["phantom"])
+        self.load_epid_layers(cfg["epid"])
+        self.load_source(cfg["source"])
+        self.set_physics(cfg["physics"])
+        self.set_options()
+
+    # ---- running
+    def reset(self):
+        self._chk(self._l.orc_reset(self._h))
+
+    def run(self, first, n, seed):
+        self._chk(self._l.orc_run(self._h, C.c_uint64(first), C.c_uint64(n), C.c_uint64(seed)))
+
+    def read(self):
+        """Raw accumulators: sums and sums of squares over histories (history-by-history estimator)."""
+        nz, ny, nx = self.nvox
+        r = getattr(self, "rebin", 1)
+        out = {
+            "epid_sum": np.zeros((self.nv, self.nu)), "epid_sq": np.zeros((self.nv, self.nu)),
+            "rb_sum": np.zeros((self.nv // r, self.nu // r)), "rb_sq": np.zeros((self.nv // r, self.nu // r)),
+            "phantom_sum": np.zeros((nz, ny, nx)),
+            "phantom_sq": np.zeros((nz, ny, nx)) if getattr(self, "_want_sq", True) else None,
+            "uncollided": np.zeros((self.nv, self.nu)),
+            "ledger": np.zeros(8), "counters": np.zeros(16, dtype=np.uint64), "aux": np.zeros(4),
+            "fc_hist": np.zeros(max(getattr(self, "fc_bins", 0), 1)),
+        }
+        self._chk(self._l.orc_read(self._h, _p(out["epid_sum"], C.c_double), _p(out["epid_sq"], C.c_double),
+                                   _p(out["rb_sum"], C.c_double), _p(out["rb_sq"], C.c_double),
+                                   _p(out["phantom_sum"], C.c_double), _p(out["phantom_sq"], C.c_double),
+                                   _p(out["uncollided"], C.c_double), _p(out["ledger"], C.c_double),
+                                   _p(out["counters"], C.c_uint64), _p(out["aux"], C.c_double), _p(out["fc_hist"], C.c_double)))
+        return out
+
+    # ---- unit-level entry points
+    def mu_partial(self, m, E):
+        o = (C.c_double * 3)(); self._l.orc_mu_partial(self._h, int(m), C.c_double(E), o); return np.array(o[:])
+
+    def stop_pow(self, m, T):
+        return self._l.orc_stop_pow(self._h, int(m), C.c_double(T))
+
+    def majorant(self, E):
+        return self._l.orc_majorant(self._h, C.c_double(E))
+
+    def highland_theta0(self, m, rho_s, Tm):
+        return self._l.orc_highland_theta0(self._h, int(m), C.c_double(rho_s), C.c_double(Tm))
+
+    def sample_source(self, first, n, seed):
+        out = np.empty((n, 7))
+        self._chk(self._l.orc_sample_source(self._h, C.c_uint64(first), C.c_uint64(n), C.c_uint64(seed), _p(out, C.c_double)))
+        return out
+
+    def field_size(self, printed_form=False):
+        return self._l.orc_field_size(self._h, int(bool(printed_form)))
+
+    def tmap(self):
+        out = np.empty((self.nv, self.nu))
+        self._chk(self._l.orc_tmap(self._h, _p(out, C.c_double)))
+        return out
+
+    def apply_lut(self, lutd, dose, tmap, s_eff):
+        a = np.ascontiguousarray(lutd["lut"], dtype=np.float64)
+        d = np.ascontiguousarray(dose, dtype=np.float64); t = np.ascontiguousarray(tmap, dtype=np.float64)
+        out = np.empty_like(d)
+        self._l.orc_apply_lut(_p(a, C.c_double), a.shape[0], a.shape[1], C.c_double(lutd["t_min"]), C.c_double(lutd["t_max"]),
+                              C.c_double(lutd["s_min"]), C.c_double(lutd["s_max"]), C.c_double(s_eff),
+                              _p(d, C.c_double), _p(t, C.c_double), C.c_size_t(d.size), _p(out, C.c_double))
+        return out
+
+
+def stats(raw):
+    """Mean per history and sigma of the mean from raw sums."""
+    n = float(raw["ledger"][6])
+    res = {"n": n}
+    for k in ("epid", "rb", "phantom"):
+        s, q = raw[k + "_sum"], raw[k + "_sq"]
+        mean = s / n
+        res[k + "_mean"] = mean
+        if q is not None:
+            var = np.maximum(q / n - mean * mean, 0.0) / max(n - 1.0, 1.0)
+            res[k + "_sigma"] = np.sqrt(var)
+    return res
+
+
+def _worker(args):
+    cfg, first, n, seed, opts = args
+    o = Oracle(cfg)
+    o.set_options(**opts)
+    o.reset()
+    o.run(first, n, seed)
+    return o.read()
+
+
+def run_sharded(cfg, n, seed, first=0, procs=None, **opts):
+    """Run histories [first, first+n) split over `procs` processes (legal: the RNG is keyed by
+    the global history index) and add the raw accumulators."""
+    import multiprocessing as mp
+    procs = procs or min(os.cpu_count() or 1, 32)
+    procs = max(1, min(procs, int(n)))
+    if procs == 1:
+        return _worker((cfg, first, n, seed, opts))
+    build()
+    bounds = np.linspace(first, first + n, procs + 1).astype(np.uint64)
+    jobs = [(cfg, int(bounds[i]), int(bounds[i + 1] - bounds[i]), seed, opts) for i in range(procs)]
+    with mp.get_context("fork").Pool(procs) as pool:
+        parts = pool.map(_worker, jobs)
+    tot = parts[0]
+    for p in parts[1:]:
+        for k, v in p.items():
+            if v is None:
+                continue
+            if k == "counters":
+                mx = max(int(tot[k][11]), int(v[11]))
+                tot[k] = tot[k] + v; tot[k][11] = mx
+            else:
+                tot[k] = tot[k] + v
+    return tot
