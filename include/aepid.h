@@ -1,0 +1,162 @@
+/* aepid.h -- C-ABI of the B200-native ARCHER-EPID hot path.
+ *
+ * What the library computes (Fig. 1, 104, 108-110, 114-123, 147-153;
+ * BASELINE.json:north_star): analog coupled photon/electron
+ * Monte Carlo transport of source photons through air, a CT-derived voxel phantom, air
+ * and a multi-layer EPID slab stack, scoring absorbed energy into the EPID image and the
+ * phantom grid, followed by the paper's dose-to-signal correction k(t, s).
+ *
+ * Conventions
+ *   - Units: cm, MeV, g/cm^3.  Tallies are energy per history [MeV]; dose is a constant
+ *     scaling by (density x voxel or pixel-layer volume) left to the caller.
+ *   - World frame = the phantom's own axis-aligned (CT) frame.  Beam frame: source at the
+ *     origin, axes u, v, w = rows of `beam_axes` written in world coordinates, beam along
+ *     +w.  Everything that is not phantom or EPID inside the world box |u|,|v| <= 100 cm,
+ *     -1 <= w <= EPID bottom is air (material 0, 1.205e-3 g/cm^3); leaving the box is
+ *     escape (SURVEY.md 8(c) "Geometry").
+ *   - Every function returns 0 on success or a negative aepid_status; nothing throws,
+ *     prints or exits.  aepid_last_error() gives the reason.
+ *   - Pointer arguments marked "host or device" are classified with
+ *     cudaPointerGetAttributes.  Inputs are copied / repacked into the workspace during
+ *     the call and may be freed on return.  Outputs are caller-owned buffers of exactly
+ *     the stated size.
+ *   - The library never allocates device memory: the caller hands it one workspace of
+ *     aepid_workspace_bytes(dims) bytes (e.g. a torch uint8 tensor) and a CUDA stream.
+ *     All work is stream-ordered; calls that fill HOST outputs synchronise the stream
+ *     before returning, calls with DEVICE outputs do not.
+ *   - One context per GPU; a context is not thread-safe.
+ *   - There is no CPU fallback: without a CUDA device aepid_create fails with AEPID_ERR_CUDA.
+ */
+#ifndef AEPID_H
+#define AEPID_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct aepid_ctx aepid_ctx;
+
+enum aepid_status {
+    AEPID_OK = 0,
+    AEPID_ERR_BAD_ARG = -1,   /* null pointer, size out of range, malformed table */
+    AEPID_ERR_BAD_STATE = -2, /* call order: something required has not been loaded */
+    AEPID_ERR_GEOMETRY = -3,  /* phantom / EPID / source overlap or lie outside the world box */
+    AEPID_ERR_CUDA = -4,      /* a CUDA runtime call failed (message holds cudaGetErrorString) */
+    AEPID_ERR_NOMEM = -5      /* workspace smaller than aepid_workspace_bytes(dims), or an input exceeds dims */
+};
+
+/* Capacities the workspace is laid out for.  Loads may use less (fewer energy bins, a smaller
+ * fluence map, fewer layers) but never more. */
+typedef struct aepid_dims {
+    int n_mat, n_E, n_T;      /* materials (<= 32), photon grid points, electron grid points */
+    int nx, ny, nz;           /* phantom grid (each <= 1024) */
+    int n_layers;             /* EPID layers (<= 8) */
+    int nu, nv;               /* EPID image */
+    int n_bins;               /* spectrum bins */
+    int fu, fv;               /* fluence map */
+    int n_batches;            /* B independent tally buffers for the batch variance estimate (2..255) */
+} aepid_dims;
+
+/* Bytes of device memory the context needs for `dims` (0 if dims are invalid). */
+size_t aepid_workspace_bytes(const aepid_dims* dims);
+
+/* Create a context on CUDA device `device`, ordered on `cuda_stream` (a cudaStream_t, e.g.
+ * torch.cuda.current_stream().cuda_stream; NULL = legacy default stream), owning nothing but
+ * host-side bookkeeping.  `workspace` is DEVICE memory, 256-byte aligned, that must outlive
+ * the context.  Tallies start zeroed. */
+int aepid_create(aepid_ctx** out, int device, void* cuda_stream, const aepid_dims* dims,
+                 void* workspace, size_t workspace_bytes);
+void aepid_destroy(aepid_ctx* ctx);
+const char* aepid_last_error(const aepid_ctx* ctx);   /* NUL-terminated, owned by the context */
+
+/* Material tables (SURVEY.md 8(c) "Cross-section / stopping-power tables"; physics list PAPER.md:104).
+ * All arrays host or device, float32.  E_grid_MeV [n_E] and T_grid_MeV [n_T] must be log-uniform and
+ * increasing.  mu_* [n_mat][n_E] are mass coefficients in cm^2/g: Compton and photoelectric are
+ * interpolated linearly in (ln E, ln mu), pair linearly in (ln E, mu).  stop_pow [n_mat][n_T] in
+ * MeV cm^2/g (log-log interpolation), rad_len_g_cm2 [n_mat].  Material 0 is the air that fills the world. */
+int aepid_init_materials(aepid_ctx* ctx, int n_mat,
+                         int n_E, const float* E_grid_MeV,
+                         const float* mu_compton, const float* mu_pe, const float* mu_pair,
+                         int n_T, const float* T_grid_MeV,
+                         const float* stop_pow, const float* rad_len_g_cm2);
+
+/* Voxel phantom ("three-dimensional density matrix").  density_g_cm3 and material are
+ * [nz][ny][nx] with x fastest, host or device; origin_cm is the world position of the corner of voxel
+ * (0,0,0).  The grid is repacked to one 32-bit word per voxel (density rounded to 19 mantissa bits,
+ * material in the low 5 bits).  Resets the tallies. */
+int aepid_load_phantom(aepid_ctx* ctx, int nx, int ny, int nz, const float spacing_cm[3],
+                       const float origin_cm[3], const float* density_g_cm3, const unsigned char* material);
+
+/* EPID slab stack: n_layers slabs normal to w, listed along +w, the upstream face of
+ * layer 0 at w = sid_cm (reading A6).  Per-layer arrays are HOST pointers [n_layers].  Energy deposited in
+ * layers with scored != 0 is binned to pixel (iu, iv) = floor((u + nu p/2)/p), floor((v + nv p/2)/p) of an
+ * nu x nv image centred on the beam axis; everything else in the stack goes to ledger[3]. */
+int aepid_load_epid_layers(aepid_ctx* ctx, int n_layers, const float* thickness_cm,
+                           const unsigned char* material, const float* density_g_cm3,
+                           const unsigned char* scored, float sid_cm, int nu, int nv, float pitch_cm);
+
+/* Source (BASELINE.json:north_star (2)): point source at src_pos_cm (world), energy
+ * from the histogram spectrum E_edges_MeV [n_bins+1] / E_pdf [n_bins] (one zero-width bin = monoenergetic),
+ * position from the planar fluence map fluence [fv][fu] (u fastest, pitch f_pitch_cm, centred on the axis) on
+ * the plane w = f_plane_dist_cm.  src_pos_cm and beam_axes are HOST pointers; the arrays host or device.
+ * May be called again between fields; it does not touch the tallies. */
+int aepid_load_source(aepid_ctx* ctx, const float src_pos_cm[3], const float beam_axes[9],
+                      int n_bins, const float* E_edges_MeV, const float* E_pdf,
+                      int fu, int fv, float f_pitch_cm, float f_plane_dist_cm, const float* fluence);
+
+/* mode 0: kerma (charged-particle energy deposited at the interaction point, configs[0]);
+ * mode 1: coupled (CSDA electron steps with Highland deflection).  Cutoffs PAPER.md:104
+ * (defaults 0.010 / 0.200 MeV); step rule f_E = 0.10, s_max = 1 cm (reading A13). */
+int aepid_set_physics(aepid_ctx* ctx, int mode, float photon_cut_MeV, float electron_cut_MeV,
+                      float f_E, float s_max_cm);
+
+int aepid_reset_tallies(aepid_ctx* ctx);
+
+/* Transport histories [first, first + n) where first = histories run since the last reset; history h
+ * draws from Philox4x32-10 keyed by `seed` with counter (h_lo, h_hi, particle, block) (reading A1).
+ * Accumulates into the B batch buffers; asynchronous on the stream. */
+int aepid_simulate(aepid_ctx* ctx, unsigned long long n_histories, unsigned long long seed);
+
+/* Mean energy per history and its standard error from the B batches.  Images [nv][nu], volumes
+ * [nz][ny][nx]; any of the four may be NULL; host or device.  ledger (HOST, may be NULL):
+ * {emitted, dep_phantom, dep_epid_scored, dep_epid_other, dep_air, escaped, n_histories, overflow flags}. */
+int aepid_read_tallies(aepid_ctx* ctx, float* epid_mean, float* epid_sigma,
+                       float* phantom_mean, float* phantom_sigma, double ledger[8]);
+
+/* Raw per-batch EPID sums [B][nv][nu] (host or device, may be NULL) and histories per batch (HOST [B]). */
+int aepid_read_batches(aepid_ctx* ctx, float* epid_batches, double* histories_per_batch);
+
+/* Event counters since the last reset (HOST [16]): Woodcock flights, air flights, EPID flights, photoelectric,
+ * Compton, pair, electron steps in phantom / air / EPID, secondaries, -, max stack depth, KN iterations,
+ * photon cutoffs, charged tracks, zero-length steps.  Only counted while aepid_set_counting(ctx, 1). */
+int aepid_set_counting(aepid_ctx* ctx, int on);
+int aepid_read_counters(aepid_ctx* ctx, unsigned long long counters[16]);
+
+/* K1 alone: source samples of histories [first, first+n): out[n][8] = {E, dx, dy, dz (world), fluence pixel,
+ * u, v on the fluence plane, 0}; host or device. */
+int aepid_sample_source(aepid_ctx* ctx, unsigned long long first, unsigned long long n,
+                        unsigned long long seed, float* out);
+
+/* Effective field size (Eq. 1; reading A16): equivalent square s = 2ab/(a+b) of the bounding
+ * box a x b (at the isocentre plane w = 100 cm) of fluence pixels with weight > 0; printed_form != 0 gives
+ * ab/(2(a+b)) exactly as printed. */
+int aepid_field_size(aepid_ctx* ctx, int printed_form, float* s_cm);
+
+/* Response post-pass: t_uv = line integral of density/(1 g cm^-3) from the source
+ * to the centre of pixel (u, v) on the EPID top plane through the phantom grid (reading A17);
+ * signal = dose * k(t_uv, s) with k bilinear in lut[it*ns + is] on uniform axes, (t, s) clamped into the table
+ * (reading A18).  s_eff_cm < 0 derives s from the loaded fluence.  epid_in NULL = current mean image.
+ * lut (nt*ns <= 65536), epid_in, signal_out [nv][nu], tmap_out [nv][nu] (may be NULL): host or device. */
+int aepid_apply_response_lut(aepid_ctx* ctx, const float* lut, int nt, int ns,
+                             float t_min, float t_max, float s_min, float s_max, float s_eff_cm,
+                             const float* epid_in, float* signal_out, float* tmap_out);
+
+/* Block until everything queued on the context's stream has finished. */
+int aepid_synchronize(aepid_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AEPID_H */

@@ -1,0 +1,249 @@
+"""Thin ctypes binding of libaepid.so (include/aepid.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C-ABI.  PyTorch is used for the
+device workspace, device tensors and the CUDA stream, nothing else.  There is no CPU fallback:
+importing works anywhere, creating an Engine without the built library or a GPU raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libaepid.so")
+_lib = None
+
+STATUS = {0: "OK", -1: "BAD_ARG", -2: "BAD_STATE", -3: "GEOMETRY", -4: "CUDA", -5: "NOMEM"}
+LEDGER_NAMES = ("emitted", "dep_phantom", "dep_epid_scored", "dep_epid_other", "dep_air", "escaped",
+                "n_histories", "overflow")
+COUNTER_NAMES = ("woodcock_flights", "air_flights", "epid_flights", "n_pe", "n_compton", "n_pair",
+                 "esteps_phantom", "esteps_air", "esteps_epid", "n_secondaries", "unused",
+                 "max_stack", "kn_iterations", "photon_cutoffs", "e_tracks", "zero_steps")
+EXPORTS = ("aepid_workspace_bytes", "aepid_create", "aepid_destroy", "aepid_last_error", "aepid_init_materials",
+           "aepid_load_phantom", "aepid_load_epid_layers", "aepid_load_source", "aepid_set_physics",
+           "aepid_reset_tallies", "aepid_simulate", "aepid_read_tallies", "aepid_read_batches",
+           "aepid_set_counting", "aepid_read_counters", "aepid_sample_source", "aepid_field_size",
+           "aepid_apply_response_lut", "aepid_synchronize")
+
+
+class AepidError(RuntimeError):
+    pass
+
+
+class Dims(C.Structure):
+    _fields_ = [(n, C.c_int) for n in ("n_mat", "n_E", "n_T", "nx", "ny", "nz", "n_layers", "nu", "nv",
+                                       "n_bins", "fu", "fv", "n_batches")]
+
+
+def load_library():
+    """dlopen libaepid.so; raise loudly if it has not been built (python -m paper_2510_24154_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise AepidError("libaepid.so is not built: run `python -m paper_2510_24154_b200.build` "
+                         "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    lib.aepid_workspace_bytes.restype = C.c_size_t
+    lib.aepid_workspace_bytes.argtypes = [C.POINTER(Dims)]
+    lib.aepid_last_error.restype = C.c_char_p
+    lib.aepid_last_error.argtypes = [C.c_void_p]
+    lib.aepid_destroy.restype = None
+    lib.aepid_destroy.argtypes = [C.c_void_p]
+    lib.aepid_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_void_p, C.POINTER(Dims), C.c_void_p, C.c_size_t]
+    vp = C.c_void_p
+    lib.aepid_init_materials.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp, vp, C.c_int, vp, vp, vp]
+    lib.aepid_load_phantom.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, vp, vp, vp]
+    lib.aepid_load_epid_layers.argtypes = [vp, C.c_int, vp, vp, vp, vp, C.c_float, C.c_int, C.c_int, C.c_float]
+    lib.aepid_load_source.argtypes = [vp, vp, vp, C.c_int, vp, vp, C.c_int, C.c_int, C.c_float, C.c_float, vp]
+    lib.aepid_set_physics.argtypes = [vp, C.c_int, C.c_float, C.c_float, C.c_float, C.c_float]
+    lib.aepid_reset_tallies.argtypes = [vp]
+    lib.aepid_simulate.argtypes = [vp, C.c_ulonglong, C.c_ulonglong]
+    lib.aepid_read_tallies.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.aepid_read_batches.argtypes = [vp, vp, vp]
+    lib.aepid_set_counting.argtypes = [vp, C.c_int]
+    lib.aepid_read_counters.argtypes = [vp, vp]
+    lib.aepid_sample_source.argtypes = [vp, C.c_ulonglong, C.c_ulonglong, C.c_ulonglong, vp]
+    lib.aepid_field_size.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
+    lib.aepid_apply_response_lut.argtypes = [vp, vp, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_float,
+                                             C.c_float, vp, vp, vp]
+    lib.aepid_synchronize.argtypes = [vp]
+    _lib = lib
+    return lib
+
+
+def workspace_bytes(dims: Dims) -> int:
+    return int(load_library().aepid_workspace_bytes(C.byref(dims)))
+
+
+def _ptr(a, dtype=None):
+    """Raw address of a numpy array (host) or a torch tensor (host or device); None -> NULL."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        if dtype is not None and a.dtype != dtype:
+            raise TypeError("expected %s, got %s" % (dtype, a.dtype))
+        if not a.flags["C_CONTIGUOUS"]:
+            raise ValueError("array must be C-contiguous")
+        return a.ctypes.data
+    if hasattr(a, "data_ptr"):
+        if not a.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        return a.data_ptr()
+    raise TypeError("expected a numpy array or a torch tensor")
+
+
+def _host_f32(a):
+    return np.ascontiguousarray(np.asarray(a, dtype=np.float32))
+
+
+class Engine:
+    """One aepid context on one GPU.  Method names follow the C-ABI: init_materials, load_phantom,
+    load_epid_layers, load_source, set_physics, simulate, read_tallies, apply_response_lut."""
+
+    def __init__(self, dims: Dims, device: int = 0, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise AepidError("no CUDA device: the ARCHER-EPID path has no CPU fallback")
+        self._lib = load_library()
+        self._torch = torch
+        self.device = torch.device("cuda", device)
+        self.dims = dims
+        nbytes = workspace_bytes(dims)
+        if nbytes == 0:
+            raise AepidError("invalid dims")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)   # device memory comes from torch
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self._h = C.c_void_p()
+        rc = self._lib.aepid_create(C.byref(self._h), device, C.c_void_p(self.stream.cuda_stream), C.byref(dims),
+                                    C.c_void_p(self.workspace.data_ptr()), nbytes)
+        self._chk(rc)
+        self.nu, self.nv = dims.nu, dims.nv
+        self.nx, self.ny, self.nz = dims.nx, dims.ny, dims.nz
+        self.n_batches = dims.n_batches
+
+    @classmethod
+    def for_config(cls, cfg, n_batches=None, device=0, stream=None):
+        """Engine sized for a gen.make_config dictionary (inputs are not loaded)."""
+        t, ph, ep, s = cfg["tables"], cfg["phantom"], cfg["epid"], cfg["source"]
+        d = Dims(n_mat=int(t["mu_compton"].shape[0]), n_E=len(t["E_grid"]), n_T=len(t["T_grid"]),
+                 nx=int(ph["nx"]), ny=int(ph["ny"]), nz=int(ph["nz"]), n_layers=len(ep["thickness"]),
+                 nu=int(ep["nu"]), nv=int(ep["nv"]), n_bins=len(s["E_pdf"]), fu=int(s["fu"]), fv=int(s["fv"]),
+                 n_batches=int(n_batches if n_batches is not None else cfg["physics"]["n_batches"]))
+        return cls(d, device=device, stream=stream)
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self._lib.aepid_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _chk(self, rc):
+        if rc != 0:
+            msg = self._lib.aepid_last_error(self._h)
+            raise AepidError("aepid %s: %s" % (STATUS.get(rc, rc), msg.decode() if msg else ""))
+
+    # ---- loading: arrays may be numpy (host) or torch tensors (host or device)
+    def init_materials(self, E_grid, mu_compton, mu_pe, mu_pair, T_grid, stop_pow, rad_len):
+        n_mat, n_E = int(mu_compton.shape[0]), int(mu_compton.shape[1])
+        self._chk(self._lib.aepid_init_materials(self._h, n_mat, n_E, _ptr(E_grid), _ptr(mu_compton), _ptr(mu_pe), _ptr(mu_pair),
+                                                 int(stop_pow.shape[1]), _ptr(T_grid), _ptr(stop_pow), _ptr(rad_len)))
+
+    def load_phantom(self, spacing, origin, density, material):
+        nz, ny, nx = (int(v) for v in density.shape)
+        sp, org = _host_f32(spacing), _host_f32(origin)
+        self._chk(self._lib.aepid_load_phantom(self._h, nx, ny, nz, _ptr(sp), _ptr(org), _ptr(density), _ptr(material)))
+
+    def load_epid_layers(self, thickness, material, density, scored, sid, nu, nv, pitch):
+        th, rho = _host_f32(thickness), _host_f32(density)
+        mat = np.ascontiguousarray(np.asarray(material, dtype=np.uint8)); sc = np.ascontiguousarray(np.asarray(scored, dtype=np.uint8))
+        self._chk(self._lib.aepid_load_epid_layers(self._h, len(th), _ptr(th), _ptr(mat), _ptr(rho), _ptr(sc),
+                                                   float(sid), int(nu), int(nv), float(pitch)))
+
+    def load_source(self, src_pos, beam_axes, E_edges, E_pdf, f_pitch, f_plane_dist, fluence):
+        src, ax = _host_f32(src_pos), _host_f32(beam_axes).reshape(9)
+        fv, fu = (int(v) for v in fluence.shape)
+        self._chk(self._lib.aepid_load_source(self._h, _ptr(src), _ptr(ax), int(E_pdf.shape[0]), _ptr(E_edges), _ptr(E_pdf),
+                                              fu, fv, float(f_pitch), float(f_plane_dist), _ptr(fluence)))
+
+    def set_physics(self, mode=1, photon_cut=0.010, electron_cut=0.200, f_E=0.10, s_max=1.0, **_):
+        self._chk(self._lib.aepid_set_physics(self._h, int(mode), float(photon_cut), float(electron_cut), float(f_E), float(s_max)))
+
+    def load_config(self, cfg):
+        """Host-array convenience: load everything of a gen.make_config dictionary."""
+        t, ph, ep, s = cfg["tables"], cfg["phantom"], cfg["epid"], cfg["source"]
+        self.init_materials(t["E_grid"], t["mu_compton"], t["mu_pe"], t["mu_pair"], t["T_grid"], t["stop_pow"], t["rad_len"])
+        self.load_phantom(ph["spacing"], ph["origin"], ph["density"], ph["material"])
+        self.load_epid_layers(ep["thickness"], ep["material"], ep["density"], ep["scored"], ep["sid"], ep["nu"], ep["nv"], ep["pitch"])
+        self.load_source(s["src_pos"], s["beam_axes"], s["E_edges"], s["E_pdf"], s["f_pitch"], s["f_plane_dist"], s["fluence"])
+        self.set_physics(**cfg["physics"])
+
+    # ---- running
+    def reset_tallies(self):
+        self._chk(self._lib.aepid_reset_tallies(self._h))
+
+    def simulate(self, n_histories, seed):
+        self._chk(self._lib.aepid_simulate(self._h, int(n_histories), int(seed)))
+
+    def synchronize(self):
+        self._chk(self._lib.aepid_synchronize(self._h))
+
+    def read_tallies(self, epid=True, phantom=True, sigma=True, out=None):
+        """Returns a dict of numpy arrays (host).  `out` may supply preallocated numpy arrays or torch
+        tensors (host or device) under the keys epid_mean / epid_sigma / phantom_mean / phantom_sigma."""
+        out = dict(out or {})
+        def buf(key, shape, want):
+            if not want:
+                return None
+            if key not in out:
+                out[key] = np.empty(shape, dtype=np.float32)
+            return out[key]
+        em = buf("epid_mean", (self.nv, self.nu), epid); es = buf("epid_sigma", (self.nv, self.nu), epid and sigma)
+        pm = buf("phantom_mean", (self.nz, self.ny, self.nx), phantom); ps = buf("phantom_sigma", (self.nz, self.ny, self.nx), phantom and sigma)
+        led = np.zeros(8, dtype=np.float64)
+        self._chk(self._lib.aepid_read_tallies(self._h, _ptr(em), _ptr(es), _ptr(pm), _ptr(ps), _ptr(led)))
+        out["ledger"] = led
+        return out
+
+    def read_batches(self):
+        b = np.empty((self.n_batches, self.nv, self.nu), dtype=np.float32)
+        n = np.zeros(self.n_batches, dtype=np.float64)
+        self._chk(self._lib.aepid_read_batches(self._h, _ptr(b), _ptr(n)))
+        return b, n
+
+    def set_counting(self, on=True):
+        self._chk(self._lib.aepid_set_counting(self._h, int(bool(on))))
+
+    def read_counters(self):
+        c = np.zeros(16, dtype=np.uint64)
+        self._chk(self._lib.aepid_read_counters(self._h, _ptr(c)))
+        return c
+
+    def sample_source(self, first, n, seed):
+        out = np.empty((int(n), 8), dtype=np.float32)
+        self._chk(self._lib.aepid_sample_source(self._h, int(first), int(n), int(seed), _ptr(out)))
+        return out
+
+    def field_size(self, printed_form=False):
+        s = C.c_float()
+        self._chk(self._lib.aepid_field_size(self._h, int(bool(printed_form)), C.byref(s)))
+        return float(s.value)
+
+    def apply_response_lut(self, lut, t_min, t_max, s_min, s_max, s_eff=-1.0, epid_in=None, signal_out=None, tmap_out=None,
+                           want_tmap=True):
+        nt, ns = (int(v) for v in lut.shape)
+        if signal_out is None:
+            signal_out = np.empty((self.nv, self.nu), dtype=np.float32)
+        if tmap_out is None and want_tmap:
+            tmap_out = np.empty((self.nv, self.nu), dtype=np.float32)
+        self._chk(self._lib.aepid_apply_response_lut(self._h, _ptr(lut), nt, ns, float(t_min), float(t_max), float(s_min), float(s_max),
+                                                     float(s_eff), _ptr(epid_in), _ptr(signal_out), _ptr(tmap_out)))
+        return signal_out, tmap_out

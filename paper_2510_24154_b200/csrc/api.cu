@@ -1,0 +1,565 @@
+// Host side of the C-ABI declared in include/aepid.h: argument checking, workspace layout, table
+// preparation (ln-domain tables, majorant, integer CDF thresholds) and kernel launches.  No device
+// allocation happens here: every device byte lives in the caller's workspace.
+#include <cuda_runtime.h>
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/aepid.h"
+#include "params.h"
+
+using namespace aepid;
+
+namespace {
+
+constexpr size_t kAlign = 256;
+constexpr size_t kMaxLut = 65536;
+inline size_t up(size_t x) { return (x + kAlign - 1) & ~(kAlign - 1); }
+
+struct Layout {
+    size_t vox, ph_batch, ep_batch, out_ph, out_ep, tmap, signal, dose_in, lut, blob, thrE, edges, thrF, small, total;
+    size_t nvox, npix, blob_bytes;
+};
+
+bool dims_ok(const aepid_dims* d) {
+    if (!d) return false;
+    if (d->n_mat < 1 || d->n_mat > kMaxMat || d->n_E < 2 || d->n_E > 4096 || d->n_T < 2 || d->n_T > 4096) return false;
+    if (d->nx < 1 || d->ny < 1 || d->nz < 1 || d->nx > 1024 || d->ny > 1024 || d->nz > 1024) return false;
+    if (d->n_layers < 1 || d->n_layers > kMaxLayers || d->nu < 1 || d->nv < 1 || d->nu > 16384 || d->nv > 16384) return false;
+    if (d->n_bins < 1 || d->n_bins > 65536 || d->fu < 1 || d->fv < 1 || d->fu > 4096 || d->fv > 4096) return false;
+    if (d->n_batches < 2 || d->n_batches > 255) return false;
+    return true;
+}
+
+Layout make_layout(const aepid_dims& d) {
+    Layout L{};
+    L.nvox = (size_t)d.nx * d.ny * d.nz;
+    L.npix = (size_t)d.nu * d.nv;
+    L.blob_bytes = ((size_t)d.n_mat * d.n_E * 4 + d.n_E + (size_t)d.n_mat * d.n_T + d.n_mat) * 4;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { const size_t at = o; o += up(bytes); return at; };
+    L.vox = take(L.nvox * 4);
+    L.ph_batch = take(L.nvox * 4 * d.n_batches);
+    L.ep_batch = take(L.npix * 4 * d.n_batches);
+    L.out_ph = take(L.nvox * 8);
+    L.out_ep = take(L.npix * 8);
+    L.tmap = take(L.npix * 4);
+    L.signal = take(L.npix * 4);
+    L.dose_in = take(L.npix * 4);
+    L.lut = take(kMaxLut * 4);
+    L.blob = take(L.blob_bytes);
+    L.thrE = take(((size_t)d.n_bins + 1) * 4);
+    L.edges = take(((size_t)d.n_bins + 1) * 4);
+    L.thrF = take(((size_t)d.fu * d.fv + 1) * 4);
+    L.small = take(1024);            // ledger [8] f64 | counters [16] u64 | chunk counter | rho_max [32] f32
+    L.total = o;
+    return L;
+}
+
+}  // namespace
+
+struct aepid_ctx {
+    int device = 0, sm_count = 148;
+    cudaStream_t stream = nullptr;
+    aepid_dims dims{};
+    Layout lay{};
+    char* ws = nullptr;
+    std::string err;
+    // host copies of what the tables are built from
+    int n_mat = 0, n_E = 0, n_T = 0;
+    std::vector<float> Eg, Tg, muC, muPE, muPP, S, X0;
+    std::vector<float> rho_max;
+    bool have_mat = false, have_phantom = false, have_epid = false, have_source = false, tables_dirty = true;
+    Geom g{};
+    Physics ph{1, 0.010f, 0.200f, 0.10f, 1.0f};
+    Tables tb{};
+    Source so{};
+    int bb_u0 = 0, bb_u1 = -1, bb_v0 = 0, bb_v1 = -1;    // bounding box of positive fluence pixels
+    unsigned long long n_done = 0;
+    double hist[256] = {0};
+    bool counting = false;
+
+    uint32_t* d_vox() { return reinterpret_cast<uint32_t*>(ws + lay.vox); }
+    float* d_ph_batch() { return reinterpret_cast<float*>(ws + lay.ph_batch); }
+    float* d_ep_batch() { return reinterpret_cast<float*>(ws + lay.ep_batch); }
+    float* d_out_ph() { return reinterpret_cast<float*>(ws + lay.out_ph); }
+    float* d_out_ep() { return reinterpret_cast<float*>(ws + lay.out_ep); }
+    float* d_tmap() { return reinterpret_cast<float*>(ws + lay.tmap); }
+    float* d_signal() { return reinterpret_cast<float*>(ws + lay.signal); }
+    float* d_dose_in() { return reinterpret_cast<float*>(ws + lay.dose_in); }
+    float* d_lut() { return reinterpret_cast<float*>(ws + lay.lut); }
+    uint32_t* d_blob() { return reinterpret_cast<uint32_t*>(ws + lay.blob); }
+    uint32_t* d_thrE() { return reinterpret_cast<uint32_t*>(ws + lay.thrE); }
+    float* d_edges() { return reinterpret_cast<float*>(ws + lay.edges); }
+    uint32_t* d_thrF() { return reinterpret_cast<uint32_t*>(ws + lay.thrF); }
+    double* d_ledger() { return reinterpret_cast<double*>(ws + lay.small); }
+    unsigned long long* d_counters() { return reinterpret_cast<unsigned long long*>(ws + lay.small + 64); }
+    unsigned int* d_chunk() { return reinterpret_cast<unsigned int*>(ws + lay.small + 192); }
+    float* d_rho_max() { return reinterpret_cast<float*>(ws + lay.small + 256); }
+};
+
+namespace {
+
+int fail(aepid_ctx* c, int code, const std::string& msg) { if (c) c->err = msg; return code; }
+#define CU(call)                                                                                         \
+    do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail(ctx, AEPID_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); } while (0)
+
+enum MemKind { MEM_HOST_PAGEABLE, MEM_HOST_PINNED, MEM_DEVICE };
+MemKind classify(const void* p) {
+    cudaPointerAttributes a{};
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return MEM_HOST_PAGEABLE; }
+    if (a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged) return MEM_DEVICE;
+    if (a.type == cudaMemoryTypeHost) return MEM_HOST_PINNED;
+    return MEM_HOST_PAGEABLE;
+}
+// Copy a host-or-device input array to a host vector (small arrays the host needs to see).
+template <class T>
+int fetch(aepid_ctx* ctx, const T* src, size_t n, std::vector<T>& out) {
+    out.resize(n);
+    if (classify(src) == MEM_DEVICE) {
+        CU(cudaMemcpyAsync(out.data(), src, n * sizeof(T), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+    } else std::memcpy(out.data(), src, n * sizeof(T));
+    return 0;
+}
+// Deliver a device result to a host-or-device output pointer.
+int deliver(aepid_ctx* ctx, void* dst, const void* dev_src, size_t bytes, bool* need_sync) {
+    const MemKind k = classify(dst);
+    CU(cudaMemcpyAsync(dst, dev_src, bytes, k == MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
+    if (k != MEM_DEVICE) *need_sync = true;
+    return 0;
+}
+
+int reset_tallies(aepid_ctx* ctx) {
+    const size_t B = ctx->dims.n_batches;
+    CU(cudaMemsetAsync(ctx->d_ph_batch(), 0, ctx->lay.nvox * 4 * B, ctx->stream));
+    CU(cudaMemsetAsync(ctx->d_ep_batch(), 0, ctx->lay.npix * 4 * B, ctx->stream));
+    CU(cudaMemsetAsync(ctx->ws + ctx->lay.small, 0, 256, ctx->stream));
+    ctx->n_done = 0;
+    std::fill(ctx->hist, ctx->hist + 256, 0.0);
+    return 0;
+}
+
+// ln-domain photon tables, majorant (reading A7 as corrected in DESIGN.md), ln stopping power, 1/X0.
+int build_tables(aepid_ctx* ctx) {
+    const int nm = ctx->n_mat, nE = ctx->n_E, nT = ctx->n_T;
+    std::vector<float> blob((size_t)nm * nE * 4 + nE + (size_t)nm * nT + nm);
+    float* phot = blob.data();
+    float* maj = phot + (size_t)nm * nE * 4;
+    float* lnS = maj + nE;
+    float* invX0 = lnS + (size_t)nm * nT;
+    for (int m = 0; m < nm; ++m)
+        for (int j = 0; j < nE; ++j) {
+            const size_t o = (size_t)m * nE + j;
+            phot[o * 4 + 0] = (float)std::log(std::max((double)ctx->muPE[o], 1e-37));
+            phot[o * 4 + 1] = (float)std::log(std::max((double)ctx->muC[o], 1e-37));
+            phot[o * 4 + 2] = ctx->muPP[o];
+            phot[o * 4 + 3] = 0.0f;
+        }
+    for (int j = 0; j < nE; ++j) {
+        double mx = 1e-30;
+        for (int m = 0; m < nm; ++m) {
+            const double r = m < (int)ctx->rho_max.size() ? ctx->rho_max[m] : 0.0;
+            if (r <= 0) continue;
+            const size_t o = (size_t)m * nE + j;
+            mx = std::max(mx, r * ((double)ctx->muPE[o] + ctx->muC[o] + ctx->muPP[o]));
+        }
+        maj[j] = (float)(mx * (1.0 + 1e-4));      // margin covers float32 rounding of the fast exp / log path
+    }
+    for (int m = 0; m < nm; ++m) {
+        for (int j = 0; j < nT; ++j) lnS[(size_t)m * nT + j] = (float)std::log(std::max((double)ctx->S[(size_t)m * nT + j], 1e-37));
+        invX0[m] = 1.0f / ctx->X0[m];
+    }
+    CU(cudaMemcpyAsync(ctx->d_blob(), blob.data(), blob.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));       // blob is a local vector
+    ctx->tb.n_mat = nm; ctx->tb.n_E = nE; ctx->tb.n_T = nT;
+    ctx->tb.lnE0 = (float)std::log((double)ctx->Eg[0]);
+    ctx->tb.inv_dlnE = (float)((nE - 1) / (std::log((double)ctx->Eg[nE - 1]) - std::log((double)ctx->Eg[0])));
+    ctx->tb.lnT0 = (float)std::log((double)ctx->Tg[0]);
+    ctx->tb.inv_dlnT = (float)((nT - 1) / (std::log((double)ctx->Tg[nT - 1]) - std::log((double)ctx->Tg[0])));
+    ctx->tb.blob = ctx->d_blob();
+    ctx->tb.blob_words = (int)blob.size();
+    ctx->tables_dirty = false;
+    return 0;
+}
+
+bool log_uniform(const std::vector<float>& g) {
+    const int n = (int)g.size();
+    if (!(g[0] > 0)) return false;
+    const double l0 = std::log((double)g[0]), d = (std::log((double)g[n - 1]) - l0) / (n - 1);
+    if (!(d > 0)) return false;
+    for (int i = 0; i < n; ++i) if (std::fabs(std::log((double)g[i]) - (l0 + i * d)) > 1e-3 * d) return false;
+    return true;
+}
+
+int check_geometry(aepid_ctx* ctx) {
+    const Geom& g = ctx->g;
+    for (int k = 0; k < 8; ++k) {
+        const double p[3] = {(k & 1) ? g.hix : g.lox, (k & 2) ? g.hiy : g.loy, (k & 4) ? g.hiz : g.loz};
+        const double r[3] = {p[0] - g.src[0], p[1] - g.src[1], p[2] - g.src[2]};
+        const double u = g.au[0] * r[0] + g.au[1] * r[1] + g.au[2] * r[2];
+        const double v = g.av[0] * r[0] + g.av[1] * r[1] + g.av[2] * r[2];
+        const double w = g.aw[0] * r[0] + g.aw[1] * r[1] + g.aw[2] * r[2];
+        if (std::fabs(u) >= kWorldHalf || std::fabs(v) >= kWorldHalf || w <= kWorldWMin || w >= g.sid)
+            return fail(ctx, AEPID_ERR_GEOMETRY, "phantom reaches outside the air region of the world box (|u|,|v| < 100 cm, -1 < w < sid)");
+    }
+    if (g.src[0] >= g.lox && g.src[0] < g.hix && g.src[1] >= g.loy && g.src[1] < g.hiy && g.src[2] >= g.loz && g.src[2] < g.hiz)
+        return fail(ctx, AEPID_ERR_GEOMETRY, "source lies inside the phantom");
+    return 0;
+}
+
+int fill_params(aepid_ctx* ctx, TransportParams& p) {
+    if (!ctx->have_mat) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_init_materials has not been called");
+    if (!ctx->have_phantom) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_load_phantom has not been called");
+    if (!ctx->have_epid) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_load_epid_layers has not been called");
+    if (!ctx->have_source) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_load_source has not been called");
+    if (int rc = check_geometry(ctx)) return rc;
+    for (int l = 0; l < ctx->g.n_layers; ++l)
+        if (ctx->g.lmat[l] >= ctx->n_mat) return fail(ctx, AEPID_ERR_BAD_ARG, "EPID layer material index out of range");
+    if (ctx->tables_dirty) if (int rc = build_tables(ctx)) return rc;
+    if (transport_smem_bytes(ctx->tb) > 200 * 1024) return fail(ctx, AEPID_ERR_NOMEM, "material tables do not fit in shared memory");
+    p.g = ctx->g; p.ph = ctx->ph; p.tb = ctx->tb; p.so = ctx->so;
+    p.vox = ctx->d_vox(); p.ep_batch = ctx->d_ep_batch(); p.ph_batch = ctx->d_ph_batch();
+    p.ledger = ctx->d_ledger(); p.counters = ctx->d_counters(); p.chunk_counter = ctx->d_chunk();
+    p.n_batches = ctx->dims.n_batches; p.nvox = ctx->lay.nvox; p.npix = ctx->lay.npix;
+    p.base = 0; p.seed = 0; p.n = 0; p.n_chunks = 0;
+    return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t aepid_workspace_bytes(const aepid_dims* dims) {
+    if (!dims_ok(dims)) return 0;
+    return make_layout(*dims).total;
+}
+
+int aepid_create(aepid_ctx** out, int device, void* cuda_stream, const aepid_dims* dims, void* workspace, size_t workspace_bytes) {
+    if (!out) return AEPID_ERR_BAD_ARG;
+    *out = nullptr;
+    aepid_ctx* ctx = new aepid_ctx();
+    *out = ctx;                                   // returned even on failure so that aepid_last_error works
+    if (!dims_ok(dims)) return fail(ctx, AEPID_ERR_BAD_ARG, "dims out of range");
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev <= 0) { cudaGetLastError(); return fail(ctx, AEPID_ERR_CUDA, "no CUDA device: this library has no CPU fallback"); }
+    if (device < 0 || device >= n_dev) return fail(ctx, AEPID_ERR_BAD_ARG, "device index out of range");
+    CU(cudaSetDevice(device));
+    cudaDeviceProp prop{};
+    CU(cudaGetDeviceProperties(&prop, device));
+    ctx->device = device; ctx->sm_count = prop.multiProcessorCount;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->dims = *dims; ctx->lay = make_layout(*dims);
+    if (!workspace || ((uintptr_t)workspace & (kAlign - 1))) return fail(ctx, AEPID_ERR_BAD_ARG, "workspace must be a 256-byte aligned device pointer");
+    if (classify(workspace) != MEM_DEVICE) return fail(ctx, AEPID_ERR_BAD_ARG, "workspace is not device memory");
+    if (workspace_bytes < ctx->lay.total) return fail(ctx, AEPID_ERR_NOMEM, "workspace smaller than aepid_workspace_bytes(dims)");
+    ctx->ws = static_cast<char*>(workspace);
+    return reset_tallies(ctx);
+}
+
+void aepid_destroy(aepid_ctx* ctx) { delete ctx; }
+
+const char* aepid_last_error(const aepid_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int aepid_synchronize(aepid_ctx* ctx) {
+    if (!ctx) return AEPID_ERR_BAD_ARG;
+    CU(cudaStreamSynchronize(ctx->stream));
+    return 0;
+}
+
+int aepid_init_materials(aepid_ctx* ctx, int n_mat, int n_E, const float* E, const float* muC, const float* muPE, const float* muPP,
+                         int n_T, const float* T, const float* S, const float* X0) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    if (!E || !muC || !muPE || !muPP || !T || !S || !X0) return fail(ctx, AEPID_ERR_BAD_ARG, "null table pointer");
+    if (n_mat < 1 || n_E < 2 || n_T < 2) return fail(ctx, AEPID_ERR_BAD_ARG, "table sizes out of range");
+    if (n_mat > ctx->dims.n_mat || n_E > ctx->dims.n_E || n_T > ctx->dims.n_T) return fail(ctx, AEPID_ERR_NOMEM, "tables exceed dims");
+    if (int rc = fetch(ctx, E, (size_t)n_E, ctx->Eg)) return rc;
+    if (int rc = fetch(ctx, T, (size_t)n_T, ctx->Tg)) return rc;
+    if (int rc = fetch(ctx, muC, (size_t)n_mat * n_E, ctx->muC)) return rc;
+    if (int rc = fetch(ctx, muPE, (size_t)n_mat * n_E, ctx->muPE)) return rc;
+    if (int rc = fetch(ctx, muPP, (size_t)n_mat * n_E, ctx->muPP)) return rc;
+    if (int rc = fetch(ctx, S, (size_t)n_mat * n_T, ctx->S)) return rc;
+    if (int rc = fetch(ctx, X0, (size_t)n_mat, ctx->X0)) return rc;
+    if (!log_uniform(ctx->Eg) || !log_uniform(ctx->Tg)) return fail(ctx, AEPID_ERR_BAD_ARG, "energy grids must be increasing and log-uniform");
+    for (float v : ctx->muC) if (!(v >= 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "negative or NaN cross section");
+    for (float v : ctx->muPE) if (!(v >= 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "negative or NaN cross section");
+    for (float v : ctx->muPP) if (!(v >= 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "negative or NaN cross section");
+    for (float v : ctx->S) if (!(v > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "stopping power must be positive");
+    for (float v : ctx->X0) if (!(v > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "radiation length must be positive");
+    ctx->n_mat = n_mat; ctx->n_E = n_E; ctx->n_T = n_T;
+    ctx->have_mat = true; ctx->tables_dirty = true;
+    return 0;
+}
+
+int aepid_load_phantom(aepid_ctx* ctx, int nx, int ny, int nz, const float sp[3], const float org[3],
+                       const float* rho, const unsigned char* mat) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    if (!ctx->have_mat) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_init_materials must come first");
+    if (!sp || !org || !rho || !mat) return fail(ctx, AEPID_ERR_BAD_ARG, "null phantom pointer");
+    if (nx < 1 || ny < 1 || nz < 1 || !(sp[0] > 0) || !(sp[1] > 0) || !(sp[2] > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "bad grid");
+    if (nx != ctx->dims.nx || ny != ctx->dims.ny || nz != ctx->dims.nz) return fail(ctx, AEPID_ERR_NOMEM, "phantom grid differs from dims");
+    const size_t n = (size_t)nx * ny * nz;
+    const MemKind kr = classify(rho), km = classify(mat);
+    const float* d_rho = rho; const unsigned char* d_mat = mat;
+    // host inputs are staged in the (about to be zeroed) phantom batch buffers: B >= 2 gives 8 bytes per voxel
+    char* stage = reinterpret_cast<char*>(ctx->d_ph_batch());
+    if (kr != MEM_DEVICE) { CU(cudaMemcpyAsync(stage, rho, n * 4, cudaMemcpyHostToDevice, ctx->stream)); d_rho = reinterpret_cast<const float*>(stage); }
+    if (km != MEM_DEVICE) { CU(cudaMemcpyAsync(stage + n * 4, mat, n, cudaMemcpyHostToDevice, ctx->stream)); d_mat = reinterpret_cast<const unsigned char*>(stage + n * 4); }
+    launch_pack_voxels(d_rho, d_mat, ctx->d_vox(), n, ctx->d_rho_max(), ctx->stream);
+    CU(cudaGetLastError());
+    ctx->rho_max.assign(kMaxMat, 0.0f);
+    CU(cudaMemcpyAsync(ctx->rho_max.data(), ctx->d_rho_max(), kMaxMat * 4, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    for (int m = ctx->n_mat; m < kMaxMat; ++m)
+        if (ctx->rho_max[m] > 0) return fail(ctx, AEPID_ERR_BAD_ARG, "material index out of range in the phantom");
+    Geom& g = ctx->g;
+    g.nx = nx; g.ny = ny; g.nz = nz;
+    g.hx = sp[0]; g.hy = sp[1]; g.hz = sp[2];
+    g.ihx = 1.0f / sp[0]; g.ihy = 1.0f / sp[1]; g.ihz = 1.0f / sp[2];
+    g.lox = org[0]; g.loy = org[1]; g.loz = org[2];
+    g.hix = org[0] + nx * sp[0]; g.hiy = org[1] + ny * sp[1]; g.hiz = org[2] + nz * sp[2];
+    ctx->have_phantom = true; ctx->tables_dirty = true;
+    return reset_tallies(ctx);
+}
+
+int aepid_load_epid_layers(aepid_ctx* ctx, int nl, const float* th, const unsigned char* mat, const float* rho,
+                           const unsigned char* scored, float sid, int nu, int nv, float pitch) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    if (!th || !mat || !rho || !scored) return fail(ctx, AEPID_ERR_BAD_ARG, "null layer pointer");
+    if (nl < 1 || nl > ctx->dims.n_layers) return fail(ctx, AEPID_ERR_NOMEM, "layer count exceeds dims");
+    if (nu != ctx->dims.nu || nv != ctx->dims.nv) return fail(ctx, AEPID_ERR_NOMEM, "EPID image differs from dims");
+    if (!(pitch > 0) || !(sid > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "pitch and sid must be positive");
+    Geom& g = ctx->g;
+    g.n_layers = nl; g.nu = nu; g.nv = nv; g.sid = sid; g.pitch = pitch; g.inv_pitch = 1.0f / pitch;
+    g.half_u = 0.5f * nu * pitch; g.half_v = 0.5f * nv * pitch;
+    double z = 0.0; g.zt[0] = 0.0f;
+    for (int l = 0; l < nl; ++l) {
+        if (!(th[l] > 0) || !(rho[l] > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "layer thickness and density must be positive");
+        z += th[l]; g.zt[l + 1] = (float)z;
+        g.lrho[l] = rho[l]; g.lmat[l] = mat[l]; g.lscored[l] = scored[l] ? 1 : 0;
+    }
+    for (int l = nl; l < kMaxLayers; ++l) { g.zt[l + 1] = g.zt[nl]; g.lrho[l] = 1.0f; g.lmat[l] = 0; g.lscored[l] = 0; }
+    ctx->have_epid = true;
+    return 0;
+}
+
+int aepid_load_source(aepid_ctx* ctx, const float src[3], const float axes[9], int nb, const float* edges, const float* pdf,
+                      int fu, int fv, float fpitch, float fdist, const float* fluence) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    if (!src || !axes || !edges || !pdf || !fluence) return fail(ctx, AEPID_ERR_BAD_ARG, "null source pointer");
+    if (nb < 1 || fu < 1 || fv < 1 || !(fpitch > 0) || !(fdist > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "bad source sizes");
+    if (nb > ctx->dims.n_bins || (size_t)fu * fv > (size_t)ctx->dims.fu * ctx->dims.fv) return fail(ctx, AEPID_ERR_NOMEM, "source exceeds dims");
+    for (int r = 0; r < 3; ++r) {                          // rows must be orthonormal
+        for (int q = r; q < 3; ++q) {
+            const double d = (double)axes[3 * r] * axes[3 * q] + (double)axes[3 * r + 1] * axes[3 * q + 1] + (double)axes[3 * r + 2] * axes[3 * q + 2];
+            if (std::fabs(d - (r == q ? 1.0 : 0.0)) > 1e-4) return fail(ctx, AEPID_ERR_BAD_ARG, "beam_axes rows are not orthonormal");
+        }
+    }
+    std::vector<float> he, hp, hf;
+    if (int rc = fetch(ctx, edges, (size_t)nb + 1, he)) return rc;
+    if (int rc = fetch(ctx, pdf, (size_t)nb, hp)) return rc;
+    if (int rc = fetch(ctx, fluence, (size_t)fu * fv, hf)) return rc;
+    // integer thresholds on the raw draw r: bin = #{k >= 1 : (r + 0.5) 2^-32 * total >= cdf[k]}
+    auto thresholds = [](const std::vector<float>& w, std::vector<uint32_t>& thr, double& total) {
+        const size_t n = w.size();
+        std::vector<double> cdf(n + 1, 0.0);
+        for (size_t i = 0; i < n; ++i) { if (!(w[i] >= 0)) return false; cdf[i + 1] = cdf[i] + (double)w[i]; }
+        total = cdf[n];
+        if (!(total > 0)) return false;
+        thr.resize(n + 1);
+        for (size_t k = 0; k <= n; ++k) {
+            const double t = std::ceil(cdf[k] / total * 4294967296.0 - 0.5);
+            thr[k] = t <= 0 ? 0u : (t >= 4294967295.0 ? 0xFFFFFFFFu : (uint32_t)t);
+        }
+        return true;
+    };
+    std::vector<uint32_t> tE, tF; double totE = 0, totF = 0;
+    if (!thresholds(hp, tE, totE)) return fail(ctx, AEPID_ERR_BAD_ARG, "spectrum pdf must be non-negative with a positive sum");
+    if (!thresholds(hf, tF, totF)) return fail(ctx, AEPID_ERR_BAD_ARG, "fluence must be non-negative with a positive sum");
+    tE[nb] = 0u;                                           // 2^32 mod 2^32: widths come out right by wrap-around
+    int j_last = 0;
+    ctx->bb_u0 = fu; ctx->bb_u1 = -1; ctx->bb_v0 = fv; ctx->bb_v1 = -1;
+    for (int j = 0; j < fv; ++j) for (int i = 0; i < fu; ++i)
+        if (hf[(size_t)j * fu + i] > 0) {
+            j_last = j * fu + i;
+            ctx->bb_u0 = std::min(ctx->bb_u0, i); ctx->bb_u1 = std::max(ctx->bb_u1, i);
+            ctx->bb_v0 = std::min(ctx->bb_v0, j); ctx->bb_v1 = std::max(ctx->bb_v1, j);
+        }
+    CU(cudaMemcpyAsync(ctx->d_thrE(), tE.data(), tE.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->d_edges(), he.data(), he.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->d_thrF(), tF.data(), tF.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));                // sources are local vectors
+    Geom& g = ctx->g;
+    for (int k = 0; k < 3; ++k) { g.src[k] = src[k]; g.au[k] = axes[k]; g.av[k] = axes[3 + k]; g.aw[k] = axes[6 + k]; }
+    Source& so = ctx->so;
+    so.n_bins = nb; so.fu = fu; so.fv = fv; so.j_last = j_last; so.fpitch = fpitch; so.fdist = fdist;
+    so.thrE = ctx->d_thrE(); so.edges = ctx->d_edges(); so.thrF = ctx->d_thrF();
+    ctx->have_source = true;
+    return 0;
+}
+
+int aepid_set_physics(aepid_ctx* ctx, int mode, float pcut, float ecut, float fE, float smax) {
+    if (!ctx) return AEPID_ERR_BAD_ARG;
+    if ((mode != 0 && mode != 1) || !(pcut > 0) || !(ecut > 0) || !(fE > 0) || !(fE <= 0.5f) || !(smax > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "physics parameters out of range");
+    ctx->ph.mode = mode; ctx->ph.pcut = pcut; ctx->ph.ecut = ecut; ctx->ph.fE = fE; ctx->ph.smax = smax;
+    return 0;
+}
+
+int aepid_reset_tallies(aepid_ctx* ctx) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    return reset_tallies(ctx);
+}
+
+int aepid_set_counting(aepid_ctx* ctx, int on) { if (!ctx) return AEPID_ERR_BAD_ARG; ctx->counting = on != 0; return 0; }
+
+int aepid_simulate(aepid_ctx* ctx, unsigned long long n_histories, unsigned long long seed) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    TransportParams p{};
+    if (int rc = fill_params(ctx, p)) return rc;
+    const int B = ctx->dims.n_batches;
+    unsigned long long left = n_histories;
+    while (left > 0) {
+        const unsigned long long n = std::min<unsigned long long>(left, 1ull << 31);
+        p.base = ctx->n_done; p.seed = seed; p.n = (uint32_t)n;
+        p.n_chunks = (uint32_t)((n + kChunk - 1) / kChunk);
+        CU(cudaMemsetAsync(ctx->d_chunk(), 0, sizeof(unsigned int), ctx->stream));
+        const int rc = launch_transport(p, ctx->counting, ctx->sm_count, ctx->stream);
+        if (rc != 0) return fail(ctx, AEPID_ERR_CUDA, std::string("transport launch: ") + cudaGetErrorString((cudaError_t)rc));
+        // histories per batch: chunk c goes to batch floor(c B / n_chunks), exactly as in the kernel
+        for (int b = 0; b < B; ++b) {
+            const uint64_t c0 = ((uint64_t)b * p.n_chunks + B - 1) / B, c1 = ((uint64_t)(b + 1) * p.n_chunks + B - 1) / B;
+            if (c1 <= c0) continue;
+            const uint64_t h0 = c0 * kChunk, h1 = std::min<uint64_t>(c1 * kChunk, n);
+            ctx->hist[b] += (double)(h1 - h0);
+        }
+        ctx->n_done += n; left -= n;
+    }
+    return 0;
+}
+
+int aepid_read_tallies(aepid_ctx* ctx, float* ep_mean, float* ep_sigma, float* ph_mean, float* ph_sigma, double ledger[8]) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    bool need_sync = false;
+    auto fold = [&](const float* batches, size_t n, float* mean, float* sigma, float* scratch) -> int {
+        if (!mean && !sigma) return 0;
+        FoldParams f{};
+        f.batches = batches; f.n = n; f.n_batches = ctx->dims.n_batches; f.total = (double)ctx->n_done;
+        std::copy(ctx->hist, ctx->hist + 256, f.hist);
+        const bool dm = mean && classify(mean) == MEM_DEVICE, ds = sigma && classify(sigma) == MEM_DEVICE;
+        f.mean = mean ? (dm ? mean : scratch) : nullptr;
+        f.sigma = sigma ? (ds ? sigma : scratch + n) : nullptr;
+        launch_fold(f, ctx->stream);
+        CU(cudaGetLastError());
+        if (mean && !dm) if (int rc = deliver(ctx, mean, scratch, n * 4, &need_sync)) return rc;
+        if (sigma && !ds) if (int rc = deliver(ctx, sigma, scratch + n, n * 4, &need_sync)) return rc;
+        return 0;
+    };
+    if (int rc = fold(ctx->d_ep_batch(), ctx->lay.npix, ep_mean, ep_sigma, ctx->d_out_ep())) return rc;
+    if (int rc = fold(ctx->d_ph_batch(), ctx->lay.nvox, ph_mean, ph_sigma, ctx->d_out_ph())) return rc;
+    if (ledger) {
+        CU(cudaMemcpyAsync(ledger, ctx->d_ledger(), 8 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        need_sync = true;
+    }
+    if (need_sync) CU(cudaStreamSynchronize(ctx->stream));
+    if (ledger) ledger[6] = (double)ctx->n_done;
+    return 0;
+}
+
+int aepid_read_batches(aepid_ctx* ctx, float* epid_batches, double* histories_per_batch) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    bool need_sync = false;
+    if (epid_batches) if (int rc = deliver(ctx, epid_batches, ctx->d_ep_batch(), ctx->lay.npix * 4 * ctx->dims.n_batches, &need_sync)) return rc;
+    if (need_sync) CU(cudaStreamSynchronize(ctx->stream));
+    if (histories_per_batch) std::copy(ctx->hist, ctx->hist + ctx->dims.n_batches, histories_per_batch);
+    return 0;
+}
+
+int aepid_read_counters(aepid_ctx* ctx, unsigned long long counters[16]) {
+    if (!ctx || !ctx->ws || !counters) return AEPID_ERR_BAD_ARG;
+    CU(cudaMemcpyAsync(counters, ctx->d_counters(), 16 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return 0;
+}
+
+int aepid_sample_source(aepid_ctx* ctx, unsigned long long first, unsigned long long n, unsigned long long seed, float* out) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    if (!out) return fail(ctx, AEPID_ERR_BAD_ARG, "null output");
+    if (!ctx->have_source) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_load_source has not been called");
+    TransportParams p{};
+    p.g = ctx->g; p.so = ctx->so; p.seed = seed;
+    if (classify(out) == MEM_DEVICE) {
+        launch_sample_source(p, first, n, out, ctx->stream);
+        CU(cudaGetLastError());
+        return 0;
+    }
+    const size_t cap = ctx->lay.nvox * 8 / 32;             // samples that fit in the phantom output scratch
+    if (cap == 0) return fail(ctx, AEPID_ERR_NOMEM, "scratch too small");
+    for (unsigned long long k = 0; k < n; k += cap) {
+        const unsigned long long m = std::min<unsigned long long>(cap, n - k);
+        launch_sample_source(p, first + k, m, ctx->d_out_ph(), ctx->stream);
+        CU(cudaGetLastError());
+        CU(cudaMemcpyAsync(out + 8 * k, ctx->d_out_ph(), m * 32, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+    }
+    return 0;
+}
+
+int aepid_field_size(aepid_ctx* ctx, int printed_form, float* s_cm) {
+    if (!ctx || !s_cm) return AEPID_ERR_BAD_ARG;
+    if (!ctx->have_source) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_load_source has not been called");
+    if (ctx->bb_u1 < 0) { *s_cm = 0.0f; return 0; }
+    const double sc = 100.0 / ctx->so.fdist;
+    const double a = (ctx->bb_u1 - ctx->bb_u0 + 1) * (double)ctx->so.fpitch * sc, b = (ctx->bb_v1 - ctx->bb_v0 + 1) * (double)ctx->so.fpitch * sc;
+    *s_cm = (float)(printed_form ? a * b / (2.0 * (a + b)) : 2.0 * a * b / (a + b));
+    return 0;
+}
+
+int aepid_apply_response_lut(aepid_ctx* ctx, const float* lut, int nt, int ns, float t_min, float t_max, float s_min, float s_max,
+                             float s_eff, const float* epid_in, float* signal_out, float* tmap_out) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    if (!lut || !signal_out) return fail(ctx, AEPID_ERR_BAD_ARG, "null lut or output");
+    if (nt < 1 || ns < 1 || (size_t)nt * ns > kMaxLut) return fail(ctx, AEPID_ERR_BAD_ARG, "LUT size out of range");
+    if ((nt > 1 && !(t_max > t_min)) || (ns > 1 && !(s_max > s_min))) return fail(ctx, AEPID_ERR_BAD_ARG, "LUT axes must be increasing");
+    if (!ctx->have_phantom || !ctx->have_epid || !ctx->have_source) return fail(ctx, AEPID_ERR_BAD_STATE, "phantom, EPID and source must be loaded");
+    const size_t n = ctx->lay.npix;
+    bool need_sync = false;
+    const float* d_lut = lut;
+    if (classify(lut) != MEM_DEVICE) {
+        CU(cudaMemcpyAsync(ctx->d_lut(), lut, (size_t)nt * ns * 4, cudaMemcpyHostToDevice, ctx->stream));
+        if (classify(lut) == MEM_HOST_PINNED) need_sync = true;
+        d_lut = ctx->d_lut();
+    }
+    if (s_eff < 0) if (int rc = aepid_field_size(ctx, 0, &s_eff)) return rc;
+    launch_tmap(ctx->g, ctx->d_vox(), ctx->d_tmap(), ctx->stream);
+    CU(cudaGetLastError());
+    const float* d_dose;
+    if (!epid_in) {
+        FoldParams f{};
+        f.batches = ctx->d_ep_batch(); f.n = n; f.n_batches = ctx->dims.n_batches; f.total = (double)ctx->n_done;
+        std::copy(ctx->hist, ctx->hist + 256, f.hist);
+        f.mean = ctx->d_dose_in(); f.sigma = nullptr;
+        launch_fold(f, ctx->stream);
+        CU(cudaGetLastError());
+        d_dose = ctx->d_dose_in();
+    } else if (classify(epid_in) == MEM_DEVICE) d_dose = epid_in;
+    else {
+        CU(cudaMemcpyAsync(ctx->d_dose_in(), epid_in, n * 4, cudaMemcpyHostToDevice, ctx->stream));
+        if (classify(epid_in) == MEM_HOST_PINNED) need_sync = true;
+        d_dose = ctx->d_dose_in();
+    }
+    const bool dev_out = classify(signal_out) == MEM_DEVICE;
+    float* d_out = dev_out ? signal_out : ctx->d_signal();
+    launch_apply_lut(d_lut, nt, ns, t_min, t_max, s_min, s_max, s_eff, d_dose, ctx->d_tmap(), d_out, n, ctx->stream);
+    CU(cudaGetLastError());
+    if (!dev_out) if (int rc = deliver(ctx, signal_out, d_out, n * 4, &need_sync)) return rc;
+    if (tmap_out) if (int rc = deliver(ctx, tmap_out, ctx->d_tmap(), n * 4, &need_sync)) return rc;
+    if (need_sync) CU(cudaStreamSynchronize(ctx->stream));
+    return 0;
+}
+
+}  // extern "C"

@@ -1,0 +1,101 @@
+// Kernel parameter blocks shared by the host API (api.cu) and the kernels (transport.cu, postpass.cu).
+// Plain structs, passed by value as __grid_constant__ kernel arguments.
+#pragma once
+#include <cstdint>
+#include <cstddef>
+
+namespace aepid {
+
+constexpr int kMaxLayers = 8;
+constexpr int kMaxMat = 32;
+constexpr int kChunk = 64;            // histories handed to a warp per grab of the global counter
+constexpr float kRhoAir = 1.205e-3f;  // world filler, material 0 (SURVEY 8(c) "Geometry")
+constexpr float kWorldHalf = 100.0f;  // |u|, |v| <= 100 cm
+constexpr float kWorldWMin = -1.0f;   // -1 <= w
+constexpr float kMec2 = 0.51099895f;
+
+enum Region : uint32_t { R_AIR = 0, R_PHANTOM = 1, R_EPID = 2 };
+enum PType : uint32_t { T_PHOTON = 0, T_ELECTRON = 1, T_POSITRON = 2 };
+
+struct Geom {
+    // phantom grid in the world frame
+    int nx, ny, nz;
+    float hx, hy, hz, ihx, ihy, ihz;
+    float lox, loy, loz, hix, hiy, hiz;
+    // beam frame
+    float src[3], au[3], av[3], aw[3];
+    // EPID slab stack; zt[] = depth of the layer tops below the EPID top plane (zt[0] = 0)
+    int n_layers, nu, nv;
+    float sid, pitch, inv_pitch, half_u, half_v;
+    float zt[kMaxLayers + 1];
+    float lrho[kMaxLayers];
+    int lmat[kMaxLayers];
+    int lscored[kMaxLayers];
+};
+
+struct Physics {
+    int mode;                          // 0 kerma, 1 coupled
+    float pcut, ecut, fE, smax;
+};
+
+// Table blob layout in global memory (copied verbatim into shared memory by every block):
+//   float4 phot[n_mat][n_E]  = {ln mu_pe, ln mu_compton, mu_pair, 0}
+//   float  maj[n_E]          majorant node values, safety margin included
+//   float  lnS[n_mat][n_T]   ln stopping power
+//   float  invX0[n_mat]
+struct Tables {
+    int n_mat, n_E, n_T;
+    float lnE0, inv_dlnE, lnT0, inv_dlnT;
+    const uint32_t* blob;
+    int blob_words;
+};
+
+struct Source {
+    int n_bins, fu, fv, j_last;
+    float fpitch, fdist;
+    const uint32_t* thrE;              // [n_bins+1] integer CDF thresholds on the raw 32-bit draw
+    const float* edges;                // [n_bins+1]
+    const uint32_t* thrF;              // [fu*fv+1]
+};
+
+struct TransportParams {
+    Geom g;
+    Physics ph;
+    Tables tb;
+    Source so;
+    const uint32_t* vox;               // packed voxels: density (19 mantissa bits) | material (5 bits)
+    float* ep_batch;                   // [B][nv*nu]
+    float* ph_batch;                   // [B][nz*ny*nx]
+    double* ledger;                    // [8]
+    unsigned long long* counters;      // [16]
+    unsigned int* chunk_counter;
+    uint64_t base;                     // global index of relative history 0 of this launch
+    uint64_t seed;
+    uint32_t n;                        // histories in this launch (< 2^32)
+    uint32_t n_chunks;
+    int n_batches;
+    size_t nvox, npix;
+};
+
+struct FoldParams {
+    const float* batches;              // [B][n]
+    size_t n;
+    int n_batches;
+    float* mean;                       // may be null
+    float* sigma;                      // may be null
+    double hist[256];                  // histories per batch
+    double total;
+};
+
+// launchers (defined in transport.cu / postpass.cu)
+int launch_transport(const TransportParams& p, bool counting, int sm_count, void* stream);
+size_t transport_smem_bytes(const Tables& t);
+void launch_pack_voxels(const float* rho, const unsigned char* mat, uint32_t* out, size_t n, float* rho_max, void* stream);
+void launch_fold(const FoldParams& p, void* stream);
+void launch_sample_source(const TransportParams& p, uint64_t first, uint64_t n, float* out, void* stream);
+void launch_tmap(const Geom& g, const uint32_t* vox, float* tmap, void* stream);
+void launch_apply_lut(const float* lut, int nt, int ns, float t_min, float t_max, float s_min, float s_max,
+                      float s_eff, const float* dose, const float* tmap, float* out, size_t n, void* stream);
+void launch_zero(void* ptr, size_t bytes, void* stream);
+
+}  // namespace aepid
