@@ -125,6 +125,20 @@ int aepid_simulate(aepid_ctx* ctx, unsigned long long n_histories, unsigned long
 int aepid_read_tallies(aepid_ctx* ctx, float* epid_mean, float* epid_sigma,
                        float* phantom_mean, float* phantom_sigma, double ledger[8]);
 
+/* Multi-GPU sharding: histories are independent, so rank r of G runs a disjoint block of the
+ * global history range.  aepid_set_history_offset makes the next aepid_simulate start at global history index
+ * `first_history` (Philox is keyed by the global index); call it after aepid_reset_tallies. */
+int aepid_set_history_offset(aepid_ctx* ctx, unsigned long long first_history);
+
+/* Per-bin sufficient statistics of this context's B batches, for the one exchange step of 8(e):
+ * s1 = sum_b x_b and s2 = sum_b x_b^2 / n_b (float64; images [nv][nu], volumes [nz][ny][nx]; DEVICE pointers, any may be
+ * NULL).  totals (HOST [2]) = {histories, non-empty batches}.  After an all-reduce(sum) of s1, s2 and totals over ranks,
+ * aepid_finalize_moments turns them into the mean per history and its standard error:
+ * mean = s1 / N, sigma^2 = (s2 - N mean^2) / ((B - 1) N).  n = number of bins; all pointers DEVICE. */
+int aepid_read_moments(aepid_ctx* ctx, double* epid_s1, double* epid_s2, double* phantom_s1, double* phantom_s2, double totals[2]);
+int aepid_finalize_moments(aepid_ctx* ctx, const double* s1, const double* s2, size_t n, double n_histories, double n_batches,
+                           float* mean, float* sigma);
+
 /* Raw per-batch EPID sums [B][nv][nu] (host or device, may be NULL) and histories per batch (HOST [B]). */
 int aepid_read_batches(aepid_ctx* ctx, float* epid_batches, double* histories_per_batch);
 

@@ -25,7 +25,8 @@ EXPORTS = ("aepid_workspace_bytes", "aepid_create", "aepid_destroy", "aepid_last
            "aepid_load_phantom", "aepid_load_epid_layers", "aepid_load_source", "aepid_set_physics",
            "aepid_reset_tallies", "aepid_simulate", "aepid_read_tallies", "aepid_read_batches",
            "aepid_set_counting", "aepid_read_counters", "aepid_sample_source", "aepid_field_size",
-           "aepid_apply_response_lut", "aepid_synchronize")
+           "aepid_apply_response_lut", "aepid_synchronize", "aepid_set_history_offset", "aepid_read_moments",
+           "aepid_finalize_moments")
 
 
 class AepidError(RuntimeError):
@@ -70,6 +71,9 @@ def load_library():
     lib.aepid_apply_response_lut.argtypes = [vp, vp, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_float,
                                              C.c_float, vp, vp, vp]
     lib.aepid_synchronize.argtypes = [vp]
+    lib.aepid_set_history_offset.argtypes = [vp, C.c_ulonglong]
+    lib.aepid_read_moments.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.aepid_finalize_moments.argtypes = [vp, vp, vp, C.c_size_t, C.c_double, C.c_double, vp, vp]
     _lib = lib
     return lib
 
@@ -212,6 +216,26 @@ class Engine:
         self._chk(self._lib.aepid_read_tallies(self._h, _ptr(em), _ptr(es), _ptr(pm), _ptr(ps), _ptr(led)))
         out["ledger"] = led
         return out
+
+    def set_history_offset(self, first_history):
+        self._chk(self._lib.aepid_set_history_offset(self._h, int(first_history)))
+
+    def read_moments(self, epid=True, phantom=True):
+        """Device tensors s1 = sum_b x_b, s2 = sum_b x_b^2/n_b and totals [histories, batches]."""
+        t = self._torch
+        mk = lambda shape: t.empty(shape, dtype=t.float64, device=self.device)
+        e1 = mk((self.nv, self.nu)) if epid else None; e2 = mk((self.nv, self.nu)) if epid else None
+        p1 = mk((self.nz, self.ny, self.nx)) if phantom else None; p2 = mk((self.nz, self.ny, self.nx)) if phantom else None
+        tot = np.zeros(2, dtype=np.float64)
+        self._chk(self._lib.aepid_read_moments(self._h, _ptr(e1), _ptr(e2), _ptr(p1), _ptr(p2), _ptr(tot)))
+        return {"epid_s1": e1, "epid_s2": e2, "phantom_s1": p1, "phantom_s2": p2, "totals": tot}
+
+    def finalize_moments(self, s1, s2, n_histories, n_batches):
+        t = self._torch
+        mean = t.empty(s1.shape, dtype=t.float32, device=s1.device); sigma = t.empty(s1.shape, dtype=t.float32, device=s1.device)
+        self._chk(self._lib.aepid_finalize_moments(self._h, _ptr(s1), _ptr(s2), s1.numel(), float(n_histories), float(n_batches),
+                                                   _ptr(mean), _ptr(sigma)))
+        return mean, sigma
 
     def read_batches(self):
         b = np.empty((self.n_batches, self.nv, self.nu), dtype=np.float32)

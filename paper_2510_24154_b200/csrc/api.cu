@@ -80,7 +80,8 @@ struct aepid_ctx {
     Tables tb{};
     Source so{};
     int bb_u0 = 0, bb_u1 = -1, bb_v0 = 0, bb_v1 = -1;    // bounding box of positive fluence pixels
-    unsigned long long n_done = 0;
+    unsigned long long n_done = 0;                         // histories since the last reset
+    unsigned long long first_history = 0;                  // global index of history 0 of this context (multi-GPU sharding)
     double hist[256] = {0};
     bool counting = false;
 
@@ -140,7 +141,7 @@ int reset_tallies(aepid_ctx* ctx) {
     CU(cudaMemsetAsync(ctx->d_ph_batch(), 0, ctx->lay.nvox * 4 * B, ctx->stream));
     CU(cudaMemsetAsync(ctx->d_ep_batch(), 0, ctx->lay.npix * 4 * B, ctx->stream));
     CU(cudaMemsetAsync(ctx->ws + ctx->lay.small, 0, 256, ctx->stream));
-    ctx->n_done = 0;
+    ctx->n_done = 0; ctx->first_history = 0;
     std::fill(ctx->hist, ctx->hist + 256, 0.0);
     return 0;
 }
@@ -425,7 +426,7 @@ int aepid_simulate(aepid_ctx* ctx, unsigned long long n_histories, unsigned long
     unsigned long long left = n_histories;
     while (left > 0) {
         const unsigned long long n = std::min<unsigned long long>(left, 1ull << 31);
-        p.base = ctx->n_done; p.seed = seed; p.n = (uint32_t)n;
+        p.base = ctx->first_history + ctx->n_done; p.seed = seed; p.n = (uint32_t)n;
         p.n_chunks = (uint32_t)((n + kChunk - 1) / kChunk);
         CU(cudaMemsetAsync(ctx->d_chunk(), 0, sizeof(unsigned int), ctx->stream));
         const int rc = launch_transport(p, ctx->counting, ctx->sm_count, ctx->stream);
@@ -467,6 +468,40 @@ int aepid_read_tallies(aepid_ctx* ctx, float* ep_mean, float* ep_sigma, float* p
     }
     if (need_sync) CU(cudaStreamSynchronize(ctx->stream));
     if (ledger) ledger[6] = (double)ctx->n_done;
+    return 0;
+}
+
+int aepid_set_history_offset(aepid_ctx* ctx, unsigned long long first_history) {
+    if (!ctx) return AEPID_ERR_BAD_ARG;
+    if (ctx->n_done != 0) return fail(ctx, AEPID_ERR_BAD_STATE, "set the history offset right after aepid_reset_tallies");
+    ctx->first_history = first_history;
+    return 0;
+}
+
+int aepid_read_moments(aepid_ctx* ctx, double* ep_s1, double* ep_s2, double* ph_s1, double* ph_s2, double totals[2]) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    for (const double* q : {ep_s1, ep_s2, ph_s1, ph_s2})
+        if (q && classify(q) != MEM_DEVICE) return fail(ctx, AEPID_ERR_BAD_ARG, "moment outputs must be device pointers");
+    FoldParams f{};
+    f.n_batches = ctx->dims.n_batches; f.total = (double)ctx->n_done;
+    std::copy(ctx->hist, ctx->hist + 256, f.hist);
+    if (ep_s1 || ep_s2) { f.batches = ctx->d_ep_batch(); f.n = ctx->lay.npix; launch_moments(f, ep_s1, ep_s2, ctx->stream); CU(cudaGetLastError()); }
+    if (ph_s1 || ph_s2) { f.batches = ctx->d_ph_batch(); f.n = ctx->lay.nvox; launch_moments(f, ph_s1, ph_s2, ctx->stream); CU(cudaGetLastError()); }
+    if (totals) {
+        totals[0] = (double)ctx->n_done; totals[1] = 0.0;
+        for (int b = 0; b < ctx->dims.n_batches; ++b) if (ctx->hist[b] > 0) totals[1] += 1.0;
+    }
+    return 0;
+}
+
+int aepid_finalize_moments(aepid_ctx* ctx, const double* s1, const double* s2, size_t n, double n_histories, double n_batches,
+                           float* mean, float* sigma) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    if (!s1 || (sigma && !s2)) return fail(ctx, AEPID_ERR_BAD_ARG, "null moment pointer");
+    for (const void* q : {(const void*)s1, (const void*)s2, (const void*)mean, (const void*)sigma})
+        if (q && classify(q) != MEM_DEVICE) return fail(ctx, AEPID_ERR_BAD_ARG, "moment buffers must be device pointers");
+    launch_finalize_moments(s1, s2, n, n_histories, n_batches, mean, sigma, ctx->stream);
+    CU(cudaGetLastError());
     return 0;
 }
 

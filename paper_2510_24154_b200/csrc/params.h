@@ -92,6 +92,8 @@ int launch_transport(const TransportParams& p, bool counting, int sm_count, void
 size_t transport_smem_bytes(const Tables& t);
 void launch_pack_voxels(const float* rho, const unsigned char* mat, uint32_t* out, size_t n, float* rho_max, void* stream);
 void launch_fold(const FoldParams& p, void* stream);
+void launch_moments(const FoldParams& p, double* s1, double* s2, void* stream);
+void launch_finalize_moments(const double* s1, const double* s2, size_t n, double total, double batches, float* mean, float* sigma, void* stream);
 void launch_sample_source(const TransportParams& p, uint64_t first, uint64_t n, float* out, void* stream);
 void launch_tmap(const Geom& g, const uint32_t* vox, float* tmap, void* stream);
 void launch_apply_lut(const float* lut, int nt, int ns, float t_min, float t_max, float s_min, float s_max,

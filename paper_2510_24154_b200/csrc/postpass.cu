@@ -61,6 +61,37 @@ void launch_fold(const FoldParams& p, void* stream) {
     fold_kernel<<<grid_for(p.n, 256), 256, 0, (cudaStream_t)stream>>>(p);
 }
 
+// ---- multi-GPU exchange: per-bin moments of the batches, and their finalisation after the all-reduce
+__global__ void moments_kernel(const __grid_constant__ FoldParams p, double* __restrict__ s1, double* __restrict__ s2) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < p.n; i += (size_t)gridDim.x * blockDim.x) {
+        double a = 0.0, q = 0.0;
+        for (int b = 0; b < p.n_batches; ++b) {
+            const double nh = p.hist[b];
+            if (nh <= 0.0) continue;
+            const double x = (double)p.batches[(size_t)b * p.n + i];
+            a += x; q += x * x / nh;
+        }
+        if (s1) s1[i] = a;
+        if (s2) s2[i] = q;
+    }
+}
+void launch_moments(const FoldParams& p, double* s1, double* s2, void* stream) {
+    if (p.n == 0) return;
+    moments_kernel<<<grid_for(p.n, 256), 256, 0, (cudaStream_t)stream>>>(p, s1, s2);
+}
+__global__ void finalize_moments_kernel(const double* __restrict__ s1, const double* __restrict__ s2, size_t n, double total, double batches,
+                                        float* __restrict__ mean, float* __restrict__ sigma) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const double m = total > 0.0 ? s1[i] / total : 0.0;
+        if (mean) mean[i] = (float)m;
+        if (sigma) sigma[i] = batches > 1.0 ? (float)sqrt(fmax(s2[i] - total * m * m, 0.0) / ((batches - 1.0) * total)) : 0.0f;
+    }
+}
+void launch_finalize_moments(const double* s1, const double* s2, size_t n, double total, double batches, float* mean, float* sigma, void* stream) {
+    if (n == 0) return;
+    finalize_moments_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)stream>>>(s1, s2, n, total, batches, mean, sigma);
+}
+
 // ---- K8 radiological thickness: one ray per EPID pixel, 3-D DDA through the packed grid (reading A17)
 __global__ void tmap_kernel(const __grid_constant__ Geom g, const uint32_t* __restrict__ vox, float* __restrict__ tmap) {
     const int ju = blockIdx.x * blockDim.x + threadIdx.x, jv = blockIdx.y * blockDim.y + threadIdx.y;

@@ -1,0 +1,324 @@
+"""Parity of the CUDA path against the CPU oracle, through the C-ABI (run with -m gpu on a B200).
+
+Monte Carlo tallies are random variables: what is compared is (a) the per-history source sample (bit-level up to
+float rounding, both sides key Philox identically), (b) tallies within combined statistical uncertainty, with the
+tolerances of BASELINE.json:north_star written out below, (c) exact invariants (energy ledger, tally sums).
+
+Tolerances:
+  * >= 99 % of EPID pixels above 20 % of max within 3 combined sigma, at the finest re-binning at which the oracle
+    has >= ~50 deposit events per tested pixel (reading A20; the factor is stated per test);
+  * integral deposited energy (EPID scored, phantom) within 0.5 % + 3 sigma of the statistical error of the comparison;
+  * energy balance to 1e-6 relative.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from gen import make_config
+from gen.configs import paper_table1_lut
+from util import slab_cfg, rebin2d
+
+pytestmark = pytest.mark.gpu
+
+
+def engine_for(cfg, **kw):
+    from paper_2510_24154_b200 import Engine
+    eng = Engine.for_config(cfg, **kw)
+    eng.load_config(cfg)
+    return eng
+
+
+def gpu_rebinned(eng, r):
+    """Mean and sigma of the EPID image re-binned by r, from the raw batch sums (exact re-binning of the batch estimator)."""
+    b, nb = eng.read_batches()
+    B = b.shape[0]
+    rb = b.reshape(B, b.shape[1] // r, r, b.shape[2] // r, r).sum(axis=(2, 4)).astype(np.float64)
+    use = nb > 0
+    rb, nb = rb[use], nb[use]
+    N = nb.sum()
+    mean = rb.sum(0) / N
+    var = (nb[:, None, None] * (rb / nb[:, None, None] - mean) ** 2).sum(0) / ((len(nb) - 1) * N)
+    return mean, np.sqrt(var)
+
+
+def check_ledger(L, n, tol=1e-6):
+    assert L[6] == n and L[7] == 0
+    assert abs(L[1] + L[2] + L[3] + L[4] + L[5] - L[0]) <= tol * L[0]
+
+
+def integral_check(g_sum_per_hist, o_raw_sum, o_raw_sq, n_o, g_sigma_total=0.0, rel=0.005):
+    """|gpu - oracle| <= rel * oracle + 3 sigma_comb for a summed tally (per history)."""
+    o_mean = o_raw_sum / n_o
+    o_var = max(o_raw_sq / n_o - o_mean ** 2, 0.0) / max(n_o - 1, 1)
+    tol = rel * o_mean + 3.0 * np.sqrt(o_var + g_sigma_total ** 2)
+    assert abs(g_sum_per_hist - o_mean) <= tol, (g_sum_per_hist, o_mean, tol)
+
+
+def compare(cfg, n_gpu, n_or, rebin, seed=None, frac_ok=0.99, procs=None, phantom_voxels=True, min_tested=30):
+    seed = cfg["seed"] if seed is None else seed
+    eng = engine_for(cfg)
+    eng.simulate(n_gpu, seed)
+    r = eng.read_tallies()
+    L = r["ledger"]
+    check_ledger(L, n_gpu)
+    # tally sums reproduce the ledger (float32 atomics vs double ledger)
+    assert abs(r["phantom_mean"].sum(dtype=np.float64) * n_gpu / L[1] - 1) < 2e-4
+    if L[2] > 0:
+        assert abs(r["epid_mean"].sum(dtype=np.float64) * n_gpu / L[2] - 1) < 2e-4
+    raw = oracle.run_sharded(cfg, n_or, seed, rebin=rebin, procs=procs, want_phantom_sq=phantom_voxels)
+    st = oracle.stats(raw)
+    Lo = raw["ledger"]
+    # ledger entries per history: every channel of the energy budget agrees
+    for k in (1, 3, 4, 5):
+        per_o, per_g = Lo[k] / n_or, L[k] / n_gpu
+        spread = 2.0 * max(per_o, 0.01)                                   # generous per-history standard deviation
+        assert abs(per_g - per_o) <= 0.005 * per_o + 4 * spread * np.sqrt(1.0 / n_or + 1.0 / n_gpu), (k, per_g, per_o)
+    # EPID image, re-binned
+    gm, gs = gpu_rebinned(eng, rebin)
+    om, os_ = st["rb_mean"], st["rb_sigma"]
+    k = om > 0.2 * om.max()
+    assert k.sum() >= min_tested
+    z = (gm[k] - om[k]) / np.sqrt(gs[k] ** 2 + os_[k] ** 2)
+    assert np.mean(np.abs(z) < 3) >= frac_ok, (np.mean(np.abs(z) < 3), z.mean(), z.std())
+    assert abs(z.mean()) < 0.35 and 0.7 < z.std() < 1.3, (z.mean(), z.std())
+    # integral EPID scored energy
+    q = raw["rb_sq"].sum()                                                # lower bound of the sum's second moment
+    g_tot_sigma = np.sqrt((gs ** 2).sum())
+    integral_check(gm.sum(), raw["rb_sum"].sum(), max(q, (raw["rb_sum"].sum() ** 2) / n_or * 1.0001), n_or, g_tot_sigma)
+    # phantom
+    pm, ps = r["phantom_mean"].astype(np.float64), r["phantom_sigma"].astype(np.float64)
+    assert abs(pm.sum() - st["phantom_mean"].sum()) <= 0.005 * st["phantom_mean"].sum() + 4 * 2.0 * np.sqrt(1.0 / n_or + 1.0 / n_gpu)
+    if phantom_voxels:
+        om, os_ = st["phantom_mean"], st["phantom_sigma"]
+        k = om > 0.2 * om.max()
+        z = (pm[k] - om[k]) / np.sqrt(ps[k] ** 2 + os_[k] ** 2 + 1e-300)
+        assert np.mean(np.abs(z) < 3) >= frac_ok, (np.mean(np.abs(z) < 3), z.mean(), z.std())
+        assert abs(z.mean()) < 0.1 and 0.9 < z.std() < 1.1, (z.mean(), z.std())
+    else:   # depth-dose profile along the beam, 1 % + statistics
+        ax = (0, 2) if cfg["source"]["beam_axes"].reshape(3, 3)[2][1] != 0 else (1, 2)
+        dg, do = pm.sum(axis=ax), st["phantom_mean"].sum(axis=ax)
+        kk = do > 0.2 * do.max()
+        assert np.abs(dg[kk] / do[kk] - 1).max() < 0.03
+    eng.close()
+    return r, raw
+
+
+# ------------------------------------------------------------------ K1
+@pytest.mark.parametrize("name,shrink,first,seed", [("C1", 4, 0, 1), ("C2", 8, 2**32 - 1000, (7 << 32) | 12345), ("C0", 2, 123456789012, 99)])
+def test_source_sample_matches_oracle_per_history(name, shrink, first, seed):
+    cfg = make_config(name, shrink=shrink)
+    eng = engine_for(cfg)
+    n = 100_000
+    g = eng.sample_source(first, n, seed).astype(np.float64)
+    o = oracle.Oracle(cfg).sample_source(first, n, seed)
+    assert np.array_equal(g[:, 4].astype(np.int64), o[:, 4].astype(np.int64))          # fluence pixel: exact
+    assert np.abs(g[:, 0] - o[:, 0]).max() <= 2e-6 * o[:, 0].max()                     # energy: float rounding
+    assert np.abs(g[:, 1:4] - o[:, 1:4]).max() < 2e-6                                  # direction (world frame)
+    assert np.abs(g[:, 5:7] - o[:, 5:7]).max() < 2e-6 * 10                             # 23-bit vs 32-bit in-pixel offset on a 0.1 cm pixel
+    eng.close()
+
+
+# ------------------------------------------------------------------ configs
+def test_c0_photon_only_kerma_full_size():
+    cfg = make_config("C0")
+    compare(cfg, 10_000_000, 10_000_000, rebin=2)      # 64x64 @ 4 mm -> 32x32 @ 8 mm: ~95 oracle events per tested pixel
+
+
+def test_c0_at_its_own_history_count_and_seed():
+    cfg = make_config("C0")
+    eng = engine_for(cfg)
+    eng.simulate(cfg["n_histories"], cfg["seed"])
+    r = eng.read_tallies()
+    check_ledger(r["ledger"], cfg["n_histories"])
+    raw = oracle.run_sharded(cfg, cfg["n_histories"], cfg["seed"])
+    # same histories, same source samples: emitted energy is identical, deposits agree statistically
+    assert r["ledger"][0] == pytest.approx(raw["ledger"][0], rel=1e-7)
+    assert abs(r["ledger"][1] - raw["ledger"][1]) / raw["ledger"][1] < 0.01
+    eng.close()
+
+
+def test_c1_coupled_full_size_bench_configuration():
+    cfg = make_config("C1")
+    compare(cfg, cfg["n_histories"], 4_000_000, rebin=8)   # 512x384 @ 0.784 mm -> 64x48 @ 6.3 mm (~100 oracle events / pixel)
+
+
+def test_c2_heterogeneous_imrt_full_grid():
+    cfg = make_config("C2")
+    compare(cfg, 40_000_000, 2_000_000, rebin=32, frac_ok=0.985, phantom_voxels=False, min_tested=15)
+
+
+def test_c3_large_patient_quarter_resolution():
+    cfg = make_config("C3", shrink=2)                   # 256x256x100 grid of the same anatomy; full grid: test_c3_full_grid_properties
+    compare(cfg, 20_000_000, 1_000_000, rebin=32, frac_ok=0.985, phantom_voxels=False, min_tested=10, procs=8)
+
+
+def test_c3_full_grid_properties():
+    cfg = make_config("C3")
+    eng = engine_for(cfg, n_batches=8)
+    n = 20_000_000
+    eng.simulate(n, 1)
+    r = eng.read_tallies(sigma=False)
+    check_ledger(r["ledger"], n)
+    assert abs(r["phantom_mean"].sum(dtype=np.float64) * n / r["ledger"][1] - 1) < 2e-4
+    # dose only where the beam and the body are: air voxels far outside the field stay (almost) empty
+    rho = cfg["phantom"]["density"]
+    assert r["phantom_mean"][rho > 0.5].sum(dtype=np.float64) > 0.9 * r["phantom_mean"].sum(dtype=np.float64)
+    eng.close()
+
+
+@pytest.mark.parametrize("field", [0, 7])
+def test_c4_field_with_response_post_pass(field):
+    cfg = make_config("C4", field=field, shrink=2)
+    r, raw = compare(cfg, 10_000_000, 1_000_000, rebin=32, frac_ok=0.98, phantom_voxels=False, min_tested=6)
+    # K8 on the GPU image against the oracle's post-pass of the same image
+    eng = engine_for(cfg)
+    lut = cfg["lut"]
+    dose = r["epid_mean"]
+    sig, tmap = eng.apply_response_lut(lut["lut"], lut["t_min"], lut["t_max"], lut["s_min"], lut["s_max"], -1.0, epid_in=dose)
+    o = oracle.Oracle(cfg)
+    s_o = o.field_size()
+    assert eng.field_size() == pytest.approx(s_o, rel=1e-6)
+    t_o = o.tmap()
+    assert np.abs(tmap - t_o).max() <= 1e-4 * t_o.max()
+    ref = o.apply_lut(lut, dose, t_o, s_o)
+    assert np.abs(sig - ref).max() <= 2e-5 * np.abs(ref).max()
+    eng.close()
+
+
+def test_rotated_gantry_general_beam_axes():
+    th = np.deg2rad(30.0)
+    cfg = slab_cfg(n=(40, 40, 40), h=(0.5, 0.5, 0.5), mode=1, epid="C1", nu=64, nv=64, pitch=0.4, sid=150.0, field_cm=8.0)
+    cfg["phantom"]["origin"] = np.array([-10.0, -10.0, -10.0], dtype=np.float32)
+    w = np.array([0.0, np.sin(th), np.cos(th)]); v = np.array([0.0, np.cos(th), -np.sin(th)]); u = np.array([1.0, 0.0, 0.0])
+    cfg["source"]["beam_axes"] = np.stack([u, v, w]).astype(np.float32)
+    cfg["source"]["src_pos"] = (-100.0 * w).astype(np.float32)
+    cfg["phantom"]["density"][10:20, :, :] = 0.3
+    cfg["phantom"]["material"][10:20, :, :] = 1
+    compare(cfg, 4_000_000, 1_000_000, rebin=4, frac_ok=0.98, seed=5, min_tested=10)
+
+
+# ------------------------------------------------------------------ invariants, edge cases, errors
+def test_partition_and_batch_invariance():
+    cfg = make_config("C1", shrink=4)
+    res = []
+    for nb, parts in ((32, (300_000,)), (8, (100_001, 199_999)), (2, (63, 1, 299_936))):
+        eng = engine_for(cfg, n_batches=nb)
+        for p in parts:
+            eng.simulate(p, 3)
+        r = eng.read_tallies()
+        check_ledger(r["ledger"], 300_000)
+        b, hist = eng.read_batches()
+        assert hist.sum() == 300_000 and len(hist) == nb
+        res.append(r)
+        eng.close()
+    # the same histories were run: per-history means agree to float32 accumulation order
+    for r in res[1:]:
+        assert np.allclose(r["ledger"][:6], res[0]["ledger"][:6], rtol=2e-6)
+        assert np.allclose(r["phantom_mean"], res[0]["phantom_mean"], rtol=1e-3, atol=1e-9)
+        assert np.allclose(r["epid_mean"].sum(), res[0]["epid_mean"].sum(), rtol=1e-4)
+
+
+def test_moments_path_equals_read_tallies():
+    cfg = make_config("C1", shrink=4)
+    eng = engine_for(cfg)
+    eng.simulate(200_000, 1)
+    r = eng.read_tallies()
+    from paper_2510_24154_b200 import parallel
+    g = parallel.global_tallies(eng)
+    assert g["n_histories"] == 200_000 and g["n_batches"] == 32
+    for k in ("epid_mean", "epid_sigma", "phantom_mean", "phantom_sigma"):
+        a, b = g[k].cpu().numpy(), r[k]
+        assert np.allclose(a, b, rtol=2e-4, atol=1e-12), k
+    # sharded run of the same global range on "two ranks" (sequentially on this GPU) reproduces the single-rank ledger
+    tot = np.zeros(8)
+    for rank in range(2):
+        parallel.simulate_sharded(eng, 200_000, 1, rank, 2)
+        tot += eng.read_tallies(epid=False, phantom=False)["ledger"]
+    assert np.allclose(tot[:6], r["ledger"][:6], rtol=2e-6)
+    eng.close()
+
+
+def test_edge_cases():
+    cfg = make_config("C0", shrink=4)
+    eng = engine_for(cfg, n_batches=2)
+    eng.simulate(0, 1)
+    r = eng.read_tallies()
+    assert r["ledger"][6] == 0 and r["epid_mean"].sum() == 0 and r["phantom_mean"].sum() == 0
+    eng.simulate(1, 1)
+    r = eng.read_tallies()
+    check_ledger(r["ledger"], 1)
+    assert r["ledger"][0] == pytest.approx(2.0)
+    eng.reset_tallies()
+    eng.simulate(65, 1)
+    check_ledger(eng.read_tallies()["ledger"], 65)
+    # vacuum-like phantom and a single-pixel fluence: every photon flies to the EPID or out of the world
+    cfg["phantom"]["density"][:] = 1e-6
+    fl = np.zeros((100, 100), np.float32); fl[50, 50] = 3.0
+    cfg["source"]["fluence"] = fl
+    eng2 = engine_for(cfg)
+    eng2.simulate(100_000, 2)
+    r = eng2.read_tallies()
+    check_ledger(r["ledger"], 100_000)
+    assert r["ledger"][1] < 1e-4 * r["ledger"][0]
+    img = r["epid_mean"]
+    assert img[6:10, 6:10].sum() > 0.9 * img.sum()                   # 16x16 image of 1.6 cm pixels: beam lands on the axis
+    assert eng2.field_size() == pytest.approx(0.1)
+    eng.close(); eng2.close()
+
+
+def test_error_codes():
+    from paper_2510_24154_b200 import AepidError, Engine
+    cfg = make_config("C0", shrink=4)
+    eng = Engine.for_config(cfg)
+    with pytest.raises(AepidError, match="BAD_STATE"):
+        eng.simulate(10, 1)                                           # nothing loaded
+    t, ph, ep, s = cfg["tables"], cfg["phantom"], cfg["epid"], cfg["source"]
+    with pytest.raises(AepidError, match="BAD_STATE"):
+        eng.load_phantom(ph["spacing"], ph["origin"], ph["density"], ph["material"])   # materials first
+    bad = t["E_grid"].copy(); bad[10] *= 1.01
+    with pytest.raises(AepidError, match="BAD_ARG"):
+        eng.init_materials(bad, t["mu_compton"], t["mu_pe"], t["mu_pair"], t["T_grid"], t["stop_pow"], t["rad_len"])
+    eng.init_materials(t["E_grid"], t["mu_compton"], t["mu_pe"], t["mu_pair"], t["T_grid"], t["stop_pow"], t["rad_len"])
+    with pytest.raises(AepidError, match="NOMEM"):
+        eng.load_phantom(ph["spacing"], ph["origin"], np.ones((3, 3, 3), np.float32), np.zeros((3, 3, 3), np.uint8))
+    m = ph["material"].copy(); m[0, 0, 0] = 9
+    with pytest.raises(AepidError, match="BAD_ARG"):
+        eng.load_phantom(ph["spacing"], ph["origin"], ph["density"], m)
+    eng.load_phantom(ph["spacing"], ph["origin"], ph["density"], ph["material"])
+    eng.load_epid_layers(ep["thickness"], ep["material"], ep["density"], ep["scored"], 110.0, ep["nu"], ep["nv"], ep["pitch"])
+    eng.load_source(s["src_pos"], s["beam_axes"], s["E_edges"], s["E_pdf"], s["f_pitch"], s["f_plane_dist"], s["fluence"])
+    with pytest.raises(AepidError, match="GEOMETRY"):
+        eng.simulate(10, 1)                                           # EPID top at 110 cm cuts the phantom (100..120)
+    with pytest.raises(AepidError, match="BAD_ARG"):
+        eng.load_source(s["src_pos"], np.ones(9, np.float32), s["E_edges"], s["E_pdf"], s["f_pitch"], s["f_plane_dist"], s["fluence"])
+    with pytest.raises(AepidError, match="BAD_ARG"):
+        eng.load_source(s["src_pos"], s["beam_axes"], s["E_edges"], s["E_pdf"], s["f_pitch"], s["f_plane_dist"], np.zeros((100, 100), np.float32))
+    with pytest.raises(AepidError, match="BAD_ARG"):
+        eng.set_physics(mode=3)
+    eng.load_epid_layers(ep["thickness"], ep["material"], ep["density"], ep["scored"], ep["sid"], ep["nu"], ep["nv"], ep["pitch"])
+    eng.simulate(1000, 1)                                             # recovers after the errors
+    check_ledger(eng.read_tallies()["ledger"], 1000)
+    eng.close()
+
+
+def test_response_post_pass_paper_table1():
+    cfg = slab_cfg(n=(40, 40, 40), h=(1.0, 1.0, 0.5), field_cm=10.0, nu=32, nv=32, pitch=0.8, sid=150.0)
+    eng = engine_for(cfg)
+    lut = paper_table1_lut()
+    dose = np.ones((32, 32), np.float32)
+    sig, tmap = eng.apply_response_lut(lut["lut"], lut["t_min"], lut["t_max"], lut["s_min"], lut["s_max"], 10.0, epid_in=dose)
+    c = (np.arange(32) + 0.5 - 16) * 0.8
+    U, V = np.meshgrid(c, c)
+    t_exp = 20.0 * np.sqrt(150.0**2 + U**2 + V**2) / 150.0           # uniform 20 cm slab: t = L / cos(theta)
+    assert np.abs(tmap - t_exp).max() < 1e-4 * 20
+    assert np.allclose(sig, 0.953, atol=1e-6)                        # t >= 20 clamps to the last column of the s = 10 row
+    for t_cm, s_cm, k in ((0.0, 5.0, 0.999), (10.0, 12.5, 0.975), (7.5, 7.5, 0.9690), (15.0, 20.0, 1.034), (50.0, 1.0, 0.949)):
+        cfg["phantom"]["density"][:] = t_cm / 20.0
+        e2 = engine_for(cfg)
+        sig, tmap = e2.apply_response_lut(lut["lut"], 0.0, 20.0, 5.0, 20.0, s_cm, epid_in=dose)
+        assert sig[16, 16] == pytest.approx(k, abs=2e-4), (t_cm, s_cm)
+        e2.close()
+    assert eng.field_size() == pytest.approx(10.0) and eng.field_size(True) == pytest.approx(2.5)
+    o = oracle.Oracle(cfg)
+    assert np.abs(engine_for(cfg).apply_response_lut(lut["lut"], 0.0, 20.0, 5.0, 20.0, -1.0, epid_in=dose)[1] - o.tmap()).max() < 1e-3
+    eng.close()
