@@ -256,7 +256,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     if world > 1: dist.barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e2e_steps = max(1, min(args.steps, 5))
+    e2e_steps = 1 if args.profile else max(1, min(args.steps, 5))
     e0.record()
     for _ in range(e2e_steps):
         e2e_step()
@@ -285,7 +285,7 @@ def run_ours(args):
     procs = os.cpu_count() or 1
     oracle.build()
     oracle.run_sharded(cfg, procs * 100, seed, procs=procs)              # fork / page-in warm-up
-    ns = args.cpu_sample
+    ns = 10_000 if args.profile else args.cpu_sample
     t0 = time.perf_counter()
     oracle.run_sharded(cfg, ns, seed, procs=procs)
     dt = time.perf_counter() - t0
@@ -318,6 +318,7 @@ def main():
     ap.add_argument("--histories", type=int, default=0, help="histories per GPU per step (default: the config's)")
     ap.add_argument("--cpu-sample", type=int, default=1_000_000, help="oracle histories timed for cpu_baseline")
     ap.add_argument("--ref-histories", type=int, default=400_000, help="oracle histories per step of --impl reference")
+    ap.add_argument("--profile", action="store_true", help="short run for ncu: one e2e step, tiny cpu_baseline sample (numbers are not bench values)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
