@@ -173,10 +173,10 @@ def test_c3_full_grid_properties():
     eng.close()
 
 
-@pytest.mark.parametrize("field", [0, 7])
-def test_c4_field_with_response_post_pass(field):
+@pytest.mark.parametrize("field,rebin,min_tested", [(0, 32, 6), (7, 8, 20)])   # 11.7x8 cm and 4.1x3.5 cm fields (reading A20)
+def test_c4_field_with_response_post_pass(field, rebin, min_tested):
     cfg = make_config("C4", field=field, shrink=2)
-    r, raw = compare(cfg, 10_000_000, 1_000_000, rebin=32, frac_ok=0.98, phantom_voxels=False, min_tested=6)
+    r, raw = compare(cfg, 10_000_000, 1_000_000, rebin=rebin, frac_ok=0.98, phantom_voxels=False, min_tested=min_tested)
     # K8 on the GPU image against the oracle's post-pass of the same image
     eng = engine_for(cfg)
     lut = cfg["lut"]
