@@ -142,11 +142,14 @@ int aepid_finalize_moments(aepid_ctx* ctx, const double* s1, const double* s2, s
 /* Raw per-batch EPID sums [B][nv][nu] (host or device, may be NULL) and histories per batch (HOST [B]). */
 int aepid_read_batches(aepid_ctx* ctx, float* epid_batches, double* histories_per_batch);
 
-/* Event counters since the last reset (HOST [16]): Woodcock flights, air flights, EPID flights, photoelectric,
- * Compton, pair, electron steps in phantom / air / EPID, secondaries, -, max stack depth, KN iterations,
- * photon cutoffs, charged tracks, zero-length steps.  Only counted while aepid_set_counting(ctx, 1). */
+/* Event and scheduler counters since the last reset (HOST [32]), only counted while aepid_set_counting(ctx, 1):
+ * [0..15] Woodcock flights, air flights, EPID flights, photoelectric, Compton, pair, electron steps in phantom / air / EPID,
+ * secondaries, -, -, KN iterations, photon cutoffs, charged tracks, zero-length steps;
+ * [16..31] scheduler: write-back/refill phases, photon loop iterations (warp level), active lanes summed over those,
+ * charged loop iterations, active lanes summed over those, source tasks, idle polls, queue claims, particles loaded,
+ * particles stored, secondaries spawned, rest unused. */
 int aepid_set_counting(aepid_ctx* ctx, int on);
-int aepid_read_counters(aepid_ctx* ctx, unsigned long long counters[16]);
+int aepid_read_counters(aepid_ctx* ctx, unsigned long long counters[32]);
 
 /* K1 alone: source samples of histories [first, first+n): out[n][8] = {E, dx, dy, dz (world), fluence pixel,
  * u, v on the fluence plane, 0}; host or device. */

@@ -20,7 +20,10 @@ LEDGER_NAMES = ("emitted", "dep_phantom", "dep_epid_scored", "dep_epid_other", "
                 "n_histories", "overflow")
 COUNTER_NAMES = ("woodcock_flights", "air_flights", "epid_flights", "n_pe", "n_compton", "n_pair",
                  "esteps_phantom", "esteps_air", "esteps_epid", "n_secondaries", "unused",
-                 "max_stack", "kn_iterations", "photon_cutoffs", "e_tracks", "zero_steps")
+                 "unused11", "kn_iterations", "photon_cutoffs", "e_tracks", "zero_steps",
+                 "sched_phases", "photon_iterations", "photon_lane_iterations", "charged_iterations", "charged_lane_iterations",
+                 "source_tasks", "idle_polls", "queue_claims", "particles_loaded", "particles_stored", "secondaries_spawned",
+                 "unused27", "unused28", "unused29", "unused30", "unused31")
 EXPORTS = ("aepid_workspace_bytes", "aepid_create", "aepid_destroy", "aepid_last_error", "aepid_init_materials",
            "aepid_load_phantom", "aepid_load_epid_layers", "aepid_load_source", "aepid_set_physics",
            "aepid_reset_tallies", "aepid_simulate", "aepid_read_tallies", "aepid_read_batches",
@@ -247,7 +250,7 @@ class Engine:
         self._chk(self._lib.aepid_set_counting(self._h, int(bool(on))))
 
     def read_counters(self):
-        c = np.zeros(16, dtype=np.uint64)
+        c = np.zeros(32, dtype=np.uint64)
         self._chk(self._lib.aepid_read_counters(self._h, _ptr(c)))
         return c
 

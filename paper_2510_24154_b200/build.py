@@ -17,7 +17,9 @@ LIB = os.path.join(HERE, "libaepid.so")
 SOURCES = ["transport.cu", "postpass.cu", "api.cu"]
 HEADERS = [os.path.join(CSRC, "params.h"), os.path.join(os.path.dirname(HERE), "include", "aepid.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "--use_fast_math=false"]
+              "-Xcompiler", "-fPIC"]
+# The transport kernel is bound by instruction fetch: approximate division / square root keep its SASS small.
+EXTRA_FLAGS = {"transport.cu": ["-prec-div=false", "-prec-sqrt=false", "-ftz=true"]}
 
 
 def nvcc():
@@ -38,14 +40,14 @@ def up_to_date():
 def build(force=False, verbose=False):
     if not force and up_to_date():
         return LIB
-    flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
     objs = []
     for s in SOURCES:
         o = os.path.join(CSRC, s.replace(".cu", ".o"))
-        cmd = [nvcc()] + flags + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, s), "-o", o]
+        cmd = ([nvcc()] + NVCC_FLAGS + EXTRA_FLAGS.get(s, []) + (["-Xptxas", "-v"] if verbose else [])
+               + ["-c", os.path.join(CSRC, s), "-o", o])
         subprocess.check_call(cmd)
         objs.append(o)
-    subprocess.check_call([nvcc(), "-shared", "-o", LIB] + objs + ["-lcudart_static", "-ldl", "-lrt", "-lpthread"])
+    subprocess.check_call([nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB] + objs + ["-lcudart_static", "-ldl", "-lrt", "-lpthread"])
     return LIB
 
 

@@ -56,7 +56,7 @@ Layout make_layout(const aepid_dims& d) {
     L.thrE = take(((size_t)d.n_bins + 1) * 4);
     L.edges = take(((size_t)d.n_bins + 1) * 4);
     L.thrF = take(((size_t)d.fu * d.fv + 1) * 4);
-    L.small = take(1024);            // ledger [8] f64 | counters [16] u64 | chunk counter | rho_max [32] f32
+    L.small = take(1024);            // ledger [8] f64 @0 | chunk counter @64 | rho_max [32] f32 @128 | counters [32] u64 @256
     L.total = o;
     return L;
 }
@@ -99,9 +99,9 @@ struct aepid_ctx {
     float* d_edges() { return reinterpret_cast<float*>(ws + lay.edges); }
     uint32_t* d_thrF() { return reinterpret_cast<uint32_t*>(ws + lay.thrF); }
     double* d_ledger() { return reinterpret_cast<double*>(ws + lay.small); }
-    unsigned long long* d_counters() { return reinterpret_cast<unsigned long long*>(ws + lay.small + 64); }
-    unsigned int* d_chunk() { return reinterpret_cast<unsigned int*>(ws + lay.small + 192); }
-    float* d_rho_max() { return reinterpret_cast<float*>(ws + lay.small + 256); }
+    unsigned long long* d_counters() { return reinterpret_cast<unsigned long long*>(ws + lay.small + 256); }
+    unsigned int* d_chunk() { return reinterpret_cast<unsigned int*>(ws + lay.small + 64); }
+    float* d_rho_max() { return reinterpret_cast<float*>(ws + lay.small + 128); }
 };
 
 namespace {
@@ -140,7 +140,8 @@ int reset_tallies(aepid_ctx* ctx) {
     const size_t B = ctx->dims.n_batches;
     CU(cudaMemsetAsync(ctx->d_ph_batch(), 0, ctx->lay.nvox * 4 * B, ctx->stream));
     CU(cudaMemsetAsync(ctx->d_ep_batch(), 0, ctx->lay.npix * 4 * B, ctx->stream));
-    CU(cudaMemsetAsync(ctx->ws + ctx->lay.small, 0, 256, ctx->stream));
+    CU(cudaMemsetAsync(ctx->ws + ctx->lay.small, 0, 128, ctx->stream));
+    CU(cudaMemsetAsync(ctx->ws + ctx->lay.small + 256, 0, 256, ctx->stream));
     ctx->n_done = 0; ctx->first_history = 0;
     std::fill(ctx->hist, ctx->hist + 256, 0.0);
     return 0;
@@ -223,12 +224,12 @@ int fill_params(aepid_ctx* ctx, TransportParams& p) {
     for (int l = 0; l < ctx->g.n_layers; ++l)
         if (ctx->g.lmat[l] >= ctx->n_mat) return fail(ctx, AEPID_ERR_BAD_ARG, "EPID layer material index out of range");
     if (ctx->tables_dirty) if (int rc = build_tables(ctx)) return rc;
-    if (transport_smem_bytes(ctx->tb) > 200 * 1024) return fail(ctx, AEPID_ERR_NOMEM, "material tables do not fit in shared memory");
+    if (transport_smem_bytes(ctx->tb) > 227 * 1024) return fail(ctx, AEPID_ERR_NOMEM, "material tables do not fit in shared memory");
     p.g = ctx->g; p.ph = ctx->ph; p.tb = ctx->tb; p.so = ctx->so;
     p.vox = ctx->d_vox(); p.ep_batch = ctx->d_ep_batch(); p.ph_batch = ctx->d_ph_batch();
-    p.ledger = ctx->d_ledger(); p.counters = ctx->d_counters(); p.chunk_counter = ctx->d_chunk();
+    p.ledger = ctx->d_ledger(); p.counters = ctx->d_counters(); p.hist_counter = ctx->d_chunk();
     p.n_batches = ctx->dims.n_batches; p.nvox = ctx->lay.nvox; p.npix = ctx->lay.npix;
-    p.base = 0; p.seed = 0; p.n = 0; p.n_chunks = 0;
+    p.base = 0; p.seed = 0; p.n = 0; p.hist_per_batch = 1;
     return 0;
 }
 
@@ -427,15 +428,13 @@ int aepid_simulate(aepid_ctx* ctx, unsigned long long n_histories, unsigned long
     while (left > 0) {
         const unsigned long long n = std::min<unsigned long long>(left, 1ull << 31);
         p.base = ctx->first_history + ctx->n_done; p.seed = seed; p.n = (uint32_t)n;
-        p.n_chunks = (uint32_t)((n + kChunk - 1) / kChunk);
+        const uint64_t hpb = (n + B - 1) / B;                  // history k of the launch -> batch k / hpb, exactly as in the kernel
+        p.hist_per_batch = (uint32_t)hpb;
         CU(cudaMemsetAsync(ctx->d_chunk(), 0, sizeof(unsigned int), ctx->stream));
         const int rc = launch_transport(p, ctx->counting, ctx->sm_count, ctx->stream);
         if (rc != 0) return fail(ctx, AEPID_ERR_CUDA, std::string("transport launch: ") + cudaGetErrorString((cudaError_t)rc));
-        // histories per batch: chunk c goes to batch floor(c B / n_chunks), exactly as in the kernel
         for (int b = 0; b < B; ++b) {
-            const uint64_t c0 = ((uint64_t)b * p.n_chunks + B - 1) / B, c1 = ((uint64_t)(b + 1) * p.n_chunks + B - 1) / B;
-            if (c1 <= c0) continue;
-            const uint64_t h0 = c0 * kChunk, h1 = std::min<uint64_t>(c1 * kChunk, n);
+            const uint64_t h0 = std::min<uint64_t>((uint64_t)b * hpb, n), h1 = std::min<uint64_t>((uint64_t)(b + 1) * hpb, n);
             ctx->hist[b] += (double)(h1 - h0);
         }
         ctx->n_done += n; left -= n;
@@ -514,9 +513,9 @@ int aepid_read_batches(aepid_ctx* ctx, float* epid_batches, double* histories_pe
     return 0;
 }
 
-int aepid_read_counters(aepid_ctx* ctx, unsigned long long counters[16]) {
+int aepid_read_counters(aepid_ctx* ctx, unsigned long long counters[32]) {
     if (!ctx || !ctx->ws || !counters) return AEPID_ERR_BAD_ARG;
-    CU(cudaMemcpyAsync(counters, ctx->d_counters(), 16 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaMemcpyAsync(counters, ctx->d_counters(), 32 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     return 0;
 }

@@ -8,7 +8,6 @@ namespace aepid {
 
 constexpr int kMaxLayers = 8;
 constexpr int kMaxMat = 32;
-constexpr int kChunk = 64;            // histories handed to a warp per grab of the global counter
 constexpr float kRhoAir = 1.205e-3f;  // world filler, material 0 (SURVEY 8(c) "Geometry")
 constexpr float kWorldHalf = 100.0f;  // |u|, |v| <= 100 cm
 constexpr float kWorldWMin = -1.0f;   // -1 <= w
@@ -67,12 +66,12 @@ struct TransportParams {
     float* ep_batch;                   // [B][nv*nu]
     float* ph_batch;                   // [B][nz*ny*nx]
     double* ledger;                    // [8]
-    unsigned long long* counters;      // [16]
-    unsigned int* chunk_counter;
+    unsigned long long* counters;      // [32]
+    unsigned int* hist_counter;        // next history of this launch that has not been started
     uint64_t base;                     // global index of relative history 0 of this launch
     uint64_t seed;
     uint32_t n;                        // histories in this launch (< 2^32)
-    uint32_t n_chunks;
+    uint32_t hist_per_batch;           // history k of the launch scores into batch min(k / hist_per_batch, B - 1)
     int n_batches;
     size_t nvox, npix;
 };

@@ -2,14 +2,35 @@
 // sampling, K5 CSDA electron steps with Highland deflection, K6 EPID slab transport and K7 tally
 // scoring (physics of SURVEY.md 8(c)).
 //
-// Design (sm_100a): one persistent grid, one particle per lane.  Every loop iteration a lane executes ONE
-// event of its particle (one photon flight or one electron step) so that lanes holding different particle
-// kinds share as much of the instruction stream as possible; a lane whose particle ends pops its private
-// secondary stack or takes the next history of the warp's chunk (chunks of 64 histories are handed out by
-// one global atomic, so the tail is balanced over the whole GPU).  Material tables live in shared memory in
-// the ln domain (one LDS.128 per node), the phantom is one packed 32-bit word per voxel gathered through
-// the read-only path (L2-resident up to ~30 M voxels), phantom deposits of consecutive steps in one voxel are
-// merged in registers and flushed with one RED, the energy ledger is kept in double.
+// Design (sm_100a): ONE persistent CTA per SM that is its own particle scheduler.
+//   * Shared memory holds the material tables (ln domain, one LDS.128 per node), a POOL of kPool particle
+//     records (SoA, 12 words) and, per event class, a ring queue of pool-slot indices, plus a ring of free slots.
+//     Classes: photon in phantom | photon in air/EPID | charged in phantom | charged in air/EPID.
+//   * Every warp runs the same scheduler loop on its own (no block-wide barrier in the steady state).  A warp
+//     works on one particle GROUP (photons or charged particles) at a time and keeps its lanes full: it runs the
+//     group's event loop; when enough lanes have run dry (particle absorbed, escaped or changed group) it writes
+//     those back (free the slot / store and queue the particle under its new class) and refills the empty lanes
+//     from the queue of its class IN PLACE, the other lanes keep their particles in registers.  A warp that runs
+//     out of work takes the class with the most waiting particles (full warps first) or, if no class can fill a
+//     warp, starts 32 new histories.  Warps therefore execute one code path with (nearly) all lanes active, and
+//     the secondaries of a history are followed concurrently by other warps instead of serially by their parent.
+//   * Secondaries go straight into the pool: the creating lane takes a free slot, stores the record and appends
+//     the slot to the queue of the secondary's class.
+//   * Queue protocol (bounded MPMC ring): pushers take tickets from tail[c] and write cell = slot | generation,
+//     then commit with avail[c] += n; poppers take n <= avail[c] committed entries, then tickets from head[c], and
+//     wait for the generation tag of their cells (the pusher holding that ticket is at most a few instructions
+//     away).  Ring capacity >= pool size, so a cell is never overwritten before it has been read.  Every wait is
+//     bounded; an exhausted bound or an exhausted pool raises the overflow flag ledger[7] (tests assert it is 0).
+//   * A particle's trajectory does not depend on the schedule: its Philox stream is keyed by (history, particle
+//     id, block) and every event consumes whole blocks (reading A1), so no draw is ever buffered across events and
+//     all lanes of a warp call Philox together.
+//   * The phantom is one packed 32-bit word per voxel gathered through the read-only path (L2-resident up to
+//     ~30 M voxels); phantom deposits of consecutive steps in one voxel are merged in registers and flushed with
+//     one RED; the energy ledger is summed per phase in float, reduced over the warp and accumulated per warp in
+//     double.
+//   * Instruction footprint matters more than anything else here (ncu: the first version of this kernel spent 78 %
+//     of its issue slots waiting for instruction fetch with 118 KB of SASS): Philox, the air navigation, the queue
+//     operations and the EPID scoring are out-of-line functions, divisions and square roots use the fast paths.
 // No tensor cores / TMA: random gathers and scalar arithmetic, nothing here is a dense contraction.
 #include <cuda_runtime.h>
 #include <cstdint>
@@ -17,50 +38,75 @@
 
 namespace aepid {
 
-constexpr int kBlock = 256;
-constexpr int kMinBlocks = 3;
-constexpr int kStackDepth = 4;
+constexpr int kWarps = 24;
+constexpr int kThreads = kWarps * 32;
+constexpr int kPoolLog = 11;
+constexpr int kPool = 1 << kPoolLog;          // particle slots per CTA; also the capacity of every ring
+constexpr int kWords = 12;                    // state words per particle
+constexpr int kRings = 5;                     // 4 classes + free slots
+constexpr int kFree = 4;
+constexpr int kSrcReserve = 384;              // free slots that must remain for secondaries before new histories start
+constexpr int kSrcMin = 8;                    // a photon warp starts new histories once this many lanes are empty
+constexpr int kKeep = 8;                      // fewer live lanes than this and a full warp of other work waiting: hand them back
+constexpr int kTransitMin = 8;                // photons in air make the transit together once this many are waiting
+constexpr int kSpinLimit = 1 << 22;
 constexpr float kPi = 3.14159265358979f;
 constexpr float kInf = 3.0e38f;
+constexpr uint32_t kNone = 0xffffffffu;
 
 #define FULL_MASK 0xffffffffu
-// flags: bits 0-1 type, 2-3 region, 4-6 layer, 8 two spare randoms buffered, 16-23 batch
+// flags: bits 0-1 type, 2-3 region, 4-6 layer, 16-23 batch
 #define F_TYPE(f) ((f) & 3u)
 #define F_REGION(f) (((f) >> 2) & 3u)
 #define F_LAYER(f) (((f) >> 4) & 7u)
 #define F_BATCH(f) (((f) >> 16) & 255u)
-#define F_HAS2 (1u << 8)
 #define SET_TYPE(f, t) ((f) = ((f) & ~3u) | (t))
 #define SET_REGION(f, r) ((f) = ((f) & ~(3u << 2)) | ((r) << 2))
 #define SET_LAYER(f, l) ((f) = ((f) & ~(7u << 4)) | ((uint32_t)(l) << 4))
+
+// event class of a particle (which queue it waits in, which warps work on it):
+// 0 photon in the phantom or in air, 1 photon inside the EPID, 2 charged in the phantom, 3 charged in air / EPID
+__device__ __forceinline__ int class_of(uint32_t flags) {
+    return F_TYPE(flags) == T_PHOTON ? (F_REGION(flags) == R_EPID ? 1 : 0) : (F_REGION(flags) == R_PHANTOM ? 2 : 3);
+}
+
+// Scheduler state and the geometry copy: static shared memory, so that the out-of-line helpers reach them
+// without arguments.
+__shared__ unsigned short s_ring[kRings * kPool];   // cell = slot | generation << kPoolLog
+__shared__ unsigned int s_tail[kRings];             // tickets handed to pushers
+__shared__ unsigned int s_head[kRings];             // tickets handed to poppers
+__shared__ int s_avail[kRings];                     // committed entries not yet claimed
+__shared__ int s_flag[2];                           // [0] no histories left, [1] error
+__shared__ Geom s_g;
+__shared__ float* s_ep_batch;
+__shared__ unsigned long long s_npix;
+extern __shared__ __align__(16) unsigned char smem_raw[];   // pool [kWords][kPool] u32 | per-warp ledger | table blob
+
+__device__ __forceinline__ uint32_t* pool_base() { return reinterpret_cast<uint32_t*>(smem_raw); }
 
 struct Shared {
     const float4* phot;
     const float* maj;
     const float* lnS;
     const float* invX0;
-    double* led;        // [8] block-level ledger
 };
-
-struct StackEntry { float x, y, z, dx, dy, dz, E; uint32_t flags, vox, pid, blk; };
 
 struct Lane {
     float x, y, z, dx, dy, dz, E;   // position: world (AIR, photon in PHANTOM), voxel fraction (charged in PHANTOM), beam (u, v, depth) in EPID
     uint32_t vox;                   // packed voxel index ix | iy << 10 | iz << 20
     uint32_t flags;
     uint32_t h, pid, blk;           // history (relative to the launch base), particle id, Philox block counter
-    uint32_t r2, r3;                // buffered raw draws
-    uint32_t cw;                    // packed word of the current voxel (charged particle in PHANTOM)
+    uint32_t cw, vlin;              // packed word and linear index of the current voxel (charged particle in PHANTOM)
     int ci; float ct, mumaj;        // photon: table cell, fraction, majorant at E
     uint32_t pidx; float pval;      // pending phantom deposit (merged while the voxel does not change)
-    double lph;                     // thread-local ledger: energy deposited in the phantom
-    int sp;
+    uint32_t slot;                  // pool slot of this particle (kNone: fresh from the source)
+    uint32_t spare;                 // a free pool slot kept by the lane for its next secondary (kNone: none)
+    float a_emit, a_ph, a_eps, a_epo, a_air, a_esc;   // ledger sums since the last flush
     bool alive;
 };
 
 // ---------------------------------------------------------------- Philox4x32-10 (own implementation; pinned on the GPU by tests)
-__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1,
-                                              uint32_t& o0, uint32_t& o1, uint32_t& o2, uint32_t& o3) {
+__device__ __noinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1) {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
         const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
@@ -69,23 +115,16 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
         c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
         k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
     }
-    o0 = c0; o1 = c1; o2 = c2; o3 = c3;
+    return make_uint4(c0, c1, c2, c3);
 }
 // uniform in (0,1) from the top 23 bits: ((r >> 9) + 0.5) 2^-23 is exact in float32 and never 0 or 1
 __device__ __forceinline__ float u01(uint32_t r) { return ((float)(r >> 9) + 0.5f) * 1.1920928955078125e-7f; }
 
-__device__ __forceinline__ void rng_block(Lane& L, const TransportParams& P, uint32_t& o0, uint32_t& o1, uint32_t& o2, uint32_t& o3) {
+__device__ __forceinline__ uint4 rng_block(Lane& L, const TransportParams& P) {
     const uint64_t h = P.base + L.h;
-    philox4x32_10((uint32_t)h, (uint32_t)(h >> 32), L.pid, L.blk, (uint32_t)P.seed, (uint32_t)(P.seed >> 32), o0, o1, o2, o3);
+    const uint4 o = philox4x32_10((uint32_t)h, (uint32_t)(h >> 32), L.pid, L.blk, (uint32_t)P.seed, (uint32_t)(P.seed >> 32));
     L.blk++;
-}
-__device__ __forceinline__ void rng_pair(Lane& L, const TransportParams& P, float& a, float& b) {
-    if (L.flags & F_HAS2) { a = u01(L.r2); b = u01(L.r3); L.flags &= ~F_HAS2; }
-    else {
-        uint32_t o0, o1;
-        rng_block(L, P, o0, o1, L.r2, L.r3);
-        a = u01(o0); b = u01(o1); L.flags |= F_HAS2;
-    }
+    return o;
 }
 __device__ __forceinline__ uint32_t child_id(const Lane& L, uint32_t sibling) {    // reading A1
     return L.pid * 0x9E3779B1u + L.blk * 2u + sibling + 1u;
@@ -134,7 +173,7 @@ __device__ __forceinline__ void dir_to_world(const Geom& g, float u, float v, fl
 // Rotate the unit vector d by polar (ct, st) and azimuth (cp, sp) using a branch-free orthonormal basis.
 __device__ __forceinline__ void rotate(float& dx, float& dy, float& dz, float ct, float st, float cp, float sp) {
     const float sg = copysignf(1.0f, dz);
-    const float a = -1.0f / (sg + dz), b = dx * dy * a;
+    const float a = -__frcp_rn(sg + dz), b = dx * dy * a;
     const float b1x = 1.0f + sg * dx * dx * a, b1y = sg * b, b1z = -sg * dx;
     const float b2x = b, b2y = sg + dy * dy * a, b2z = -dy;
     const float sc = st * cp, ss = st * sp;
@@ -158,48 +197,51 @@ __device__ __forceinline__ uint32_t vox_linear(const Geom& g, uint32_t v) {
 __device__ __forceinline__ void dep_vox(Lane& L, const TransportParams& P, uint32_t idx, float e) {
     if (idx != L.pidx) { flush_pending(L, P); L.pidx = idx; }
     L.pval += e;
-    L.lph += (double)e;
+    L.a_ph += e;
 }
-__device__ __forceinline__ void dep_epid(Lane& L, const TransportParams& P, const Shared& sh, int layer, float u, float v, float e) {
-    if (P.g.lscored[layer]) {
-        const float fu = floorf((u + P.g.half_u) * P.g.inv_pitch), fv = floorf((v + P.g.half_v) * P.g.inv_pitch);
-        if (fu >= 0.0f && fu < (float)P.g.nu && fv >= 0.0f && fv < (float)P.g.nv) {
-            atomicAdd(P.ep_batch + (size_t)F_BATCH(L.flags) * P.npix + (size_t)fv * P.g.nu + (size_t)fu, e);
-            atomicAdd(&sh.led[2], (double)e);
-            return;
-        }
-    }
-    atomicAdd(&sh.led[3], (double)e);
+// Energy e deposited at (u, v) of an EPID layer: scores the pixel and returns true if the layer is scored and
+// (u, v) lies inside the image (SURVEY 8(c) "Geometry").
+__device__ __noinline__ bool score_epid(uint32_t flags, float u, float v, float e) {
+    if (!s_g.lscored[F_LAYER(flags)]) return false;
+    const float fu = floorf((u + s_g.half_u) * s_g.inv_pitch), fv = floorf((v + s_g.half_v) * s_g.inv_pitch);
+    if (!(fu >= 0.0f && fu < (float)s_g.nu && fv >= 0.0f && fv < (float)s_g.nv)) return false;
+    atomicAdd(s_ep_batch + (size_t)F_BATCH(flags) * s_npix + (size_t)fv * s_g.nu + (size_t)fu, e);
+    return true;
+}
+__device__ __forceinline__ void dep_epid(Lane& L, float u, float v, float e) {
+    if (score_epid(L.flags, u, v, e)) L.a_eps += e; else L.a_epo += e;
 }
 // deposit at the particle's position
-__device__ __forceinline__ void dep_here(Lane& L, const TransportParams& P, const Shared& sh, float e) {
+__device__ __forceinline__ void dep_here(Lane& L, const TransportParams& P, float e) {
     const uint32_t reg = F_REGION(L.flags);
     if (reg == R_PHANTOM) dep_vox(L, P, vox_linear(P.g, L.vox), e);
-    else if (reg == R_AIR) atomicAdd(&sh.led[4], (double)e);
-    else dep_epid(L, P, sh, F_LAYER(L.flags), L.x, L.y, e);
+    else if (reg == R_AIR) L.a_air += e;
+    else dep_epid(L, L.x, L.y, e);
 }
 
 // ---------------------------------------------------------------- geometry
 // Nearest boundary seen from AIR: kind 0 phantom AABB entry, 1 EPID top plane, 2 world exit.
-__device__ __forceinline__ float air_boundary(const Geom& g, const Lane& L, int& kind, int& axis) {
+struct AirHit { float t; int code; };      // code = kind | axis << 2
+__device__ __noinline__ AirHit air_boundary(float x, float y, float z, float dx, float dy, float dz) {
+    const Geom& g = s_g;
     float tn = -kInf, tf = kInf; int ax = 0; bool miss = false;
 #define SLAB(P_, D_, LO_, HI_, A_)                                            \
     if (fabsf(D_) > 1e-20f) {                                                  \
-        const float inv = 1.0f / (D_);                                         \
+        const float inv = __frcp_rn(D_);                                       \
         float t1 = ((LO_) - (P_)) * inv, t2 = ((HI_) - (P_)) * inv;           \
         if (t1 > t2) { const float t = t1; t1 = t2; t2 = t; }                  \
         if (t1 > tn) { tn = t1; ax = A_; }                                     \
         tf = fminf(tf, t2);                                                    \
     } else if ((P_) < (LO_) || (P_) >= (HI_)) miss = true;
-    SLAB(L.x, L.dx, g.lox, g.hix, 0)
-    SLAB(L.y, L.dy, g.loy, g.hiy, 1)
-    SLAB(L.z, L.dz, g.loz, g.hiz, 2)
+    SLAB(x, dx, g.lox, g.hix, 0)
+    SLAB(y, dy, g.loy, g.hiy, 1)
+    SLAB(z, dz, g.loz, g.hiz, 2)
 #undef SLAB
     float tb = (miss || !(tf > 0.0f) || tn >= tf) ? kInf : fmaxf(tn, 0.0f);
-    kind = 0; axis = ax;
+    int kind = 0;
     float pu, pv, pw, du, dv, dw;
-    to_beam(g, L.x, L.y, L.z, pu, pv, pw);
-    dir_to_beam(g, L.dx, L.dy, L.dz, du, dv, dw);
+    to_beam(g, x, y, z, pu, pv, pw);
+    dir_to_beam(g, dx, dy, dz, du, dv, dw);
     if (dw > 0.0f) { const float te = fmaxf((g.sid - pw) / dw, 0.0f); if (te < tb) { tb = te; kind = 1; } }
     float tw = kInf;
     if (du > 0.0f) tw = fminf(tw, (kWorldHalf - pu) / du); else if (du < 0.0f) tw = fminf(tw, (-kWorldHalf - pu) / du);
@@ -207,7 +249,8 @@ __device__ __forceinline__ float air_boundary(const Geom& g, const Lane& L, int&
     if (dw < 0.0f) tw = fminf(tw, (kWorldWMin - pw) / dw);
     tw = fmaxf(tw, 0.0f);
     if (tw < tb) { tb = tw; kind = 2; }
-    return tb;
+    AirHit r; r.t = tb; r.code = kind | (ax << 2);
+    return r;
 }
 __device__ __forceinline__ float lateral_exit(float u, float v, float du, float dv) {
     float t = kInf;
@@ -232,7 +275,8 @@ __device__ __forceinline__ void enter_phantom(Lane& L, const TransportParams& P,
         else { iz = pos_dir ? 0 : g.nz - 1; fz = pos_dir ? 0.0f : 1.0f; }
         L.x = fx; L.y = fy; L.z = fz;
         L.vox = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20);
-        L.cw = __ldg(P.vox + vox_linear(g, L.vox));
+        L.vlin = vox_linear(g, L.vox);
+        L.cw = __ldg(P.vox + L.vlin);
     }
 }
 __device__ __forceinline__ void enter_epid(Lane& L, const Geom& g) {       // position already on the top plane
@@ -257,222 +301,386 @@ __device__ __forceinline__ void frac_to_world(Lane& L, const Geom& g) {
     L.y = fmaf(((float)((L.vox >> 10) & 1023u) + L.y), g.hy, g.loy);
     L.z = fmaf(((float)((L.vox >> 20) & 1023u) + L.z), g.hz, g.loz);
 }
-
-// ---------------------------------------------------------------- stack
-__device__ __forceinline__ void push(Lane& L, StackEntry* stk, float x, float y, float z, float dx, float dy, float dz, float E,
-                                     uint32_t flags, uint32_t vox, uint32_t pid, uint32_t blk, const Shared& sh) {
-    if (L.sp >= kStackDepth) { atomicAdd(&sh.led[7], 1.0); atomicAdd(&sh.led[5], (double)E); return; }   // cannot happen (depth <= 2); flagged
-    StackEntry& s = stk[L.sp++];
-    s.x = x; s.y = y; s.z = z; s.dx = dx; s.dy = dy; s.dz = dz; s.E = E; s.flags = flags & ~F_HAS2; s.vox = vox; s.pid = pid; s.blk = blk;
+// photon (world position in PHANTOM) -> charged particle representation
+__device__ __forceinline__ void world_to_frac(const Geom& g, uint32_t vox, float& x, float& y, float& z) {
+    const float gx = (x - g.lox) * g.ihx - (float)(vox & 1023u);
+    const float gy = (y - g.loy) * g.ihy - (float)((vox >> 10) & 1023u);
+    const float gz = (z - g.loz) * g.ihz - (float)((vox >> 20) & 1023u);
+    x = fminf(fmaxf(gx, 0.0f), 1.0f); y = fminf(fmaxf(gy, 0.0f), 1.0f); z = fminf(fmaxf(gz, 0.0f), 1.0f);
 }
 
-// Two 0.511 MeV photons, isotropic and back to back (reading A11): the lane becomes the first, the second is pushed.
+// ---------------------------------------------------------------- queues (protocol in the header comment)
+// error bits (summed over CTAs into ledger[7]): 1 queue wait timed out, 2 no slot for a secondary, 4 particle without a slot,
+// 8 idle bound ran out
+__device__ __forceinline__ void raise_error(int bit) { atomicOr(s_flag + 1, bit); }
+
+// wait for the cell of ticket t in ring r; returns the slot (kNone if the bound ran out)
+__device__ __noinline__ uint32_t ring_take(int r, uint32_t t) {
+    const uint32_t idx = t & (kPool - 1), gen = (t >> kPoolLog) & 31u;
+    volatile unsigned short* cell = s_ring + r * kPool + idx;
+#pragma unroll 1
+    for (int spin = 0; spin < kSpinLimit; ++spin) {
+        const uint32_t v = *cell;
+        if ((v >> kPoolLog) == gen) return v & (kPool - 1);
+    }
+    raise_error(1);
+    return kNone;
+}
+// one lane appends one slot to ring r (divergent code)
+__device__ __noinline__ void ring_push_one(int r, uint32_t slot) {
+    const uint32_t t = atomicAdd(s_tail + r, 1u);
+    const uint32_t idx = t & (kPool - 1), gen = (t >> kPoolLog) & 31u;
+    *((volatile unsigned short*)(s_ring + r * kPool + idx)) = (unsigned short)(slot | (gen << kPoolLog));
+    __threadfence_block();
+    atomicAdd(s_avail + r, 1);
+}
+// one lane takes one entry of ring r, if there is a committed one (divergent code)
+__device__ __noinline__ uint32_t ring_pop_one(int r) {
+    if (*((volatile int*)(s_avail + r)) <= 0) return kNone;
+    if (atomicSub(s_avail + r, 1) <= 0) { atomicAdd(s_avail + r, 1); return kNone; }
+    return ring_take(r, atomicAdd(s_head + r, 1u));
+}
+
+// lane 0 claims up to `want` committed entries of ring r; returns count | first ticket << 32 (warp-uniform, all lanes call)
+__device__ __noinline__ unsigned long long ring_claim_packed(int r, int want) {
+    int n = 0; uint32_t t = 0;
+    if ((threadIdx.x & 31u) == 0) {
+        int a = *((volatile int*)(s_avail + r));
+#pragma unroll 1
+        while (a > 0) {
+            n = min(a, want);
+            const int old = atomicCAS(s_avail + r, a, a - n);
+            if (old == a) break;
+            a = old; n = 0;
+        }
+        if (a <= 0) n = 0;
+        if (n > 0) t = atomicAdd(s_head + r, (unsigned)n);
+    }
+    n = __shfl_sync(FULL_MASK, n, 0);
+    t = __shfl_sync(FULL_MASK, t, 0);
+    return (unsigned long long)(uint32_t)n | ((unsigned long long)t << 32);
+}
+
+// Store a particle record in pool slot `slot` and append the slot to the queue of the particle's class.
+__device__ __noinline__ void queue_particle(uint32_t slot, float x, float y, float z, float dx, float dy, float dz, float E,
+                                            uint32_t vox, uint32_t flags, uint32_t h, uint32_t pid, uint32_t blk) {
+    uint32_t* p = pool_base() + slot;
+    p[0 * kPool] = __float_as_uint(x);  p[1 * kPool] = __float_as_uint(y);  p[2 * kPool] = __float_as_uint(z);
+    p[3 * kPool] = __float_as_uint(dx); p[4 * kPool] = __float_as_uint(dy); p[5 * kPool] = __float_as_uint(dz);
+    p[6 * kPool] = __float_as_uint(E);  p[7 * kPool] = vox; p[8 * kPool] = flags;
+    p[9 * kPool] = h; p[10 * kPool] = pid; p[11 * kPool] = blk;
+    __threadfence_block();
+    ring_push_one(class_of(flags), slot);
+}
+// Slot discipline: every particle owns a pool slot from birth, so handing it over never needs a new one; a lane
+// keeps at most one SPARE free slot (the slot of a particle that died in it, else one from the free ring) and only
+// runs an event that can create a secondary while it holds one.  Hence the pool cannot overflow: when the free ring
+// runs dry the photon lanes wait, the charged-particle warps drain the queues and slots come back.
+__device__ __forceinline__ bool ensure_spare(Lane& L) {
+    if (L.spare == kNone) L.spare = ring_pop_one(kFree);
+    return L.spare != kNone;
+}
+// A secondary goes straight into the pool (the lane's spare slot) and into the queue of its class.  Without a spare
+// (cannot happen: see ensure_spare; flagged) its energy is booked as escaped so that the ledger still closes.
+__device__ __forceinline__ void spawn_from(Lane& L, float x, float y, float z, float dx, float dy, float dz, float E,
+                                           uint32_t flags, uint32_t pid) {
+    const uint32_t s = L.spare; L.spare = kNone;
+    if (s == kNone) { raise_error(2); L.a_esc += E + (F_TYPE(flags) == T_POSITRON ? 2.0f * kMec2 : 0.0f); return; }
+    queue_particle(s, x, y, z, dx, dy, dz, E, L.vox, flags, L.h, pid, 0u);
+}
+
+// Two 0.511 MeV photons, isotropic and back to back (reading A11): the lane becomes the first, the second is spawned.
 // Position must already be in the frame photons use in this region.
-__device__ __forceinline__ void annihilate(Lane& L, const TransportParams& P, const Shared& sh, StackEntry* stk) {
-    float a, b; rng_pair(L, P, a, b);
-    const float ct = 2.0f * a - 1.0f, st = sqrtf(fmaxf(0.0f, 1.0f - ct * ct));
-    float sp, cp; __sincosf(2.0f * kPi * b - kPi, &sp, &cp);
+__device__ __forceinline__ void annihilate(Lane& L, const TransportParams& P) {
+    const uint4 r = rng_block(L, P);
+    const float ct = 2.0f * u01(r.x) - 1.0f, st = sqrtf(fmaxf(0.0f, 1.0f - ct * ct));
+    float sp, cp; __sincosf(2.0f * kPi * u01(r.y) - kPi, &sp, &cp);
     const float dx = st * cp, dy = st * sp, dz = ct;
     uint32_t f = L.flags; SET_TYPE(f, T_PHOTON);
-    push(L, stk, L.x, L.y, L.z, -dx, -dy, -dz, kMec2, f, L.vox, child_id(L, 1), 0u, sh);
+    spawn_from(L, L.x, L.y, L.z, -dx, -dy, -dz, kMec2, f, child_id(L, 1));
     L.pid = child_id(L, 0); L.blk = 0;
-    L.flags = f & ~F_HAS2;
+    L.flags = f;
     L.dx = dx; L.dy = dy; L.dz = dz; L.E = kMec2;
-    set_energy(L, P, sh);
-}
-
-// photon (world position in PHANTOM) -> charged particle representation
-__device__ __forceinline__ void world_to_frac(Lane& L, const Geom& g) {
-    const float gx = (L.x - g.lox) * g.ihx - (float)(L.vox & 1023u);
-    const float gy = (L.y - g.loy) * g.ihy - (float)((L.vox >> 10) & 1023u);
-    const float gz = (L.z - g.loz) * g.ihz - (float)((L.vox >> 20) & 1023u);
-    L.x = fminf(fmaxf(gx, 0.0f), 1.0f); L.y = fminf(fmaxf(gy, 0.0f), 1.0f); L.z = fminf(fmaxf(gz, 0.0f), 1.0f);
 }
 
 // ---------------------------------------------------------------- K4 interaction
 template <bool COUNT>
-__device__ __forceinline__ void interact(Lane& L, const TransportParams& P, const Shared& sh, StackEntry* stk,
-                                         float xsel, float pe, float co, uint32_t* cnt) {
+__device__ __forceinline__ void interact(Lane& L, const TransportParams& P, const Shared& sh, float xsel, float pe, float co, uint32_t* cnt) {
     const bool coupled = P.ph.mode != 0;
     const uint32_t reg = F_REGION(L.flags);
     if (xsel < pe) {                                                       // photoelectric: electron T = E along d
         if (COUNT) cnt[3]++;
-        if (!coupled || L.E <= P.ph.ecut) { dep_here(L, P, sh, L.E); L.alive = false; return; }
+        if (!coupled || L.E <= P.ph.ecut) { dep_here(L, P, L.E); L.alive = false; return; }
         SET_TYPE(L.flags, T_ELECTRON);
-        L.pid = child_id(L, 0); L.blk = 0; L.flags &= ~F_HAS2;
+        L.pid = child_id(L, 0); L.blk = 0;
         if (COUNT) { cnt[9]++; cnt[14]++; }
-        if (reg == R_PHANTOM) world_to_frac(L, P.g);
+        if (reg == R_PHANTOM) { world_to_frac(P.g, L.vox, L.x, L.y, L.z); }
         return;
     }
     if (xsel < pe + co) {                                                  // Compton: Klein-Nishina by epsilon-mixture rejection
         if (COUNT) cnt[4]++;
-        const float k = L.E * (1.0f / kMec2), e0 = 1.0f / (1.0f + 2.0f * k), e02 = e0 * e0;
+        const float k = L.E * (1.0f / kMec2), e0 = __frcp_rn(1.0f + 2.0f * k), e02 = e0 * e0;
         const float a1 = -__logf(e0), a2 = 0.5f * (1.0f - e02);
         float eps, t, x4;
+#pragma unroll 1
         for (;;) {
-            float x1, x2, x3;
-            rng_pair(L, P, x1, x2); rng_pair(L, P, x3, x4);
+            const uint4 r = rng_block(L, P);                               // one block per trial
+            const float x1 = u01(r.x), x2 = u01(r.y), x3 = u01(r.z); x4 = u01(r.w);
             if (COUNT) cnt[12]++;
             eps = (x1 * (a1 + a2) < a1) ? __expf(-x2 * a1) : sqrtf(fmaf(1.0f - e02, x2, e02));
-            t = (1.0f - eps) / (k * eps);
-            const float g = 1.0f - eps * t * (2.0f - t) / (1.0f + eps * eps);
+            t = __fdividef(1.0f - eps, k * eps);
+            const float g = 1.0f - __fdividef(eps * t * (2.0f - t), 1.0f + eps * eps);
             if (g >= x3) break;
         }
         const float ct = 1.0f - t, st = sqrtf(fmaxf(0.0f, t * (2.0f - t)));
         float sp, cp; __sincosf(2.0f * kPi * x4 - kPi, &sp, &cp);
-        const float E1 = eps * L.E, T = L.E - E1;
+        const float E0 = L.E, E1 = eps * E0, T = E0 - E1;
         float d1x = L.dx, d1y = L.dy, d1z = L.dz;
         rotate(d1x, d1y, d1z, ct, st, cp, sp);
-        if (!coupled || T <= P.ph.ecut) {                                  // kerma, or electron born below its cutoff: local deposit
-            dep_here(L, P, sh, T);
+        if (coupled && T > P.ph.ecut) {
+            // electron from momentum conservation: spawned into the pool with its own stream (reading A1)
+            float ex = E0 * L.dx - E1 * d1x, ey = E0 * L.dy - E1 * d1y, ez = E0 * L.dz - E1 * d1z;
+            const float inv = rsqrtf(ex * ex + ey * ey + ez * ez);
+            float px = L.x, py = L.y, pz = L.z;
+            if (reg == R_PHANTOM) world_to_frac(P.g, L.vox, px, py, pz);
+            uint32_t f = L.flags; SET_TYPE(f, T_ELECTRON);
+            if (COUNT) { cnt[9]++; cnt[14]++; }
+            spawn_from(L, px, py, pz, ex * inv, ey * inv, ez * inv, T, f, child_id(L, 0));
+        } else {                                                           // kerma, or electron born below its cutoff: local deposit
+            dep_here(L, P, T);
             if (COUNT && coupled) { cnt[9]++; cnt[14]++; }
-            L.E = E1; L.dx = d1x; L.dy = d1y; L.dz = d1z;
-            set_energy(L, P, sh);
-            return;
         }
-        // electron from momentum conservation; the scattered photon waits on the stack
-        float ex = L.E * L.dx - E1 * d1x, ey = L.E * L.dy - E1 * d1y, ez = L.E * L.dz - E1 * d1z;
-        const float inv = rsqrtf(ex * ex + ey * ey + ez * ez);
-        const uint32_t epid = child_id(L, 0);
-        if (E1 < P.ph.pcut) dep_here(L, P, sh, E1);
-        else {
-            // the scattered photon keeps its own stream (same particle id, block counter carried on the stack)
-            push(L, stk, L.x, L.y, L.z, d1x, d1y, d1z, E1, L.flags, L.vox, L.pid, L.blk, sh);
-        }
-        SET_TYPE(L.flags, T_ELECTRON);
-        L.pid = epid; L.blk = 0; L.flags &= ~F_HAS2;
-        L.E = T; L.dx = ex * inv; L.dy = ey * inv; L.dz = ez * inv;
-        if (COUNT) { cnt[9]++; cnt[14]++; }
-        if (reg == R_PHANTOM) world_to_frac(L, P.g);
+        // the scattered photon keeps its own stream
+        L.E = E1; L.dx = d1x; L.dy = d1y; L.dz = d1z;
+        if (E1 < P.ph.pcut) { if (COUNT) cnt[13]++; dep_here(L, P, E1); L.alive = false; return; }
+        set_energy(L, P, sh);
         return;
     }
     // pair production: uniform kinetic split, both along d (reading A10)
     if (COUNT) cnt[5]++;
-    float a, b; rng_pair(L, P, a, b);
+    const float a = u01(rng_block(L, P).x);
     const float Ttot = L.E - 2.0f * kMec2;
     const float Tm = a * Ttot, Tp = Ttot - Tm;
     if (!coupled) {
-        dep_here(L, P, sh, Ttot);
+        dep_here(L, P, Ttot);
         if (COUNT) cnt[9] += 2;
-        annihilate(L, P, sh, stk);                                         // 2 m_e c^2 re-emitted at the interaction point (A11)
+        annihilate(L, P);                                                  // 2 m_e c^2 re-emitted at the interaction point (A11)
+        set_energy(L, P, sh);
         return;
     }
     if (COUNT) { cnt[9] += 2; cnt[14] += 2; }
     uint32_t fpos = L.flags; SET_TYPE(fpos, T_POSITRON);
     const uint32_t id0 = child_id(L, 0), id1 = child_id(L, 1);
-    if (reg == R_PHANTOM) world_to_frac(L, P.g);
-    push(L, stk, L.x, L.y, L.z, L.dx, L.dy, L.dz, Tp, fpos, L.vox, id1, 0u, sh);
+    if (reg == R_PHANTOM) world_to_frac(P.g, L.vox, L.x, L.y, L.z);
+    spawn_from(L, L.x, L.y, L.z, L.dx, L.dy, L.dz, Tp, fpos, id1);
     SET_TYPE(L.flags, T_ELECTRON);
-    L.pid = id0; L.blk = 0; L.flags &= ~F_HAS2;
+    L.pid = id0; L.blk = 0;
     L.E = Tm;
 }
 
-// ---------------------------------------------------------------- photon event: one flight (K2, K3, K6) + interaction (K4)
+// ---------------------------------------------------------------- photon flights.  Each returns true with (xsel, pe, co)
+// set if the photon collides at its new position (K4 follows).
+// K3: one Woodcock flight in the phantom against the majorant.
 template <bool COUNT>
-__device__ __forceinline__ void photon_event(Lane& L, const TransportParams& P, const Shared& sh, StackEntry* stk, uint32_t* cnt) {
+__device__ __forceinline__ bool woodcock_flight(Lane& L, const TransportParams& P, const Shared& sh, float& xsel, float& pe, float& co, uint32_t* cnt) {
     const Geom& g = P.g;
-    if (L.E < P.ph.pcut) { if (COUNT) cnt[13]++; dep_here(L, P, sh, L.E); L.alive = false; return; }   // PAPER.md:104, 10 keV
-    float u1, u2; rng_pair(L, P, u1, u2);
-    const float nl = -__logf(u1);
-    const uint32_t reg = F_REGION(L.flags);
-    float pe, co, pp, xsel = 0.0f; bool hit = false;
-    if (reg == R_PHANTOM) {                                                // Woodcock flight against the majorant
-        if (COUNT) cnt[0]++;
-        const float s = __fdividef(nl, L.mumaj);
-        const float nx = fmaf(s, L.dx, L.x), ny = fmaf(s, L.dy, L.y), nz = fmaf(s, L.dz, L.z);
-        if (!(nx >= g.lox && nx < g.hix && ny >= g.loy && ny < g.hiy && nz >= g.loz && nz < g.hiz)) {
-            // left the grid: place on the AABB exit point, snapped onto the crossed face
-            float tx = kInf, ty = kInf, tz = kInf;
-            if (L.dx > 0.0f) tx = (g.hix - L.x) / L.dx; else if (L.dx < 0.0f) tx = (g.lox - L.x) / L.dx;
-            if (L.dy > 0.0f) ty = (g.hiy - L.y) / L.dy; else if (L.dy < 0.0f) ty = (g.loy - L.y) / L.dy;
-            if (L.dz > 0.0f) tz = (g.hiz - L.z) / L.dz; else if (L.dz < 0.0f) tz = (g.loz - L.z) / L.dz;
-            const float t = fmaxf(fminf(tx, fminf(ty, tz)), 0.0f);
-            L.x = fmaf(t, L.dx, L.x); L.y = fmaf(t, L.dy, L.y); L.z = fmaf(t, L.dz, L.z);
-            if (tx <= ty && tx <= tz) L.x = L.dx > 0.0f ? g.hix : g.lox;
-            else if (ty <= tz) L.y = L.dy > 0.0f ? g.hiy : g.loy;
-            else L.z = L.dz > 0.0f ? g.hiz : g.loz;
-            SET_REGION(L.flags, R_AIR);
-            return;
-        }
-        L.x = nx; L.y = ny; L.z = nz;
-        const int ix = min((int)((nx - g.lox) * g.ihx), g.nx - 1), iy = min((int)((ny - g.loy) * g.ihy), g.ny - 1), iz = min((int)((nz - g.loz) * g.ihz), g.nz - 1);
-        const uint32_t w = __ldg(P.vox + ((size_t)iz * g.ny + iy) * g.nx + ix);
-        const float rho = __uint_as_float(w & ~31u);
-        mu3(P, sh, (int)(w & 31u), L.ci, L.ct, pe, co, pp);
-        xsel = u2 * L.mumaj;
-        if (xsel < rho * (pe + co + pp)) {
-            hit = true; xsel = __fdividef(xsel, rho);                      // reuse the accept draw for the channel (reading A8)
-            L.cw = w; L.vox = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20);
-        }
-    } else if (reg == R_AIR) {
-        if (COUNT) cnt[1]++;
-        int kind, axis;
-        const float tb = air_boundary(g, L, kind, axis);
-        mu3(P, sh, 0, L.ci, L.ct, pe, co, pp);
-        const float mt = pe + co + pp;
-        const float s = nl / (kRhoAir * mt);
-        if (s < tb) { L.x = fmaf(s, L.dx, L.x); L.y = fmaf(s, L.dy, L.y); L.z = fmaf(s, L.dz, L.z); hit = true; xsel = u2 * mt; }
-        else {
-            L.x = fmaf(tb, L.dx, L.x); L.y = fmaf(tb, L.dy, L.y); L.z = fmaf(tb, L.dz, L.z);
-            if (kind == 0) enter_phantom(L, P, axis);
-            else if (kind == 1) enter_epid(L, g);
-            else { atomicAdd(&sh.led[5], (double)L.E); L.alive = false; }
-            return;
-        }
-    } else {                                                               // EPID: surface tracking layer by layer
-        if (COUNT) cnt[2]++;
-        const int l = F_LAYER(L.flags);
-        mu3(P, sh, g.lmat[l], L.ci, L.ct, pe, co, pp);
-        const float mt = pe + co + pp;
-        const float s = nl / (g.lrho[l] * mt);
-        float tf = kInf;
-        if (L.dz > 0.0f) tf = (g.zt[l + 1] - L.z) / L.dz; else if (L.dz < 0.0f) tf = (g.zt[l] - L.z) / L.dz;
-        tf = fmaxf(tf, 0.0f);
-        const float tl = lateral_exit(L.x, L.y, L.dx, L.dy);
-        if (s < tf && s < tl) { L.x = fmaf(s, L.dx, L.x); L.y = fmaf(s, L.dy, L.y); L.z = fmaf(s, L.dz, L.z); hit = true; xsel = u2 * mt; }
-        else if (tl < tf) { atomicAdd(&sh.led[5], (double)L.E); L.alive = false; return; }
-        else {
-            L.x = fmaf(tf, L.dx, L.x); L.y = fmaf(tf, L.dy, L.y);
-            if (L.dz > 0.0f) {
-                L.z = g.zt[l + 1];
-                if (l + 1 >= g.n_layers) { atomicAdd(&sh.led[5], (double)L.E); L.alive = false; }
-                else SET_LAYER(L.flags, l + 1);
-            } else {
-                L.z = g.zt[l];
-                if (l == 0) epid_to_air(L, g); else SET_LAYER(L.flags, l - 1);
-            }
-            return;
-        }
+    const uint4 rr = rng_block(L, P);
+    const float u1 = u01(rr.x), u2 = u01(rr.y);
+    if (COUNT) cnt[0]++;
+    const float s = __fdividef(-__logf(u1), L.mumaj);
+    const float nx = fmaf(s, L.dx, L.x), ny = fmaf(s, L.dy, L.y), nz = fmaf(s, L.dz, L.z);
+    if (!(nx >= g.lox && nx < g.hix && ny >= g.loy && ny < g.hiy && nz >= g.loz && nz < g.hiz)) {
+        // left the grid: place on the AABB exit point, snapped onto the crossed face
+        float tx = kInf, ty = kInf, tz = kInf;
+        if (L.dx > 0.0f) tx = (g.hix - L.x) / L.dx; else if (L.dx < 0.0f) tx = (g.lox - L.x) / L.dx;
+        if (L.dy > 0.0f) ty = (g.hiy - L.y) / L.dy; else if (L.dy < 0.0f) ty = (g.loy - L.y) / L.dy;
+        if (L.dz > 0.0f) tz = (g.hiz - L.z) / L.dz; else if (L.dz < 0.0f) tz = (g.loz - L.z) / L.dz;
+        const float t = fmaxf(fminf(tx, fminf(ty, tz)), 0.0f);
+        L.x = fmaf(t, L.dx, L.x); L.y = fmaf(t, L.dy, L.y); L.z = fmaf(t, L.dz, L.z);
+        if (tx <= ty && tx <= tz) L.x = L.dx > 0.0f ? g.hix : g.lox;
+        else if (ty <= tz) L.y = L.dy > 0.0f ? g.hiy : g.loy;
+        else L.z = L.dz > 0.0f ? g.hiz : g.loz;
+        SET_REGION(L.flags, R_AIR);
+        return false;
     }
-    if (hit) interact<COUNT>(L, P, sh, stk, xsel, pe, co, cnt);
+    L.x = nx; L.y = ny; L.z = nz;
+    const int ix = min((int)((nx - g.lox) * g.ihx), g.nx - 1), iy = min((int)((ny - g.loy) * g.ihy), g.ny - 1), iz = min((int)((nz - g.loz) * g.ihz), g.nz - 1);
+    const uint32_t w = __ldg(P.vox + ((size_t)iz * g.ny + iy) * g.nx + ix);
+    const float rho = __uint_as_float(w & ~31u);
+    float pp;
+    mu3(P, sh, (int)(w & 31u), L.ci, L.ct, pe, co, pp);
+    xsel = u2 * L.mumaj;
+    if (xsel < rho * (pe + co + pp)) {
+        xsel = __fdividef(xsel, rho);                                      // reuse the accept draw for the channel (reading A8)
+        L.cw = w; L.vox = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20);
+        return true;
+    }
+    return false;
+}
+// K2 + K6: a photon in AIR flies to wherever it goes.  One exponential optical depth is spent along the straight
+// path through the air and - if the path crosses the whole EPID stack inside the world box - through the layers (a
+// sequence of exponential flights that stop at boundaries is one exponential flight in optical depth).  Outcomes:
+// collision in air or in a layer (true), phantom entry, EPID entry (the rare path that leaves the stack sideways:
+// left to the layer-by-layer code), escape.
+template <bool COUNT>
+__device__ __forceinline__ bool air_transit(Lane& L, const TransportParams& P, const Shared& sh, float& xsel, float& pe, float& co, uint32_t* cnt) {
+    const Geom& g = P.g;
+    if (COUNT) cnt[1]++;
+    const AirHit ah = air_boundary(L.x, L.y, L.z, L.dx, L.dy, L.dz);
+    const uint4 rr = rng_block(L, P);
+    const float u1 = u01(rr.x), u2 = u01(rr.y);
+    float nl = -__logf(u1);
+    float pp;
+    mu3(P, sh, 0, L.ci, L.ct, pe, co, pp);
+    float mt = pe + co + pp;
+    const float mua = kRhoAir * mt;
+    if (nl < mua * ah.t) {                                                 // collision in air
+        const float s = __fdividef(nl, mua);
+        L.x = fmaf(s, L.dx, L.x); L.y = fmaf(s, L.dy, L.y); L.z = fmaf(s, L.dz, L.z);
+        xsel = u2 * mt;
+        return true;
+    }
+    L.x = fmaf(ah.t, L.dx, L.x); L.y = fmaf(ah.t, L.dy, L.y); L.z = fmaf(ah.t, L.dz, L.z);
+    const int kind = ah.code & 3;
+    if (kind == 0) { enter_phantom(L, P, ah.code >> 2); return false; }
+    if (kind == 2) { L.a_esc += L.E; L.alive = false; return false; }
+    enter_epid(L, g);                                                      // (u, v, depth 0), beam-frame direction, dw > 0
+    const float idw = __frcp_rn(L.dz);
+    if (lateral_exit(L.x, L.y, L.dx, L.dy) < g.zt[g.n_layers] * idw) return false;   // leaves the stack sideways: layer-by-layer code
+    nl -= mua * ah.t;
+    if (COUNT) cnt[2]++;
+#pragma unroll 1
+    for (int l = 0; l < g.n_layers; ++l) {
+        mu3(P, sh, g.lmat[l], L.ci, L.ct, pe, co, pp);
+        mt = pe + co + pp;
+        const float mul = g.lrho[l] * mt, path = (g.zt[l + 1] - g.zt[l]) * idw;
+        if (nl < mul * path) {                                             // collision in layer l
+            const float s = __fdividef(nl, mul) + g.zt[l] * idw;           // path length from the top plane
+            L.x = fmaf(s, L.dx, L.x); L.y = fmaf(s, L.dy, L.y); L.z = fminf(fmaxf(s * L.dz, g.zt[l]), g.zt[l + 1]);
+            SET_LAYER(L.flags, l);
+            xsel = u2 * mt;
+            return true;
+        }
+        nl -= mul * path;
+    }
+    L.a_esc += L.E; L.alive = false;                                       // through the bottom of the stack
+    return false;
+}
+// K6: one flight of a photon inside the EPID, surface tracking layer by layer.
+template <bool COUNT>
+__device__ __forceinline__ bool epid_flight(Lane& L, const TransportParams& P, const Shared& sh, float& xsel, float& pe, float& co, uint32_t* cnt) {
+    const Geom& g = P.g;
+    const uint4 rr = rng_block(L, P);
+    const float u1 = u01(rr.x), u2 = u01(rr.y);
+    if (COUNT) cnt[2]++;
+    const int l = F_LAYER(L.flags);
+    float pp;
+    mu3(P, sh, g.lmat[l], L.ci, L.ct, pe, co, pp);
+    const float mt = pe + co + pp;
+    const float s = __fdividef(-__logf(u1), g.lrho[l] * mt);
+    float tf = kInf;
+    if (L.dz > 0.0f) tf = (g.zt[l + 1] - L.z) / L.dz; else if (L.dz < 0.0f) tf = (g.zt[l] - L.z) / L.dz;
+    tf = fmaxf(tf, 0.0f);
+    const float tl = lateral_exit(L.x, L.y, L.dx, L.dy);
+    if (s < tf && s < tl) { L.x = fmaf(s, L.dx, L.x); L.y = fmaf(s, L.dy, L.y); L.z = fmaf(s, L.dz, L.z); xsel = u2 * mt; return true; }
+    if (tl < tf) { L.a_esc += L.E; L.alive = false; return false; }
+    L.x = fmaf(tf, L.dx, L.x); L.y = fmaf(tf, L.dy, L.y);
+    if (L.dz > 0.0f) {
+        L.z = g.zt[l + 1];
+        if (l + 1 >= g.n_layers) { L.a_esc += L.E; L.alive = false; }
+        else SET_LAYER(L.flags, l + 1);
+    } else {
+        L.z = g.zt[l];
+        if (l == 0) epid_to_air(L, g); else SET_LAYER(L.flags, l - 1);
+    }
+    return false;
 }
 
 // ---------------------------------------------------------------- K5 electron / positron step
+// Energy loss of the step (midpoint rule), deposit-independent part shared by the two step functions.
+struct StepLoss { float s, dep, Tmid; };
+__device__ __forceinline__ StepLoss step_loss(Lane& L, const TransportParams& P, const Shared& sh, int m, float rho, float tb) {
+    const float T = L.E;
+    const float S = stop_pow(P, sh, m, T);
+    StepLoss r;
+    r.s = fminf(tb, fminf(__fdividef(P.ph.fE * T, rho * S), P.ph.smax));
+    const float S2 = stop_pow(P, sh, m, T - 0.5f * rho * r.s * S);        // midpoint rule
+    const float dE = fminf(T, rho * r.s * S2);
+    const float Tn = T - dE;
+    r.dep = T - Tn;                                                        // exactly what the particle loses (ledger closes)
+    r.Tmid = T - 0.5f * dE;
+    L.E = Tn;
+    return r;
+}
+// Highland deflection angles for a step of mass thickness rho*s at mid-step energy Tmid from the draws (ra, rb)
+// (reading A13).  A zero-length step gives theta = 0, i.e. no deflection.
+__device__ __forceinline__ void highland(const Shared& sh, int m, float rho_s, float Tmid, uint32_t ra, uint32_t rb,
+                                         float& ct, float& st, float& cp, float& sp) {
+    const float t = fmaxf(rho_s * sh.invX0[m], 1e-30f);
+    const float ibpc = __fdividef(Tmid + kMec2, Tmid * (Tmid + 2.0f * kMec2));
+    const float th0 = 13.6f * ibpc * sqrtf(t) * fmaxf(0.25f, fmaf(0.038f, __logf(t), 1.0f));
+    const float th = rho_s > 0.0f ? fminf(kPi, th0 * sqrtf(-2.0f * __logf(u01(ra)))) : 0.0f;
+    __sincosf(th, &st, &ct);
+    __sincosf(2.0f * kPi * u01(rb) - kPi, &sp, &cp);
+}
+// charged particle at or below its cutoff (PAPER.md:104, 200 keV): local deposit; a positron annihilates
 template <bool COUNT>
-__device__ __forceinline__ void electron_event(Lane& L, const TransportParams& P, const Shared& sh, StackEntry* stk, uint32_t* cnt) {
+__device__ __forceinline__ void stop_charged(Lane& L, const TransportParams& P, uint32_t* cnt) {
+    dep_here(L, P, L.E);
+    if (F_TYPE(L.flags) == T_POSITRON) {
+        if (F_REGION(L.flags) == R_PHANTOM) frac_to_world(L, P.g);
+        if (COUNT) cnt[9] += 2;
+        annihilate(L, P);
+    } else L.alive = false;
+}
+// One step inside the phantom with the draws (ra, rb): the hot loop of the whole path, written without branches up
+// to the face crossing.  The particle is above its cutoff.
+template <bool COUNT>
+__device__ __forceinline__ void electron_step_phantom(Lane& L, const TransportParams& P, const Shared& sh, uint32_t ra, uint32_t rb, uint32_t* cnt) {
     const Geom& g = P.g;
-    const uint32_t reg = F_REGION(L.flags);
-    if (L.E <= P.ph.ecut) {                                                // PAPER.md:104, 200 keV: local deposit
-        dep_here(L, P, sh, L.E);
-        if (F_TYPE(L.flags) == T_POSITRON) {
-            if (reg == R_PHANTOM) frac_to_world(L, g);
-            if (COUNT) cnt[9] += 2;
-            annihilate(L, P, sh, stk);
-        } else L.alive = false;
-        return;
+    const float rho = __uint_as_float(L.cw & ~31u); const int m = (int)(L.cw & 31u);
+    // distance to the voxel face in the direction of travel, per axis (a vanishing component gives a huge distance)
+    const float tx = (L.dx > 0.0f ? 1.0f - L.x : L.x) * g.hx * __frcp_rn(fabsf(L.dx) + 1e-30f);
+    const float ty = (L.dy > 0.0f ? 1.0f - L.y : L.y) * g.hy * __frcp_rn(fabsf(L.dy) + 1e-30f);
+    const float tz = (L.dz > 0.0f ? 1.0f - L.z : L.z) * g.hz * __frcp_rn(fabsf(L.dz) + 1e-30f);
+    const float tb = fmaxf(fminf(tx, fminf(ty, tz)), 0.0f);
+    const int axis = (tx <= ty && tx <= tz) ? 0 : (ty <= tz ? 1 : 2);
+    const StepLoss sl = step_loss(L, P, sh, m, rho, tb);
+    if (COUNT) { cnt[6]++; if (!(sl.s > 0.0f)) cnt[15]++; }
+    dep_vox(L, P, L.vlin, sl.dep);
+    L.x = fmaf(sl.s * g.ihx, L.dx, L.x); L.y = fmaf(sl.s * g.ihy, L.dy, L.y); L.z = fmaf(sl.s * g.ihz, L.dz, L.z);
+    float ct, st, cp, sp;
+    highland(sh, m, rho * sl.s, sl.Tmid, ra, rb, ct, st, cp, sp);
+    if (sl.s == tb) {                                                      // the step ended on a face: neighbouring voxel or out of the grid
+        const bool up = (axis == 0 ? L.dx : (axis == 1 ? L.dy : L.dz)) > 0.0f;
+        const float nf = up ? 0.0f : 1.0f;
+        L.x = axis == 0 ? nf : L.x; L.y = axis == 1 ? nf : L.y; L.z = axis == 2 ? nf : L.z;
+        const int sh10 = axis * 10;
+        const int ni = (int)((L.vox >> sh10) & 1023u) + (up ? 1 : -1);
+        const int nmax = axis == 0 ? g.nx : (axis == 1 ? g.ny : g.nz);
+        if (ni < 0 || ni >= nmax) {
+            frac_to_world(L, g);                                           // uses the old index; then snap the crossed axis
+            if (axis == 0) L.x = up ? g.hix : g.lox; else if (axis == 1) L.y = up ? g.hiy : g.loy; else L.z = up ? g.hiz : g.loz;
+            SET_REGION(L.flags, R_AIR);
+        } else {
+            const int stride = axis == 0 ? 1 : (axis == 1 ? g.nx : g.nx * g.ny);
+            L.vox = (L.vox & ~(1023u << sh10)) | ((uint32_t)ni << sh10);
+            L.vlin += up ? (uint32_t)stride : (uint32_t)(-stride);
+            L.cw = __ldg(P.vox + L.vlin);
+        }
     }
+    rotate(L.dx, L.dy, L.dz, ct, st, cp, sp);
+}
+// one step in the air or inside the EPID (the particle is above its cutoff)
+template <bool COUNT>
+__device__ __forceinline__ void electron_step_outside(Lane& L, const TransportParams& P, const Shared& sh, uint32_t ra, uint32_t rb, uint32_t* cnt) {
+    const Geom& g = P.g;
+    const bool in_air = F_REGION(L.flags) == R_AIR;
     float rho, tb; int m, axis = 0, kind = 0;
-    if (reg == R_PHANTOM) {
-        rho = __uint_as_float(L.cw & ~31u); m = (int)(L.cw & 31u);
-        float tx = kInf, ty = kInf, tz = kInf;
-        if (L.dx > 0.0f) tx = (1.0f - L.x) * g.hx / L.dx; else if (L.dx < 0.0f) tx = -L.x * g.hx / L.dx;
-        if (L.dy > 0.0f) ty = (1.0f - L.y) * g.hy / L.dy; else if (L.dy < 0.0f) ty = -L.y * g.hy / L.dy;
-        if (L.dz > 0.0f) tz = (1.0f - L.z) * g.hz / L.dz; else if (L.dz < 0.0f) tz = -L.z * g.hz / L.dz;
-        if (tx <= ty && tx <= tz) { tb = tx; axis = 0; } else if (ty <= tz) { tb = ty; axis = 1; } else { tb = tz; axis = 2; }
-        tb = fmaxf(tb, 0.0f);
-    } else if (reg == R_AIR) {
+    if (in_air) {
         rho = kRhoAir; m = 0;
-        tb = air_boundary(g, L, kind, axis);
+        const AirHit ah = air_boundary(L.x, L.y, L.z, L.dx, L.dy, L.dz);
+        tb = ah.t; kind = ah.code & 3; axis = ah.code >> 2;
     } else {
         const int l = F_LAYER(L.flags);
         rho = g.lrho[l]; m = g.lmat[l];
@@ -482,67 +690,25 @@ __device__ __forceinline__ void electron_event(Lane& L, const TransportParams& P
         const float tl = lateral_exit(L.x, L.y, L.dx, L.dy);
         if (tl < tf) { tb = tl; kind = 2; } else { tb = tf; kind = 0; }
     }
-    const float T = L.E;
-    const float S = stop_pow(P, sh, m, T);
-    const float s = fminf(tb, fminf(P.ph.fE * T / (rho * S), P.ph.smax));
-    const float S2 = stop_pow(P, sh, m, T - 0.5f * rho * s * S);          // midpoint rule
-    const float dE = fminf(T, rho * s * S2);
-    const float Tn = T - dE;
-    const float dep = T - Tn;                                              // exactly what the particle loses (ledger closes)
-    const float Tmid = T - 0.5f * dE;
-    if (reg == R_PHANTOM) {
-        if (COUNT) cnt[6]++;
-        dep_vox(L, P, vox_linear(g, L.vox), dep);
-        L.x = fmaf(s * g.ihx, L.dx, L.x); L.y = fmaf(s * g.ihy, L.dy, L.y); L.z = fmaf(s * g.ihz, L.dz, L.z);
-    } else if (reg == R_AIR) {
-        if (COUNT) cnt[7]++;
-        atomicAdd(&sh.led[4], (double)dep);
-        L.x = fmaf(s, L.dx, L.x); L.y = fmaf(s, L.dy, L.y); L.z = fmaf(s, L.dz, L.z);
-    } else {
-        if (COUNT) cnt[8]++;
-        dep_epid(L, P, sh, F_LAYER(L.flags), fmaf(0.5f * s, L.dx, L.x), fmaf(0.5f * s, L.dy, L.y), dep);   // pixel of the step midpoint (A24)
-        L.x = fmaf(s, L.dx, L.x); L.y = fmaf(s, L.dy, L.y); L.z = fmaf(s, L.dz, L.z);
-    }
-    L.E = Tn;
-    // Highland deflection, applied at the end of the step (reading A13)
-    const bool deflect = s > 0.0f;
-    float ct = 1.0f, st = 0.0f, cp = 1.0f, sp = 0.0f;
-    if (deflect) {
-        const float t = rho * s * sh.invX0[m];
-        const float bpc = Tmid * (Tmid + 2.0f * kMec2) / (Tmid + kMec2);
-        const float th0 = (13.6f / bpc) * sqrtf(t) * fmaxf(0.25f, fmaf(0.038f, __logf(t), 1.0f));
-        float ua, ub; rng_pair(L, P, ua, ub);
-        const float th = fminf(kPi, th0 * sqrtf(-2.0f * __logf(ua)));
-        __sincosf(th, &st, &ct);
-        __sincosf(2.0f * kPi * ub - kPi, &sp, &cp);
-    } else if (COUNT) cnt[15]++;
-    if (s == tb) {                                                         // the step ended on a face: neighbouring voxel / layer / region
+    const StepLoss sl = step_loss(L, P, sh, m, rho, tb);
+    if (COUNT && !(sl.s > 0.0f)) cnt[15]++;
+    if (in_air) { if (COUNT) cnt[7]++; L.a_air += sl.dep; }
+    else { if (COUNT) cnt[8]++; dep_epid(L, fmaf(0.5f * sl.s, L.dx, L.x), fmaf(0.5f * sl.s, L.dy, L.y), sl.dep); }   // pixel of the step midpoint (A24)
+    L.x = fmaf(sl.s, L.dx, L.x); L.y = fmaf(sl.s, L.dy, L.y); L.z = fmaf(sl.s, L.dz, L.z);
+    float ct, st, cp, sp;
+    highland(sh, m, rho * sl.s, sl.Tmid, ra, rb, ct, st, cp, sp);
+    if (sl.s == tb) {                                                      // the step ended on a boundary
         const float e_out = L.E + (F_TYPE(L.flags) == T_POSITRON ? 2.0f * kMec2 : 0.0f);
-        if (reg == R_PHANTOM) {
-            const bool up = comp3(L.dx, L.dy, L.dz, axis) > 0.0f;
-            int ix = (int)(L.vox & 1023u), iy = (int)((L.vox >> 10) & 1023u), iz = (int)((L.vox >> 20) & 1023u);
-            bool out;
-            if (axis == 0) { ix += up ? 1 : -1; L.x = up ? 0.0f : 1.0f; out = ix < 0 || ix >= g.nx; }
-            else if (axis == 1) { iy += up ? 1 : -1; L.y = up ? 0.0f : 1.0f; out = iy < 0 || iy >= g.ny; }
-            else { iz += up ? 1 : -1; L.z = up ? 0.0f : 1.0f; out = iz < 0 || iz >= g.nz; }
-            if (out) {
-                frac_to_world(L, g);                                       // uses the old index; then snap the crossed axis
-                if (axis == 0) L.x = up ? g.hix : g.lox; else if (axis == 1) L.y = up ? g.hiy : g.loy; else L.z = up ? g.hiz : g.loz;
-                SET_REGION(L.flags, R_AIR);
-            } else {
-                L.vox = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20);
-                L.cw = __ldg(P.vox + vox_linear(g, L.vox));
-            }
-        } else if (reg == R_AIR) {
+        if (in_air) {
             if (kind == 0) enter_phantom(L, P, axis);
             else if (kind == 1) enter_epid(L, g);
-            else { atomicAdd(&sh.led[5], (double)e_out); L.alive = false; return; }
+            else { L.a_esc += e_out; L.alive = false; return; }
         } else {
             const int l = F_LAYER(L.flags);
-            if (kind == 2) { atomicAdd(&sh.led[5], (double)e_out); L.alive = false; return; }
+            if (kind == 2) { L.a_esc += e_out; L.alive = false; return; }
             if (L.dz > 0.0f) {
                 L.z = g.zt[l + 1];
-                if (l + 1 >= g.n_layers) { atomicAdd(&sh.led[5], (double)e_out); L.alive = false; return; }
+                if (l + 1 >= g.n_layers) { L.a_esc += e_out; L.alive = false; return; }
                 SET_LAYER(L.flags, l + 1);
             } else {
                 L.z = g.zt[l];
@@ -550,7 +716,19 @@ __device__ __forceinline__ void electron_event(Lane& L, const TransportParams& P
             }
         }
     }
-    if (deflect) rotate(L.dx, L.dy, L.dz, ct, st, cp, sp);
+    rotate(L.dx, L.dy, L.dz, ct, st, cp, sp);
+}
+// K5 for one lane: one Philox block feeds up to two consecutive steps
+template <bool COUNT, bool PHANTOM>
+__device__ __forceinline__ void charged_event(Lane& L, const TransportParams& P, const Shared& sh, uint32_t* cnt) {
+    if (L.E <= P.ph.ecut) { stop_charged<COUNT>(L, P, cnt); return; }
+    const uint4 r = rng_block(L, P);
+#pragma unroll 1
+    for (int k = 0; k < 2; ++k) {
+        if (PHANTOM) electron_step_phantom<COUNT>(L, P, sh, k ? r.z : r.x, k ? r.w : r.y, cnt);
+        else electron_step_outside<COUNT>(L, P, sh, k ? r.z : r.x, k ? r.w : r.y, cnt);
+        if (!L.alive || L.E <= P.ph.ecut || (F_REGION(L.flags) == R_PHANTOM) != PHANTOM) break;
+    }
 }
 
 // ---------------------------------------------------------------- K1 source
@@ -586,125 +764,267 @@ __device__ __forceinline__ SourceSample sample_source(const TransportParams& P, 
 }
 
 // ---------------------------------------------------------------- the kernel
-template <bool COUNT>
-__global__ void __launch_bounds__(kBlock, kMinBlocks) transport_kernel(const __grid_constant__ TransportParams P) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    {
-        uint32_t* dst = reinterpret_cast<uint32_t*>(smem_raw);
-        for (int i = threadIdx.x; i < P.tb.blob_words; i += kBlock) dst[i] = __ldg(P.tb.blob + i);
+// Add the warp's sum of v to *dst (lane 0); all lanes must call.
+__device__ __noinline__ void ledger_add(float v, double* dst) {
+    if (__ballot_sync(FULL_MASK, v != 0.0f) == 0u) return;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL_MASK, v, o);
+    if ((threadIdx.x & 31u) == 0) *dst += (double)v;
+}
+__device__ __forceinline__ void ledger_flush(Lane& L, double* led) {
+    ledger_add(L.a_emit, led + 0); ledger_add(L.a_ph, led + 1); ledger_add(L.a_eps, led + 2);
+    ledger_add(L.a_epo, led + 3); ledger_add(L.a_air, led + 4); ledger_add(L.a_esc, led + 5);
+    L.a_emit = L.a_ph = L.a_eps = L.a_epo = L.a_air = L.a_esc = 0.0f;
+}
+
+// Scheduler state changes under the warp's feet: every decision taken on it is made by lane 0 and broadcast, so that
+// the warp never splits on it.
+enum Decision { D_GO = 0, D_SOURCE = 1, D_RESELECT = 2, D_EVICT = 3 };
+__device__ __forceinline__ bool can_source(const volatile int* q, int lanes) {
+    return *((volatile int*)s_flag) == 0 && q[kFree] >= lanes + kSrcReserve;
+}
+// A warp of class wcls has `a` < 32 live lanes after the refill attempt: what now?
+__device__ __noinline__ int decide(int a, int wcls, uint32_t it) {
+    int d = D_GO;
+    if ((threadIdx.x & 31u) == 0) {
+        const volatile int* q = s_avail;
+        if (wcls == 0 && 32 - a >= kSrcMin && can_source(q, 32)) d = D_SOURCE;
+        else if (a == 0) d = D_RESELECT;
+        else if (a < kKeep && (it & 3u) == 0u && (q[0] >= 32 || q[1] >= 32 || q[2] >= 32 || q[3] >= 32 || can_source(q, 32))) d = D_EVICT;
     }
+    return __shfl_sync(FULL_MASK, d, 0);
+}
+// A warp with no particles picks its next class: 0..3 a queue (the fullest; charged particles first when the pool is
+// nearly exhausted), 4 new histories, 5 nothing to do right now, 6 nothing left at all.
+__device__ __noinline__ int pick_class() {
+    int d = 5;
+    if ((threadIdx.x & 31u) == 0) {
+        const volatile int* q = s_avail;
+        const int a0 = q[0], a1 = q[1], a2 = q[2], a3 = q[3], af = q[kFree];
+        int best = 0, ab = a0;
+        if (a1 > ab) { ab = a1; best = 1; }
+        if (a2 > ab) { ab = a2; best = 2; }
+        if (a3 > ab) { ab = a3; best = 3; }
+        if (af < 128 && (a2 > 0 || a3 > 0)) { best = a2 >= a3 ? 2 : 3; ab = 32; }
+        const bool src_done = *((volatile int*)s_flag) != 0;
+        if (ab >= 32) d = best;
+        else if (!src_done && af >= 32 + kSrcReserve) d = 4;
+        else if (ab > 0) d = best;
+        else if (src_done && af == kPool) d = 6;
+    }
+    return __shfl_sync(FULL_MASK, d, 0);
+}
+
+template <bool COUNT>
+__global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_constant__ TransportParams P) {
+    // dynamic shared memory: pool | per-warp ledger | table blob
+    double* const led_all = reinterpret_cast<double*>(smem_raw + (size_t)kWords * kPool * 4);
+    uint32_t* const blob = reinterpret_cast<uint32_t*>(smem_raw + (size_t)kWords * kPool * 4 + kWarps * 8 * sizeof(double));
+    for (int i = threadIdx.x; i < P.tb.blob_words; i += kThreads) blob[i] = __ldg(P.tb.blob + i);
     Shared sh;
-    sh.phot = reinterpret_cast<const float4*>(smem_raw);
+    sh.phot = reinterpret_cast<const float4*>(blob);
     sh.maj = reinterpret_cast<const float*>(sh.phot + P.tb.n_mat * P.tb.n_E);
     sh.lnS = sh.maj + P.tb.n_E;
     sh.invX0 = sh.lnS + P.tb.n_mat * P.tb.n_T;
-    sh.led = reinterpret_cast<double*>(smem_raw + (((size_t)P.tb.blob_words * 4 + 15) & ~(size_t)15));
-    if (threadIdx.x < 8) sh.led[threadIdx.x] = 0.0;
+    for (int i = threadIdx.x; i < kRings * kPool; i += kThreads)
+        s_ring[i] = (unsigned short)(i >= kFree * kPool ? (i - kFree * kPool) : 0xffff);    // free ring: slot i, generation 0
+    for (int i = threadIdx.x; i < kWarps * 8; i += kThreads) led_all[i] = 0.0;
+    if (threadIdx.x < kRings) {
+        const bool fr = threadIdx.x == kFree;
+        s_tail[threadIdx.x] = fr ? kPool : 0u; s_head[threadIdx.x] = 0u; s_avail[threadIdx.x] = fr ? kPool : 0;
+    }
+    if (threadIdx.x < 2) s_flag[threadIdx.x] = 0;
+    if (threadIdx.x == 0) { s_g = P.g; s_ep_batch = P.ep_batch; s_npix = P.npix; }
     __syncthreads();
 
-    StackEntry stk[kStackDepth];
-    uint32_t cnt[16];
+    uint32_t cnt[COUNT ? 32 : 1];
     if (COUNT) {
 #pragma unroll
-        for (int i = 0; i < 16; ++i) cnt[i] = 0;
+        for (int i = 0; i < 32; ++i) cnt[i] = 0;
     }
-    Lane L;
-    L.alive = false; L.sp = 0; L.pval = 0.0f; L.pidx = 0xffffffffu; L.lph = 0.0; L.flags = 0; L.blk = 0; L.pid = 0; L.h = 0;
-    L.x = L.y = L.z = 0.0f; L.dx = L.dy = 0.0f; L.dz = 1.0f; L.E = 0.0f; L.vox = 0; L.cw = 0; L.ci = 0; L.ct = 0.0f; L.mumaj = 1.0f; L.r2 = L.r3 = 0;
-    const unsigned lane = threadIdx.x & 31u;
+    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const unsigned lt_mask = (1u << lane) - 1u;
-    uint32_t wnext = 0, wend = 0, wbatch = 0;      // warp-uniform: current chunk of relative history indices
-    bool wdone = false;
-    double emitted = 0.0;
-    uint32_t max_sp = 0;
+    double* const led = led_all + warp * 8;
+    Lane L;
+    L.x = L.y = L.z = 0.0f; L.dx = L.dy = 0.0f; L.dz = 1.0f; L.E = 0.0f; L.vox = 0; L.flags = 0; L.h = L.pid = L.blk = 0;
+    L.cw = 0; L.vlin = 0; L.ci = 0; L.ct = 0.0f; L.mumaj = 1.0f;
+    L.pval = 0.0f; L.pidx = kNone; L.slot = kNone; L.spare = kNone; L.alive = false;
+    L.a_emit = L.a_ph = L.a_eps = L.a_epo = L.a_air = L.a_esc = 0.0f;
+    int wcls = 0;           // event class this warp works on (warp-uniform)
+    bool evict = false;     // hand every particle back at the top of the next iteration
+    bool drain = false;     // ... and then take other work instead of refilling (the free ring ran dry)
+    int idle = 0;
 
-    for (;;) {
-        if (!L.alive && L.sp > 0) {                // next secondary of this lane's history
-            const StackEntry& s = stk[--L.sp];
-            L.x = s.x; L.y = s.y; L.z = s.z; L.dx = s.dx; L.dy = s.dy; L.dz = s.dz; L.E = s.E;
-            L.flags = s.flags; L.vox = s.vox; L.pid = s.pid; L.blk = s.blk;
-            L.alive = true;
-            if (F_TYPE(L.flags) == T_PHOTON) set_energy(L, P, sh);
-            else if (F_REGION(L.flags) == R_PHANTOM) L.cw = __ldg(P.vox + vox_linear(P.g, L.vox));
-        }
-        if (!wdone) {
-            const unsigned need = __ballot_sync(FULL_MASK, !L.alive);
-            if (need) {
-                if (wnext == wend) {               // grab the next chunk
-                    uint32_t c = 0;
-                    if (lane == 0) c = atomicAdd(P.chunk_counter, 1u);
-                    c = __shfl_sync(FULL_MASK, c, 0);
-                    if (c >= P.n_chunks) wdone = true;
-                    else {
-                        wnext = c * (uint32_t)kChunk;
-                        wend = min(P.n, wnext + (uint32_t)kChunk);
-                        wbatch = (uint32_t)(((uint64_t)c * (uint64_t)P.n_batches) / P.n_chunks);
-                    }
-                }
-                if (!wdone) {
-                    const uint32_t rank = __popc(need & lt_mask);
-                    const uint32_t avail = wend - wnext;
-                    if (!L.alive && rank < avail) {                        // start history wnext + rank
-                        flush_pending(L, P);
-                        L.h = wnext + rank; L.pid = 0; L.blk = 0;
-                        uint32_t r0, r1, r2, r3;
-                        rng_block(L, P, r0, r1, r2, r3);                   // block 0 of particle 0: E, pixel, u, v (reading A1)
-                        const SourceSample s = sample_source(P, r0, r1, r2, r3);
-                        L.x = P.g.src[0]; L.y = P.g.src[1]; L.z = P.g.src[2];
-                        L.dx = s.dx; L.dy = s.dy; L.dz = s.dz; L.E = s.E;
-                        L.flags = T_PHOTON | (R_AIR << 2) | (wbatch << 16);
-                        L.alive = true; L.sp = 0;
-                        emitted += (double)s.E;
-                        set_energy(L, P, sh);
-                    }
-                    wnext += min((uint32_t)__popc(need), avail);
-                }
+    for (uint32_t it = 1;; ++it) {
+        // ---- A: particles that left the class go to the queue of their new class; the slot of a dead particle becomes the lane's spare
+        if (!(L.alive && !evict && class_of(L.flags) == wcls)) {
+            flush_pending(L, P);
+            if (L.alive) {
+                const uint32_t s = L.slot;
+                if (s == kNone) {                                          // cannot happen (flagged): drop, ledger still closes
+                    raise_error(4);
+                    L.a_esc += L.E + (F_TYPE(L.flags) == T_POSITRON ? 2.0f * kMec2 : 0.0f);
+                } else queue_particle(s, L.x, L.y, L.z, L.dx, L.dy, L.dz, L.E, L.vox, L.flags, L.h, L.pid, L.blk);
+                if (COUNT) cnt[23]++;
+                L.alive = false; L.slot = kNone;
+            } else if (L.slot != kNone) {
+                if (wcls < 2 && L.spare == kNone) L.spare = L.slot; else ring_push_one(kFree, L.slot);   // photon lanes keep one spare
+                L.slot = kNone;
             }
         }
-        if (!__any_sync(FULL_MASK, L.alive)) { if (wdone) break; else continue; }
-        if (L.alive) {
-            if (F_TYPE(L.flags) == T_PHOTON) photon_event<COUNT>(L, P, sh, stk, cnt);
-            else electron_event<COUNT>(L, P, sh, stk, cnt);
-            if (COUNT) max_sp = max(max_sp, (uint32_t)L.sp);
+        evict = false;
+        // ---- B: empty lanes refill from the queue of the class
+        if (!L.alive && !drain && *((volatile int*)(s_avail + wcls)) > 0) {
+            const uint32_t s = ring_pop_one(wcls);
+            if (s != kNone) {
+                const uint32_t* p = pool_base() + s;
+                L.x = __uint_as_float(p[0 * kPool]); L.y = __uint_as_float(p[1 * kPool]); L.z = __uint_as_float(p[2 * kPool]);
+                L.dx = __uint_as_float(p[3 * kPool]); L.dy = __uint_as_float(p[4 * kPool]); L.dz = __uint_as_float(p[5 * kPool]);
+                L.E = __uint_as_float(p[6 * kPool]); L.vox = p[7 * kPool]; L.flags = p[8 * kPool];
+                L.h = p[9 * kPool]; L.pid = p[10 * kPool]; L.blk = p[11 * kPool];
+                L.slot = s; L.alive = true;
+                L.pval = 0.0f; L.pidx = kNone;
+                if (COUNT) cnt[24]++;
+                if (F_TYPE(L.flags) == T_PHOTON) set_energy(L, P, sh);
+                else if (F_REGION(L.flags) == R_PHANTOM) { L.vlin = vox_linear(P.g, L.vox); L.cw = __ldg(P.vox + L.vlin); }
+            }
         }
+        // ---- C: lanes still empty: start new histories, take another class, or carry on
+        const unsigned live = __ballot_sync(FULL_MASK, L.alive);
+        const int n_live = __popc(live);
+        if (drain || n_live == 0 || (wcls == 0 && 32 - n_live >= kSrcMin) || (n_live < kKeep && (it & 3u) == 0u)) {
+            const int dec = drain ? D_RESELECT : decide(n_live, wcls, it);
+            drain = false;
+            if (dec == D_SOURCE) {
+                // K1: new histories in the empty lanes
+                const unsigned long long cl = ring_claim_packed(kFree, 32 - __popc(live));   // one slot per new history
+                const int nd = (int)(uint32_t)cl;   // (32 - n_live at most)
+                const int rk = __popc(~live & lt_mask);
+                uint32_t myslot = kNone;
+                if (!L.alive && rk < nd) myslot = ring_take(kFree, (uint32_t)(cl >> 32) + (uint32_t)rk);
+                uint32_t h0 = 0;
+                if (lane == 0 && nd > 0) h0 = atomicAdd(P.hist_counter, (unsigned)nd);
+                h0 = __shfl_sync(FULL_MASK, h0, 0);
+                if (nd > 0 && h0 >= P.n && lane == 0) atomicExch(s_flag, 1);
+                {
+                    if (COUNT && lane == 0) cnt[21]++;
+                    const uint32_t h = h0 + (uint32_t)rk;
+                    if (myslot != kNone && h >= P.n) { ring_push_one(kFree, myslot); myslot = kNone; }
+                    if (myslot != kNone) {
+                        L.h = h; L.pid = 0; L.blk = 0;
+                        const uint4 r = rng_block(L, P);                   // block 0 of particle 0: E, pixel, u, v (reading A1)
+                        const SourceSample s = sample_source(P, r.x, r.y, r.z, r.w);
+                        L.x = P.g.src[0]; L.y = P.g.src[1]; L.z = P.g.src[2];
+                        L.dx = s.dx; L.dy = s.dy; L.dz = s.dz; L.E = s.E;
+                        L.vox = 0;
+                        L.flags = T_PHOTON | (R_AIR << 2) | (min(h / P.hist_per_batch, (uint32_t)P.n_batches - 1u) << 16);
+                        L.alive = true; L.slot = myslot;
+                        L.pval = 0.0f; L.pidx = kNone;
+                        L.a_emit += s.E;
+                        set_energy(L, P, sh);
+                    }
+                }
+                idle = 0;
+            } else if (dec == D_RESELECT) {
+                ledger_flush(L, led);
+                const int pc = pick_class();
+                if (COUNT && lane == 0) cnt[27]++;
+                if (pc < 4) {
+                    wcls = pc; idle = 0;
+                    if (pc >= 2 && L.spare != kNone) { ring_push_one(kFree, L.spare); L.spare = kNone; }   // charged-particle warps need no spares
+                }
+                else if (pc == 4) { wcls = 0; idle = 0; }
+                else {
+                    if (L.spare != kNone) { ring_push_one(kFree, L.spare); L.spare = kNone; }   // idle: give the spare slots back
+                    if (pc == 6) break;                                    // nothing queued, nothing in flight, nothing left to start
+                    if (++idle > kSpinLimit) { raise_error(8); break; }
+                    if (COUNT && lane == 0) cnt[22]++;
+                    __nanosleep(200);
+                }
+                continue;
+            } else if (dec == D_EVICT) {
+                evict = true;
+                if (COUNT && lane == 0) cnt[28]++;
+            }
+        }
+        // ---- D: one event per live lane
+        if (COUNT && lane == 0) cnt[16]++;
+        if (wcls < 2) {
+            bool on = L.alive && class_of(L.flags) == wcls;
+            if (on && !ensure_spare(L)) on = false;                        // an interaction may create a secondary: wait for a slot
+            if (__ballot_sync(FULL_MASK, on) == 0u) { evict = true; drain = true; continue; }   // every photon waits for a slot: drain queues instead
+            bool hit = false; float xsel = 0.0f, pe = 0.0f, co = 0.0f;
+            if (COUNT) { if (lane == 0) cnt[17]++; if (on) cnt[18]++; }
+            if (wcls == 0) {
+                // photons in AIR wait until enough of them can make the transit together
+                const bool in_air = on && F_REGION(L.flags) == R_AIR;
+                const unsigned m_air = __ballot_sync(FULL_MASK, in_air), m_on = __ballot_sync(FULL_MASK, on);
+                const bool do_air = __popc(m_air) >= kTransitMin || m_air == m_on;
+                if (on && L.E < P.ph.pcut) { if (COUNT) cnt[13]++; dep_here(L, P, L.E); L.alive = false; }   // PAPER.md:104, 10 keV
+                else if (on && !in_air) hit = woodcock_flight<COUNT>(L, P, sh, xsel, pe, co, cnt);
+                else if (in_air && do_air) {
+                    if (COUNT) { cnt[26]++; }
+                    hit = air_transit<COUNT>(L, P, sh, xsel, pe, co, cnt);
+                }
+                if (COUNT && lane == 0 && do_air && m_air) cnt[25]++;
+            } else {
+                if (on && L.E < P.ph.pcut) { if (COUNT) cnt[13]++; dep_here(L, P, L.E); L.alive = false; }
+                else if (on) hit = epid_flight<COUNT>(L, P, sh, xsel, pe, co, cnt);
+            }
+            if (hit) interact<COUNT>(L, P, sh, xsel, pe, co, cnt);
+        } else if (wcls == 2) {
+            bool on = L.alive && class_of(L.flags) == 2;
+            if (on && F_TYPE(L.flags) == T_POSITRON && L.E <= P.ph.ecut && !ensure_spare(L)) on = false;   // annihilation needs a slot
+            if (COUNT) { if (lane == 0) cnt[19]++; if (on) cnt[20]++; }
+            if (on) charged_event<COUNT, true>(L, P, sh, cnt);
+        } else {
+            bool on = L.alive && class_of(L.flags) == 3;
+            if (on && F_TYPE(L.flags) == T_POSITRON && L.E <= P.ph.ecut && !ensure_spare(L)) on = false;
+            if (COUNT) { if (lane == 0) cnt[19]++; if (on) cnt[20]++; }
+            if (on) charged_event<COUNT, false>(L, P, sh, cnt);
+        }
+        // ---- E: ledger of the last iterations: float per lane -> warp sum -> the warp's double accumulators
+        if ((it & 63u) == 0u) ledger_flush(L, led);
     }
     flush_pending(L, P);
-    atomicAdd(&sh.led[0], emitted);
-    atomicAdd(&sh.led[1], L.lph);
+    ledger_flush(L, led);
+
     __syncthreads();
-    if (threadIdx.x < 8 && threadIdx.x != 6) { const double v = sh.led[threadIdx.x]; if (v != 0.0) atomicAdd(P.ledger + threadIdx.x, v); }
+    if (threadIdx.x < 6) {
+        double v = 0.0;
+        for (int w = 0; w < kWarps; ++w) v += led_all[w * 8 + threadIdx.x];
+        if (v != 0.0) atomicAdd(P.ledger + threadIdx.x, v);
+    }
+    if (threadIdx.x == 0 && s_flag[1]) atomicAdd(P.ledger + 7, (double)s_flag[1]);
     if (COUNT) {
 #pragma unroll
-        for (int i = 0; i < 16; ++i) {
-            if (i == 11) continue;
+        for (int i = 0; i < 32; ++i) {
             uint32_t v = cnt[i];
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL_MASK, v, o);
             if (lane == 0 && v) atomicAdd(P.counters + i, (unsigned long long)v);
         }
-        atomicMax(P.counters + 11, (unsigned long long)max_sp);
     }
 }
 
-size_t transport_smem_bytes(const Tables& t) { return (((size_t)t.blob_words * 4 + 15) & ~(size_t)15) + 8 * sizeof(double); }
+size_t transport_smem_bytes(const Tables& t) {      // dynamic + static shared memory of the kernel
+    return (size_t)kWords * kPool * 4 + kWarps * 8 * sizeof(double) + (size_t)t.blob_words * 4 +
+           sizeof(unsigned short) * kRings * kPool + sizeof(Geom) + 256;
+}
 
 int launch_transport(const TransportParams& p, bool counting, int sm_count, void* stream) {
-    const size_t smem = transport_smem_bytes(p.tb);
+    const size_t smem = (size_t)kWords * kPool * 4 + kWarps * 8 * sizeof(double) + (size_t)p.tb.blob_words * 4;
     cudaError_t e;
     if (counting) e = cudaFuncSetAttribute(transport_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     else e = cudaFuncSetAttribute(transport_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return (int)e;
-    int per_sm = 0;
-    if (counting) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, transport_kernel<true>, kBlock, smem);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, transport_kernel<false>, kBlock, smem);
-    if (per_sm < 1) per_sm = 1;
-    // persistent grid: every resident CTA slot of every SM, but no more warps than chunks
-    long long blocks = (long long)sm_count * per_sm;
-    const long long need = ((long long)p.n_chunks + (kBlock / 32) - 1) / (kBlock / 32);
+    // persistent grid: one CTA per SM, but no more CTAs than there is work for
+    long long blocks = sm_count;
+    const long long need = ((long long)p.n + 255) / 256;
     if (blocks > need) blocks = need;
     if (blocks < 1) blocks = 1;
-    if (counting) transport_kernel<true><<<(unsigned)blocks, kBlock, smem, (cudaStream_t)stream>>>(p);
-    else transport_kernel<false><<<(unsigned)blocks, kBlock, smem, (cudaStream_t)stream>>>(p);
+    if (counting) transport_kernel<true><<<(unsigned)blocks, kThreads, smem, (cudaStream_t)stream>>>(p);
+    else transport_kernel<false><<<(unsigned)blocks, kThreads, smem, (cudaStream_t)stream>>>(p);
     return (int)cudaGetLastError();
 }
 
@@ -713,9 +1033,8 @@ __global__ void sample_source_kernel(const __grid_constant__ TransportParams P, 
     const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n) return;
     const uint64_t h = first + k;
-    uint32_t r0, r1, r2, r3;
-    philox4x32_10((uint32_t)h, (uint32_t)(h >> 32), 0u, 0u, (uint32_t)P.seed, (uint32_t)(P.seed >> 32), r0, r1, r2, r3);
-    const SourceSample s = sample_source(P, r0, r1, r2, r3);
+    const uint4 r = philox4x32_10((uint32_t)h, (uint32_t)(h >> 32), 0u, 0u, (uint32_t)P.seed, (uint32_t)(P.seed >> 32));
+    const SourceSample s = sample_source(P, r.x, r.y, r.z, r.w);
     float4* o = reinterpret_cast<float4*>(out + 8 * k);
     o[0] = make_float4(s.E, s.dx, s.dy, s.dz);
     o[1] = make_float4((float)s.pixel, s.u, s.v, 0.0f);
