@@ -3,6 +3,7 @@
 #pragma once
 #include <cstdint>
 #include <cstddef>
+#include <vector_types.h>
 
 namespace aepid {
 
@@ -12,6 +13,9 @@ constexpr float kRhoAir = 1.205e-3f;  // world filler, material 0 (SURVEY 8(c) "
 constexpr float kWorldHalf = 100.0f;  // |u|, |v| <= 100 cm
 constexpr float kWorldWMin = -1.0f;   // -1 <= w
 constexpr float kMec2 = 0.51099895f;
+constexpr int kPoolSlots = 8192;      // particle records per CTA of the transport kernel (transport.cu)
+constexpr int kRecordBytes = 48;      // three 16-byte vectors per particle
+constexpr int kMaxCtas = 192;         // CTAs of the transport kernel the workspace provides a pool for (one per SM)
 
 enum Region : uint32_t { R_AIR = 0, R_PHANTOM = 1, R_EPID = 2 };
 enum PType : uint32_t { T_PHOTON = 0, T_ELECTRON = 1, T_POSITRON = 2 };
@@ -68,6 +72,7 @@ struct TransportParams {
     double* ledger;                    // [8]
     unsigned long long* counters;      // [32]
     unsigned int* hist_counter;        // next history of this launch that has not been started
+    uint4* pool;                       // particle records [kMaxCtas][kPoolSlots][3], scratch of one launch
     uint64_t base;                     // global index of relative history 0 of this launch
     uint64_t seed;
     uint32_t n;                        // histories in this launch (< 2^32)

@@ -2,35 +2,39 @@
 // sampling, K5 CSDA electron steps with Highland deflection, K6 EPID slab transport and K7 tally
 // scoring (physics of SURVEY.md 8(c)).
 //
-// Design (sm_100a): ONE persistent CTA per SM that is its own particle scheduler.
-//   * Shared memory holds the material tables (ln domain, one LDS.128 per node), a POOL of kPool particle
-//     records (SoA, 12 words) and, per event class, a ring queue of pool-slot indices, plus a ring of free slots.
-//     Classes: photon in phantom | photon in air/EPID | charged in phantom | charged in air/EPID.
-//   * Every warp runs the same scheduler loop on its own (no block-wide barrier in the steady state).  A warp
-//     works on one particle GROUP (photons or charged particles) at a time and keeps its lanes full: it runs the
-//     group's event loop; when enough lanes have run dry (particle absorbed, escaped or changed group) it writes
-//     those back (free the slot / store and queue the particle under its new class) and refills the empty lanes
-//     from the queue of its class IN PLACE, the other lanes keep their particles in registers.  A warp that runs
-//     out of work takes the class with the most waiting particles (full warps first) or, if no class can fill a
-//     warp, starts 32 new histories.  Warps therefore execute one code path with (nearly) all lanes active, and
-//     the secondaries of a history are followed concurrently by other warps instead of serially by their parent.
-//   * Secondaries go straight into the pool: the creating lane takes a free slot, stores the record and appends
-//     the slot to the queue of the secondary's class.
-//   * Queue protocol (bounded MPMC ring): pushers take tickets from tail[c] and write cell = slot | generation,
-//     then commit with avail[c] += n; poppers take n <= avail[c] committed entries, then tickets from head[c], and
-//     wait for the generation tag of their cells (the pusher holding that ticket is at most a few instructions
-//     away).  Ring capacity >= pool size, so a cell is never overwritten before it has been read.  Every wait is
-//     bounded; an exhausted bound or an exhausted pool raises the overflow flag ledger[7] (tests assert it is 0).
+// Design (sm_100a): ONE persistent CTA per SM that runs a LOCAL WAVEFRONT.  Measured on B200 (profiles/r01b_*,
+// profiles/r01c_icache_microbench.md): warps of one SM that execute different parts of a code body larger than the
+// 32 KB instruction cache starve on instruction fetch (IPC 0.3-1.1 of 4), warps that execute the same part do not.
+// So all warps of a CTA work on the same event class at any time:
+//   * Event classes: A photon in air (new histories start here), W photon in the phantom, E charged particle in the
+//     phantom, P photon inside the EPID or with a collision pending outside the phantom, X charged particle outside
+//     the phantom.  The CTA runs PHASES, one class per phase, separated by block barriers; thread 0 picks the next
+//     phase: new histories while the particle pool has room, else the class with the most waiting particles.
+//   * Particle records (48 B, three 16 B vectors) live in a per-CTA POOL in global memory (kPool slots, L2 resident,
+//     written and read with .cg accesses); shared memory holds the material tables (ln domain, one LDS.128 per node)
+//     and, per class, a ring of pool-slot indices, plus a ring of free slots.  A pool this large (8192 particles
+//     for 768 lanes) makes a phase many waves long, so that the phase switch (two barriers, a cold instruction
+//     cache) and the tail of a phase cost little.
+//   * Within a phase every lane follows its particle event by event while it stays in the class; a lane whose
+//     particle has died or changed class writes it back (record to the pool, slot to the ring of the new class) and
+//     is refilled IN PLACE from the ring of the phase, so warps run one code path with nearly all lanes active.
+//     Secondaries go straight into the pool: the creating lane holds a spare free slot, stores the record and
+//     appends the slot to the ring of the secondary's class.
+//   * Ring protocol: head/tail are monotonic counters; pushes take a ticket from tail and write the cell; pops take
+//     tickets from head but only below the SNAPSHOT of tail taken at the last barrier, so a cell is never read
+//     before the barrier that publishes it and no generation tags or spin waits are needed.  What is pushed during a
+//     phase (also into the phase's own ring: parked or evicted particles) becomes visible in the next phase.
+//   * A phase ends softly: once its ring is exhausted a warp with fewer than kKeepLanes live lanes, or any warp
+//     after half of the warps have gone, writes its particles back and leaves; the survivors join the next phase of
+//     their class.  Phases that start with fewer than two waves of particles run until every lane is dry.
+//   * Slot discipline: every particle owns a pool slot from birth, so writing it back never needs a new one; a lane
+//     runs an event that can create a secondary only while it holds a spare slot, otherwise it parks its particle.
+//     New histories start only while kReserve slots stay free.  Hence the pool cannot overflow.
 //   * A particle's trajectory does not depend on the schedule: its Philox stream is keyed by (history, particle
-//     id, block) and every event consumes whole blocks (reading A1), so no draw is ever buffered across events and
-//     all lanes of a warp call Philox together.
-//   * The phantom is one packed 32-bit word per voxel gathered through the read-only path (L2-resident up to
-//     ~30 M voxels); phantom deposits of consecutive steps in one voxel are merged in registers and flushed with
-//     one RED; the energy ledger is summed per phase in float, reduced over the warp and accumulated per warp in
-//     double.
-//   * Instruction footprint matters more than anything else here (ncu: the first version of this kernel spent 78 %
-//     of its issue slots waiting for instruction fetch with 118 KB of SASS): Philox, the air navigation, the queue
-//     operations and the EPID scoring are out-of-line functions, divisions and square roots use the fast paths.
+//     id, block) and every event consumes whole blocks (reading A1).
+//   * The phantom is one packed 32-bit word per voxel gathered through the read-only path; phantom deposits of
+//     consecutive steps in one voxel are merged in registers and flushed with one RED; the energy ledger is summed
+//     per lane in float, reduced over the warp and accumulated per warp in double.
 // No tensor cores / TMA: random gathers and scalar arithmetic, nothing here is a dense contraction.
 #include <cuda_runtime.h>
 #include <cstdint>
@@ -40,50 +44,56 @@ namespace aepid {
 
 constexpr int kWarps = 24;
 constexpr int kThreads = kWarps * 32;
-constexpr int kPoolLog = 11;
+constexpr int kPoolLog = 13;
 constexpr int kPool = 1 << kPoolLog;          // particle slots per CTA; also the capacity of every ring
-constexpr int kWords = 12;                    // state words per particle
-constexpr int kRings = 5;                     // 4 classes + free slots
-constexpr int kFree = 4;
-constexpr int kSrcReserve = 384;              // free slots that must remain for secondaries before new histories start
-constexpr int kSrcMin = 8;                    // a photon warp starts new histories once this many lanes are empty
-constexpr int kKeep = 8;                      // fewer live lanes than this and a full warp of other work waiting: hand them back
-constexpr int kTransitMin = 8;                // photons in air make the transit together once this many are waiting
-constexpr int kSpinLimit = 1 << 22;
+static_assert(kPool == kPoolSlots, "params.h and transport.cu disagree on the pool size");
+constexpr int kReserve = 3 * kPool / 8;       // free slots that must remain for secondaries when new histories start
+constexpr int kRefillMin = 8;                 // a warp refills its empty lanes once this many are empty
+constexpr int kKeepLanes = 12;                // ring exhausted and fewer live lanes than this: write back and leave the phase
+constexpr int kLongPhase = 2 * kThreads;      // phases that start with at least this many particles end softly
+constexpr int kStarved = 256;                 // fewer free slots than this: prefer phases that need none
+constexpr uint32_t kIterLimit = 1u << 20;     // iterations of one warp in one phase before it hands its particles back
+constexpr uint32_t kPhaseLimit = 1u << 24;
 constexpr float kPi = 3.14159265358979f;
 constexpr float kInf = 3.0e38f;
 constexpr uint32_t kNone = 0xffffffffu;
 
+// event classes = rings = phases
+enum : int { C_A = 0, C_W = 1, C_E = 2, C_P = 3, C_X = 4, kClasses = 5, kFree = 5, kRings = 6 };
+
 #define FULL_MASK 0xffffffffu
-// flags: bits 0-1 type, 2-3 region, 4-6 layer, 16-23 batch
+// flags: bits 0-1 type, 2-3 region, 4-6 layer, 7 collision pending (photon outside the phantom), 16-23 batch
 #define F_TYPE(f) ((f) & 3u)
 #define F_REGION(f) (((f) >> 2) & 3u)
 #define F_LAYER(f) (((f) >> 4) & 7u)
+#define F_HIT (1u << 7)
 #define F_BATCH(f) (((f) >> 16) & 255u)
 #define SET_TYPE(f, t) ((f) = ((f) & ~3u) | (t))
 #define SET_REGION(f, r) ((f) = ((f) & ~(3u << 2)) | ((r) << 2))
 #define SET_LAYER(f, l) ((f) = ((f) & ~(7u << 4)) | ((uint32_t)(l) << 4))
 
-// event class of a particle (which queue it waits in, which warps work on it):
-// 0 photon in the phantom or in air, 1 photon inside the EPID, 2 charged in the phantom, 3 charged in air / EPID
+// event class of a particle: which ring it waits in, which phase works on it
 __device__ __forceinline__ int class_of(uint32_t flags) {
-    return F_TYPE(flags) == T_PHOTON ? (F_REGION(flags) == R_EPID ? 1 : 0) : (F_REGION(flags) == R_PHANTOM ? 2 : 3);
+    const uint32_t reg = F_REGION(flags);
+    if (F_TYPE(flags) == T_PHOTON) return reg == R_PHANTOM ? C_W : ((reg == R_EPID || (flags & F_HIT)) ? C_P : C_A);
+    return reg == R_PHANTOM ? C_E : C_X;
 }
 
 // Scheduler state and the geometry copy: static shared memory, so that the out-of-line helpers reach them
 // without arguments.
-__shared__ unsigned short s_ring[kRings * kPool];   // cell = slot | generation << kPoolLog
 __shared__ unsigned int s_tail[kRings];             // tickets handed to pushers
 __shared__ unsigned int s_head[kRings];             // tickets handed to poppers
-__shared__ int s_avail[kRings];                     // committed entries not yet claimed
-__shared__ int s_flag[2];                           // [0] no histories left, [1] error
+__shared__ unsigned int s_snap[kRings];             // tail at the last barrier: pops stay below it
+__shared__ int s_flag[2];                           // [0] no histories left, [1] error bits
+__shared__ int s_phase, s_keep, s_budget, s_left;   // class of the phase (-1: done), soft-end threshold, new histories allowed, warps gone
+__shared__ unsigned int s_nphase;
 __shared__ Geom s_g;
 __shared__ float* s_ep_batch;
 __shared__ unsigned long long s_npix;
-extern __shared__ __align__(16) unsigned char smem_raw[];   // pool [kWords][kPool] u32 | per-warp ledger | table blob
+__shared__ uint4* s_pool;                           // this CTA's particle records [kPool][3]
+extern __shared__ __align__(16) unsigned char smem_raw[];   // rings [kRings][kPool] u16 | per-warp ledger | table blob
 
-__device__ __forceinline__ uint32_t* pool_base() { return reinterpret_cast<uint32_t*>(smem_raw); }
-
+__device__ __forceinline__ unsigned short* ring_cells(int r) { return reinterpret_cast<unsigned short*>(smem_raw) + r * kPool; }
 struct Shared {
     const float4* phot;
     const float* maj;
@@ -309,78 +319,62 @@ __device__ __forceinline__ void world_to_frac(const Geom& g, uint32_t vox, float
     x = fminf(fmaxf(gx, 0.0f), 1.0f); y = fminf(fmaxf(gy, 0.0f), 1.0f); z = fminf(fmaxf(gz, 0.0f), 1.0f);
 }
 
-// ---------------------------------------------------------------- queues (protocol in the header comment)
-// error bits (summed over CTAs into ledger[7]): 1 queue wait timed out, 2 no slot for a secondary, 4 particle without a slot,
-// 8 idle bound ran out
+// ---------------------------------------------------------------- rings (protocol in the header comment)
+// error bits (summed over CTAs into ledger[7]): 2 no slot for a secondary, 4 particle without a slot, 8 scheduler found no
+// runnable phase or ran out of phases
 __device__ __forceinline__ void raise_error(int bit) { atomicOr(s_flag + 1, bit); }
 
-// wait for the cell of ticket t in ring r; returns the slot (kNone if the bound ran out)
-__device__ __noinline__ uint32_t ring_take(int r, uint32_t t) {
-    const uint32_t idx = t & (kPool - 1), gen = (t >> kPoolLog) & 31u;
-    volatile unsigned short* cell = s_ring + r * kPool + idx;
-#pragma unroll 1
-    for (int spin = 0; spin < kSpinLimit; ++spin) {
-        const uint32_t v = *cell;
-        if ((v >> kPoolLog) == gen) return v & (kPool - 1);
-    }
-    raise_error(1);
-    return kNone;
-}
-// one lane appends one slot to ring r (divergent code)
+// one lane appends one slot to ring r (divergent code); visible to poppers after the next barrier
 __device__ __noinline__ void ring_push_one(int r, uint32_t slot) {
     const uint32_t t = atomicAdd(s_tail + r, 1u);
-    const uint32_t idx = t & (kPool - 1), gen = (t >> kPoolLog) & 31u;
-    *((volatile unsigned short*)(s_ring + r * kPool + idx)) = (unsigned short)(slot | (gen << kPoolLog));
-    __threadfence_block();
-    atomicAdd(s_avail + r, 1);
+    ring_cells(r)[t & (kPool - 1)] = (unsigned short)slot;
 }
-// one lane takes one entry of ring r, if there is a committed one (divergent code)
+// one lane takes one entry of ring r, if one is left below the snapshot (divergent code)
 __device__ __noinline__ uint32_t ring_pop_one(int r) {
-    if (*((volatile int*)(s_avail + r)) <= 0) return kNone;
-    if (atomicSub(s_avail + r, 1) <= 0) { atomicAdd(s_avail + r, 1); return kNone; }
-    return ring_take(r, atomicAdd(s_head + r, 1u));
+    if ((int)(s_snap[r] - *((volatile unsigned int*)(s_head + r))) <= 0) return kNone;
+    const uint32_t t = atomicAdd(s_head + r, 1u);
+    if ((int)(s_snap[r] - t) <= 0) { atomicSub(s_head + r, 1u); return kNone; }
+    return ring_cells(r)[t & (kPool - 1)];
 }
-
-// lane 0 claims up to `want` committed entries of ring r; returns count | first ticket << 32 (warp-uniform, all lanes call)
-__device__ __noinline__ unsigned long long ring_claim_packed(int r, int want) {
+// lane 0 claims up to `want` entries of ring r; returns count | first ticket << 32 (warp-uniform, all lanes call)
+__device__ __noinline__ unsigned long long ring_claim(int r, int want) {
     int n = 0; uint32_t t = 0;
-    if ((threadIdx.x & 31u) == 0) {
-        int a = *((volatile int*)(s_avail + r));
-#pragma unroll 1
-        while (a > 0) {
-            n = min(a, want);
-            const int old = atomicCAS(s_avail + r, a, a - n);
-            if (old == a) break;
-            a = old; n = 0;
-        }
-        if (a <= 0) n = 0;
-        if (n > 0) t = atomicAdd(s_head + r, (unsigned)n);
+    if ((threadIdx.x & 31u) == 0 && want > 0 && (int)(s_snap[r] - *((volatile unsigned int*)(s_head + r))) > 0) {
+        t = atomicAdd(s_head + r, (unsigned)want);
+        n = min(max((int)(s_snap[r] - t), 0), want);
+        if (n < want) atomicSub(s_head + r, (unsigned)(want - n));
     }
     n = __shfl_sync(FULL_MASK, n, 0);
     t = __shfl_sync(FULL_MASK, t, 0);
     return (unsigned long long)(uint32_t)n | ((unsigned long long)t << 32);
 }
+// lane 0 claims up to `want` of the new histories this phase may start (warp-uniform, all lanes call)
+__device__ __noinline__ int budget_claim(int want) {
+    int n = 0;
+    if ((threadIdx.x & 31u) == 0 && want > 0 && *((volatile int*)&s_budget) > 0) {
+        const int b = atomicSub(&s_budget, want);
+        n = min(max(b, 0), want);
+        if (n < want) atomicAdd(&s_budget, want - n);
+    }
+    return __shfl_sync(FULL_MASK, n, 0);
+}
 
-// Store a particle record in pool slot `slot` and append the slot to the queue of the particle's class.
+// Store a particle record in pool slot `slot` and append the slot to the ring of the particle's class.
 __device__ __noinline__ void queue_particle(uint32_t slot, float x, float y, float z, float dx, float dy, float dz, float E,
                                             uint32_t vox, uint32_t flags, uint32_t h, uint32_t pid, uint32_t blk) {
-    uint32_t* p = pool_base() + slot;
-    p[0 * kPool] = __float_as_uint(x);  p[1 * kPool] = __float_as_uint(y);  p[2 * kPool] = __float_as_uint(z);
-    p[3 * kPool] = __float_as_uint(dx); p[4 * kPool] = __float_as_uint(dy); p[5 * kPool] = __float_as_uint(dz);
-    p[6 * kPool] = __float_as_uint(E);  p[7 * kPool] = vox; p[8 * kPool] = flags;
-    p[9 * kPool] = h; p[10 * kPool] = pid; p[11 * kPool] = blk;
-    __threadfence_block();
+    uint4* rec = s_pool + (size_t)slot * 3;
+    __stcg(rec + 0, make_uint4(__float_as_uint(x), __float_as_uint(y), __float_as_uint(z), __float_as_uint(dx)));
+    __stcg(rec + 1, make_uint4(__float_as_uint(dy), __float_as_uint(dz), __float_as_uint(E), vox));
+    __stcg(rec + 2, make_uint4(flags, h, pid, blk));
     ring_push_one(class_of(flags), slot);
 }
-// Slot discipline: every particle owns a pool slot from birth, so handing it over never needs a new one; a lane
-// keeps at most one SPARE free slot (the slot of a particle that died in it, else one from the free ring) and only
-// runs an event that can create a secondary while it holds one.  Hence the pool cannot overflow: when the free ring
-// runs dry the photon lanes wait, the charged-particle warps drain the queues and slots come back.
+// A lane keeps at most one SPARE free slot (the slot of a particle that died in it, else one from the free ring)
+// and only runs an event that can create a secondary while it holds one (header comment, "slot discipline").
 __device__ __forceinline__ bool ensure_spare(Lane& L) {
     if (L.spare == kNone) L.spare = ring_pop_one(kFree);
     return L.spare != kNone;
 }
-// A secondary goes straight into the pool (the lane's spare slot) and into the queue of its class.  Without a spare
+// A secondary goes straight into the pool (the lane's spare slot) and into the ring of its class.  Without a spare
 // (cannot happen: see ensure_spare; flagged) its energy is booked as escaped so that the ledger still closes.
 __device__ __forceinline__ void spawn_from(Lane& L, float x, float y, float z, float dx, float dy, float dz, float E,
                                            uint32_t flags, uint32_t pid) {
@@ -388,7 +382,6 @@ __device__ __forceinline__ void spawn_from(Lane& L, float x, float y, float z, f
     if (s == kNone) { raise_error(2); L.a_esc += E + (F_TYPE(flags) == T_POSITRON ? 2.0f * kMec2 : 0.0f); return; }
     queue_particle(s, x, y, z, dx, dy, dz, E, L.vox, flags, L.h, pid, 0u);
 }
-
 // Two 0.511 MeV photons, isotropic and back to back (reading A11): the lane becomes the first, the second is spawned.
 // Position must already be in the frame photons use in this region.
 __device__ __forceinline__ void annihilate(Lane& L, const TransportParams& P) {
@@ -777,64 +770,202 @@ __device__ __forceinline__ void ledger_flush(Lane& L, double* led) {
     L.a_emit = L.a_ph = L.a_eps = L.a_epo = L.a_air = L.a_esc = 0.0f;
 }
 
-// Scheduler state changes under the warp's feet: every decision taken on it is made by lane 0 and broadcast, so that
-// the warp never splits on it.
-enum Decision { D_GO = 0, D_SOURCE = 1, D_RESELECT = 2, D_EVICT = 3 };
-__device__ __forceinline__ bool can_source(const volatile int* q, int lanes) {
-    return *((volatile int*)s_flag) == 0 && q[kFree] >= lanes + kSrcReserve;
-}
-// A warp of class wcls has `a` < 32 live lanes after the refill attempt: what now?
-__device__ __noinline__ int decide(int a, int wcls, uint32_t it) {
-    int d = D_GO;
-    if ((threadIdx.x & 31u) == 0) {
-        const volatile int* q = s_avail;
-        if (wcls == 0 && 32 - a >= kSrcMin && can_source(q, 32)) d = D_SOURCE;
-        else if (a == 0) d = D_RESELECT;
-        else if (a < kKeep && (it & 3u) == 0u && (q[0] >= 32 || q[1] >= 32 || q[2] >= 32 || q[3] >= 32 || can_source(q, 32))) d = D_EVICT;
+// Thread 0, between two barriers: publish what the last phase pushed (snapshot of every tail) and pick the next
+// phase: new histories (class A) while the pool has room for a full wave of them, else the class with the most
+// waiting particles.  W and P need free slots for their secondaries, so they wait while the pool is nearly full and
+// another class can run (E and X give slots back).
+__device__ __noinline__ void choose_phase(const TransportParams& P, unsigned long long* phase_count) {
+    int n[kRings];
+#pragma unroll
+    for (int r = 0; r < kRings; ++r) { s_snap[r] = s_tail[r]; n[r] = (int)(s_snap[r] - s_head[r]); }
+    const int nf = n[kFree];
+    bool more = s_flag[0] == 0;
+    int budget = 0;
+    if (more) {
+        const uint32_t done = *((volatile unsigned int*)P.hist_counter);
+        const uint32_t left = done < P.n ? P.n - done : 0u;
+        if (left == 0u) { more = false; s_flag[0] = 1; }
+        // towards the end of the launch take no more than a share of what is left, so that the CTAs finish together
+        const uint32_t share = max(left / (2u * gridDim.x), (uint32_t)kThreads);
+        budget = (int)min((uint32_t)max(nf - kReserve, 0), share);
     }
-    return __shfl_sync(FULL_MASK, d, 0);
-}
-// A warp with no particles picks its next class: 0..3 a queue (the fullest; charged particles first when the pool is
-// nearly exhausted), 4 new histories, 5 nothing to do right now, 6 nothing left at all.
-__device__ __noinline__ int pick_class() {
-    int d = 5;
-    if ((threadIdx.x & 31u) == 0) {
-        const volatile int* q = s_avail;
-        const int a0 = q[0], a1 = q[1], a2 = q[2], a3 = q[3], af = q[kFree];
-        int best = 0, ab = a0;
-        if (a1 > ab) { ab = a1; best = 1; }
-        if (a2 > ab) { ab = a2; best = 2; }
-        if (a3 > ab) { ab = a3; best = 3; }
-        if (af < 128 && (a2 > 0 || a3 > 0)) { best = a2 >= a3 ? 2 : 3; ab = 32; }
-        const bool src_done = *((volatile int*)s_flag) != 0;
-        if (ab >= 32) d = best;
-        else if (!src_done && af >= 32 + kSrcReserve) d = 4;
-        else if (ab > 0) d = best;
-        else if (src_done && af == kPool) d = 6;
+    int ph = -1;
+    if (more && budget >= kThreads) ph = C_A;
+    else {
+        const bool starved = nf < kStarved && (n[C_E] + n[C_X] + n[C_A]) > 0;
+        int nb = 0;
+#pragma unroll
+        for (int c = 0; c < kClasses; ++c) {
+            if (starved && (c == C_W || c == C_P)) continue;
+            if (n[c] > nb) { nb = n[c]; ph = c; }
+        }
+        if (ph >= 0) budget = 0;
+        else if (more && budget > 0) ph = C_A;                 // fewer histories left than lanes
+        else if (more) raise_error(8);                         // cannot happen: nothing queued, yet no room for a history
     }
-    return __shfl_sync(FULL_MASK, d, 0);
+    if (ph >= 0 && ++s_nphase > kPhaseLimit) { raise_error(8); ph = -1; }
+    s_phase = ph; s_left = 0; s_budget = ph == C_A ? budget : 0;
+    const int n_start = ph < 0 ? 0 : n[ph] + (ph == C_A ? budget : 0);
+    s_keep = n_start >= kLongPhase ? kKeepLanes : 0;
+    if (phase_count && ph >= 0) atomicAdd(phase_count, 1ull);
+}
+
+// One phase of class C for one warp (header comment).  On return every lane is empty and holds no slot.
+template <bool COUNT, int C>
+__device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, const Shared& sh, double* led, uint32_t* cnt) {
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    constexpr bool kSpawns = C == C_W || C == C_P;             // classes whose events create secondaries all the time
+    const int keep = *((volatile int*)&s_keep);
+    bool leaving = false, park = false;
+#pragma unroll 1
+    for (uint32_t it = 1;; ++it) {
+        // ---- A: particles that left the class (or all of them, when the warp leaves) go to the ring of their class;
+        //         the slot of a dead particle becomes the lane's spare or goes back to the free ring
+        if (!(L.alive && !leaving && !park && class_of(L.flags) == C)) {
+            flush_pending(L, P);
+            if (L.alive) {
+                if (L.slot == kNone) {                                     // cannot happen (flagged): drop, ledger still closes
+                    raise_error(4);
+                    L.a_esc += L.E + (F_TYPE(L.flags) == T_POSITRON ? 2.0f * kMec2 : 0.0f);
+                } else queue_particle(L.slot, L.x, L.y, L.z, L.dx, L.dy, L.dz, L.E, L.vox, L.flags, L.h, L.pid, L.blk);
+                if (COUNT) cnt[27]++;
+                L.alive = false; L.slot = kNone;
+            } else if (L.slot != kNone) {
+                if (kSpawns && !leaving && L.spare == kNone) L.spare = L.slot; else ring_push_one(kFree, L.slot);
+                L.slot = kNone;
+            }
+            park = false;
+        }
+        if (leaving) break;
+        // ---- B: refill the empty lanes from the ring of the class; class A then starts new histories
+        unsigned empty = __ballot_sync(FULL_MASK, !L.alive);
+        if (__popc(empty) >= kRefillMin) {
+            const unsigned long long cl = ring_claim(C, __popc(empty));
+            const int got = (int)(uint32_t)cl;
+            const int rk = __popc(empty & lt_mask);
+            if (!L.alive && rk < got) {
+                const uint32_t s = ring_cells(C)[((uint32_t)(cl >> 32) + (uint32_t)rk) & (kPool - 1)];
+                const uint4* rec = s_pool + (size_t)s * 3;
+                const uint4 a = __ldcg(rec), b = __ldcg(rec + 1), c = __ldcg(rec + 2);
+                L.x = __uint_as_float(a.x); L.y = __uint_as_float(a.y); L.z = __uint_as_float(a.z); L.dx = __uint_as_float(a.w);
+                L.dy = __uint_as_float(b.x); L.dz = __uint_as_float(b.y); L.E = __uint_as_float(b.z); L.vox = b.w;
+                L.flags = c.x; L.h = c.y; L.pid = c.z; L.blk = c.w;
+                L.slot = s; L.alive = true;
+                L.pval = 0.0f; L.pidx = kNone;
+                if (COUNT) cnt[28]++;
+                if (C == C_A || C == C_W || C == C_P) set_energy(L, P, sh);
+                if (C == C_E) { L.vlin = vox_linear(P.g, L.vox); L.cw = __ldg(P.vox + L.vlin); }
+            }
+            if (C == C_A) {
+                // K1: new histories in the lanes that are still empty, one free slot each
+                empty = __ballot_sync(FULL_MASK, !L.alive);
+                int nd = budget_claim(__popc(empty));
+                if (nd > 0) {
+                    const unsigned long long fl = ring_claim(kFree, nd);
+                    const int nslots = (int)(uint32_t)fl;                  // = nd: the budget never exceeds the free slots below the snapshot
+                    const int rk2 = __popc(empty & lt_mask);
+                    uint32_t h0 = 0;
+                    if (lane == 0) h0 = atomicAdd(P.hist_counter, (unsigned)nslots);
+                    h0 = __shfl_sync(FULL_MASK, h0, 0);
+                    if (!L.alive && rk2 < nslots) {
+                        const uint32_t myslot = ring_cells(kFree)[((uint32_t)(fl >> 32) + (uint32_t)rk2) & (kPool - 1)];
+                        const uint32_t h = h0 + (uint32_t)rk2;
+                        if (h >= P.n) { ring_push_one(kFree, myslot); atomicExch(s_flag, 1); }
+                        else {
+                            L.h = h; L.pid = 0; L.blk = 0;
+                            const uint4 r = rng_block(L, P);               // block 0 of particle 0: E, pixel, u, v (reading A1)
+                            const SourceSample s = sample_source(P, r.x, r.y, r.z, r.w);
+                            L.x = P.g.src[0]; L.y = P.g.src[1]; L.z = P.g.src[2];
+                            L.dx = s.dx; L.dy = s.dy; L.dz = s.dz; L.E = s.E;
+                            L.vox = 0;
+                            L.flags = T_PHOTON | (R_AIR << 2) | (min(h / P.hist_per_batch, (uint32_t)P.n_batches - 1u) << 16);
+                            L.alive = true; L.slot = myslot;
+                            L.pval = 0.0f; L.pidx = kNone;
+                            L.a_emit += s.E;
+                            set_energy(L, P, sh);
+                        }
+                    }
+                    if (COUNT && lane == 0) cnt[30]++;
+                }
+            }
+        }
+        // ---- C: leave the phase?
+        const int n_live = __popc(__ballot_sync(FULL_MASK, L.alive));
+        int go = 0;                                                        // 0 carry on, 1 nothing to do right now, 2 write back and leave, 3 leave
+        if (lane == 0) {
+            bool dry = (int)(s_snap[C] - *((volatile unsigned int*)(s_head + C))) <= 0;
+            if (C == C_A && *((volatile int*)&s_budget) > 0 && *((volatile int*)s_flag) == 0) dry = false;
+            if (n_live == 0) go = dry ? 3 : 1;
+            else if (it >= kIterLimit) go = 2;
+            else if (dry && keep > 0 && (n_live < keep || 2 * *((volatile int*)&s_left) >= kWarps)) go = 2;
+        }
+        go = __shfl_sync(FULL_MASK, go, 0);
+        if (go == 3) break;
+        if (go == 2) { leaving = true; continue; }
+        if (go == 1) continue;
+        // ---- D: one event per live lane
+        if (COUNT) { if (lane == 0) cnt[16 + C]++; if (L.alive) cnt[21 + C]++; }
+        bool on = L.alive;
+        if (C == C_W || C == C_P) {
+            if (on && !ensure_spare(L)) { park = true; on = false; if (COUNT) cnt[29]++; }   // an interaction may create a secondary
+        } else if (C == C_E || C == C_X) {
+            if (on && F_TYPE(L.flags) == T_POSITRON && L.E <= P.ph.ecut && !ensure_spare(L)) { park = true; on = false; if (COUNT) cnt[29]++; }   // annihilation needs a slot
+        }
+        if (on) {
+            if (C == C_E) charged_event<COUNT, true>(L, P, sh, cnt);
+            else if (C == C_X) charged_event<COUNT, false>(L, P, sh, cnt);
+            else if (L.E < P.ph.pcut) { if (COUNT) cnt[13]++; dep_here(L, P, L.E); L.alive = false; }   // PAPER.md:104, 10 keV
+            else {
+                bool hit = false; float xsel = 0.0f, pe = 0.0f, co = 0.0f;
+                if (C == C_A) {
+                    if (air_transit<COUNT>(L, P, sh, xsel, pe, co, cnt)) L.flags |= F_HIT;   // collision in air or in a layer: class P
+                } else if (C == C_W) {
+                    hit = woodcock_flight<COUNT>(L, P, sh, xsel, pe, co, cnt);
+                } else {
+                    if (L.flags & F_HIT) {                                 // collision found by the transit: channel from a fresh draw (reading A8)
+                        L.flags &= ~F_HIT;
+                        const bool in_air = F_REGION(L.flags) == R_AIR;
+                        float pp;
+                        mu3(P, sh, in_air ? 0 : P.g.lmat[F_LAYER(L.flags)], L.ci, L.ct, pe, co, pp);
+                        xsel = u01(rng_block(L, P).x) * (pe + co + pp);
+                        hit = true;
+                    } else hit = epid_flight<COUNT>(L, P, sh, xsel, pe, co, cnt);
+                }
+                if (hit) interact<COUNT>(L, P, sh, xsel, pe, co, cnt);
+            }
+        }
+        // ---- E: ledger of the last iterations: float per lane -> warp sum -> the warp's double accumulators
+        if ((it & 63u) == 0u) ledger_flush(L, led);
+    }
+    if (L.spare != kNone) { ring_push_one(kFree, L.spare); L.spare = kNone; }
+    ledger_flush(L, led);
+    if (lane == 0) atomicAdd(&s_left, 1);
 }
 
 template <bool COUNT>
 __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_constant__ TransportParams P) {
-    // dynamic shared memory: pool | per-warp ledger | table blob
-    double* const led_all = reinterpret_cast<double*>(smem_raw + (size_t)kWords * kPool * 4);
-    uint32_t* const blob = reinterpret_cast<uint32_t*>(smem_raw + (size_t)kWords * kPool * 4 + kWarps * 8 * sizeof(double));
+    // dynamic shared memory: rings | per-warp ledger | table blob
+    constexpr size_t kRingBytes = (size_t)kRings * kPool * sizeof(unsigned short);
+    double* const led_all = reinterpret_cast<double*>(smem_raw + kRingBytes);
+    uint32_t* const blob = reinterpret_cast<uint32_t*>(smem_raw + kRingBytes + kWarps * 8 * sizeof(double));
     for (int i = threadIdx.x; i < P.tb.blob_words; i += kThreads) blob[i] = __ldg(P.tb.blob + i);
     Shared sh;
     sh.phot = reinterpret_cast<const float4*>(blob);
     sh.maj = reinterpret_cast<const float*>(sh.phot + P.tb.n_mat * P.tb.n_E);
     sh.lnS = sh.maj + P.tb.n_E;
     sh.invX0 = sh.lnS + P.tb.n_mat * P.tb.n_T;
-    for (int i = threadIdx.x; i < kRings * kPool; i += kThreads)
-        s_ring[i] = (unsigned short)(i >= kFree * kPool ? (i - kFree * kPool) : 0xffff);    // free ring: slot i, generation 0
+    for (int i = threadIdx.x; i < kPool; i += kThreads) ring_cells(kFree)[i] = (unsigned short)i;
     for (int i = threadIdx.x; i < kWarps * 8; i += kThreads) led_all[i] = 0.0;
     if (threadIdx.x < kRings) {
         const bool fr = threadIdx.x == kFree;
-        s_tail[threadIdx.x] = fr ? kPool : 0u; s_head[threadIdx.x] = 0u; s_avail[threadIdx.x] = fr ? kPool : 0;
+        s_tail[threadIdx.x] = fr ? kPool : 0u; s_head[threadIdx.x] = 0u; s_snap[threadIdx.x] = 0u;
     }
     if (threadIdx.x < 2) s_flag[threadIdx.x] = 0;
-    if (threadIdx.x == 0) { s_g = P.g; s_ep_batch = P.ep_batch; s_npix = P.npix; }
+    if (threadIdx.x == 0) {
+        s_g = P.g; s_ep_batch = P.ep_batch; s_npix = P.npix; s_nphase = 0u;
+        s_pool = P.pool + (size_t)blockIdx.x * kPool * 3;
+    }
     __syncthreads();
 
     uint32_t cnt[COUNT ? 32 : 1];
@@ -843,153 +974,29 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
         for (int i = 0; i < 32; ++i) cnt[i] = 0;
     }
     const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    const unsigned lt_mask = (1u << lane) - 1u;
     double* const led = led_all + warp * 8;
     Lane L;
     L.x = L.y = L.z = 0.0f; L.dx = L.dy = 0.0f; L.dz = 1.0f; L.E = 0.0f; L.vox = 0; L.flags = 0; L.h = L.pid = L.blk = 0;
     L.cw = 0; L.vlin = 0; L.ci = 0; L.ct = 0.0f; L.mumaj = 1.0f;
     L.pval = 0.0f; L.pidx = kNone; L.slot = kNone; L.spare = kNone; L.alive = false;
     L.a_emit = L.a_ph = L.a_eps = L.a_epo = L.a_air = L.a_esc = 0.0f;
-    int wcls = 0;           // event class this warp works on (warp-uniform)
-    bool evict = false;     // hand every particle back at the top of the next iteration
-    bool drain = false;     // ... and then take other work instead of refilling (the free ring ran dry)
-    int idle = 0;
 
-    for (uint32_t it = 1;; ++it) {
-        // ---- A: particles that left the class go to the queue of their new class; the slot of a dead particle becomes the lane's spare
-        if (!(L.alive && !evict && class_of(L.flags) == wcls)) {
-            flush_pending(L, P);
-            if (L.alive) {
-                const uint32_t s = L.slot;
-                if (s == kNone) {                                          // cannot happen (flagged): drop, ledger still closes
-                    raise_error(4);
-                    L.a_esc += L.E + (F_TYPE(L.flags) == T_POSITRON ? 2.0f * kMec2 : 0.0f);
-                } else queue_particle(s, L.x, L.y, L.z, L.dx, L.dy, L.dz, L.E, L.vox, L.flags, L.h, L.pid, L.blk);
-                if (COUNT) cnt[23]++;
-                L.alive = false; L.slot = kNone;
-            } else if (L.slot != kNone) {
-                if (wcls < 2 && L.spare == kNone) L.spare = L.slot; else ring_push_one(kFree, L.slot);   // photon lanes keep one spare
-                L.slot = kNone;
-            }
+#pragma unroll 1
+    for (;;) {
+        if (threadIdx.x == 0) choose_phase(P, COUNT ? P.counters + 26 : nullptr);
+        __syncthreads();
+        const int ph = s_phase;
+        if (ph < 0) break;
+        switch (ph) {
+            case C_A: run_phase<COUNT, C_A>(L, P, sh, led, cnt); break;
+            case C_W: run_phase<COUNT, C_W>(L, P, sh, led, cnt); break;
+            case C_E: run_phase<COUNT, C_E>(L, P, sh, led, cnt); break;
+            case C_P: run_phase<COUNT, C_P>(L, P, sh, led, cnt); break;
+            default:  run_phase<COUNT, C_X>(L, P, sh, led, cnt); break;
         }
-        evict = false;
-        // ---- B: empty lanes refill from the queue of the class
-        if (!L.alive && !drain && *((volatile int*)(s_avail + wcls)) > 0) {
-            const uint32_t s = ring_pop_one(wcls);
-            if (s != kNone) {
-                const uint32_t* p = pool_base() + s;
-                L.x = __uint_as_float(p[0 * kPool]); L.y = __uint_as_float(p[1 * kPool]); L.z = __uint_as_float(p[2 * kPool]);
-                L.dx = __uint_as_float(p[3 * kPool]); L.dy = __uint_as_float(p[4 * kPool]); L.dz = __uint_as_float(p[5 * kPool]);
-                L.E = __uint_as_float(p[6 * kPool]); L.vox = p[7 * kPool]; L.flags = p[8 * kPool];
-                L.h = p[9 * kPool]; L.pid = p[10 * kPool]; L.blk = p[11 * kPool];
-                L.slot = s; L.alive = true;
-                L.pval = 0.0f; L.pidx = kNone;
-                if (COUNT) cnt[24]++;
-                if (F_TYPE(L.flags) == T_PHOTON) set_energy(L, P, sh);
-                else if (F_REGION(L.flags) == R_PHANTOM) { L.vlin = vox_linear(P.g, L.vox); L.cw = __ldg(P.vox + L.vlin); }
-            }
-        }
-        // ---- C: lanes still empty: start new histories, take another class, or carry on
-        const unsigned live = __ballot_sync(FULL_MASK, L.alive);
-        const int n_live = __popc(live);
-        if (drain || n_live == 0 || (wcls == 0 && 32 - n_live >= kSrcMin) || (n_live < kKeep && (it & 3u) == 0u)) {
-            const int dec = drain ? D_RESELECT : decide(n_live, wcls, it);
-            drain = false;
-            if (dec == D_SOURCE) {
-                // K1: new histories in the empty lanes
-                const unsigned long long cl = ring_claim_packed(kFree, 32 - __popc(live));   // one slot per new history
-                const int nd = (int)(uint32_t)cl;   // (32 - n_live at most)
-                const int rk = __popc(~live & lt_mask);
-                uint32_t myslot = kNone;
-                if (!L.alive && rk < nd) myslot = ring_take(kFree, (uint32_t)(cl >> 32) + (uint32_t)rk);
-                uint32_t h0 = 0;
-                if (lane == 0 && nd > 0) h0 = atomicAdd(P.hist_counter, (unsigned)nd);
-                h0 = __shfl_sync(FULL_MASK, h0, 0);
-                if (nd > 0 && h0 >= P.n && lane == 0) atomicExch(s_flag, 1);
-                {
-                    if (COUNT && lane == 0) cnt[21]++;
-                    const uint32_t h = h0 + (uint32_t)rk;
-                    if (myslot != kNone && h >= P.n) { ring_push_one(kFree, myslot); myslot = kNone; }
-                    if (myslot != kNone) {
-                        L.h = h; L.pid = 0; L.blk = 0;
-                        const uint4 r = rng_block(L, P);                   // block 0 of particle 0: E, pixel, u, v (reading A1)
-                        const SourceSample s = sample_source(P, r.x, r.y, r.z, r.w);
-                        L.x = P.g.src[0]; L.y = P.g.src[1]; L.z = P.g.src[2];
-                        L.dx = s.dx; L.dy = s.dy; L.dz = s.dz; L.E = s.E;
-                        L.vox = 0;
-                        L.flags = T_PHOTON | (R_AIR << 2) | (min(h / P.hist_per_batch, (uint32_t)P.n_batches - 1u) << 16);
-                        L.alive = true; L.slot = myslot;
-                        L.pval = 0.0f; L.pidx = kNone;
-                        L.a_emit += s.E;
-                        set_energy(L, P, sh);
-                    }
-                }
-                idle = 0;
-            } else if (dec == D_RESELECT) {
-                ledger_flush(L, led);
-                const int pc = pick_class();
-                if (COUNT && lane == 0) cnt[27]++;
-                if (pc < 4) {
-                    wcls = pc; idle = 0;
-                    if (pc >= 2 && L.spare != kNone) { ring_push_one(kFree, L.spare); L.spare = kNone; }   // charged-particle warps need no spares
-                }
-                else if (pc == 4) { wcls = 0; idle = 0; }
-                else {
-                    if (L.spare != kNone) { ring_push_one(kFree, L.spare); L.spare = kNone; }   // idle: give the spare slots back
-                    if (pc == 6) break;                                    // nothing queued, nothing in flight, nothing left to start
-                    if (++idle > kSpinLimit) { raise_error(8); break; }
-                    if (COUNT && lane == 0) cnt[22]++;
-                    __nanosleep(200);
-                }
-                continue;
-            } else if (dec == D_EVICT) {
-                evict = true;
-                if (COUNT && lane == 0) cnt[28]++;
-            }
-        }
-        // ---- D: one event per live lane
-        if (COUNT && lane == 0) cnt[16]++;
-        if (wcls < 2) {
-            bool on = L.alive && class_of(L.flags) == wcls;
-            if (on && !ensure_spare(L)) on = false;                        // an interaction may create a secondary: wait for a slot
-            if (__ballot_sync(FULL_MASK, on) == 0u) { evict = true; drain = true; continue; }   // every photon waits for a slot: drain queues instead
-            bool hit = false; float xsel = 0.0f, pe = 0.0f, co = 0.0f;
-            if (COUNT) { if (lane == 0) cnt[17]++; if (on) cnt[18]++; }
-            if (wcls == 0) {
-                // photons in AIR wait until enough of them can make the transit together
-                const bool in_air = on && F_REGION(L.flags) == R_AIR;
-                const unsigned m_air = __ballot_sync(FULL_MASK, in_air), m_on = __ballot_sync(FULL_MASK, on);
-                const bool do_air = __popc(m_air) >= kTransitMin || m_air == m_on;
-                if (on && L.E < P.ph.pcut) { if (COUNT) cnt[13]++; dep_here(L, P, L.E); L.alive = false; }   // PAPER.md:104, 10 keV
-                else if (on && !in_air) hit = woodcock_flight<COUNT>(L, P, sh, xsel, pe, co, cnt);
-                else if (in_air && do_air) {
-                    if (COUNT) { cnt[26]++; }
-                    hit = air_transit<COUNT>(L, P, sh, xsel, pe, co, cnt);
-                }
-                if (COUNT && lane == 0 && do_air && m_air) cnt[25]++;
-            } else {
-                if (on && L.E < P.ph.pcut) { if (COUNT) cnt[13]++; dep_here(L, P, L.E); L.alive = false; }
-                else if (on) hit = epid_flight<COUNT>(L, P, sh, xsel, pe, co, cnt);
-            }
-            if (hit) interact<COUNT>(L, P, sh, xsel, pe, co, cnt);
-        } else if (wcls == 2) {
-            bool on = L.alive && class_of(L.flags) == 2;
-            if (on && F_TYPE(L.flags) == T_POSITRON && L.E <= P.ph.ecut && !ensure_spare(L)) on = false;   // annihilation needs a slot
-            if (COUNT) { if (lane == 0) cnt[19]++; if (on) cnt[20]++; }
-            if (on) charged_event<COUNT, true>(L, P, sh, cnt);
-        } else {
-            bool on = L.alive && class_of(L.flags) == 3;
-            if (on && F_TYPE(L.flags) == T_POSITRON && L.E <= P.ph.ecut && !ensure_spare(L)) on = false;
-            if (COUNT) { if (lane == 0) cnt[19]++; if (on) cnt[20]++; }
-            if (on) charged_event<COUNT, false>(L, P, sh, cnt);
-        }
-        // ---- E: ledger of the last iterations: float per lane -> warp sum -> the warp's double accumulators
-        if ((it & 63u) == 0u) ledger_flush(L, led);
+        __syncthreads();
     }
-    flush_pending(L, P);
-    ledger_flush(L, led);
 
-    __syncthreads();
     if (threadIdx.x < 6) {
         double v = 0.0;
         for (int w = 0; w < kWarps; ++w) v += led_all[w * 8 + threadIdx.x];
@@ -1007,19 +1014,20 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
     }
 }
 
+constexpr size_t kDynSmemFixed = (size_t)kRings * kPool * sizeof(unsigned short) + kWarps * 8 * sizeof(double);
+
 size_t transport_smem_bytes(const Tables& t) {      // dynamic + static shared memory of the kernel
-    return (size_t)kWords * kPool * 4 + kWarps * 8 * sizeof(double) + (size_t)t.blob_words * 4 +
-           sizeof(unsigned short) * kRings * kPool + sizeof(Geom) + 256;
+    return kDynSmemFixed + (size_t)t.blob_words * 4 + sizeof(Geom) + 512;
 }
 
 int launch_transport(const TransportParams& p, bool counting, int sm_count, void* stream) {
-    const size_t smem = (size_t)kWords * kPool * 4 + kWarps * 8 * sizeof(double) + (size_t)p.tb.blob_words * 4;
+    const size_t smem = kDynSmemFixed + (size_t)p.tb.blob_words * 4;
     cudaError_t e;
     if (counting) e = cudaFuncSetAttribute(transport_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     else e = cudaFuncSetAttribute(transport_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return (int)e;
-    // persistent grid: one CTA per SM, but no more CTAs than there is work for
-    long long blocks = sm_count;
+    // persistent grid: one CTA per SM (each with its own slice of the particle pool), but no more CTAs than there is work for
+    long long blocks = sm_count < kMaxCtas ? sm_count : kMaxCtas;
     const long long need = ((long long)p.n + 255) / 256;
     if (blocks > need) blocks = need;
     if (blocks < 1) blocks = 1;
@@ -1027,7 +1035,6 @@ int launch_transport(const TransportParams& p, bool counting, int sm_count, void
     else transport_kernel<false><<<(unsigned)blocks, kThreads, smem, (cudaStream_t)stream>>>(p);
     return (int)cudaGetLastError();
 }
-
 // K1 alone (aepid_sample_source): out[k] = {E, dx, dy, dz, pixel, u, v, 0} for history first + k
 __global__ void sample_source_kernel(const __grid_constant__ TransportParams P, uint64_t first, uint64_t n, float* __restrict__ out) {
     const uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
