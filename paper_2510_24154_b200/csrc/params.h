@@ -13,9 +13,13 @@ constexpr float kRhoAir = 1.205e-3f;  // world filler, material 0 (SURVEY 8(c) "
 constexpr float kWorldHalf = 100.0f;  // |u|, |v| <= 100 cm
 constexpr float kWorldWMin = -1.0f;   // -1 <= w
 constexpr float kMec2 = 0.51099895f;
-constexpr int kPoolSlots = 8192;      // particle records per CTA of the transport kernel (transport.cu)
+#ifndef AEPID_POOL_LOG
+#define AEPID_POOL_LOG 16
+#endif
+constexpr int kPoolSlots = 1 << AEPID_POOL_LOG;   // particle records per CTA of the transport kernel (transport.cu), at most 65536
+constexpr int kRingCount = 6;         // slot-index rings per CTA: five event classes and the free slots
 constexpr int kRecordBytes = 48;      // three 16-byte vectors per particle
-constexpr int kMaxCtas = 192;         // CTAs of the transport kernel the workspace provides a pool for (one per SM)
+constexpr int kMaxCtas = 160;         // CTAs of the transport kernel the workspace provides a pool for (one per SM)
 
 enum Region : uint32_t { R_AIR = 0, R_PHANTOM = 1, R_EPID = 2 };
 enum PType : uint32_t { T_PHOTON = 0, T_ELECTRON = 1, T_POSITRON = 2 };
@@ -73,6 +77,7 @@ struct TransportParams {
     unsigned long long* counters;      // [32]
     unsigned int* hist_counter;        // next history of this launch that has not been started
     uint4* pool;                       // particle records [kMaxCtas][kPoolSlots][3], scratch of one launch
+    unsigned short* rings;             // slot-index rings [kMaxCtas][kRingCount][kPoolSlots], scratch of one launch
     uint64_t base;                     // global index of relative history 0 of this launch
     uint64_t seed;
     uint32_t n;                        // histories in this launch (< 2^32)

@@ -24,9 +24,10 @@
 //     tickets from head but only below the SNAPSHOT of tail taken at the last barrier, so a cell is never read
 //     before the barrier that publishes it and no generation tags or spin waits are needed.  What is pushed during a
 //     phase (also into the phase's own ring: parked or evicted particles) becomes visible in the next phase.
-//   * A phase ends softly: once its ring is exhausted a warp with fewer than kKeepLanes live lanes, or any warp
-//     after half of the warps have gone, writes its particles back and leaves; the survivors join the next phase of
-//     their class.  Phases that start with fewer than two waves of particles run until every lane is dry.
+//   * A phase ends softly: a warp that can no longer keep its lanes full (ring exhausted, kRefillMin lanes empty)
+//     writes its particles back and leaves, so all warps reach the barrier within about one event of each other and
+//     the survivors join the next phase of their class (a write-back and reload costs a fraction of one event).
+//     Phases that start with fewer than two waves of particles run until every lane is dry.
 //   * Slot discipline: every particle owns a pool slot from birth, so writing it back never needs a new one; a lane
 //     runs an event that can create a secondary only while it holds a spare slot, otherwise it parks its particle.
 //     New histories start only while kReserve slots stay free.  Hence the pool cannot overflow.
@@ -44,12 +45,17 @@ namespace aepid {
 
 constexpr int kWarps = 24;
 constexpr int kThreads = kWarps * 32;
-constexpr int kPoolLog = 13;
+constexpr int kPoolLog = AEPID_POOL_LOG;
 constexpr int kPool = 1 << kPoolLog;          // particle slots per CTA; also the capacity of every ring
-static_assert(kPool == kPoolSlots, "params.h and transport.cu disagree on the pool size");
-constexpr int kReserve = 3 * kPool / 8;       // free slots that must remain for secondaries when new histories start
-constexpr int kRefillMin = 8;                 // a warp refills its empty lanes once this many are empty
-constexpr int kKeepLanes = 12;                // ring exhausted and fewer live lanes than this: write back and leave the phase
+static_assert(kPool == kPoolSlots && kPool <= 65536, "ring cells are 16-bit slot indices");
+#ifndef AEPID_RESERVE_8THS
+#define AEPID_RESERVE_8THS 3
+#endif
+#ifndef AEPID_REFILL_MIN
+#define AEPID_REFILL_MIN 8
+#endif
+constexpr int kReserve = AEPID_RESERVE_8THS * kPool / 8;       // free slots that must remain for secondaries when new histories start
+constexpr int kRefillMin = AEPID_REFILL_MIN;                 // a warp refills its empty lanes once this many are empty
 constexpr int kLongPhase = 2 * kThreads;      // phases that start with at least this many particles end softly
 constexpr int kStarved = 256;                 // fewer free slots than this: prefer phases that need none
 constexpr uint32_t kIterLimit = 1u << 20;     // iterations of one warp in one phase before it hands its particles back
@@ -59,7 +65,7 @@ constexpr float kInf = 3.0e38f;
 constexpr uint32_t kNone = 0xffffffffu;
 
 // event classes = rings = phases
-enum : int { C_A = 0, C_W = 1, C_E = 2, C_P = 3, C_X = 4, kClasses = 5, kFree = 5, kRings = 6 };
+enum : int { C_A = 0, C_W = 1, C_E = 2, C_P = 3, C_X = 4, kClasses = 5, kFree = 5, kRings = kRingCount };
 
 #define FULL_MASK 0xffffffffu
 // flags: bits 0-1 type, 2-3 region, 4-6 layer, 7 collision pending (photon outside the phantom), 16-23 batch
@@ -91,9 +97,10 @@ __shared__ Geom s_g;
 __shared__ float* s_ep_batch;
 __shared__ unsigned long long s_npix;
 __shared__ uint4* s_pool;                           // this CTA's particle records [kPool][3]
-extern __shared__ __align__(16) unsigned char smem_raw[];   // rings [kRings][kPool] u16 | per-warp ledger | table blob
+__shared__ unsigned short* s_rings;                 // this CTA's rings [kRings][kPool]
+extern __shared__ __align__(16) unsigned char smem_raw[];   // per-warp ledger | table blob
 
-__device__ __forceinline__ unsigned short* ring_cells(int r) { return reinterpret_cast<unsigned short*>(smem_raw) + r * kPool; }
+__device__ __forceinline__ unsigned short* ring_cells(int r) { return s_rings + r * kPool; }
 struct Shared {
     const float4* phot;
     const float* maj;
@@ -129,6 +136,9 @@ __device__ __noinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c
 }
 // uniform in (0,1) from the top 23 bits: ((r >> 9) + 0.5) 2^-23 is exact in float32 and never 0 or 1
 __device__ __forceinline__ float u01(uint32_t r) { return ((float)(r >> 9) + 0.5f) * 1.1920928955078125e-7f; }
+
+// approximate reciprocal (MUFU.RCP): geometry distances and sampling formulas do not need the IEEE one
+__device__ __forceinline__ float rcp(float x) { return __fdividef(1.0f, x); }
 
 __device__ __forceinline__ uint4 rng_block(Lane& L, const TransportParams& P) {
     const uint64_t h = P.base + L.h;
@@ -183,7 +193,7 @@ __device__ __forceinline__ void dir_to_world(const Geom& g, float u, float v, fl
 // Rotate the unit vector d by polar (ct, st) and azimuth (cp, sp) using a branch-free orthonormal basis.
 __device__ __forceinline__ void rotate(float& dx, float& dy, float& dz, float ct, float st, float cp, float sp) {
     const float sg = copysignf(1.0f, dz);
-    const float a = -__frcp_rn(sg + dz), b = dx * dy * a;
+    const float a = -rcp(sg + dz), b = dx * dy * a;
     const float b1x = 1.0f + sg * dx * dx * a, b1y = sg * b, b1z = -sg * dx;
     const float b2x = b, b2y = sg + dy * dy * a, b2z = -dy;
     const float sc = st * cp, ss = st * sp;
@@ -237,7 +247,7 @@ __device__ __noinline__ AirHit air_boundary(float x, float y, float z, float dx,
     float tn = -kInf, tf = kInf; int ax = 0; bool miss = false;
 #define SLAB(P_, D_, LO_, HI_, A_)                                            \
     if (fabsf(D_) > 1e-20f) {                                                  \
-        const float inv = __frcp_rn(D_);                                       \
+        const float inv = rcp(D_);                                       \
         float t1 = ((LO_) - (P_)) * inv, t2 = ((HI_) - (P_)) * inv;           \
         if (t1 > t2) { const float t = t1; t1 = t2; t2 = t; }                  \
         if (t1 > tn) { tn = t1; ax = A_; }                                     \
@@ -327,14 +337,14 @@ __device__ __forceinline__ void raise_error(int bit) { atomicOr(s_flag + 1, bit)
 // one lane appends one slot to ring r (divergent code); visible to poppers after the next barrier
 __device__ __noinline__ void ring_push_one(int r, uint32_t slot) {
     const uint32_t t = atomicAdd(s_tail + r, 1u);
-    ring_cells(r)[t & (kPool - 1)] = (unsigned short)slot;
+    __stcg(ring_cells(r) + (t & (kPool - 1)), (unsigned short)slot);
 }
 // one lane takes one entry of ring r, if one is left below the snapshot (divergent code)
 __device__ __noinline__ uint32_t ring_pop_one(int r) {
     if ((int)(s_snap[r] - *((volatile unsigned int*)(s_head + r))) <= 0) return kNone;
     const uint32_t t = atomicAdd(s_head + r, 1u);
     if ((int)(s_snap[r] - t) <= 0) { atomicSub(s_head + r, 1u); return kNone; }
-    return ring_cells(r)[t & (kPool - 1)];
+    return __ldcg(ring_cells(r) + (t & (kPool - 1)));
 }
 // lane 0 claims up to `want` entries of ring r; returns count | first ticket << 32 (warp-uniform, all lanes call)
 __device__ __noinline__ unsigned long long ring_claim(int r, int want) {
@@ -412,7 +422,7 @@ __device__ __forceinline__ void interact(Lane& L, const TransportParams& P, cons
     }
     if (xsel < pe + co) {                                                  // Compton: Klein-Nishina by epsilon-mixture rejection
         if (COUNT) cnt[4]++;
-        const float k = L.E * (1.0f / kMec2), e0 = __frcp_rn(1.0f + 2.0f * k), e02 = e0 * e0;
+        const float k = L.E * (1.0f / kMec2), e0 = rcp(1.0f + 2.0f * k), e02 = e0 * e0;
         const float a1 = -__logf(e0), a2 = 0.5f * (1.0f - e02);
         float eps, t, x4;
 #pragma unroll 1
@@ -485,9 +495,9 @@ __device__ __forceinline__ bool woodcock_flight(Lane& L, const TransportParams& 
     if (!(nx >= g.lox && nx < g.hix && ny >= g.loy && ny < g.hiy && nz >= g.loz && nz < g.hiz)) {
         // left the grid: place on the AABB exit point, snapped onto the crossed face
         float tx = kInf, ty = kInf, tz = kInf;
-        if (L.dx > 0.0f) tx = (g.hix - L.x) / L.dx; else if (L.dx < 0.0f) tx = (g.lox - L.x) / L.dx;
-        if (L.dy > 0.0f) ty = (g.hiy - L.y) / L.dy; else if (L.dy < 0.0f) ty = (g.loy - L.y) / L.dy;
-        if (L.dz > 0.0f) tz = (g.hiz - L.z) / L.dz; else if (L.dz < 0.0f) tz = (g.loz - L.z) / L.dz;
+        if (L.dx != 0.0f) tx = ((L.dx > 0.0f ? g.hix : g.lox) - L.x) * rcp(L.dx);
+        if (L.dy != 0.0f) ty = ((L.dy > 0.0f ? g.hiy : g.loy) - L.y) * rcp(L.dy);
+        if (L.dz != 0.0f) tz = ((L.dz > 0.0f ? g.hiz : g.loz) - L.z) * rcp(L.dz);
         const float t = fmaxf(fminf(tx, fminf(ty, tz)), 0.0f);
         L.x = fmaf(t, L.dx, L.x); L.y = fmaf(t, L.dy, L.y); L.z = fmaf(t, L.dz, L.z);
         if (tx <= ty && tx <= tz) L.x = L.dx > 0.0f ? g.hix : g.lox;
@@ -538,7 +548,7 @@ __device__ __forceinline__ bool air_transit(Lane& L, const TransportParams& P, c
     if (kind == 0) { enter_phantom(L, P, ah.code >> 2); return false; }
     if (kind == 2) { L.a_esc += L.E; L.alive = false; return false; }
     enter_epid(L, g);                                                      // (u, v, depth 0), beam-frame direction, dw > 0
-    const float idw = __frcp_rn(L.dz);
+    const float idw = rcp(L.dz);
     if (lateral_exit(L.x, L.y, L.dx, L.dy) < g.zt[g.n_layers] * idw) return false;   // leaves the stack sideways: layer-by-layer code
     nl -= mua * ah.t;
     if (COUNT) cnt[2]++;
@@ -633,9 +643,9 @@ __device__ __forceinline__ void electron_step_phantom(Lane& L, const TransportPa
     const Geom& g = P.g;
     const float rho = __uint_as_float(L.cw & ~31u); const int m = (int)(L.cw & 31u);
     // distance to the voxel face in the direction of travel, per axis (a vanishing component gives a huge distance)
-    const float tx = (L.dx > 0.0f ? 1.0f - L.x : L.x) * g.hx * __frcp_rn(fabsf(L.dx) + 1e-30f);
-    const float ty = (L.dy > 0.0f ? 1.0f - L.y : L.y) * g.hy * __frcp_rn(fabsf(L.dy) + 1e-30f);
-    const float tz = (L.dz > 0.0f ? 1.0f - L.z : L.z) * g.hz * __frcp_rn(fabsf(L.dz) + 1e-30f);
+    const float tx = (L.dx > 0.0f ? 1.0f - L.x : L.x) * g.hx * rcp(fabsf(L.dx) + 1e-30f);
+    const float ty = (L.dy > 0.0f ? 1.0f - L.y : L.y) * g.hy * rcp(fabsf(L.dy) + 1e-30f);
+    const float tz = (L.dz > 0.0f ? 1.0f - L.z : L.z) * g.hz * rcp(fabsf(L.dz) + 1e-30f);
     const float tb = fmaxf(fminf(tx, fminf(ty, tz)), 0.0f);
     const int axis = (tx <= ty && tx <= tz) ? 0 : (ty <= tz ? 1 : 2);
     const StepLoss sl = step_loss(L, P, sh, m, rho, tb);
@@ -806,7 +816,7 @@ __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned lon
     if (ph >= 0 && ++s_nphase > kPhaseLimit) { raise_error(8); ph = -1; }
     s_phase = ph; s_left = 0; s_budget = ph == C_A ? budget : 0;
     const int n_start = ph < 0 ? 0 : n[ph] + (ph == C_A ? budget : 0);
-    s_keep = n_start >= kLongPhase ? kKeepLanes : 0;
+    s_keep = n_start >= kLongPhase ? 1 : 0;
     if (phase_count && ph >= 0) atomicAdd(phase_count, 1ull);
 }
 
@@ -840,12 +850,12 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
         if (leaving) break;
         // ---- B: refill the empty lanes from the ring of the class; class A then starts new histories
         unsigned empty = __ballot_sync(FULL_MASK, !L.alive);
-        if (__popc(empty) >= kRefillMin) {
+        if (__popc(empty) >= kRefillMin || it >= kIterLimit) {
             const unsigned long long cl = ring_claim(C, __popc(empty));
             const int got = (int)(uint32_t)cl;
             const int rk = __popc(empty & lt_mask);
             if (!L.alive && rk < got) {
-                const uint32_t s = ring_cells(C)[((uint32_t)(cl >> 32) + (uint32_t)rk) & (kPool - 1)];
+                const uint32_t s = __ldcg(ring_cells(C) + (((uint32_t)(cl >> 32) + (uint32_t)rk) & (kPool - 1)));
                 const uint4* rec = s_pool + (size_t)s * 3;
                 const uint4 a = __ldcg(rec), b = __ldcg(rec + 1), c = __ldcg(rec + 2);
                 L.x = __uint_as_float(a.x); L.y = __uint_as_float(a.y); L.z = __uint_as_float(a.z); L.dx = __uint_as_float(a.w);
@@ -869,7 +879,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                     if (lane == 0) h0 = atomicAdd(P.hist_counter, (unsigned)nslots);
                     h0 = __shfl_sync(FULL_MASK, h0, 0);
                     if (!L.alive && rk2 < nslots) {
-                        const uint32_t myslot = ring_cells(kFree)[((uint32_t)(fl >> 32) + (uint32_t)rk2) & (kPool - 1)];
+                        const uint32_t myslot = __ldcg(ring_cells(kFree) + (((uint32_t)(fl >> 32) + (uint32_t)rk2) & (kPool - 1)));
                         const uint32_t h = h0 + (uint32_t)rk2;
                         if (h >= P.n) { ring_push_one(kFree, myslot); atomicExch(s_flag, 1); }
                         else {
@@ -889,21 +899,21 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                     if (COUNT && lane == 0) cnt[30]++;
                 }
             }
+            // ---- C: leave the phase?
+            const int n_live = __popc(__ballot_sync(FULL_MASK, L.alive));
+            int go = 0;                                                        // 0 carry on, 1 nothing to do right now, 2 write back and leave, 3 leave
+            if (lane == 0) {
+                bool dry = (int)(s_snap[C] - *((volatile unsigned int*)(s_head + C))) <= 0;
+                if (C == C_A && *((volatile int*)&s_budget) > 0 && *((volatile int*)s_flag) == 0) dry = false;
+                if (n_live == 0) go = dry ? 3 : 1;
+                else if (it >= kIterLimit) go = 2;
+                else if (dry && keep > 0 && 32 - n_live >= kRefillMin) go = 2;    // cannot keep its lanes full any more
+            }
+            go = __shfl_sync(FULL_MASK, go, 0);
+            if (go == 3) break;
+            if (go == 2) { leaving = true; continue; }
+            if (go == 1) continue;
         }
-        // ---- C: leave the phase?
-        const int n_live = __popc(__ballot_sync(FULL_MASK, L.alive));
-        int go = 0;                                                        // 0 carry on, 1 nothing to do right now, 2 write back and leave, 3 leave
-        if (lane == 0) {
-            bool dry = (int)(s_snap[C] - *((volatile unsigned int*)(s_head + C))) <= 0;
-            if (C == C_A && *((volatile int*)&s_budget) > 0 && *((volatile int*)s_flag) == 0) dry = false;
-            if (n_live == 0) go = dry ? 3 : 1;
-            else if (it >= kIterLimit) go = 2;
-            else if (dry && keep > 0 && (n_live < keep || 2 * *((volatile int*)&s_left) >= kWarps)) go = 2;
-        }
-        go = __shfl_sync(FULL_MASK, go, 0);
-        if (go == 3) break;
-        if (go == 2) { leaving = true; continue; }
-        if (go == 1) continue;
         // ---- D: one event per live lane
         if (COUNT) { if (lane == 0) cnt[16 + C]++; if (L.alive) cnt[21 + C]++; }
         bool on = L.alive;
@@ -945,17 +955,15 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
 
 template <bool COUNT>
 __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_constant__ TransportParams P) {
-    // dynamic shared memory: rings | per-warp ledger | table blob
-    constexpr size_t kRingBytes = (size_t)kRings * kPool * sizeof(unsigned short);
-    double* const led_all = reinterpret_cast<double*>(smem_raw + kRingBytes);
-    uint32_t* const blob = reinterpret_cast<uint32_t*>(smem_raw + kRingBytes + kWarps * 8 * sizeof(double));
+    // dynamic shared memory: per-warp ledger | table blob
+    double* const led_all = reinterpret_cast<double*>(smem_raw);
+    uint32_t* const blob = reinterpret_cast<uint32_t*>(smem_raw + kWarps * 8 * sizeof(double));
     for (int i = threadIdx.x; i < P.tb.blob_words; i += kThreads) blob[i] = __ldg(P.tb.blob + i);
     Shared sh;
     sh.phot = reinterpret_cast<const float4*>(blob);
     sh.maj = reinterpret_cast<const float*>(sh.phot + P.tb.n_mat * P.tb.n_E);
     sh.lnS = sh.maj + P.tb.n_E;
     sh.invX0 = sh.lnS + P.tb.n_mat * P.tb.n_T;
-    for (int i = threadIdx.x; i < kPool; i += kThreads) ring_cells(kFree)[i] = (unsigned short)i;
     for (int i = threadIdx.x; i < kWarps * 8; i += kThreads) led_all[i] = 0.0;
     if (threadIdx.x < kRings) {
         const bool fr = threadIdx.x == kFree;
@@ -965,7 +973,10 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
     if (threadIdx.x == 0) {
         s_g = P.g; s_ep_batch = P.ep_batch; s_npix = P.npix; s_nphase = 0u;
         s_pool = P.pool + (size_t)blockIdx.x * kPool * 3;
+        s_rings = P.rings + (size_t)blockIdx.x * kRings * kPool;
     }
+    __syncthreads();
+    for (int i = threadIdx.x; i < kPool; i += kThreads) __stcg(ring_cells(kFree) + i, (unsigned short)i);   // every slot is free
     __syncthreads();
 
     uint32_t cnt[COUNT ? 32 : 1];
@@ -1014,7 +1025,7 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
     }
 }
 
-constexpr size_t kDynSmemFixed = (size_t)kRings * kPool * sizeof(unsigned short) + kWarps * 8 * sizeof(double);
+constexpr size_t kDynSmemFixed = kWarps * 8 * sizeof(double);
 
 size_t transport_smem_bytes(const Tables& t) {      // dynamic + static shared memory of the kernel
     return kDynSmemFixed + (size_t)t.blob_words * 4 + sizeof(Geom) + 512;
