@@ -57,6 +57,11 @@ static_assert(kPool == kPoolSlots && kPool <= 65536, "ring cells are 16-bit slot
 constexpr int kReserve = AEPID_RESERVE_8THS * kPool / 8;       // free slots that must remain for secondaries when new histories start
 constexpr int kRefillMin = AEPID_REFILL_MIN;                 // a warp refills its empty lanes once this many are empty
 constexpr int kLongPhase = 2 * kThreads;      // phases that start with at least this many particles end softly
+#ifndef AEPID_HIT_MIN
+#define AEPID_HIT_MIN 16
+#endif
+constexpr int kHitMin = AEPID_HIT_MIN;          // photon flights go on until this many lanes of the warp have a collision to sample
+constexpr int kMaxRounds = 8;                 // ... but no more than this many flights per event
 constexpr int kStarved = 256;                 // fewer free slots than this: prefer phases that need none
 constexpr uint32_t kIterLimit = 1u << 20;     // iterations of one warp in one phase before it hands its particles back
 constexpr uint32_t kPhaseLimit = 1u << 24;
@@ -730,7 +735,12 @@ __device__ __forceinline__ void charged_event(Lane& L, const TransportParams& P,
     for (int k = 0; k < 2; ++k) {
         if (PHANTOM) electron_step_phantom<COUNT>(L, P, sh, k ? r.z : r.x, k ? r.w : r.y, cnt);
         else electron_step_outside<COUNT>(L, P, sh, k ? r.z : r.x, k ? r.w : r.y, cnt);
-        if (!L.alive || L.E <= P.ph.ecut || (F_REGION(L.flags) == R_PHANTOM) != PHANTOM) break;
+        if (!L.alive) break;
+        if (L.E <= P.ph.ecut) {                                            // cutoff reached: an electron stops here and now;
+            if (F_TYPE(L.flags) == T_ELECTRON) { dep_here(L, P, L.E); L.alive = false; }   // a positron first needs a slot for its second photon
+            break;
+        }
+        if ((F_REGION(L.flags) == R_PHANTOM) != PHANTOM) break;
     }
 }
 
@@ -922,7 +932,19 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
         } else if (C == C_E || C == C_X) {
             if (on && F_TYPE(L.flags) == T_POSITRON && L.E <= P.ph.ecut && !ensure_spare(L)) { park = true; on = false; if (COUNT) cnt[29]++; }   // annihilation needs a slot
         }
-        if (on) {
+        if (C == C_W) {
+            // K3 + K4: flights against the majorant until at least kHitMin lanes have a collision to sample (or nobody flies
+            // any more), then the interactions together: keeps both halves of the event well filled when few flights collide
+            bool fly = on;
+            if (on && L.E < P.ph.pcut) { if (COUNT) cnt[13]++; dep_here(L, P, L.E); L.alive = false; fly = false; }   // PAPER.md:104, 10 keV
+            bool hit = false; float xsel = 0.0f, pe = 0.0f, co = 0.0f;
+#pragma unroll 1
+            for (int round = 0; round < kMaxRounds; ++round) {
+                if (fly) { hit = woodcock_flight<COUNT>(L, P, sh, xsel, pe, co, cnt); fly = !hit && F_REGION(L.flags) == R_PHANTOM; }
+                if (__popc(__ballot_sync(FULL_MASK, hit)) >= kHitMin || __ballot_sync(FULL_MASK, fly) == 0u) break;
+            }
+            if (hit) interact<COUNT>(L, P, sh, xsel, pe, co, cnt);
+        } else if (on) {
             if (C == C_E) charged_event<COUNT, true>(L, P, sh, cnt);
             else if (C == C_X) charged_event<COUNT, false>(L, P, sh, cnt);
             else if (L.E < P.ph.pcut) { if (COUNT) cnt[13]++; dep_here(L, P, L.E); L.alive = false; }   // PAPER.md:104, 10 keV
@@ -930,8 +952,6 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                 bool hit = false; float xsel = 0.0f, pe = 0.0f, co = 0.0f;
                 if (C == C_A) {
                     if (air_transit<COUNT>(L, P, sh, xsel, pe, co, cnt)) L.flags |= F_HIT;   // collision in air or in a layer: class P
-                } else if (C == C_W) {
-                    hit = woodcock_flight<COUNT>(L, P, sh, xsel, pe, co, cnt);
                 } else {
                     if (L.flags & F_HIT) {                                 // collision found by the transit: channel from a fresh draw (reading A8)
                         L.flags &= ~F_HIT;
