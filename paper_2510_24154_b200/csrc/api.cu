@@ -22,7 +22,7 @@ constexpr size_t kMaxLut = 65536;
 inline size_t up(size_t x) { return (x + kAlign - 1) & ~(kAlign - 1); }
 
 struct Layout {
-    size_t vox, ph_batch, ep_batch, out_ph, out_ep, tmap, signal, dose_in, lut, blob, thrE, edges, thrF, pool, rings, small, total;
+    size_t vox, ph_batch, ep_batch, out_ph, out_ep, tmap, signal, dose_in, lut, blob, thrE, edges, thrF, guideF, pool, rings, small, total;
     size_t nvox, npix, blob_bytes;
 };
 
@@ -56,6 +56,7 @@ Layout make_layout(const aepid_dims& d) {
     L.thrE = take(((size_t)d.n_bins + 1) * 4);
     L.edges = take(((size_t)d.n_bins + 1) * 4);
     L.thrF = take(((size_t)d.fu * d.fv + 1) * 4);
+    L.guideF = take(((size_t)kGuideSize + 1) * 4);
     L.pool = take((size_t)kMaxCtas * kPoolSlots * kRecordBytes);   // particle pools of the transport kernel (scratch)
     L.rings = take((size_t)kMaxCtas * kRingCount * kPoolSlots * 2);
     L.small = take(1024);            // ledger [8] f64 @0 | chunk counter @64 | rho_max [32] f32 @128 | counters [32] u64 @256
@@ -100,6 +101,7 @@ struct aepid_ctx {
     uint32_t* d_thrE() { return reinterpret_cast<uint32_t*>(ws + lay.thrE); }
     float* d_edges() { return reinterpret_cast<float*>(ws + lay.edges); }
     uint32_t* d_thrF() { return reinterpret_cast<uint32_t*>(ws + lay.thrF); }
+    uint32_t* d_guideF() { return reinterpret_cast<uint32_t*>(ws + lay.guideF); }
     double* d_ledger() { return reinterpret_cast<double*>(ws + lay.small); }
     unsigned long long* d_counters() { return reinterpret_cast<unsigned long long*>(ws + lay.small + 256); }
     unsigned int* d_chunk() { return reinterpret_cast<unsigned int*>(ws + lay.small + 64); }
@@ -388,6 +390,19 @@ int aepid_load_source(aepid_ctx* ctx, const float src[3], const float axes[9], i
     if (!thresholds(hp, tE, totE)) return fail(ctx, AEPID_ERR_BAD_ARG, "spectrum pdf must be non-negative with a positive sum");
     if (!thresholds(hf, tF, totF)) return fail(ctx, AEPID_ERR_BAD_ARG, "fluence must be non-negative with a positive sum");
     tE[nb] = 0u;                                           // 2^32 mod 2^32: widths come out right by wrap-around
+    // guide table of the fluence search: guide[k] = #{j < n : thrF[1 + j] <= k 2^(32 - kGuideLog)}, so that the upper
+    // bound of a draw r lies in [guide[r >> s], guide[(r >> s) + 1]] and the search touches 2-3 words instead of 16
+    std::vector<uint32_t> gF((size_t)kGuideSize + 1);
+    {
+        const size_t n = (size_t)fu * fv - 1;
+        size_t j = 0;
+        for (int k = 0; k < kGuideSize; ++k) {
+            const uint32_t key = (uint32_t)k << (32 - kGuideLog);
+            while (j < n && tF[1 + j] <= key) ++j;
+            gF[k] = (uint32_t)j;
+        }
+        gF[kGuideSize] = (uint32_t)n;
+    }
     int j_last = 0;
     ctx->bb_u0 = fu; ctx->bb_u1 = -1; ctx->bb_v0 = fv; ctx->bb_v1 = -1;
     for (int j = 0; j < fv; ++j) for (int i = 0; i < fu; ++i)
@@ -399,12 +414,13 @@ int aepid_load_source(aepid_ctx* ctx, const float src[3], const float axes[9], i
     CU(cudaMemcpyAsync(ctx->d_thrE(), tE.data(), tE.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(ctx->d_edges(), he.data(), he.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(ctx->d_thrF(), tF.data(), tF.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->d_guideF(), gF.data(), gF.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));                // sources are local vectors
     Geom& g = ctx->g;
     for (int k = 0; k < 3; ++k) { g.src[k] = src[k]; g.au[k] = axes[k]; g.av[k] = axes[3 + k]; g.aw[k] = axes[6 + k]; }
     Source& so = ctx->so;
     so.n_bins = nb; so.fu = fu; so.fv = fv; so.j_last = j_last; so.fpitch = fpitch; so.fdist = fdist;
-    so.thrE = ctx->d_thrE(); so.edges = ctx->d_edges(); so.thrF = ctx->d_thrF();
+    so.thrE = ctx->d_thrE(); so.edges = ctx->d_edges(); so.thrF = ctx->d_thrF(); so.guideF = ctx->d_guideF();
     ctx->have_source = true;
     return 0;
 }

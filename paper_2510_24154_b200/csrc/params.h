@@ -19,7 +19,9 @@ constexpr float kMec2 = 0.51099895f;
 constexpr int kPoolSlots = 1 << AEPID_POOL_LOG;   // particle records per CTA of the transport kernel (transport.cu), at most 65536
 constexpr int kRingCount = 6;         // slot-index rings per CTA: five event classes and the free slots
 constexpr int kRecordBytes = 48;      // three 16-byte vectors per particle
-constexpr int kMaxCtas = 160;         // CTAs of the transport kernel the workspace provides a pool for (one per SM)
+constexpr int kMaxCtas = 160;
+constexpr int kGuideLog = 12;         // the fluence search starts from a guide table indexed by the top kGuideLog bits of the draw
+constexpr int kGuideSize = 1 << kGuideLog;         // CTAs of the transport kernel the workspace provides a pool for (one per SM)
 
 enum Region : uint32_t { R_AIR = 0, R_PHANTOM = 1, R_EPID = 2 };
 enum PType : uint32_t { T_PHOTON = 0, T_ELECTRON = 1, T_POSITRON = 2 };
@@ -63,6 +65,7 @@ struct Source {
     const uint32_t* thrE;              // [n_bins+1] integer CDF thresholds on the raw 32-bit draw
     const float* edges;                // [n_bins+1]
     const uint32_t* thrF;              // [fu*fv+1]
+    const uint32_t* guideF;            // [kGuideSize+1] bracket of the search in thrF per top-bits bucket of the draw
 };
 
 struct TransportParams {

@@ -43,7 +43,10 @@
 
 namespace aepid {
 
-constexpr int kWarps = 24;
+#ifndef AEPID_WARPS
+#define AEPID_WARPS 32
+#endif
+constexpr int kWarps = AEPID_WARPS;
 constexpr int kThreads = kWarps * 32;
 constexpr int kPoolLog = AEPID_POOL_LOG;
 constexpr int kPool = 1 << kPoolLog;          // particle slots per CTA; also the capacity of every ring
@@ -56,6 +59,17 @@ static_assert(kPool == kPoolSlots && kPool <= 65536, "ring cells are 16-bit slot
 #endif
 constexpr int kReserve = AEPID_RESERVE_8THS * kPool / 8;       // free slots that must remain for secondaries when new histories start
 constexpr int kRefillMin = AEPID_REFILL_MIN;                 // a warp refills its empty lanes once this many are empty
+#ifndef AEPID_MIN_ITER
+#define AEPID_MIN_ITER 12
+#endif
+constexpr uint32_t kMinIter = AEPID_MIN_ITER;   // events per lane before a warp may leave a short phase early
+#ifndef AEPID_STEPS_E
+#define AEPID_STEPS_E 4
+#endif
+#ifndef AEPID_STEPS_X
+#define AEPID_STEPS_X 4
+#endif
+constexpr int kStepsE = AEPID_STEPS_E, kStepsX = AEPID_STEPS_X;   // steps per event of a charged particle in / outside the phantom
 constexpr int kLongPhase = 2 * kThreads;      // phases that start with at least this many particles end softly
 #ifndef AEPID_HIT_MIN
 #define AEPID_HIT_MIN 16
@@ -642,7 +656,9 @@ __device__ __forceinline__ void stop_charged(Lane& L, const TransportParams& P, 
     } else L.alive = false;
 }
 // One step inside the phantom with the draws (ra, rb): the hot loop of the whole path, written without branches up
-// to the face crossing.  The particle is above its cutoff.
+// to the rare exit from the grid (selects instead of per-axis branches: a face is crossed by a few lanes of nearly
+// every warp, so divergent code there is paid by all).  The particle is above its cutoff.  Invariant of class E: the
+// pending deposit of the lane belongs to the current voxel (L.pidx == L.vlin, set when the particle is loaded).
 template <bool COUNT>
 __device__ __forceinline__ void electron_step_phantom(Lane& L, const TransportParams& P, const Shared& sh, uint32_t ra, uint32_t rb, uint32_t* cnt) {
     const Geom& g = P.g;
@@ -652,30 +668,35 @@ __device__ __forceinline__ void electron_step_phantom(Lane& L, const TransportPa
     const float ty = (L.dy > 0.0f ? 1.0f - L.y : L.y) * g.hy * rcp(fabsf(L.dy) + 1e-30f);
     const float tz = (L.dz > 0.0f ? 1.0f - L.z : L.z) * g.hz * rcp(fabsf(L.dz) + 1e-30f);
     const float tb = fmaxf(fminf(tx, fminf(ty, tz)), 0.0f);
-    const int axis = (tx <= ty && tx <= tz) ? 0 : (ty <= tz ? 1 : 2);
+    const bool ax0 = tx <= ty && tx <= tz, ax1 = !ax0 && ty <= tz, ax2 = !ax0 && !ax1;
     const StepLoss sl = step_loss(L, P, sh, m, rho, tb);
     if (COUNT) { cnt[6]++; if (!(sl.s > 0.0f)) cnt[15]++; }
-    dep_vox(L, P, L.vlin, sl.dep);
+    L.pval += sl.dep; L.a_ph += sl.dep;
     L.x = fmaf(sl.s * g.ihx, L.dx, L.x); L.y = fmaf(sl.s * g.ihy, L.dy, L.y); L.z = fmaf(sl.s * g.ihz, L.dz, L.z);
     float ct, st, cp, sp;
     highland(sh, m, rho * sl.s, sl.Tmid, ra, rb, ct, st, cp, sp);
-    if (sl.s == tb) {                                                      // the step ended on a face: neighbouring voxel or out of the grid
-        const bool up = (axis == 0 ? L.dx : (axis == 1 ? L.dy : L.dz)) > 0.0f;
-        const float nf = up ? 0.0f : 1.0f;
-        L.x = axis == 0 ? nf : L.x; L.y = axis == 1 ? nf : L.y; L.z = axis == 2 ? nf : L.z;
-        const int sh10 = axis * 10;
-        const int ni = (int)((L.vox >> sh10) & 1023u) + (up ? 1 : -1);
-        const int nmax = axis == 0 ? g.nx : (axis == 1 ? g.ny : g.nz);
-        if (ni < 0 || ni >= nmax) {
-            frac_to_world(L, g);                                           // uses the old index; then snap the crossed axis
-            if (axis == 0) L.x = up ? g.hix : g.lox; else if (axis == 1) L.y = up ? g.hiy : g.loy; else L.z = up ? g.hiz : g.loz;
-            SET_REGION(L.flags, R_AIR);
-        } else {
-            const int stride = axis == 0 ? 1 : (axis == 1 ? g.nx : g.nx * g.ny);
-            L.vox = (L.vox & ~(1023u << sh10)) | ((uint32_t)ni << sh10);
-            L.vlin += up ? (uint32_t)stride : (uint32_t)(-stride);
-            L.cw = __ldg(P.vox + L.vlin);
-        }
+    // the step ended on a face: neighbouring voxel (index +-1 on the crossed axis, never re-derived from the position) or out of the grid
+    const bool cross = sl.s == tb;
+    const bool up = (ax0 ? L.dx : (ax1 ? L.dy : L.dz)) > 0.0f;
+    const float nf = up ? 0.0f : 1.0f;
+    const int sh10 = ax0 ? 0 : (ax1 ? 10 : 20);
+    const int nmax = ax0 ? g.nx : (ax1 ? g.ny : g.nz);
+    const int stride = ax0 ? 1 : (ax1 ? g.nx : g.nx * g.ny);
+    const int ni = (int)((L.vox >> sh10) & 1023u) + (up ? 1 : -1);
+    const bool inside = ni >= 0 && ni < nmax;
+    L.x = (cross && ax0) ? nf : L.x; L.y = (cross && ax1) ? nf : L.y; L.z = (cross && ax2) ? nf : L.z;
+    if (cross && inside) {
+        if (L.pval != 0.0f) atomicAdd(P.ph_batch + (size_t)F_BATCH(L.flags) * P.nvox + L.vlin, L.pval);
+        L.pval = 0.0f;
+        L.vox = (L.vox & ~(1023u << sh10)) | ((uint32_t)ni << sh10);
+        L.vlin += (uint32_t)(up ? stride : -stride);
+        L.pidx = L.vlin;
+        L.cw = __ldg(P.vox + L.vlin);
+    }
+    if (cross && !inside) {                                                // rare: leaves the grid
+        frac_to_world(L, g);                                               // uses the old index; then snap the crossed axis
+        if (ax0) L.x = up ? g.hix : g.lox; else if (ax1) L.y = up ? g.hiy : g.loy; else L.z = up ? g.hiz : g.loz;
+        SET_REGION(L.flags, R_AIR);
     }
     rotate(L.dx, L.dy, L.dz, ct, st, cp, sp);
 }
@@ -687,8 +708,19 @@ __device__ __forceinline__ void electron_step_outside(Lane& L, const TransportPa
     float rho, tb; int m, axis = 0, kind = 0;
     if (in_air) {
         rho = kRhoAir; m = 0;
-        const AirHit ah = air_boundary(L.x, L.y, L.z, L.dx, L.dy, L.dz);
-        tb = ah.t; kind = ah.code & 3; axis = ah.code >> 2;
+        // Open air: farther than s_max from the phantom box, the EPID top plane and the world walls, so the step (at most
+        // s_max long) cannot reach a boundary and the exact distances are not needed.  An electron crosses the air gap in
+        // hundreds of such steps.
+        const float far = P.ph.smax * 1.0001f;
+        const float gap = fmaxf(fmaxf(fmaxf(g.lox - L.x, L.x - g.hix), fmaxf(g.loy - L.y, L.y - g.hiy)), fmaxf(g.loz - L.z, L.z - g.hiz));
+        float pu, pv, pw;
+        to_beam(g, L.x, L.y, L.z, pu, pv, pw);
+        const float wall = fminf(fminf(kWorldHalf - fabsf(pu), kWorldHalf - fabsf(pv)), fminf(pw - kWorldWMin, g.sid - pw));
+        if (gap > far && wall > far) { tb = kInf; }
+        else {
+            const AirHit ah = air_boundary(L.x, L.y, L.z, L.dx, L.dy, L.dz);
+            tb = ah.t; kind = ah.code & 3; axis = ah.code >> 2;
+        }
     } else {
         const int l = F_LAYER(L.flags);
         rho = g.lrho[l]; m = g.lmat[l];
@@ -726,15 +758,16 @@ __device__ __forceinline__ void electron_step_outside(Lane& L, const TransportPa
     }
     rotate(L.dx, L.dy, L.dz, ct, st, cp, sp);
 }
-// K5 for one lane: one Philox block feeds up to two consecutive steps
+// K5 for one lane: up to kStepsE / kStepsX consecutive steps per event, one Philox block per two steps
 template <bool COUNT, bool PHANTOM>
 __device__ __forceinline__ void charged_event(Lane& L, const TransportParams& P, const Shared& sh, uint32_t* cnt) {
     if (L.E <= P.ph.ecut) { stop_charged<COUNT>(L, P, cnt); return; }
-    const uint4 r = rng_block(L, P);
+    uint4 r = rng_block(L, P);
 #pragma unroll 1
-    for (int k = 0; k < 2; ++k) {
-        if (PHANTOM) electron_step_phantom<COUNT>(L, P, sh, k ? r.z : r.x, k ? r.w : r.y, cnt);
-        else electron_step_outside<COUNT>(L, P, sh, k ? r.z : r.x, k ? r.w : r.y, cnt);
+    for (int k = 0; k < (PHANTOM ? kStepsE : kStepsX); ++k) {
+        if (k && !(k & 1)) r = rng_block(L, P);
+        if (PHANTOM) electron_step_phantom<COUNT>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, cnt);
+        else electron_step_outside<COUNT>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, cnt);
         if (!L.alive) break;
         if (L.E <= P.ph.ecut) {                                            // cutoff reached: an electron stops here and now;
             if (F_TYPE(L.flags) == T_ELECTRON) { dep_here(L, P, L.E); L.alive = false; }   // a positron first needs a slot for its second photon
@@ -765,7 +798,12 @@ __device__ __forceinline__ SourceSample sample_source(const TransportParams& P, 
         const float e0 = __ldg(so.edges + i), e1 = __ldg(so.edges + i + 1);
         s.E = fmaf(t, e1 - e0, e0);
     }
-    uint32_t j = upper_bound_u32(so.thrF + 1, (uint32_t)(so.fu * so.fv - 1), r1);
+    uint32_t j;
+    {   // fluence pixel: #{k : thrF[1 + k] <= r1}, searched inside the bracket the guide table gives for the top bits of r1
+        uint32_t lo = __ldg(so.guideF + (r1 >> (32 - kGuideLog))), hi = __ldg(so.guideF + (r1 >> (32 - kGuideLog)) + 1);
+        while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (__ldg(so.thrF + 1 + mid) <= r1) lo = mid + 1; else hi = mid; }
+        j = lo;
+    }
     j = min(j, (uint32_t)so.j_last);
     s.pixel = j;
     const int ju = (int)(j % (uint32_t)so.fu), jv = (int)(j / (uint32_t)so.fu);
@@ -826,7 +864,12 @@ __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned lon
     if (ph >= 0 && ++s_nphase > kPhaseLimit) { raise_error(8); ph = -1; }
     s_phase = ph; s_left = 0; s_budget = ph == C_A ? budget : 0;
     const int n_start = ph < 0 ? 0 : n[ph] + (ph == C_A ? budget : 0);
-    s_keep = n_start >= kLongPhase ? 1 : 0;
+    // soft end (header comment): always for a long phase; for a short one only while there is other work to switch to,
+    // and then not before kMinIter events per lane, so that every phase makes progress
+    int n_other = 0;
+#pragma unroll
+    for (int c = 0; c < kClasses; ++c) n_other += c == ph ? 0 : n[c];
+    s_keep = n_start >= kLongPhase ? 1 : ((more || n_other > 0) ? 2 : 0);
     if (phase_count && ph >= 0) atomicAdd(phase_count, 1ull);
 }
 
@@ -875,7 +918,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                 L.pval = 0.0f; L.pidx = kNone;
                 if (COUNT) cnt[28]++;
                 if (C == C_A || C == C_W || C == C_P) set_energy(L, P, sh);
-                if (C == C_E) { L.vlin = vox_linear(P.g, L.vox); L.cw = __ldg(P.vox + L.vlin); }
+                if (C == C_E) { L.vlin = vox_linear(P.g, L.vox); L.cw = __ldg(P.vox + L.vlin); L.pidx = L.vlin; }
             }
             if (C == C_A) {
                 // K1: new histories in the lanes that are still empty, one free slot each
@@ -917,7 +960,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                 if (C == C_A && *((volatile int*)&s_budget) > 0 && *((volatile int*)s_flag) == 0) dry = false;
                 if (n_live == 0) go = dry ? 3 : 1;
                 else if (it >= kIterLimit) go = 2;
-                else if (dry && keep > 0 && 32 - n_live >= kRefillMin) go = 2;    // cannot keep its lanes full any more
+                else if (dry && 32 - n_live >= kRefillMin && (keep == 1 || (keep == 2 && it >= kMinIter))) go = 2;    // cannot keep its lanes full any more
             }
             go = __shfl_sync(FULL_MASK, go, 0);
             if (go == 3) break;
@@ -925,7 +968,9 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
             if (go == 1) continue;
         }
         // ---- D: one event per live lane
+        #ifndef AEPID_PHASE_CLOCK
         if (COUNT) { if (lane == 0) cnt[16 + C]++; if (L.alive) cnt[21 + C]++; }
+#endif
         bool on = L.alive;
         if (C == C_W || C == C_P) {
             if (on && !ensure_spare(L)) { park = true; on = false; if (COUNT) cnt[29]++; }   // an interaction may create a secondary
@@ -1018,6 +1063,9 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
         __syncthreads();
         const int ph = s_phase;
         if (ph < 0) break;
+#ifdef AEPID_PHASE_CLOCK
+        const long long t0 = clock64();
+#endif
         switch (ph) {
             case C_A: run_phase<COUNT, C_A>(L, P, sh, led, cnt); break;
             case C_W: run_phase<COUNT, C_W>(L, P, sh, led, cnt); break;
@@ -1025,7 +1073,17 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
             case C_P: run_phase<COUNT, C_P>(L, P, sh, led, cnt); break;
             default:  run_phase<COUNT, C_X>(L, P, sh, led, cnt); break;
         }
+#ifdef AEPID_PHASE_CLOCK
+        if (COUNT && lane == 0) atomicAdd(P.counters + 10, (unsigned long long)(clock64() - t0));   // busy warp-cycles
+#endif
         __syncthreads();
+#ifdef AEPID_PHASE_CLOCK
+        if (COUNT && threadIdx.x == 0) {
+            atomicAdd(P.counters + 16 + ph, (unsigned long long)(clock64() - t0));                  // cycles per class
+            atomicAdd(P.counters + 21 + ph, 1ull);                                                    // phases per class
+            atomicAdd(P.counters + 11, (unsigned long long)(clock64() - t0) * kWarps);
+        }
+#endif
     }
 
     if (threadIdx.x < 6) {
