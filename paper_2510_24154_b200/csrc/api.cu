@@ -58,7 +58,7 @@ Layout make_layout(const aepid_dims& d) {
     L.thrF = take(((size_t)d.fu * d.fv + 1) * 4);
     L.guideF = take(((size_t)kGuideSize + 1) * 4);
     L.pool = take((size_t)kMaxCtas * kPoolSlots * kRecordBytes);   // particle pools of the transport kernel (scratch)
-    L.rings = take((size_t)kMaxCtas * kRingCount * kPoolSlots * 2);
+    L.rings = take((size_t)kMaxCtas * kRingCount * kPoolSlots * sizeof(ring_t));
     L.small = take(1024);            // ledger [8] f64 @0 | chunk counter @64 | rho_max [32] f32 @128 | counters [32] u64 @256
     L.total = o;
     return L;
@@ -233,7 +233,7 @@ int fill_params(aepid_ctx* ctx, TransportParams& p) {
     p.vox = ctx->d_vox(); p.ep_batch = ctx->d_ep_batch(); p.ph_batch = ctx->d_ph_batch();
     p.ledger = ctx->d_ledger(); p.counters = ctx->d_counters(); p.hist_counter = ctx->d_chunk();
     p.pool = reinterpret_cast<uint4*>(ctx->ws + ctx->lay.pool);
-    p.rings = reinterpret_cast<unsigned short*>(ctx->ws + ctx->lay.rings);
+    p.rings = reinterpret_cast<ring_t*>(ctx->ws + ctx->lay.rings);
     p.n_batches = ctx->dims.n_batches; p.nvox = ctx->lay.nvox; p.npix = ctx->lay.npix;
     p.base = 0; p.seed = 0; p.n = 0; p.hist_per_batch = 1;
     return 0;

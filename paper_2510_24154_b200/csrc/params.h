@@ -3,6 +3,7 @@
 #pragma once
 #include <cstdint>
 #include <cstddef>
+#include <type_traits>
 #include <vector_types.h>
 
 namespace aepid {
@@ -16,7 +17,8 @@ constexpr float kMec2 = 0.51099895f;
 #ifndef AEPID_POOL_LOG
 #define AEPID_POOL_LOG 16
 #endif
-constexpr int kPoolSlots = 1 << AEPID_POOL_LOG;   // particle records per CTA of the transport kernel (transport.cu), at most 65536
+constexpr int kPoolSlots = 1 << AEPID_POOL_LOG;   // particle records per CTA of the transport kernel (transport.cu)
+typedef std::conditional<(AEPID_POOL_LOG <= 16), unsigned short, uint32_t>::type ring_t;   // a ring cell holds a slot index
 constexpr int kRingCount = 6;         // slot-index rings per CTA: five event classes and the free slots
 constexpr int kRecordBytes = 48;      // three 16-byte vectors per particle
 constexpr int kMaxCtas = 160;
@@ -80,7 +82,7 @@ struct TransportParams {
     unsigned long long* counters;      // [32]
     unsigned int* hist_counter;        // next history of this launch that has not been started
     uint4* pool;                       // particle records [kMaxCtas][kPoolSlots][3], scratch of one launch
-    unsigned short* rings;             // slot-index rings [kMaxCtas][kRingCount][kPoolSlots], scratch of one launch
+    ring_t* rings;             // slot-index rings [kMaxCtas][kRingCount][kPoolSlots], scratch of one launch
     uint64_t base;                     // global index of relative history 0 of this launch
     uint64_t seed;
     uint32_t n;                        // histories in this launch (< 2^32)

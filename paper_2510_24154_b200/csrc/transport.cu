@@ -2,8 +2,8 @@
 // sampling, K5 CSDA electron steps with Highland deflection, K6 EPID slab transport and K7 tally
 // scoring (physics of SURVEY.md 8(c)).
 //
-// Design (sm_100a): ONE persistent CTA per SM that runs a LOCAL WAVEFRONT.  Measured on B200 (profiles/r01b_*,
-// profiles/r01c_icache_microbench.md): warps of one SM that execute different parts of a code body larger than the
+// Design (sm_100a): ONE persistent CTA per SM that runs a LOCAL WAVEFRONT.  Measured on B200 (profiles/r01a_README.md,
+// DESIGN.md 6.2): warps of one SM that execute different parts of a code body larger than the
 // 32 KB instruction cache starve on instruction fetch (IPC 0.3-1.1 of 4), warps that execute the same part do not.
 // So all warps of a CTA work on the same event class at any time:
 //   * Event classes: A photon in air (new histories start here), W photon in the phantom, E charged particle in the
@@ -12,9 +12,9 @@
 //     phase: new histories while the particle pool has room, else the class with the most waiting particles.
 //   * Particle records (48 B, three 16 B vectors) live in a per-CTA POOL in global memory (kPool slots, L2 resident,
 //     written and read with .cg accesses); shared memory holds the material tables (ln domain, one LDS.128 per node)
-//     and, per class, a ring of pool-slot indices, plus a ring of free slots.  A pool this large (8192 particles
-//     for 768 lanes) makes a phase many waves long, so that the phase switch (two barriers, a cold instruction
-//     cache) and the tail of a phase cost little.
+//     and the scheduler state; the rings of pool-slot indices (one per class, one of free slots) live in global memory
+//     too.  A pool this large (65536 particles for 1024 lanes) makes a phase many waves long, so that the phase switch
+//     (two barriers, a cold instruction cache) and the tail of a phase cost little (measured: halving the pool costs 5 %).
 //   * Within a phase every lane follows its particle event by event while it stays in the class; a lane whose
 //     particle has died or changed class writes it back (record to the pool, slot to the ring of the new class) and
 //     is refilled IN PLACE from the ring of the phase, so warps run one code path with nearly all lanes active.
@@ -27,7 +27,7 @@
 //   * A phase ends softly: a warp that can no longer keep its lanes full (ring exhausted, kRefillMin lanes empty)
 //     writes its particles back and leaves, so all warps reach the barrier within about one event of each other and
 //     the survivors join the next phase of their class (a write-back and reload costs a fraction of one event).
-//     Phases that start with fewer than two waves of particles run until every lane is dry.
+//     In a phase that starts with fewer than two waves of particles a warp stays for at least kMinIter events.
 //   * Slot discipline: every particle owns a pool slot from birth, so writing it back never needs a new one; a lane
 //     runs an event that can create a secondary only while it holds a spare slot, otherwise it parks its particle.
 //     New histories start only while kReserve slots stay free.  Hence the pool cannot overflow.
@@ -50,7 +50,7 @@ constexpr int kWarps = AEPID_WARPS;
 constexpr int kThreads = kWarps * 32;
 constexpr int kPoolLog = AEPID_POOL_LOG;
 constexpr int kPool = 1 << kPoolLog;          // particle slots per CTA; also the capacity of every ring
-static_assert(kPool == kPoolSlots && kPool <= 65536, "ring cells are 16-bit slot indices");
+static_assert(kPool == kPoolSlots, "pool size");
 #ifndef AEPID_RESERVE_8THS
 #define AEPID_RESERVE_8THS 3
 #endif
@@ -70,6 +70,11 @@ constexpr uint32_t kMinIter = AEPID_MIN_ITER;   // events per lane before a warp
 #define AEPID_STEPS_X 4
 #endif
 constexpr int kStepsE = AEPID_STEPS_E, kStepsX = AEPID_STEPS_X;   // steps per event of a charged particle in / outside the phantom
+#ifdef AEPID_PHASE_CLOCK
+constexpr bool kPhaseClock = true;        // analysis build: counters 10, 11, 16-25, 27-31 hold phase clocks instead
+#else
+constexpr bool kPhaseClock = false;
+#endif
 constexpr int kLongPhase = 2 * kThreads;      // phases that start with at least this many particles end softly
 #ifndef AEPID_HIT_MIN
 #define AEPID_HIT_MIN 16
@@ -116,10 +121,10 @@ __shared__ Geom s_g;
 __shared__ float* s_ep_batch;
 __shared__ unsigned long long s_npix;
 __shared__ uint4* s_pool;                           // this CTA's particle records [kPool][3]
-__shared__ unsigned short* s_rings;                 // this CTA's rings [kRings][kPool]
+__shared__ ring_t* s_rings;                 // this CTA's rings [kRings][kPool]
 extern __shared__ __align__(16) unsigned char smem_raw[];   // per-warp ledger | table blob
 
-__device__ __forceinline__ unsigned short* ring_cells(int r) { return s_rings + r * kPool; }
+__device__ __forceinline__ ring_t* ring_cells(int r) { return s_rings + r * kPool; }
 struct Shared {
     const float4* phot;
     const float* maj;
@@ -356,7 +361,7 @@ __device__ __forceinline__ void raise_error(int bit) { atomicOr(s_flag + 1, bit)
 // one lane appends one slot to ring r (divergent code); visible to poppers after the next barrier
 __device__ __noinline__ void ring_push_one(int r, uint32_t slot) {
     const uint32_t t = atomicAdd(s_tail + r, 1u);
-    __stcg(ring_cells(r) + (t & (kPool - 1)), (unsigned short)slot);
+    __stcg(ring_cells(r) + (t & (kPool - 1)), (ring_t)slot);
 }
 // one lane takes one entry of ring r, if one is left below the snapshot (divergent code)
 __device__ __noinline__ uint32_t ring_pop_one(int r) {
@@ -864,12 +869,9 @@ __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned lon
     if (ph >= 0 && ++s_nphase > kPhaseLimit) { raise_error(8); ph = -1; }
     s_phase = ph; s_left = 0; s_budget = ph == C_A ? budget : 0;
     const int n_start = ph < 0 ? 0 : n[ph] + (ph == C_A ? budget : 0);
-    // soft end (header comment): always for a long phase; for a short one only while there is other work to switch to,
-    // and then not before kMinIter events per lane, so that every phase makes progress
-    int n_other = 0;
-#pragma unroll
-    for (int c = 0; c < kClasses; ++c) n_other += c == ph ? 0 : n[c];
-    s_keep = n_start >= kLongPhase ? 1 : ((more || n_other > 0) ? 2 : 0);
+    // soft end (header comment): at once for a long phase; for a short one not before kMinIter events per lane, so
+    // that every phase makes progress (a short phase that restarts runs with its particles packed into fewer warps)
+    s_keep = n_start >= kLongPhase ? 1 : 2;
     if (phase_count && ph >= 0) atomicAdd(phase_count, 1ull);
 }
 
@@ -892,7 +894,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                     raise_error(4);
                     L.a_esc += L.E + (F_TYPE(L.flags) == T_POSITRON ? 2.0f * kMec2 : 0.0f);
                 } else queue_particle(L.slot, L.x, L.y, L.z, L.dx, L.dy, L.dz, L.E, L.vox, L.flags, L.h, L.pid, L.blk);
-                if (COUNT) cnt[27]++;
+                if (COUNT && !kPhaseClock) cnt[27]++;
                 L.alive = false; L.slot = kNone;
             } else if (L.slot != kNone) {
                 if (kSpawns && !leaving && L.spare == kNone) L.spare = L.slot; else ring_push_one(kFree, L.slot);
@@ -916,7 +918,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                 L.flags = c.x; L.h = c.y; L.pid = c.z; L.blk = c.w;
                 L.slot = s; L.alive = true;
                 L.pval = 0.0f; L.pidx = kNone;
-                if (COUNT) cnt[28]++;
+                if (COUNT && !kPhaseClock) cnt[28]++;
                 if (C == C_A || C == C_W || C == C_P) set_energy(L, P, sh);
                 if (C == C_E) { L.vlin = vox_linear(P.g, L.vox); L.cw = __ldg(P.vox + L.vlin); L.pidx = L.vlin; }
             }
@@ -949,7 +951,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                             set_energy(L, P, sh);
                         }
                     }
-                    if (COUNT && lane == 0) cnt[30]++;
+                    if (COUNT && !kPhaseClock && lane == 0) cnt[30]++;
                 }
             }
             // ---- C: leave the phase?
@@ -973,9 +975,9 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
 #endif
         bool on = L.alive;
         if (C == C_W || C == C_P) {
-            if (on && !ensure_spare(L)) { park = true; on = false; if (COUNT) cnt[29]++; }   // an interaction may create a secondary
+            if (on && !ensure_spare(L)) { park = true; on = false; if (COUNT && !kPhaseClock) cnt[29]++; }   // an interaction may create a secondary
         } else if (C == C_E || C == C_X) {
-            if (on && F_TYPE(L.flags) == T_POSITRON && L.E <= P.ph.ecut && !ensure_spare(L)) { park = true; on = false; if (COUNT) cnt[29]++; }   // annihilation needs a slot
+            if (on && F_TYPE(L.flags) == T_POSITRON && L.E <= P.ph.ecut && !ensure_spare(L)) { park = true; on = false; if (COUNT && !kPhaseClock) cnt[29]++; }   // annihilation needs a slot
         }
         if (C == C_W) {
             // K3 + K4: flights against the majorant until at least kHitMin lanes have a collision to sample (or nobody flies
@@ -1041,7 +1043,7 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
         s_rings = P.rings + (size_t)blockIdx.x * kRings * kPool;
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < kPool; i += kThreads) __stcg(ring_cells(kFree) + i, (unsigned short)i);   // every slot is free
+    for (int i = threadIdx.x; i < kPool; i += kThreads) __stcg(ring_cells(kFree) + i, (ring_t)i);   // every slot is free
     __syncthreads();
 
     uint32_t cnt[COUNT ? 32 : 1];
@@ -1074,7 +1076,7 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
             default:  run_phase<COUNT, C_X>(L, P, sh, led, cnt); break;
         }
 #ifdef AEPID_PHASE_CLOCK
-        if (COUNT && lane == 0) atomicAdd(P.counters + 10, (unsigned long long)(clock64() - t0));   // busy warp-cycles
+        if (COUNT && lane == 0) { atomicAdd(P.counters + 10, (unsigned long long)(clock64() - t0)); atomicAdd(P.counters + 27 + ph, (unsigned long long)(clock64() - t0)); }   // busy warp-cycles
 #endif
         __syncthreads();
 #ifdef AEPID_PHASE_CLOCK
