@@ -235,7 +235,7 @@ int fill_params(aepid_ctx* ctx, TransportParams& p) {
     p.pool = reinterpret_cast<uint4*>(ctx->ws + ctx->lay.pool);
     p.rings = reinterpret_cast<ring_t*>(ctx->ws + ctx->lay.rings);
     p.n_batches = ctx->dims.n_batches; p.nvox = ctx->lay.nvox; p.npix = ctx->lay.npix;
-    p.base = 0; p.seed = 0; p.n = 0; p.hist_per_batch = 1;
+    p.base = 0; set_seed(p, 0); p.n = 0; p.hist_per_batch = 1;
     return 0;
 }
 
@@ -447,7 +447,7 @@ int aepid_simulate(aepid_ctx* ctx, unsigned long long n_histories, unsigned long
     unsigned long long left = n_histories;
     while (left > 0) {
         const unsigned long long n = std::min<unsigned long long>(left, 1ull << 31);
-        p.base = ctx->first_history + ctx->n_done; p.seed = seed; p.n = (uint32_t)n;
+        p.base = ctx->first_history + ctx->n_done; set_seed(p, seed); p.n = (uint32_t)n;
         const uint64_t hpb = (n + B - 1) / B;                  // history k of the launch -> batch k / hpb, exactly as in the kernel
         p.hist_per_batch = (uint32_t)hpb;
         CU(cudaMemsetAsync(ctx->d_chunk(), 0, sizeof(unsigned int), ctx->stream));
@@ -545,7 +545,7 @@ int aepid_sample_source(aepid_ctx* ctx, unsigned long long first, unsigned long 
     if (!out) return fail(ctx, AEPID_ERR_BAD_ARG, "null output");
     if (!ctx->have_source) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_load_source has not been called");
     TransportParams p{};
-    p.g = ctx->g; p.so = ctx->so; p.seed = seed;
+    p.g = ctx->g; p.so = ctx->so; set_seed(p, seed);
     if (classify(out) == MEM_DEVICE) {
         launch_sample_source(p, first, n, out, ctx->stream);
         CU(cudaGetLastError());

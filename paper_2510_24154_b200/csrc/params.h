@@ -85,6 +85,7 @@ struct TransportParams {
     ring_t* rings;             // slot-index rings [kMaxCtas][kRingCount][kPoolSlots], scratch of one launch
     uint64_t base;                     // global index of relative history 0 of this launch
     uint64_t seed;
+    uint32_t rk[20];                   // Philox round keys of `seed` (set_seed): rk[2r], rk[2r+1] = key of round r
     uint32_t n;                        // histories in this launch (< 2^32)
     uint32_t hist_per_batch;           // history k of the launch scores into batch min(k / hist_per_batch, B - 1)
     int n_batches;
@@ -100,6 +101,11 @@ struct FoldParams {
     double hist[256];                  // histories per batch
     double total;
 };
+
+inline void set_seed(TransportParams& p, uint64_t seed) {
+    p.seed = seed;
+    for (int r = 0; r < 10; ++r) { p.rk[2 * r] = (uint32_t)seed + 0x9E3779B9u * (uint32_t)r; p.rk[2 * r + 1] = (uint32_t)(seed >> 32) + 0xBB67AE85u * (uint32_t)r; }
+}
 
 // launchers (defined in transport.cu / postpass.cu)
 int launch_transport(const TransportParams& p, bool counting, int sm_count, void* stream);

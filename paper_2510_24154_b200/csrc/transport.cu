@@ -159,7 +159,8 @@ __device__ __noinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c
     return make_uint4(c0, c1, c2, c3);
 }
 // uniform in (0,1) from the top 23 bits: ((r >> 9) + 0.5) 2^-23 is exact in float32 and never 0 or 1
-__device__ __forceinline__ float u01(uint32_t r) { return ((float)(r >> 9) + 0.5f) * 1.1920928955078125e-7f; }
+// (built in the mantissa of a float in [1, 2), no integer conversion; the subtraction is exact)
+__device__ __forceinline__ float u01(uint32_t r) { return __uint_as_float(0x3f800000u | (r >> 9)) - 0.99999994f; }
 
 // approximate reciprocal (MUFU.RCP): geometry distances and sampling formulas do not need the IEEE one
 __device__ __forceinline__ float rcp(float x) { return __fdividef(1.0f, x); }
@@ -169,6 +170,21 @@ __device__ __forceinline__ uint4 rng_block(Lane& L, const TransportParams& P) {
     const uint4 o = philox4x32_10((uint32_t)h, (uint32_t)(h >> 32), L.pid, L.blk, (uint32_t)P.seed, (uint32_t)(P.seed >> 32));
     L.blk++;
     return o;
+}
+// The same block, expanded in place with the round keys taken from the kernel parameters (constant-bank operands: no
+// key arithmetic, no call): for the three hottest draw sites (electron steps, Woodcock flights, Klein-Nishina trials).
+__device__ __forceinline__ uint4 rng_block_hot(Lane& L, const TransportParams& P) {
+    const uint64_t h = P.base + L.h;
+    uint32_t c0 = (uint32_t)h, c1 = (uint32_t)(h >> 32), c2 = L.pid, c3 = L.blk;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ P.rk[2 * r], n2 = hi0 ^ c3 ^ P.rk[2 * r + 1];
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    }
+    L.blk++;
+    return make_uint4(c0, c1, c2, c3);
 }
 __device__ __forceinline__ uint32_t child_id(const Lane& L, uint32_t sibling) {    // reading A1
     return L.pid * 0x9E3779B1u + L.blk * 2u + sibling + 1u;
@@ -451,7 +467,7 @@ __device__ __forceinline__ void interact(Lane& L, const TransportParams& P, cons
         float eps, t, x4;
 #pragma unroll 1
         for (;;) {
-            const uint4 r = rng_block(L, P);                               // one block per trial
+            const uint4 r = rng_block_hot(L, P);                           // one block per trial
             const float x1 = u01(r.x), x2 = u01(r.y), x3 = u01(r.z); x4 = u01(r.w);
             if (COUNT) cnt[12]++;
             eps = (x1 * (a1 + a2) < a1) ? __expf(-x2 * a1) : sqrtf(fmaf(1.0f - e02, x2, e02));
@@ -511,7 +527,7 @@ __device__ __forceinline__ void interact(Lane& L, const TransportParams& P, cons
 template <bool COUNT>
 __device__ __forceinline__ bool woodcock_flight(Lane& L, const TransportParams& P, const Shared& sh, float& xsel, float& pe, float& co, uint32_t* cnt) {
     const Geom& g = P.g;
-    const uint4 rr = rng_block(L, P);
+    const uint4 rr = rng_block_hot(L, P);
     const float u1 = u01(rr.x), u2 = u01(rr.y);
     if (COUNT) cnt[0]++;
     const float s = __fdividef(-__logf(u1), L.mumaj);
@@ -767,10 +783,10 @@ __device__ __forceinline__ void electron_step_outside(Lane& L, const TransportPa
 template <bool COUNT, bool PHANTOM>
 __device__ __forceinline__ void charged_event(Lane& L, const TransportParams& P, const Shared& sh, uint32_t* cnt) {
     if (L.E <= P.ph.ecut) { stop_charged<COUNT>(L, P, cnt); return; }
-    uint4 r = rng_block(L, P);
+    uint4 r = PHANTOM ? rng_block_hot(L, P) : rng_block(L, P);
 #pragma unroll 1
     for (int k = 0; k < (PHANTOM ? kStepsE : kStepsX); ++k) {
-        if (k && !(k & 1)) r = rng_block(L, P);
+        if (k && !(k & 1)) r = PHANTOM ? rng_block_hot(L, P) : rng_block(L, P);
         if (PHANTOM) electron_step_phantom<COUNT>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, cnt);
         else electron_step_outside<COUNT>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, cnt);
         if (!L.alive) break;
