@@ -93,10 +93,10 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def build_cfg(name):
+def build_cfg(name, field=0):
     from gen import make_config
     from gen.configs import paper_table1_lut
-    cfg = make_config(name)
+    cfg = make_config(name, field=field)
     if cfg.get("lut") is None:
         cfg["lut"] = paper_table1_lut()          # PAPER.md:157-162 Table 1 as the response LUT (C4 brings its own)
     return cfg
@@ -109,7 +109,7 @@ def run_reference(args):
     if rank != 0:
         return
     import oracle
-    cfg = build_cfg(args.config)
+    cfg = build_cfg(args.config, args.field)
     procs = os.cpu_count() or 1
     sample = args.ref_histories
     oracle.build()
@@ -155,7 +155,7 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    cfg = build_cfg(args.config)
+    cfg = build_cfg(args.config, args.field)
     n = int(args.histories or cfg["n_histories"])
     n_total = n * world
     seed = cfg["seed"]
@@ -295,7 +295,7 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": "%s (BASELINE.json configs[%s])" % (args.config, args.config[1:]), "histories_per_gpu_per_step": n,
+            "config": {"workload": "%s (BASELINE.json configs[%s])%s" % (args.config, args.config[1:], " field %d" % args.field if args.config == "C4" else ""), "histories_per_gpu_per_step": n,
                        "n_batches": eng.n_batches, "l2": "flushed between timed steps (256 MiB write)",
                        "parallelism": "history-range sharding x%d, one all-reduce of tally moments per step" % world if world > 1 else "single GPU"},
             "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
@@ -315,6 +315,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3", "C4"])
+    ap.add_argument("--field", type=int, default=0, help="which of C4's 25 IMRT fields (seeds per reading A23)")
     ap.add_argument("--histories", type=int, default=0, help="histories per GPU per step (default: the config's)")
     ap.add_argument("--cpu-sample", type=int, default=1_000_000, help="oracle histories timed for cpu_baseline")
     ap.add_argument("--ref-histories", type=int, default=400_000, help="oracle histories per step of --impl reference")
