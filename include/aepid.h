@@ -170,6 +170,21 @@ int aepid_apply_response_lut(aepid_ctx* ctx, const float* lut, int nt, int ns,
                              float t_min, float t_max, float s_min, float s_max, float s_eff_cm,
                              const float* epid_in, float* signal_out, float* tmap_out);
 
+/* Analysis chain (section 2.3.3).
+ * aepid_upsample: out [mv][mu] = bilinear interpolant of in [nv][nu] over the same physical area: output pixel (j, i)
+ * is taken at x = (i + 0.5) nu/mu - 0.5, y = (j + 0.5) nv/mv - 0.5 in input pixels (centres at the integers), clamped to
+ * [0, n - 1] (reading A28).  DEVICE pointers, caller-owned; asynchronous on the context's stream.
+ * aepid_gamma_index: global 2-D gamma of `eval` against `ref` (same grid [nv][nu], non-negative, pixel pitch pitch_cm):
+ * gamma = min over evaluated pixels within gamma_cap * dta_cm of sqrt(dist^2/dta^2 + (D_e - D_r)^2/(dose_frac max(ref))^2),
+ * reported as min(gamma_cap, gamma); reference pixels below threshold_frac * max(ref) get -1 and are not counted
+ * (reading A29).  ref, eval, gamma_out: DEVICE [nv][nu].  stats (HOST [4], may be NULL; when given the call
+ * synchronises) = tested pixels, pixels with gamma <= 1, mean gamma, max gamma over the tested pixels.
+ * AEPID_ERR_NOMEM if the window of gamma_cap * dta_cm / pitch_cm pixels does not fit in shared memory (about 90 pixels). */
+int aepid_upsample(aepid_ctx* ctx, const float* in, int nu, int nv, float* out, int mu, int mv);
+int aepid_gamma_index(aepid_ctx* ctx, const float* ref, const float* eval, int nu, int nv, float pitch_cm,
+                      float dose_frac, float dta_cm, float threshold_frac, float gamma_cap,
+                      float* gamma_out, double stats[4]);
+
 /* Block until everything queued on the context's stream has finished. */
 int aepid_synchronize(aepid_ctx* ctx);
 

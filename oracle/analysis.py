@@ -45,13 +45,15 @@ def gamma_index(ref, ev, pitch_cm, dose_frac, dta_cm, threshold_frac=0.10, cap=2
     gamma(r) = min over evaluated grid points e of sqrt(|x_e - x_r|^2 / DTA^2 + (D_e - D_r)^2 / (dose_frac D_max)^2),
     D_max = max of the reference (global normalisation), reported as min(cap, gamma): grid points farther than
     cap * DTA cannot bring gamma below cap, so the search window is the disc of that radius.
-    Reference pixels below threshold_frac * D_max are not tested and get gamma = -1.
+    Reference pixels below threshold_frac * D_max are not tested and get gamma = -1; an all-zero reference tests nothing.
     Returns (gamma [nv][nu], stats) with stats = (n_tested, n_pass (gamma <= 1), mean gamma, max gamma) over tested pixels.
     """
     r = np.asarray(ref, dtype=np.float64)
     e = np.asarray(ev, dtype=np.float64)
     nv, nu = r.shape
     dmax = r.max()
+    if not dmax > 0.0:
+        return np.full((nv, nu), -1.0), (0, 0, 0.0, 0.0)
     dd = dose_frac * dmax
     w = int(np.floor(cap * dta_cm / pitch_cm + 1e-9))
     g2 = np.full((nv, nu), cap * cap, dtype=np.float64)

@@ -29,7 +29,7 @@ EXPORTS = ("aepid_workspace_bytes", "aepid_create", "aepid_destroy", "aepid_last
            "aepid_reset_tallies", "aepid_simulate", "aepid_read_tallies", "aepid_read_batches",
            "aepid_set_counting", "aepid_read_counters", "aepid_sample_source", "aepid_field_size",
            "aepid_apply_response_lut", "aepid_synchronize", "aepid_set_history_offset", "aepid_read_moments",
-           "aepid_finalize_moments")
+           "aepid_finalize_moments", "aepid_upsample", "aepid_gamma_index")
 
 
 class AepidError(RuntimeError):
@@ -77,6 +77,8 @@ def load_library():
     lib.aepid_set_history_offset.argtypes = [vp, C.c_ulonglong]
     lib.aepid_read_moments.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.aepid_finalize_moments.argtypes = [vp, vp, vp, C.c_size_t, C.c_double, C.c_double, vp, vp]
+    lib.aepid_upsample.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int, C.c_int]
+    lib.aepid_gamma_index.argtypes = [vp, vp, vp, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_float, C.c_float, vp, vp]
     _lib = lib
     return lib
 
@@ -263,6 +265,39 @@ class Engine:
         s = C.c_float()
         self._chk(self._lib.aepid_field_size(self._h, int(bool(printed_form)), C.byref(s)))
         return float(s.value)
+
+    def _device_image(self, a):
+        """float32 device tensor of a numpy array or tensor (marshalling: the C-ABI wants device pointers here)."""
+        import torch
+        if isinstance(a, np.ndarray):
+            a = torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32))
+        return a.to(device=self.device, dtype=torch.float32).contiguous()
+
+    def upsample(self, image, mv, mu, out=None):
+        """K9: bilinear up-sampling of image [nv][nu] to [mv][mu]; returns a device tensor."""
+        import torch
+        a = self._device_image(image)
+        nv, nu = (int(v) for v in a.shape)
+        if out is None:
+            out = torch.empty((int(mv), int(mu)), dtype=torch.float32, device=self.device)
+        self._chk(self._lib.aepid_upsample(self._h, _ptr(a), nu, nv, _ptr(out), int(mu), int(mv)))
+        return out
+
+    def gamma_index(self, ref, ev, pitch_cm, dose_frac=0.03, dta_cm=0.3, threshold_frac=0.10, cap=2.0, out=None):
+        """K10: global gamma index of ev against ref (same grid); returns (gamma device tensor, stats dict)."""
+        import torch
+        r, e = self._device_image(ref), self._device_image(ev)
+        if r.shape != e.shape or r.dim() != 2:
+            raise ValueError("ref and ev must be 2-D images of the same shape")
+        nv, nu = (int(v) for v in r.shape)
+        if out is None:
+            out = torch.empty((nv, nu), dtype=torch.float32, device=self.device)
+        st = np.zeros(4, dtype=np.float64)
+        self._chk(self._lib.aepid_gamma_index(self._h, _ptr(r), _ptr(e), nu, nv, float(pitch_cm), float(dose_frac), float(dta_cm),
+                                              float(threshold_frac), float(cap), _ptr(out), _ptr(st)))
+        n = int(st[0])
+        return out, {"n_tested": n, "n_pass": int(st[1]), "pass_rate": (st[1] / st[0]) if n else float("nan"),
+                     "mean_gamma": float(st[2]), "max_gamma": float(st[3])}
 
     def apply_response_lut(self, lut, t_min, t_max, s_min, s_max, s_eff=-1.0, epid_in=None, signal_out=None, tmap_out=None,
                            want_tmap=True):

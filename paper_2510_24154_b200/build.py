@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libaepid.so")
-SOURCES = ["transport.cu", "postpass.cu", "api.cu"]
+SOURCES = ["transport.cu", "postpass.cu", "analysis.cu", "api.cu"]
 HEADERS = [os.path.join(CSRC, "params.h"), os.path.join(os.path.dirname(HERE), "include", "aepid.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]

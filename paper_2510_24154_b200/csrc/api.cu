@@ -59,7 +59,7 @@ Layout make_layout(const aepid_dims& d) {
     L.guideF = take(((size_t)kGuideSize + 1) * 4);
     L.pool = take((size_t)kMaxCtas * kPoolSlots * kRecordBytes);   // particle pools of the transport kernel (scratch)
     L.rings = take((size_t)kMaxCtas * kRingCount * kPoolSlots * sizeof(ring_t));
-    L.small = take(1024);            // ledger [8] f64 @0 | chunk counter @64 | rho_max [32] f32 @128 | counters [32] u64 @256
+    L.small = take(1024);            // ledger [8] f64 @0 | chunk counter @64 | rho_max [32] f32 @128 | counters [32] u64 @256 | gamma stats [4] f64 @512, max bits @544
     L.total = o;
     return L;
 }
@@ -106,6 +106,8 @@ struct aepid_ctx {
     unsigned long long* d_counters() { return reinterpret_cast<unsigned long long*>(ws + lay.small + 256); }
     unsigned int* d_chunk() { return reinterpret_cast<unsigned int*>(ws + lay.small + 64); }
     float* d_rho_max() { return reinterpret_cast<float*>(ws + lay.small + 128); }
+    double* d_gamma_stats() { return reinterpret_cast<double*>(ws + lay.small + 512); }
+    unsigned int* d_gamma_max() { return reinterpret_cast<unsigned int*>(ws + lay.small + 544); }
 };
 
 namespace {
@@ -613,6 +615,39 @@ int aepid_apply_response_lut(aepid_ctx* ctx, const float* lut, int nt, int ns, f
     if (!dev_out) if (int rc = deliver(ctx, signal_out, d_out, n * 4, &need_sync)) return rc;
     if (tmap_out) if (int rc = deliver(ctx, tmap_out, ctx->d_tmap(), n * 4, &need_sync)) return rc;
     if (need_sync) CU(cudaStreamSynchronize(ctx->stream));
+    return 0;
+}
+
+int aepid_upsample(aepid_ctx* ctx, const float* in, int nu, int nv, float* out, int mu, int mv) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    if (!in || !out) return fail(ctx, AEPID_ERR_BAD_ARG, "null image pointer");
+    if (nu < 1 || nv < 1 || mu < 1 || mv < 1 || nu > 32768 || nv > 32768 || mu > 32768 || mv > 32768) return fail(ctx, AEPID_ERR_BAD_ARG, "image size out of range");
+    if (classify(in) != MEM_DEVICE || classify(out) != MEM_DEVICE) return fail(ctx, AEPID_ERR_BAD_ARG, "aepid_upsample takes device pointers");
+    launch_upsample(in, nu, nv, out, mu, mv, ctx->stream);
+    CU(cudaGetLastError());
+    return 0;
+}
+
+int aepid_gamma_index(aepid_ctx* ctx, const float* ref, const float* eval, int nu, int nv, float pitch_cm, float dose_frac, float dta_cm,
+                      float threshold_frac, float gamma_cap, float* gamma_out, double stats[4]) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    if (!ref || !eval || !gamma_out) return fail(ctx, AEPID_ERR_BAD_ARG, "null image pointer");
+    if (nu < 1 || nv < 1 || nu > 32768 || nv > 32768) return fail(ctx, AEPID_ERR_BAD_ARG, "image size out of range");
+    if (!(pitch_cm > 0) || !(dose_frac > 0) || !(dta_cm > 0) || !(threshold_frac >= 0) || !(gamma_cap >= 1))
+        return fail(ctx, AEPID_ERR_BAD_ARG, "gamma criteria out of range (pitch, dose fraction, DTA > 0; threshold >= 0; cap >= 1)");
+    if (classify(ref) != MEM_DEVICE || classify(eval) != MEM_DEVICE || classify(gamma_out) != MEM_DEVICE)
+        return fail(ctx, AEPID_ERR_BAD_ARG, "aepid_gamma_index takes device pointers for the images");
+    if (launch_gamma(ref, eval, gamma_out, nu, nv, pitch_cm, dose_frac, dta_cm, threshold_frac, gamma_cap, ctx->d_gamma_max(),
+                     ctx->d_gamma_stats(), ctx->stream) != 0)
+        return fail(ctx, AEPID_ERR_NOMEM, "search window (cap x DTA / pitch pixels) does not fit in shared memory");
+    CU(cudaGetLastError());
+    if (stats) {
+        double h[4];
+        CU(cudaMemcpyAsync(h, ctx->d_gamma_stats(), sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        stats[0] = h[0]; stats[1] = h[1]; stats[2] = h[0] > 0 ? h[2] / h[0] : 0.0;
+        stats[3] = h[3];                                               // kept on the device as the bit pattern of a non-negative double
+    }
     return 0;
 }
 

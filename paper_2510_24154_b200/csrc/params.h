@@ -119,5 +119,9 @@ void launch_tmap(const Geom& g, const uint32_t* vox, float* tmap, void* stream);
 void launch_apply_lut(const float* lut, int nt, int ns, float t_min, float t_max, float s_min, float s_max,
                       float s_eff, const float* dose, const float* tmap, float* out, size_t n, void* stream);
 void launch_zero(void* ptr, size_t bytes, void* stream);
+// analysis.cu
+void launch_upsample(const float* in, int nu, int nv, float* out, int mu, int mv, void* stream);
+int launch_gamma(const float* ref, const float* ev, float* gamma, int nu, int nv, float pitch, float dose_frac, float dta,
+                 float thr_frac, float cap, unsigned int* dmax_bits, double* stats, void* stream);
 
 }  // namespace aepid

@@ -1,0 +1,116 @@
+"""GPU parity of the analysis chain (K9 up-sampling, K10 gamma index) against oracle/analysis.py,
+through the C-ABI.  Tolerances: the kernels work in float32, the oracle in float64."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def eng():
+    from gen import make_config
+    from paper_2510_24154_b200 import Engine
+    cfg = make_config("C0")
+    e = Engine.for_config(cfg)
+    e.load_config(cfg)
+    yield e
+    e.close()
+
+
+def synthetic_epid_image(nv, nu, seed, noise=0.0):
+    """Smooth IMRT-like image: a few soft-edged rectangles on a low background (inputs only, no method arithmetic)."""
+    rng = np.random.default_rng(seed)
+    y, x = np.mgrid[0:nv, 0:nu].astype(np.float64)
+    img = np.full((nv, nu), 0.02)
+    for _ in range(5):
+        cx, cy = rng.uniform(0.3, 0.7) * nu, rng.uniform(0.3, 0.7) * nv
+        wx, wy = rng.uniform(0.08, 0.25) * nu, rng.uniform(0.08, 0.25) * nv
+        edge = 0.015 * nu
+        img += rng.uniform(0.2, 1.0) / ((1 + np.exp((np.abs(x - cx) - wx) / edge)) * (1 + np.exp((np.abs(y - cy) - wy) / edge)))
+    if noise:
+        img *= 1 + noise * rng.standard_normal(img.shape)
+    return np.maximum(img, 0.0)
+
+
+@pytest.mark.parametrize("nv,nu,mv,mu", [(23, 37, 67, 101), (160, 160, 1190, 1190), (5, 1, 9, 4), (64, 48, 64, 48), (40, 60, 13, 7)])
+def test_upsample_matches_oracle(eng, nv, nu, mv, mu):
+    from oracle import analysis as A
+    img = synthetic_epid_image(nv, nu, 7, noise=0.05).astype(np.float32)
+    got = eng.upsample(img, mv, mu).cpu().numpy()
+    exp = A.upsample_bilinear(img, mv, mu)
+    assert got.shape == exp.shape
+    assert np.abs(got - exp).max() <= 3e-6 * img.max()
+
+
+def _compare_gamma(g, st, go, sto, ref, thr):
+    tested_o = go >= 0
+    tested_g = g >= 0
+    edge = np.abs(ref - thr * ref.max()) <= 1e-6 * ref.max()            # threshold decided in float32 vs float64
+    assert np.all((tested_o == tested_g) | edge)
+    both = tested_o & tested_g
+    assert np.abs(g[both] - go[both]).max() <= 3e-5
+    assert abs(st["n_tested"] - sto[0]) <= edge.sum()
+    near_one = int((np.abs(go[both] - 1.0) <= 3e-5).sum())
+    assert abs(st["n_pass"] - sto[1]) <= near_one + edge.sum()
+    assert abs(st["mean_gamma"] - sto[2]) <= 1e-4
+    assert abs(st["max_gamma"] - sto[3]) <= 1e-4
+
+
+@pytest.mark.parametrize("nv,nu,pitch,frac,dta", [(45, 70, 0.05, 0.03, 0.3), (33, 31, 0.0784, 0.02, 0.2), (16, 200, 0.1, 0.03, 0.2), (1, 1, 0.1, 0.03, 0.3)])
+def test_gamma_matches_oracle_elementwise(eng, nv, nu, pitch, frac, dta):
+    from oracle import analysis as A
+    ref = synthetic_epid_image(nv, nu, 21).astype(np.float32)
+    ev = (synthetic_epid_image(nv, nu, 21) * (1 + 0.03 * np.random.default_rng(4).standard_normal((nv, nu)))).astype(np.float32)
+    ev = np.roll(ev, 1, axis=1)                                          # plus a one-pixel shift along u
+    g, st = eng.gamma_index(ref, ev, pitch, frac, dta, 0.10, 2.0)
+    go, sto = A.gamma_index(ref, ev, pitch, frac, dta, 0.10, 2.0)
+    _compare_gamma(g.cpu().numpy(), st, go, sto, ref.astype(np.float64), 0.10)
+
+
+def test_gamma_full_size_paper_criteria(eng):
+    """1190 x 1190 at 0.336 mm (the measured grid of PAPER.md:141), 3 %/3 mm, 3 %/2 mm, 2 %/2 mm, 10 % threshold."""
+    from oracle import analysis as A
+    n, pitch = 1190, 40.0 / 1190
+    ref = synthetic_epid_image(160, 160, 33)
+    ev = synthetic_epid_image(160, 160, 33, noise=0.02)
+    ref_up = eng.upsample(ref.astype(np.float32), n, n)
+    ev_up = eng.upsample(ev.astype(np.float32), n, n)
+    r, e = ref_up.cpu().numpy(), ev_up.cpu().numpy()
+    for k, (frac, dta) in enumerate(((0.03, 0.3), (0.03, 0.2), (0.02, 0.2))):
+        g, st = eng.gamma_index(ref_up, ev_up, pitch, frac, dta, 0.10, 2.0)
+        if k == 0:                                                       # full oracle once (about 20 s), sampled strips for the others
+            go, sto = A.gamma_index(r, e, pitch, frac, dta, 0.10, 2.0)
+            _compare_gamma(g.cpu().numpy(), st, go, sto, r.astype(np.float64), 0.10)
+        else:
+            # a strip of rows with its full search halo is an exact sub-problem once the global maximum is pinned by
+            # keeping the row that holds it
+            jm = int(np.unravel_index(np.argmax(r), r.shape)[0])
+            w = int(2.0 * dta / pitch) + 1
+            lo, hi = max(jm - 40 - w, 0), min(jm + 40 + w, n)
+            go, _ = A.gamma_index(r[lo:hi], e[lo:hi], pitch, frac, dta, 0.10, 2.0)
+            gg = g.cpu().numpy()[lo:hi]
+            inner = slice(w if lo > 0 else 0, (hi - lo) - (w if hi < n else 0))
+            both = (go[inner] >= 0) & (gg[inner] >= 0)
+            assert both.sum() > 10000
+            assert np.abs(gg[inner][both] - go[inner][both]).max() <= 3e-5
+        assert 0.0 <= st["pass_rate"] <= 1.0
+
+
+def test_gamma_degenerate_and_errors(eng):
+    import torch
+    from paper_2510_24154_b200.binding import AepidError
+    z = np.zeros((8, 9), dtype=np.float32)
+    g, st = eng.gamma_index(z, z, 0.1)
+    assert st["n_tested"] == 0 and np.all(g.cpu().numpy() == -1.0)
+    a = synthetic_epid_image(12, 12, 1).astype(np.float32)
+    g, st = eng.gamma_index(a, a, 0.1)
+    assert st["n_pass"] == st["n_tested"] > 0 and st["max_gamma"] == 0.0
+    with pytest.raises(AepidError):                                      # window of 2 * 3 cm / 0.01 cm = 600 pixels
+        eng.gamma_index(a, a, 0.01, 0.03, 3.0)
+    with pytest.raises(AepidError):
+        eng.gamma_index(a, a, 0.1, dose_frac=0.0)
+    lib = eng._lib
+    host = np.zeros((4, 4), dtype=np.float32)
+    dev = torch.zeros((4, 4), dtype=torch.float32, device=eng.device)
+    assert lib.aepid_upsample(eng._h, host.ctypes.data, 4, 4, dev.data_ptr(), 4, 4) == -1      # host pointer: BAD_ARG
+    assert lib.aepid_gamma_index(eng._h, dev.data_ptr(), host.ctypes.data, 4, 4, 0.1, 0.03, 0.3, 0.1, 2.0, dev.data_ptr(), None) == -1

@@ -149,6 +149,14 @@ def test_c1_coupled_full_size_bench_configuration():
     compare(cfg, cfg["n_histories"], 4_000_000, rebin=8)   # 512x384 @ 0.784 mm -> 64x48 @ 6.3 mm (~100 oracle events / pixel)
 
 
+def test_paper_scoring_grid_160x160_at_2p5mm():
+    """The scoring grid the paper itself uses (2.5 mm pixels, 160 x 160 image) on the C1 workload."""
+    from gen.configs import epid_stack
+    cfg = make_config("C1")
+    cfg["epid"] = epid_stack("C1", 160, 160, 0.25, 150.0)
+    compare(cfg, cfg["n_histories"], 4_000_000, rebin=4, phantom_voxels=False)   # 40x40 @ 1 cm: ~90 oracle events per tested pixel
+
+
 def test_c2_heterogeneous_imrt_full_grid():
     cfg = make_config("C2")
     compare(cfg, 40_000_000, 2_000_000, rebin=32, frac_ok=0.985, phantom_voxels=False, min_tested=15)
