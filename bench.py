@@ -38,6 +38,11 @@ EVENTS_PER_HISTORY = {
 }
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of transport_kernel per history, from the committed ncu --set full capture
+# (profiles/r01f_README.md: 2.385 GB + 1.948 GB for 1e7 histories of C1); None where no capture exists.
+DRAM_BYTES_PER_HISTORY = {"C1": 433.3}
+
+
 def alg_instr_per_history(name):
     ev = EVENTS_PER_HISTORY.get(name, EVENTS_PER_HISTORY["C1"])
     return float(sum(INSTR_PER_EVENT[k] * v for k, v in ev.items()))
@@ -276,7 +281,7 @@ def run_ours(args):
     alg = alg_instr_per_history(args.config)
     achieved = alg * n / (kernel_ms / args.steps * 1e-3) / 1e9
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_ginstr, "unit": "Gthread-instr/s", "frac": achieved / peak_ginstr,
-                "traffic": None, "kernel": "transport_kernel", "kernel_ms_per_launch": kernel_ms / args.steps,
+                "traffic": DRAM_BYTES_PER_HISTORY.get(args.config) and DRAM_BYTES_PER_HISTORY[args.config] * n, "kernel": "transport_kernel", "kernel_ms_per_launch": kernel_ms / args.steps,
                 "alg_thread_instr_per_history": alg, "peak_source": "%s sm_max_mhz x %d SMs x 4 schedulers x 32 lanes" % (which, sm_count),
                 "hbm_gbs_peak": peaks.get("hbm_gbs")}
 
