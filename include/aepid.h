@@ -170,6 +170,17 @@ int aepid_apply_response_lut(aepid_ctx* ctx, const float* lut, int nt, int ns,
                              float t_min, float t_max, float s_min, float s_max, float s_eff_cm,
                              const float* epid_in, float* signal_out, float* tmap_out);
 
+/* Phase Space 3 ("an additional scoring plane, Phase Space 3, is generated to store all particles exiting
+ * the patient"; reading A30): while a buffer is set, every particle that arrives at the EPID top plane (w = sid) from the
+ * air is copied into it as two float4 = {u, v, du, dv} {dw, E, type bits, history bits}: position and direction in the beam
+ * frame (cm; dw > 0), photon energy or kinetic energy (MeV), type 0 photon / 1 electron / 2 positron and the global history
+ * index modulo 2^32 as raw 32-bit patterns.  The particle itself flies on (the hand-off stays in flight); the order of the
+ * records is not defined.  records: DEVICE, 16-byte aligned, 32 * capacity bytes, caller-owned and kept alive while set;
+ * NULL switches the recording off.  Setting a buffer and aepid_reset_tallies zero the arrival count.
+ * aepid_read_phase_space_count (synchronises): arrivals since then; only the first `capacity` claimed records are stored. */
+int aepid_set_phase_space(aepid_ctx* ctx, void* records, unsigned long long capacity);
+int aepid_read_phase_space_count(aepid_ctx* ctx, unsigned long long* n_arrived);
+
 /* Analysis chain (section 2.3.3).
  * aepid_upsample: out [mv][mu] = bilinear interpolant of in [nv][nu] over the same physical area: output pixel (j, i)
  * is taken at x = (i + 0.5) nu/mu - 0.5, y = (j + 0.5) nv/mv - 0.5 in input pixels (centres at the integers), clamped to

@@ -38,6 +38,7 @@ def lib():
         _lib = C.CDLL(build())
         _lib.orc_create.restype = C.c_void_p
         _lib.orc_last_error.restype = C.c_char_p
+        _lib.orc_ps3_count.restype = C.c_uint64
         for f in ("orc_stop_pow", "orc_majorant", "orc_highland_theta0", "orc_field_size", "orc_lut_bilinear"):
             getattr(_lib, f).restype = C.c_double
     return _lib
@@ -179,6 +180,17 @@ class Oracle:
                                    _p(out["phantom_sum"], C.c_double), _p(out["phantom_sq"], C.c_double),
                                    _p(out["uncollided"], C.c_double), _p(out["ledger"], C.c_double),
                                    _p(out["counters"], C.c_uint64), _p(out["aux"], C.c_double), _p(out["fc_hist"], C.c_double)))
+        return out
+
+    # ---- Phase Space 3 (reading A30)
+    def set_ps3(self, on=True):
+        self._chk(self._l.orc_set_ps3(self._h, int(bool(on))))
+
+    def read_ps3(self):
+        """Records [n][8] = {type, E, u, v, du, dv, dw, history} of every particle that arrived at the EPID top plane."""
+        n = int(self._l.orc_ps3_count(self._h))
+        out = np.empty((n, 8))
+        self._chk(self._l.orc_read_ps3(self._h, _p(out, C.c_double)))
         return out
 
     # ---- unit-level entry points

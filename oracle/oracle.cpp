@@ -163,6 +163,9 @@ struct Ctx {
     // per-history scratch
     std::vector<std::pair<int64_t, double>> hpix, hvox;
     std::vector<Particle> stack;
+    // Phase Space 3 (reading A30): every particle arriving at the EPID top plane from the air,
+    // 8 doubles per record = {type, E, u, v, du, dv, dw (beam frame), history index}
+    bool ps3_on = false; uint64_t cur_h = 0; std::vector<double> ps3;
 };
 
 // ---------------------------------------------------------------- tables
@@ -369,6 +372,7 @@ void enter_epid(Ctx& c, Particle& p, double t) {
     p.pos = p.pos + t * p.dir;
     Vec3 pb = to_beam(c, p.pos); pb.z = c.sid;
     p.dir = dir_to_beam(c, p.dir); p.pos = pb; p.region = EPID; p.layer = 0;
+    if (c.ps3_on) { const double rec[8] = {(double)p.type, p.E, pb.x, pb.y, p.dir.x, p.dir.y, p.dir.z, (double)c.cur_h}; c.ps3.insert(c.ps3.end(), rec, rec + 8); }
     if (p.type == PHOTON && p.uncollided) {                        // pin P3 / P10 tally
         c.counters[10]++;
         const double fu = std::floor((pb.x + 0.5 * c.nu * c.pitch) / c.pitch);
@@ -819,6 +823,7 @@ int orc_run(orc_ctx* x, uint64_t first, uint64_t n, uint64_t seed) {
     Run r{seed};
     for (uint64_t h = first; h < first + n; ++h) {
         Particle p{};
+        c.cur_h = h;
         p.rng.init(seed, h, 0);
         const SourceSample s = sample_source(c, p.rng);             // block 0 of particle 0 (reading A1)
         p.type = PHOTON; p.E = s.E; p.pos = c.src; p.dir = s.dir_world; p.region = AIR; p.uncollided = true;
@@ -858,6 +863,11 @@ int orc_read(orc_ctx* x, double* ep_sum, double* ep_sq, double* rb_sum, double* 
     if (aux) std::memcpy(aux, c.aux, sizeof(c.aux));
     return 0;
 }
+
+// Phase Space 3: switch the recording on / off (clears the store), number of records, copy out [n][8].
+int orc_set_ps3(orc_ctx* x, int on) { Ctx& c = C(x); c.ps3_on = on != 0; c.ps3.clear(); return 0; }
+uint64_t orc_ps3_count(orc_ctx* x) { return C(x).ps3.size() / 8; }
+int orc_read_ps3(orc_ctx* x, double* out) { Ctx& c = C(x); if (!c.ps3.empty()) std::memcpy(out, c.ps3.data(), c.ps3.size() * sizeof(double)); return 0; }
 
 // ---- unit-level entry points for the pins
 int orc_mu_partial(orc_ctx* x, int m, double E, double out[3]) { mu_partial(C(x), m, E, out); return 0; }

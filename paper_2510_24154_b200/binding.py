@@ -29,7 +29,8 @@ EXPORTS = ("aepid_workspace_bytes", "aepid_create", "aepid_destroy", "aepid_last
            "aepid_reset_tallies", "aepid_simulate", "aepid_read_tallies", "aepid_read_batches",
            "aepid_set_counting", "aepid_read_counters", "aepid_sample_source", "aepid_field_size",
            "aepid_apply_response_lut", "aepid_synchronize", "aepid_set_history_offset", "aepid_read_moments",
-           "aepid_finalize_moments", "aepid_upsample", "aepid_gamma_index")
+           "aepid_finalize_moments", "aepid_upsample", "aepid_gamma_index",
+           "aepid_set_phase_space", "aepid_read_phase_space_count")
 
 
 class AepidError(RuntimeError):
@@ -77,6 +78,8 @@ def load_library():
     lib.aepid_set_history_offset.argtypes = [vp, C.c_ulonglong]
     lib.aepid_read_moments.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.aepid_finalize_moments.argtypes = [vp, vp, vp, C.c_size_t, C.c_double, C.c_double, vp, vp]
+    lib.aepid_set_phase_space.argtypes = [vp, vp, C.c_ulonglong]
+    lib.aepid_read_phase_space_count.argtypes = [vp, vp]
     lib.aepid_upsample.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int, C.c_int]
     lib.aepid_gamma_index.argtypes = [vp, vp, vp, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_float, C.c_float, vp, vp]
     _lib = lib
@@ -265,6 +268,27 @@ class Engine:
         s = C.c_float()
         self._chk(self._lib.aepid_field_size(self._h, int(bool(printed_form)), C.byref(s)))
         return float(s.value)
+
+    def set_phase_space(self, capacity):
+        """Record Phase Space 3 into a device buffer of `capacity` records (0: switch off)."""
+        import torch
+        if not capacity:
+            self._ps3 = None
+            self._chk(self._lib.aepid_set_phase_space(self._h, None, 0))
+            return
+        self._ps3 = torch.empty((int(capacity), 8), dtype=torch.float32, device=self.device)
+        self._chk(self._lib.aepid_set_phase_space(self._h, _ptr(self._ps3), int(capacity)))
+
+    def read_phase_space(self):
+        """(records [n][8] float64 = {type, E, u, v, du, dv, dw, history}, arrivals): the stored records and the total count."""
+        n = C.c_ulonglong(0)
+        self._chk(self._lib.aepid_read_phase_space_count(self._h, C.byref(n)))
+        k = min(int(n.value), int(self._ps3.shape[0]))
+        raw = self._ps3[:k].cpu().numpy()
+        bits = raw.view(np.uint32)
+        out = np.empty((k, 8))
+        out[:, 0] = bits[:, 6]; out[:, 1] = raw[:, 5]; out[:, 2:6] = raw[:, 0:4]; out[:, 6] = raw[:, 4]; out[:, 7] = bits[:, 7]
+        return out, int(n.value)
 
     def _device_image(self, a):
         """float32 device tensor of a numpy array or tensor (marshalling: the C-ABI wants device pointers here)."""

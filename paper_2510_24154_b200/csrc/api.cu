@@ -59,7 +59,7 @@ Layout make_layout(const aepid_dims& d) {
     L.guideF = take(((size_t)kGuideSize + 1) * 4);
     L.pool = take((size_t)kMaxCtas * kPoolSlots * kRecordBytes);   // particle pools of the transport kernel (scratch)
     L.rings = take((size_t)kMaxCtas * kRingCount * kPoolSlots * sizeof(ring_t));
-    L.small = take(1024);            // ledger [8] f64 @0 | chunk counter @64 | rho_max [32] f32 @128 | counters [32] u64 @256 | gamma stats [4] f64 @512, max bits @544
+    L.small = take(1024);            // ledger [8] f64 @0 | chunk counter @64 | rho_max [32] f32 @128 | counters [32] u64 @256 | gamma stats [4] f64 @512, max bits @544 | PS3 count u64 @576
     L.total = o;
     return L;
 }
@@ -87,6 +87,7 @@ struct aepid_ctx {
     unsigned long long first_history = 0;                  // global index of history 0 of this context (multi-GPU sharding)
     double hist[256] = {0};
     bool counting = false;
+    float4* ps3 = nullptr; unsigned long long ps3_cap = 0;       // caller-owned Phase Space 3 buffer (aepid_set_phase_space)
 
     uint32_t* d_vox() { return reinterpret_cast<uint32_t*>(ws + lay.vox); }
     float* d_ph_batch() { return reinterpret_cast<float*>(ws + lay.ph_batch); }
@@ -108,6 +109,7 @@ struct aepid_ctx {
     float* d_rho_max() { return reinterpret_cast<float*>(ws + lay.small + 128); }
     double* d_gamma_stats() { return reinterpret_cast<double*>(ws + lay.small + 512); }
     unsigned int* d_gamma_max() { return reinterpret_cast<unsigned int*>(ws + lay.small + 544); }
+    unsigned long long* d_ps3_count() { return reinterpret_cast<unsigned long long*>(ws + lay.small + 576); }
 };
 
 namespace {
@@ -148,6 +150,7 @@ int reset_tallies(aepid_ctx* ctx) {
     CU(cudaMemsetAsync(ctx->d_ep_batch(), 0, ctx->lay.npix * 4 * B, ctx->stream));
     CU(cudaMemsetAsync(ctx->ws + ctx->lay.small, 0, 128, ctx->stream));
     CU(cudaMemsetAsync(ctx->ws + ctx->lay.small + 256, 0, 256, ctx->stream));
+    CU(cudaMemsetAsync(ctx->d_ps3_count(), 0, 8, ctx->stream));
     ctx->n_done = 0; ctx->first_history = 0;
     std::fill(ctx->hist, ctx->hist + 256, 0.0);
     return 0;
@@ -237,6 +240,7 @@ int fill_params(aepid_ctx* ctx, TransportParams& p) {
     p.pool = reinterpret_cast<uint4*>(ctx->ws + ctx->lay.pool);
     p.rings = reinterpret_cast<ring_t*>(ctx->ws + ctx->lay.rings);
     p.n_batches = ctx->dims.n_batches; p.nvox = ctx->lay.nvox; p.npix = ctx->lay.npix;
+    p.ps3 = ctx->ps3; p.ps3_count = ctx->d_ps3_count(); p.ps3_cap = ctx->ps3 ? ctx->ps3_cap : 0;
     p.base = 0; set_seed(p, 0); p.n = 0; p.hist_per_batch = 1;
     return 0;
 }
@@ -615,6 +619,23 @@ int aepid_apply_response_lut(aepid_ctx* ctx, const float* lut, int nt, int ns, f
     if (!dev_out) if (int rc = deliver(ctx, signal_out, d_out, n * 4, &need_sync)) return rc;
     if (tmap_out) if (int rc = deliver(ctx, tmap_out, ctx->d_tmap(), n * 4, &need_sync)) return rc;
     if (need_sync) CU(cudaStreamSynchronize(ctx->stream));
+    return 0;
+}
+
+int aepid_set_phase_space(aepid_ctx* ctx, void* records, unsigned long long capacity) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    if (records && (classify(records) != MEM_DEVICE || ((uintptr_t)records & 15))) return fail(ctx, AEPID_ERR_BAD_ARG, "phase-space buffer must be 16-byte aligned device memory");
+    if (records && capacity == 0) return fail(ctx, AEPID_ERR_BAD_ARG, "phase-space capacity is zero");
+    ctx->ps3 = reinterpret_cast<float4*>(records); ctx->ps3_cap = records ? capacity : 0;
+    CU(cudaMemsetAsync(ctx->d_ps3_count(), 0, 8, ctx->stream));
+    return 0;
+}
+
+int aepid_read_phase_space_count(aepid_ctx* ctx, unsigned long long* n_arrived) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    if (!n_arrived) return fail(ctx, AEPID_ERR_BAD_ARG, "null output");
+    CU(cudaMemcpyAsync(n_arrived, ctx->d_ps3_count(), 8, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
     return 0;
 }
 

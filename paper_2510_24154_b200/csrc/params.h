@@ -83,6 +83,9 @@ struct TransportParams {
     unsigned int* hist_counter;        // next history of this launch that has not been started
     uint4* pool;                       // particle records [kMaxCtas][kPoolSlots][3], scratch of one launch
     ring_t* rings;             // slot-index rings [kMaxCtas][kRingCount][kPoolSlots], scratch of one launch
+    float4* ps3;                       // Phase Space 3 records [ps3_cap][2] (null: not recorded), see aepid_set_phase_space
+    unsigned long long* ps3_count;     // arrivals at the EPID top plane so far (also beyond the capacity)
+    unsigned long long ps3_cap;
     uint64_t base;                     // global index of relative history 0 of this launch
     uint64_t seed;
     uint32_t rk[20];                   // Philox round keys of `seed` (set_seed): rk[2r], rk[2r+1] = key of round r

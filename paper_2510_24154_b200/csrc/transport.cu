@@ -346,6 +346,26 @@ __device__ __forceinline__ void enter_epid(Lane& L, const Geom& g) {       // po
     L.x = pu; L.y = pv; L.z = 0.0f; L.dx = du; L.dy = dv; L.dz = dw;
     SET_REGION(L.flags, R_EPID); SET_LAYER(L.flags, 0);
 }
+// Phase Space 3 (reading A30): the particle has just arrived at the EPID top plane from the air (position
+// (u, v, 0) and direction already in the beam frame).  One counter request per group of lanes that arrive together; the
+// hand-off stays in flight, the record is a copy.
+__device__ __noinline__ void record_ps3(float4* rec, unsigned long long* count, unsigned long long cap,
+                                        float u, float v, float du, float dv, float dw, float E, uint32_t type, uint32_t hist) {
+    const unsigned act = __activemask(), lane = threadIdx.x & 31u;
+    const int leader = __ffs(act) - 1;
+    unsigned long long base = 0;
+    if ((int)lane == leader) base = atomicAdd(count, (unsigned long long)__popc(act));
+    base = __shfl_sync(act, base, leader);
+    const unsigned long long k = base + (unsigned long long)__popc(act & ((1u << lane) - 1u));
+    if (k < cap) {
+        __stcs(rec + 2 * k, make_float4(u, v, du, dv));
+        __stcs(rec + 2 * k + 1, make_float4(dw, E, __uint_as_float(type), __uint_as_float(hist)));
+    }
+}
+__device__ __forceinline__ void enter_epid_ps3(Lane& L, const TransportParams& P) {
+    enter_epid(L, P.g);
+    if (P.ps3) record_ps3(P.ps3, P.ps3_count, P.ps3_cap, L.x, L.y, L.dx, L.dy, L.dz, L.E, F_TYPE(L.flags), (uint32_t)(P.base + L.h));
+}
 __device__ __forceinline__ void epid_to_air(Lane& L, const Geom& g) {      // leaving through the top face
     const float u = L.x, v = L.y, w = g.sid;
     float x, y, z;
@@ -587,7 +607,7 @@ __device__ __forceinline__ bool air_transit(Lane& L, const TransportParams& P, c
     const int kind = ah.code & 3;
     if (kind == 0) { enter_phantom(L, P, ah.code >> 2); return false; }
     if (kind == 2) { L.a_esc += L.E; L.alive = false; return false; }
-    enter_epid(L, g);                                                      // (u, v, depth 0), beam-frame direction, dw > 0
+    enter_epid_ps3(L, P);                                                  // (u, v, depth 0), beam-frame direction, dw > 0
     const float idw = rcp(L.dz);
     if (lateral_exit(L.x, L.y, L.dx, L.dy) < g.zt[g.n_layers] * idw) return false;   // leaves the stack sideways: layer-by-layer code
     nl -= mua * ah.t;
@@ -762,7 +782,7 @@ __device__ __forceinline__ void electron_step_outside(Lane& L, const TransportPa
         const float e_out = L.E + (F_TYPE(L.flags) == T_POSITRON ? 2.0f * kMec2 : 0.0f);
         if (in_air) {
             if (kind == 0) enter_phantom(L, P, axis);
-            else if (kind == 1) enter_epid(L, g);
+            else if (kind == 1) enter_epid_ps3(L, P);
             else { L.a_esc += e_out; L.alive = false; return; }
         } else {
             const int l = F_LAYER(L.flags);
