@@ -22,7 +22,7 @@ constexpr size_t kMaxLut = 65536;
 inline size_t up(size_t x) { return (x + kAlign - 1) & ~(kAlign - 1); }
 
 struct Layout {
-    size_t vox, ph_batch, ep_batch, out_ph, out_ep, tmap, signal, dose_in, lut, blob, thrE, edges, thrF, guideF, pool, rings, small, total;
+    size_t vox, ph_batch, ep_batch, out_ph, out_ep, tmap, signal, dose_in, lut, blob, thrE, edges, thrF, guideF, queues, small, total;
     size_t nvox, npix, blob_bytes;
 };
 
@@ -57,8 +57,7 @@ Layout make_layout(const aepid_dims& d) {
     L.edges = take(((size_t)d.n_bins + 1) * 4);
     L.thrF = take(((size_t)d.fu * d.fv + 1) * 4);
     L.guideF = take(((size_t)kGuideSize + 1) * 4);
-    L.pool = take((size_t)kMaxCtas * kPoolSlots * kRecordBytes);   // particle pools of the transport kernel (scratch)
-    L.rings = take((size_t)kMaxCtas * kRingCount * kPoolSlots * sizeof(ring_t));
+    L.queues = take((size_t)kMaxCtas * kRingCount * kPoolSlots * kRecordBytes);   // class queues of the transport kernel (scratch)
     L.small = take(1024);            // ledger [8] f64 @0 | chunk counter @64 | rho_max [32] f32 @128 | counters [32] u64 @256 | gamma stats [4] f64 @512, max bits @544 | PS3 count u64 @576
     L.total = o;
     return L;
@@ -237,8 +236,7 @@ int fill_params(aepid_ctx* ctx, TransportParams& p) {
     p.g = ctx->g; p.ph = ctx->ph; p.tb = ctx->tb; p.so = ctx->so;
     p.vox = ctx->d_vox(); p.ep_batch = ctx->d_ep_batch(); p.ph_batch = ctx->d_ph_batch();
     p.ledger = ctx->d_ledger(); p.counters = ctx->d_counters(); p.hist_counter = ctx->d_chunk();
-    p.pool = reinterpret_cast<uint4*>(ctx->ws + ctx->lay.pool);
-    p.rings = reinterpret_cast<ring_t*>(ctx->ws + ctx->lay.rings);
+    p.queues = reinterpret_cast<uint4*>(ctx->ws + ctx->lay.queues);
     p.n_batches = ctx->dims.n_batches; p.nvox = ctx->lay.nvox; p.npix = ctx->lay.npix;
     p.ps3 = ctx->ps3; p.ps3_count = ctx->d_ps3_count(); p.ps3_cap = ctx->ps3 ? ctx->ps3_cap : 0;
     p.base = 0; set_seed(p, 0); p.n = 0; p.hist_per_batch = 1;

@@ -15,11 +15,10 @@ constexpr float kWorldHalf = 100.0f;  // |u|, |v| <= 100 cm
 constexpr float kWorldWMin = -1.0f;   // -1 <= w
 constexpr float kMec2 = 0.51099895f;
 #ifndef AEPID_POOL_LOG
-#define AEPID_POOL_LOG 16
+#define AEPID_POOL_LOG 17
 #endif
 constexpr int kPoolSlots = 1 << AEPID_POOL_LOG;   // particle records per CTA of the transport kernel (transport.cu)
-typedef std::conditional<(AEPID_POOL_LOG <= 16), unsigned short, uint32_t>::type ring_t;   // a ring cell holds a slot index
-constexpr int kRingCount = 6;         // slot-index rings per CTA: five event classes and the free slots
+constexpr int kRingCount = 5;         // class queues per CTA: the five event classes
 constexpr int kRecordBytes = 48;      // three 16-byte vectors per particle
 constexpr int kMaxCtas = 160;
 constexpr int kGuideLog = 12;         // the fluence search starts from a guide table indexed by the top kGuideLog bits of the draw
@@ -81,8 +80,7 @@ struct TransportParams {
     double* ledger;                    // [8]
     unsigned long long* counters;      // [32]
     unsigned int* hist_counter;        // next history of this launch that has not been started
-    uint4* pool;                       // particle records [kMaxCtas][kPoolSlots][3], scratch of one launch
-    ring_t* rings;             // slot-index rings [kMaxCtas][kRingCount][kPoolSlots], scratch of one launch
+    uint4* queues;                     // class queues of particle records [kMaxCtas][kRingCount][kPoolSlots][3], scratch of one launch
     float4* ps3;                       // Phase Space 3 records [ps3_cap][2] (null: not recorded), see aepid_set_phase_space
     unsigned long long* ps3_count;     // arrivals at the EPID top plane so far (also beyond the capacity)
     unsigned long long ps3_cap;

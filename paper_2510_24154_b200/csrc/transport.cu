@@ -10,27 +10,31 @@
 //     phantom, P photon inside the EPID or with a collision pending outside the phantom, X charged particle outside
 //     the phantom.  The CTA runs PHASES, one class per phase, separated by block barriers; thread 0 picks the next
 //     phase: new histories while the particle pool has room, else the class with the most waiting particles.
-//   * Particle records (48 B, three 16 B vectors) live in a per-CTA POOL in global memory (kPool slots, L2 resident,
-//     written and read with .cg accesses); shared memory holds the material tables (ln domain, one LDS.128 per node)
-//     and the scheduler state; the rings of pool-slot indices (one per class, one of free slots) live in global memory
-//     too.  A pool this large (65536 particles for 1024 lanes) makes a phase many waves long, so that the phase switch
-//     (two barriers, a cold instruction cache) and the tail of a phase cost little (measured: halving the pool costs 5 %).
+//   * Particle records (48 B, three 16 B vectors) live in per-CTA CLASS QUEUES in global memory: one ring of kPool
+//     records per event class (L2 / HBM, written and read with .cg accesses, consecutive tickets = consecutive records,
+//     so a refill is one coalesced, prefetchable read with no index to chase).  Shared memory holds the material tables
+//     (ln domain, one LDS.128 per node) and the scheduler state.  Up to kLiveMax = 65536 particles for 1024 lanes
+//     make a phase many waves long, so that the phase switch (two barriers, a cold instruction cache) and the tail of
+//     a phase cost little (measured: half as many cost 3.5 %).
 //   * Within a phase every lane follows its particle event by event while it stays in the class; a lane whose
-//     particle has died or changed class writes it back (record to the pool, slot to the ring of the new class) and
-//     is refilled IN PLACE from the ring of the phase, so warps run one code path with nearly all lanes active.
-//     Secondaries go straight into the pool: the creating lane holds a spare free slot, stores the record and
-//     appends the slot to the ring of the secondary's class.
-//   * Ring protocol: head/tail are monotonic counters; pushes take a ticket from tail and write the cell; pops take
-//     tickets from head but only below the SNAPSHOT of tail taken at the last barrier, so a cell is never read
-//     before the barrier that publishes it and no generation tags or spin waits are needed.  What is pushed during a
-//     phase (also into the phase's own ring: parked or evicted particles) becomes visible in the next phase.
+//     particle has died or changed class writes it back (record appended to the queue of the new class) and is
+//     refilled IN PLACE from the queue of the phase, so warps run one code path with nearly all lanes active.
+//     Secondaries are appended straight to the queue of their class.
+//   * Queue protocol: head/tail are monotonic ticket counters; a push takes a ticket from tail and writes the record;
+//     pops take tickets from head but only below the SNAPSHOT of tail taken at the last barrier, so a record is never
+//     read before the barrier that publishes it and no generation tags or spin waits are needed.  What is pushed
+//     during a phase (also into the phase's own queue: parked or evicted particles) becomes visible in the next phase.
+//     A push may not wrap onto a record that can still be read in this phase: tail at the end of the phase minus head
+//     at its start must stay <= kPool.  That difference is (particles popped) + (particles in the queue at the end),
+//     each at most the number of particles alive in the CTA, which s_live keeps <= kLiveMax = kPool / 2.
 //   * A phase ends softly: a warp that can no longer keep its lanes full (ring exhausted, kRefillMin lanes empty)
 //     writes its particles back and leaves, so all warps reach the barrier within about one event of each other and
 //     the survivors join the next phase of their class (a write-back and reload costs a fraction of one event).
 //     In a phase that starts with fewer than two waves of particles a warp stays for at least kMinIter events.
-//   * Slot discipline: every particle owns a pool slot from birth, so writing it back never needs a new one; a lane
-//     runs an event that can create a secondary only while it holds a spare slot, otherwise it parks its particle.
-//     New histories start only while kReserve slots stay free.  Hence the pool cannot overflow.
+//   * Head room: s_live counts the particles alive in the CTA plus the credits held by lanes.  A lane runs an event
+//     that can create a secondary only while it holds a credit (its own count when its particle died, else a fresh
+//     one), otherwise it parks its particle; new histories start only while kReserve of head room stays free.  Hence
+//     s_live <= kLiveMax always, and writing a particle back never needs anything.
 //   * A particle's trajectory does not depend on the schedule: its Philox stream is keyed by (history, particle
 //     id, block) and every event consumes whole blocks (reading A1).
 //   * The phantom is one packed 32-bit word per voxel gathered through the read-only path; phantom deposits of
@@ -49,20 +53,24 @@ namespace aepid {
 constexpr int kWarps = AEPID_WARPS;
 constexpr int kThreads = kWarps * 32;
 constexpr int kPoolLog = AEPID_POOL_LOG;
-constexpr int kPool = 1 << kPoolLog;          // particle slots per CTA; also the capacity of every ring
-static_assert(kPool == kPoolSlots, "pool size");
+constexpr int kPool = 1 << kPoolLog;          // records per class queue of a CTA
+static_assert(kPool == kPoolSlots, "queue size");
+constexpr int kLiveMax = kPool / 2;           // particles alive in a CTA at any time: half a queue, see "queue protocol" in the header comment
 #ifndef AEPID_RESERVE_8THS
 #define AEPID_RESERVE_8THS 3
 #endif
 #ifndef AEPID_REFILL_MIN
 #define AEPID_REFILL_MIN 8
 #endif
-constexpr int kReserve = AEPID_RESERVE_8THS * kPool / 8;       // free slots that must remain for secondaries when new histories start
+constexpr int kReserve = AEPID_RESERVE_8THS * kLiveMax / 8;    // head room that must remain for secondaries when new histories start
 constexpr int kRefillMin = AEPID_REFILL_MIN;                 // a warp refills its empty lanes once this many are empty
 #ifndef AEPID_MIN_ITER
 #define AEPID_MIN_ITER 12
 #endif
 constexpr uint32_t kMinIter = AEPID_MIN_ITER;   // events per lane before a warp may leave a short phase early
+#ifndef AEPID_PREFETCH
+#define AEPID_PREFETCH 2048
+#endif
 #ifndef AEPID_STEPS_E
 #define AEPID_STEPS_E 4
 #endif
@@ -81,7 +89,7 @@ constexpr int kLongPhase = 2 * kThreads;      // phases that start with at least
 #endif
 constexpr int kHitMin = AEPID_HIT_MIN;          // photon flights go on until this many lanes of the warp have a collision to sample
 constexpr int kMaxRounds = 8;                 // ... but no more than this many flights per event
-constexpr int kStarved = 256;                 // fewer free slots than this: prefer phases that need none
+constexpr int kStarved = 256;                 // less head room than this: prefer phases that need none
 constexpr uint32_t kIterLimit = 1u << 20;     // iterations of one warp in one phase before it hands its particles back
 constexpr uint32_t kPhaseLimit = 1u << 24;
 constexpr float kPi = 3.14159265358979f;
@@ -89,7 +97,7 @@ constexpr float kInf = 3.0e38f;
 constexpr uint32_t kNone = 0xffffffffu;
 
 // event classes = rings = phases
-enum : int { C_A = 0, C_W = 1, C_E = 2, C_P = 3, C_X = 4, kClasses = 5, kFree = 5, kRings = kRingCount };
+enum : int { C_A = 0, C_W = 1, C_E = 2, C_P = 3, C_X = 4, kClasses = 5, kRings = kRingCount };
 
 #define FULL_MASK 0xffffffffu
 // flags: bits 0-1 type, 2-3 region, 4-6 layer, 7 collision pending (photon outside the phantom), 16-23 batch
@@ -120,11 +128,11 @@ __shared__ unsigned int s_nphase;
 __shared__ Geom s_g;
 __shared__ float* s_ep_batch;
 __shared__ unsigned long long s_npix;
-__shared__ uint4* s_pool;                           // this CTA's particle records [kPool][3]
-__shared__ ring_t* s_rings;                 // this CTA's rings [kRings][kPool]
+__shared__ uint4* s_queue;                          // this CTA's class queues of particle records [kClasses][kPool][3]
+__shared__ int s_live;                              // particles alive in this CTA (in the queues, in lanes) + head-room credits held by lanes
 extern __shared__ __align__(16) unsigned char smem_raw[];   // per-warp ledger | table blob
 
-__device__ __forceinline__ ring_t* ring_cells(int r) { return s_rings + r * kPool; }
+__device__ __forceinline__ uint4* queue_rec(int r, uint32_t ticket) { return s_queue + ((size_t)r * kPool + (ticket & (uint32_t)(kPool - 1))) * 3; }
 struct Shared {
     const float4* phot;
     const float* maj;
@@ -140,8 +148,8 @@ struct Lane {
     uint32_t cw, vlin;              // packed word and linear index of the current voxel (charged particle in PHANTOM)
     int ci; float ct, mumaj;        // photon: table cell, fraction, majorant at E
     uint32_t pidx; float pval;      // pending phantom deposit (merged while the voxel does not change)
-    uint32_t slot;                  // pool slot of this particle (kNone: fresh from the source)
-    uint32_t spare;                 // a free pool slot kept by the lane for its next secondary (kNone: none)
+    uint32_t slot;                  // 1: the lane holds a particle that is counted in s_live (alive, or dead and not yet released); kNone: none
+    uint32_t spare;                 // 1: the lane holds a head-room credit for its next secondary (kNone: none)
     float a_emit, a_ph, a_eps, a_epo, a_air, a_esc;   // ledger sums since the last flush
     bool alive;
 };
@@ -389,23 +397,11 @@ __device__ __forceinline__ void world_to_frac(const Geom& g, uint32_t vox, float
     x = fminf(fmaxf(gx, 0.0f), 1.0f); y = fminf(fmaxf(gy, 0.0f), 1.0f); z = fminf(fmaxf(gz, 0.0f), 1.0f);
 }
 
-// ---------------------------------------------------------------- rings (protocol in the header comment)
-// error bits (summed over CTAs into ledger[7]): 2 no slot for a secondary, 4 particle without a slot, 8 scheduler found no
+// ---------------------------------------------------------------- class queues (protocol in the header comment)
+// error bits (summed over CTAs into ledger[7]): 2 no head room for a secondary, 8 scheduler found no
 // runnable phase or ran out of phases
 __device__ __forceinline__ void raise_error(int bit) { atomicOr(s_flag + 1, bit); }
 
-// one lane appends one slot to ring r (divergent code); visible to poppers after the next barrier
-__device__ __noinline__ void ring_push_one(int r, uint32_t slot) {
-    const uint32_t t = atomicAdd(s_tail + r, 1u);
-    __stcg(ring_cells(r) + (t & (kPool - 1)), (ring_t)slot);
-}
-// one lane takes one entry of ring r, if one is left below the snapshot (divergent code)
-__device__ __noinline__ uint32_t ring_pop_one(int r) {
-    if ((int)(s_snap[r] - *((volatile unsigned int*)(s_head + r))) <= 0) return kNone;
-    const uint32_t t = atomicAdd(s_head + r, 1u);
-    if ((int)(s_snap[r] - t) <= 0) { atomicSub(s_head + r, 1u); return kNone; }
-    return __ldcg(ring_cells(r) + (t & (kPool - 1)));
-}
 // lane 0 claims up to `want` entries of ring r; returns count | first ticket << 32 (warp-uniform, all lanes call)
 __device__ __noinline__ unsigned long long ring_claim(int r, int want) {
     int n = 0; uint32_t t = 0;
@@ -429,28 +425,35 @@ __device__ __noinline__ int budget_claim(int want) {
     return __shfl_sync(FULL_MASK, n, 0);
 }
 
-// Store a particle record in pool slot `slot` and append the slot to the ring of the particle's class.
-__device__ __noinline__ void queue_particle(uint32_t slot, float x, float y, float z, float dx, float dy, float dz, float E,
+// Append a particle record to the queue of its class (one lane, divergent code); visible to poppers after the next barrier.
+__device__ __noinline__ void queue_particle(float x, float y, float z, float dx, float dy, float dz, float E,
                                             uint32_t vox, uint32_t flags, uint32_t h, uint32_t pid, uint32_t blk) {
-    uint4* rec = s_pool + (size_t)slot * 3;
+    const int r = class_of(flags);
+    uint4* rec = queue_rec(r, atomicAdd(s_tail + r, 1u));
     __stcg(rec + 0, make_uint4(__float_as_uint(x), __float_as_uint(y), __float_as_uint(z), __float_as_uint(dx)));
     __stcg(rec + 1, make_uint4(__float_as_uint(dy), __float_as_uint(dz), __float_as_uint(E), vox));
     __stcg(rec + 2, make_uint4(flags, h, pid, blk));
-    ring_push_one(class_of(flags), slot);
 }
-// A lane keeps at most one SPARE free slot (the slot of a particle that died in it, else one from the free ring)
-// and only runs an event that can create a secondary while it holds one (header comment, "slot discipline").
+// Head room: s_live counts the particles alive in the CTA plus the credits lanes hold for secondaries they may create; it
+// never exceeds kLiveMax, which is what keeps every queue from wrapping onto unread records (header comment).  A lane
+// keeps at most one credit (its own, when its particle died, else a fresh one) and only runs an event that can create a
+// secondary while it holds one.
+__device__ __noinline__ uint32_t take_credit() {
+    if (*((volatile int*)&s_live) >= kLiveMax) return kNone;
+    if (atomicAdd(&s_live, 1) >= kLiveMax) { atomicSub(&s_live, 1); return kNone; }
+    return 1u;
+}
 __device__ __forceinline__ bool ensure_spare(Lane& L) {
-    if (L.spare == kNone) L.spare = ring_pop_one(kFree);
+    if (L.spare == kNone) L.spare = take_credit();
     return L.spare != kNone;
 }
-// A secondary goes straight into the pool (the lane's spare slot) and into the ring of its class.  Without a spare
-// (cannot happen: see ensure_spare; flagged) its energy is booked as escaped so that the ledger still closes.
+// A secondary goes straight into the queue of its class, on the lane's credit.  Without one (cannot happen: see
+// ensure_spare; flagged) its energy is booked as escaped so that the ledger still closes.
 __device__ __forceinline__ void spawn_from(Lane& L, float x, float y, float z, float dx, float dy, float dz, float E,
                                            uint32_t flags, uint32_t pid) {
-    const uint32_t s = L.spare; L.spare = kNone;
-    if (s == kNone) { raise_error(2); L.a_esc += E + (F_TYPE(flags) == T_POSITRON ? 2.0f * kMec2 : 0.0f); return; }
-    queue_particle(s, x, y, z, dx, dy, dz, E, L.vox, flags, L.h, pid, 0u);
+    if (L.spare == kNone) { raise_error(2); L.a_esc += E + (F_TYPE(flags) == T_POSITRON ? 2.0f * kMec2 : 0.0f); return; }
+    L.spare = kNone;
+    queue_particle(x, y, z, dx, dy, dz, E, L.vox, flags, L.h, pid, 0u);
 }
 // Two 0.511 MeV photons, isotropic and back to back (reading A11): the lane becomes the first, the second is spawned.
 // Position must already be in the frame photons use in this region.
@@ -877,7 +880,11 @@ __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned lon
     int n[kRings];
 #pragma unroll
     for (int r = 0; r < kRings; ++r) { s_snap[r] = s_tail[r]; n[r] = (int)(s_snap[r] - s_head[r]); }
-    const int nf = n[kFree];
+    int n_live = 0;
+#pragma unroll
+    for (int c = 0; c < kClasses; ++c) n_live += n[c];
+    s_live = n_live;                                           // between phases every particle sits in a queue and no lane holds a credit
+    const int nf = kLiveMax - n_live;
     bool more = s_flag[0] == 0;
     int budget = 0;
     if (more) {
@@ -921,19 +928,16 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
     bool leaving = false, park = false;
 #pragma unroll 1
     for (uint32_t it = 1;; ++it) {
-        // ---- A: particles that left the class (or all of them, when the warp leaves) go to the ring of their class;
-        //         the slot of a dead particle becomes the lane's spare or goes back to the free ring
+        // ---- A: particles that left the class (or all of them, when the warp leaves) go to the queue of their class;
+        //         the count of a dead particle becomes the lane's credit or is given back
         if (!(L.alive && !leaving && !park && class_of(L.flags) == C)) {
             flush_pending(L, P);
             if (L.alive) {
-                if (L.slot == kNone) {                                     // cannot happen (flagged): drop, ledger still closes
-                    raise_error(4);
-                    L.a_esc += L.E + (F_TYPE(L.flags) == T_POSITRON ? 2.0f * kMec2 : 0.0f);
-                } else queue_particle(L.slot, L.x, L.y, L.z, L.dx, L.dy, L.dz, L.E, L.vox, L.flags, L.h, L.pid, L.blk);
+                queue_particle(L.x, L.y, L.z, L.dx, L.dy, L.dz, L.E, L.vox, L.flags, L.h, L.pid, L.blk);
                 if (COUNT && !kPhaseClock) cnt[27]++;
                 L.alive = false; L.slot = kNone;
             } else if (L.slot != kNone) {
-                if (kSpawns && !leaving && L.spare == kNone) L.spare = L.slot; else ring_push_one(kFree, L.slot);
+                if (kSpawns && !leaving && L.spare == kNone) L.spare = 1u; else atomicSub(&s_live, 1);
                 L.slot = kNone;
             }
             park = false;
@@ -946,33 +950,38 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
             const int got = (int)(uint32_t)cl;
             const int rk = __popc(empty & lt_mask);
             if (!L.alive && rk < got) {
-                const uint32_t s = __ldcg(ring_cells(C) + (((uint32_t)(cl >> 32) + (uint32_t)rk) & (kPool - 1)));
-                const uint4* rec = s_pool + (size_t)s * 3;
+                const uint32_t tk = (uint32_t)(cl >> 32) + (uint32_t)rk;
+                const uint4* rec = queue_rec(C, tk);
                 const uint4 a = __ldcg(rec), b = __ldcg(rec + 1), c = __ldcg(rec + 2);
+#if AEPID_PREFETCH > 0
+                // the records a later refill will want (same queue, AEPID_PREFETCH tickets ahead, if published): into the L2
+                if ((int)(s_snap[C] - (tk + AEPID_PREFETCH)) > 0) {
+                    const uint4* nx = queue_rec(C, tk + AEPID_PREFETCH);
+                    asm volatile("prefetch.global.L2 [%0];" :: "l"(nx));
+                    asm volatile("prefetch.global.L2 [%0];" :: "l"(nx + 2));
+                }
+#endif
                 L.x = __uint_as_float(a.x); L.y = __uint_as_float(a.y); L.z = __uint_as_float(a.z); L.dx = __uint_as_float(a.w);
                 L.dy = __uint_as_float(b.x); L.dz = __uint_as_float(b.y); L.E = __uint_as_float(b.z); L.vox = b.w;
                 L.flags = c.x; L.h = c.y; L.pid = c.z; L.blk = c.w;
-                L.slot = s; L.alive = true;
+                L.slot = 1u; L.alive = true;
                 L.pval = 0.0f; L.pidx = kNone;
                 if (COUNT && !kPhaseClock) cnt[28]++;
                 if (C == C_A || C == C_W || C == C_P) set_energy(L, P, sh);
                 if (C == C_E) { L.vlin = vox_linear(P.g, L.vox); L.cw = __ldg(P.vox + L.vlin); L.pidx = L.vlin; }
             }
             if (C == C_A) {
-                // K1: new histories in the lanes that are still empty, one free slot each
+                // K1: new histories in the lanes that are still empty (the budget of the phase is head room set aside for them)
                 empty = __ballot_sync(FULL_MASK, !L.alive);
-                int nd = budget_claim(__popc(empty));
-                if (nd > 0) {
-                    const unsigned long long fl = ring_claim(kFree, nd);
-                    const int nslots = (int)(uint32_t)fl;                  // = nd: the budget never exceeds the free slots below the snapshot
+                const int nslots = budget_claim(__popc(empty));
+                if (nslots > 0) {
                     const int rk2 = __popc(empty & lt_mask);
                     uint32_t h0 = 0;
-                    if (lane == 0) h0 = atomicAdd(P.hist_counter, (unsigned)nslots);
+                    if (lane == 0) { h0 = atomicAdd(P.hist_counter, (unsigned)nslots); atomicAdd(&s_live, nslots); }
                     h0 = __shfl_sync(FULL_MASK, h0, 0);
                     if (!L.alive && rk2 < nslots) {
-                        const uint32_t myslot = __ldcg(ring_cells(kFree) + (((uint32_t)(fl >> 32) + (uint32_t)rk2) & (kPool - 1)));
                         const uint32_t h = h0 + (uint32_t)rk2;
-                        if (h >= P.n) { ring_push_one(kFree, myslot); atomicExch(s_flag, 1); }
+                        if (h >= P.n) { atomicSub(&s_live, 1); atomicExch(s_flag, 1); }
                         else {
                             L.h = h; L.pid = 0; L.blk = 0;
                             const uint4 r = rng_block(L, P);               // block 0 of particle 0: E, pixel, u, v (reading A1)
@@ -981,7 +990,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                             L.dx = s.dx; L.dy = s.dy; L.dz = s.dz; L.E = s.E;
                             L.vox = 0;
                             L.flags = T_PHOTON | (R_AIR << 2) | (min(h / P.hist_per_batch, (uint32_t)P.n_batches - 1u) << 16);
-                            L.alive = true; L.slot = myslot;
+                            L.alive = true; L.slot = 1u;
                             L.pval = 0.0f; L.pidx = kNone;
                             L.a_emit += s.E;
                             set_energy(L, P, sh);
@@ -1051,7 +1060,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
         // ---- E: ledger of the last iterations: float per lane -> warp sum -> the warp's double accumulators
         if ((it & 63u) == 0u) ledger_flush(L, led);
     }
-    if (L.spare != kNone) { ring_push_one(kFree, L.spare); L.spare = kNone; }
+    if (L.spare != kNone) { atomicSub(&s_live, 1); L.spare = kNone; }
     ledger_flush(L, led);
     if (lane == 0) atomicAdd(&s_left, 1);
 }
@@ -1068,18 +1077,13 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
     sh.lnS = sh.maj + P.tb.n_E;
     sh.invX0 = sh.lnS + P.tb.n_mat * P.tb.n_T;
     for (int i = threadIdx.x; i < kWarps * 8; i += kThreads) led_all[i] = 0.0;
-    if (threadIdx.x < kRings) {
-        const bool fr = threadIdx.x == kFree;
-        s_tail[threadIdx.x] = fr ? kPool : 0u; s_head[threadIdx.x] = 0u; s_snap[threadIdx.x] = 0u;
-    }
+    if (threadIdx.x < kRings) { s_tail[threadIdx.x] = 0u; s_head[threadIdx.x] = 0u; s_snap[threadIdx.x] = 0u; }
     if (threadIdx.x < 2) s_flag[threadIdx.x] = 0;
     if (threadIdx.x == 0) {
         s_g = P.g; s_ep_batch = P.ep_batch; s_npix = P.npix; s_nphase = 0u;
-        s_pool = P.pool + (size_t)blockIdx.x * kPool * 3;
-        s_rings = P.rings + (size_t)blockIdx.x * kRings * kPool;
+        s_queue = P.queues + (size_t)blockIdx.x * kClasses * kPool * 3;
+        s_live = 0;
     }
-    __syncthreads();
-    for (int i = threadIdx.x; i < kPool; i += kThreads) __stcg(ring_cells(kFree) + i, (ring_t)i);   // every slot is free
     __syncthreads();
 
     uint32_t cnt[COUNT ? 32 : 1];

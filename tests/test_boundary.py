@@ -38,7 +38,7 @@ def test_workspace_bytes_validates_dims(lib):
     n = pkg.workspace_bytes(d)
     vox, pix = 120 * 120 * 80, 512 * 384
     assert n >= 4 * vox * (1 + 32 + 2) + 4 * pix * (32 + 2 + 3)
-    pool = 160 * 65536 * (48 + 6 * 2)                        # particle pools and slot rings of the transport kernel (params.h)
+    pool = 160 * 5 * 131072 * 48                             # class queues of particle records of the transport kernel (params.h)
     assert n < 1.1 * (4 * vox * 35 + 4 * pix * 37) + pool + (2 << 20)
     for field, bad in (("n_batches", 1), ("n_batches", 256), ("nx", 0), ("nx", 2000), ("n_mat", 33), ("n_layers", 9), ("fu", 0)):
         e = pkg.Dims.from_buffer_copy(d)
