@@ -60,7 +60,7 @@ constexpr int kLiveMax = kPool / 2;           // particles alive in a CTA at any
 #define AEPID_RESERVE_8THS 3
 #endif
 #ifndef AEPID_REFILL_MIN
-#define AEPID_REFILL_MIN 8
+#define AEPID_REFILL_MIN 3
 #endif
 constexpr int kReserve = AEPID_RESERVE_8THS * kLiveMax / 8;    // head room that must remain for secondaries when new histories start
 constexpr int kRefillMin = AEPID_REFILL_MIN;                 // a warp refills its empty lanes once this many are empty
