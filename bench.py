@@ -39,8 +39,8 @@ EVENTS_PER_HISTORY = {
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of transport_kernel per history, from the committed ncu --set full capture
-# (profiles/r01f_README.md: 2.385 GB + 1.948 GB for 1e7 histories of C1); None where no capture exists.
-DRAM_BYTES_PER_HISTORY = {"C1": 433.3}
+# (profiles/r01g_README.md: 1.823 GB + 1.676 GB for 1e7 histories of C1); None where no capture exists.
+DRAM_BYTES_PER_HISTORY = {"C1": 349.9}
 
 
 def alg_instr_per_history(name):

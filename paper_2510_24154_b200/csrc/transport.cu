@@ -68,6 +68,10 @@ constexpr int kRefillMin = AEPID_REFILL_MIN;                 // a warp refills i
 #define AEPID_MIN_ITER 12
 #endif
 constexpr uint32_t kMinIter = AEPID_MIN_ITER;   // events per lane before a warp may leave a short phase early
+#ifndef AEPID_SHARE_NUM
+#define AEPID_SHARE_NUM 1u
+#define AEPID_SHARE_DEN 1u
+#endif
 #ifndef AEPID_PREFETCH
 #define AEPID_PREFETCH 2048
 #endif
@@ -891,8 +895,8 @@ __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned lon
         const uint32_t done = *((volatile unsigned int*)P.hist_counter);
         const uint32_t left = done < P.n ? P.n - done : 0u;
         if (left == 0u) { more = false; s_flag[0] = 1; }
-        // towards the end of the launch take no more than a share of what is left, so that the CTAs finish together
-        const uint32_t share = max(left / (2u * gridDim.x), (uint32_t)kThreads);
+        // take no more than this CTA's share of what is left, so that the CTAs finish together
+        const uint32_t share = max((uint32_t)((unsigned long long)left * AEPID_SHARE_NUM / (AEPID_SHARE_DEN * gridDim.x)), (uint32_t)kThreads);
         budget = (int)min((uint32_t)max(nf - kReserve, 0), share);
     }
     int ph = -1;
