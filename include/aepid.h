@@ -170,6 +170,11 @@ int aepid_apply_response_lut(aepid_ctx* ctx, const float* lut, int nt, int ns,
                              float t_min, float t_max, float s_min, float s_max, float s_eff_cm,
                              const float* epid_in, float* signal_out, float* tmap_out);
 
+/* Scheduler knob of the transport kernel: the most particles a CTA keeps alive at a time, 64 .. 65536
+ * (0 = the default, 65536 = half a class queue).  Results do not depend on it (every particle has its own Philox stream);
+ * small values make lanes wait for head room and exist to test exactly that path. */
+int aepid_set_live_limit(aepid_ctx* ctx, int max_live_per_cta);
+
 /* Phase Space 3 ("an additional scoring plane, Phase Space 3, is generated to store all particles exiting
  * the patient"; reading A30): while a buffer is set, every particle that arrives at the EPID top plane (w = sid) from the
  * air is copied into it as two float4 = {u, v, du, dv} {dw, E, type bits, history bits}: position and direction in the beam

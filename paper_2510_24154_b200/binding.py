@@ -30,7 +30,7 @@ EXPORTS = ("aepid_workspace_bytes", "aepid_create", "aepid_destroy", "aepid_last
            "aepid_set_counting", "aepid_read_counters", "aepid_sample_source", "aepid_field_size",
            "aepid_apply_response_lut", "aepid_synchronize", "aepid_set_history_offset", "aepid_read_moments",
            "aepid_finalize_moments", "aepid_upsample", "aepid_gamma_index",
-           "aepid_set_phase_space", "aepid_read_phase_space_count")
+           "aepid_set_phase_space", "aepid_read_phase_space_count", "aepid_set_live_limit")
 
 
 class AepidError(RuntimeError):
@@ -78,6 +78,7 @@ def load_library():
     lib.aepid_set_history_offset.argtypes = [vp, C.c_ulonglong]
     lib.aepid_read_moments.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.aepid_finalize_moments.argtypes = [vp, vp, vp, C.c_size_t, C.c_double, C.c_double, vp, vp]
+    lib.aepid_set_live_limit.argtypes = [vp, C.c_int]
     lib.aepid_set_phase_space.argtypes = [vp, vp, C.c_ulonglong]
     lib.aepid_read_phase_space_count.argtypes = [vp, vp]
     lib.aepid_upsample.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int, C.c_int]
@@ -268,6 +269,9 @@ class Engine:
         s = C.c_float()
         self._chk(self._lib.aepid_field_size(self._h, int(bool(printed_form)), C.byref(s)))
         return float(s.value)
+
+    def set_live_limit(self, max_live_per_cta=0):
+        self._chk(self._lib.aepid_set_live_limit(self._h, int(max_live_per_cta)))
 
     def set_phase_space(self, capacity):
         """Record Phase Space 3 into a device buffer of `capacity` records (0: switch off)."""

@@ -86,6 +86,7 @@ struct aepid_ctx {
     unsigned long long first_history = 0;                  // global index of history 0 of this context (multi-GPU sharding)
     double hist[256] = {0};
     bool counting = false;
+    int live_max = kPoolSlots / 2;
     float4* ps3 = nullptr; unsigned long long ps3_cap = 0;       // caller-owned Phase Space 3 buffer (aepid_set_phase_space)
 
     uint32_t* d_vox() { return reinterpret_cast<uint32_t*>(ws + lay.vox); }
@@ -237,7 +238,7 @@ int fill_params(aepid_ctx* ctx, TransportParams& p) {
     p.vox = ctx->d_vox(); p.ep_batch = ctx->d_ep_batch(); p.ph_batch = ctx->d_ph_batch();
     p.ledger = ctx->d_ledger(); p.counters = ctx->d_counters(); p.hist_counter = ctx->d_chunk();
     p.queues = reinterpret_cast<uint4*>(ctx->ws + ctx->lay.queues);
-    p.n_batches = ctx->dims.n_batches; p.nvox = ctx->lay.nvox; p.npix = ctx->lay.npix;
+    p.n_batches = ctx->dims.n_batches; p.nvox = ctx->lay.nvox; p.npix = ctx->lay.npix; p.live_max = ctx->live_max;
     p.ps3 = ctx->ps3; p.ps3_count = ctx->d_ps3_count(); p.ps3_cap = ctx->ps3 ? ctx->ps3_cap : 0;
     p.base = 0; set_seed(p, 0); p.n = 0; p.hist_per_batch = 1;
     return 0;
@@ -617,6 +618,14 @@ int aepid_apply_response_lut(aepid_ctx* ctx, const float* lut, int nt, int ns, f
     if (!dev_out) if (int rc = deliver(ctx, signal_out, d_out, n * 4, &need_sync)) return rc;
     if (tmap_out) if (int rc = deliver(ctx, tmap_out, ctx->d_tmap(), n * 4, &need_sync)) return rc;
     if (need_sync) CU(cudaStreamSynchronize(ctx->stream));
+    return 0;
+}
+
+int aepid_set_live_limit(aepid_ctx* ctx, int max_live_per_cta) {
+    if (!ctx) return AEPID_ERR_BAD_ARG;
+    if (max_live_per_cta == 0) max_live_per_cta = kPoolSlots / 2;
+    if (max_live_per_cta < 64 || max_live_per_cta > kPoolSlots / 2) return fail(ctx, AEPID_ERR_BAD_ARG, "live limit out of range (64 .. half a class queue)");
+    ctx->live_max = max_live_per_cta;
     return 0;
 }
 

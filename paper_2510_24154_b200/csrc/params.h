@@ -90,6 +90,7 @@ struct TransportParams {
     uint32_t n;                        // histories in this launch (< 2^32)
     uint32_t hist_per_batch;           // history k of the launch scores into batch min(k / hist_per_batch, B - 1)
     int n_batches;
+    int live_max;                      // most particles alive per CTA (<= kPoolSlots / 2), aepid_set_live_limit
     size_t nvox, npix;
 };
 

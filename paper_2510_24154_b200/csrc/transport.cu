@@ -55,14 +55,15 @@ constexpr int kThreads = kWarps * 32;
 constexpr int kPoolLog = AEPID_POOL_LOG;
 constexpr int kPool = 1 << kPoolLog;          // records per class queue of a CTA
 static_assert(kPool == kPoolSlots, "queue size");
-constexpr int kLiveMax = kPool / 2;           // particles alive in a CTA at any time: half a queue, see "queue protocol" in the header comment
+constexpr int kLiveMax = kPool / 2;           // most particles alive in a CTA at any time: half a queue, see "queue protocol" in the header
+                                              // comment; the limit in force is TransportParams::live_max <= kLiveMax (s_live_max)
 #ifndef AEPID_RESERVE_8THS
 #define AEPID_RESERVE_8THS 3
 #endif
 #ifndef AEPID_REFILL_MIN
 #define AEPID_REFILL_MIN 3
 #endif
-constexpr int kReserve = AEPID_RESERVE_8THS * kLiveMax / 8;    // head room that must remain for secondaries when new histories start
+constexpr int kReserve8ths = AEPID_RESERVE_8THS;             // eighths of the limit that must remain free for secondaries when new histories start
 constexpr int kRefillMin = AEPID_REFILL_MIN;                 // a warp refills its empty lanes once this many are empty
 #ifndef AEPID_MIN_ITER
 #define AEPID_MIN_ITER 12
@@ -133,6 +134,7 @@ __shared__ Geom s_g;
 __shared__ float* s_ep_batch;
 __shared__ unsigned long long s_npix;
 __shared__ uint4* s_queue;                          // this CTA's class queues of particle records [kClasses][kPool][3]
+__shared__ int s_live_max;                          // limit of s_live for this launch
 __shared__ int s_live;                              // particles alive in this CTA (in the queues, in lanes) + head-room credits held by lanes
 extern __shared__ __align__(16) unsigned char smem_raw[];   // per-warp ledger | table blob
 
@@ -443,8 +445,8 @@ __device__ __noinline__ void queue_particle(float x, float y, float z, float dx,
 // keeps at most one credit (its own, when its particle died, else a fresh one) and only runs an event that can create a
 // secondary while it holds one.
 __device__ __noinline__ uint32_t take_credit() {
-    if (*((volatile int*)&s_live) >= kLiveMax) return kNone;
-    if (atomicAdd(&s_live, 1) >= kLiveMax) { atomicSub(&s_live, 1); return kNone; }
+    if (*((volatile int*)&s_live) >= s_live_max) return kNone;
+    if (atomicAdd(&s_live, 1) >= s_live_max) { atomicSub(&s_live, 1); return kNone; }
     return 1u;
 }
 __device__ __forceinline__ bool ensure_spare(Lane& L) {
@@ -888,7 +890,7 @@ __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned lon
 #pragma unroll
     for (int c = 0; c < kClasses; ++c) n_live += n[c];
     s_live = n_live;                                           // between phases every particle sits in a queue and no lane holds a credit
-    const int nf = kLiveMax - n_live;
+    const int nf = s_live_max - n_live;
     bool more = s_flag[0] == 0;
     int budget = 0;
     if (more) {
@@ -897,7 +899,7 @@ __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned lon
         if (left == 0u) { more = false; s_flag[0] = 1; }
         // take no more than this CTA's share of what is left, so that the CTAs finish together
         const uint32_t share = max((uint32_t)((unsigned long long)left * AEPID_SHARE_NUM / (AEPID_SHARE_DEN * gridDim.x)), (uint32_t)kThreads);
-        budget = (int)min((uint32_t)max(nf - kReserve, 0), share);
+        budget = (int)min((uint32_t)max(nf - kReserve8ths * s_live_max / 8, 0), share);
     }
     int ph = -1;
     if (more && budget >= kThreads) ph = C_A;
@@ -1086,7 +1088,7 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
     if (threadIdx.x == 0) {
         s_g = P.g; s_ep_batch = P.ep_batch; s_npix = P.npix; s_nphase = 0u;
         s_queue = P.queues + (size_t)blockIdx.x * kClasses * kPool * 3;
-        s_live = 0;
+        s_live = 0; s_live_max = min(max(P.live_max, 64), kLiveMax);
     }
     __syncthreads();
 
