@@ -111,16 +111,18 @@ def make_tables(n_E=500, E_min=1e-3, E_max=20.0, n_T=200, T_min=0.01, T_max=20.0
     T = np.exp(np.linspace(np.log(T_min), np.log(T_max), n_T))
     n_mat = len(MATERIALS)
     mc = np.empty((n_mat, n_E)); mp = np.empty((n_mat, n_E)); mpp = np.empty((n_mat, n_E))
-    sp = np.empty((n_mat, n_T)); x0 = np.empty(n_mat)
+    sp = np.empty((n_mat, n_T)); x0 = np.empty(n_mat); ne = np.empty(n_mat)
     for m, (_, comp, _) in enumerate(MATERIALS):
         mc[m] = mu_compton(comp, E)
         mp[m] = mu_photoelectric(comp, E)
         mpp[m] = mu_pair(comp, E)
         sp[m] = stopping_power(comp, T)
         x0[m] = radiation_length(comp)
+        ne[m] = N_A * sum(w * ELEMENTS[el][0] / ELEMENTS[el][1] for el, w in _fractions(comp).items())
     f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
     return {
         "n_mat": n_mat, "names": [m[0] for m in MATERIALS],
         "E_grid": f32(E), "mu_compton": f32(mc), "mu_pe": f32(mp), "mu_pair": f32(mpp),
         "T_grid": f32(T), "stop_pow": f32(sp), "rad_len": f32(x0),
+        "electrons_per_gram": f32(ne),      # N_A sum_i w_i Z_i / A_i: input of the Class II (Moller) mode
     }

@@ -39,6 +39,7 @@ def lib():
         _lib.orc_create.restype = C.c_void_p
         _lib.orc_last_error.restype = C.c_char_p
         _lib.orc_ps3_count.restype = C.c_uint64
+        _lib.orc_moller_cos.restype = C.c_double
         for f in ("orc_stop_pow", "orc_majorant", "orc_highland_theta0", "orc_field_size", "orc_lut_bilinear"):
             getattr(_lib, f).restype = C.c_double
     return _lib
@@ -80,6 +81,23 @@ def sample_deflection(d0, theta0, seed, n):
     return out
 
 
+def moller_xs(T, Tc):
+    """(cross section per electron [cm^2], integral of W d sigma [MeV cm^2]) for energy transfers above Tc (reading A31)."""
+    o = (C.c_double * 2)()
+    lib().orc_moller_xs(C.c_double(T), C.c_double(Tc), o)
+    return o[0], o[1]
+
+
+def sample_moller(T, Tc, seed, n):
+    eps = np.empty(n)
+    lib().orc_sample_moller(C.c_double(T), C.c_double(Tc), C.c_uint64(seed), C.c_uint64(n), _p(eps, C.c_double))
+    return eps
+
+
+def moller_cos(T_out, T_in):
+    return lib().orc_moller_cos(C.c_double(T_out), C.c_double(T_in))
+
+
 def lut_bilinear(lut, t_min, t_max, s_min, s_max, t, s):
     a = np.ascontiguousarray(lut, dtype=np.float64)
     return lib().orc_lut_bilinear(_p(a, C.c_double), a.shape[0], a.shape[1], C.c_double(t_min), C.c_double(t_max),
@@ -109,6 +127,9 @@ class Oracle:
         E, T = _f32(t["E_grid"]), _f32(t["T_grid"])
         mc, mp, mpp, sp, x0 = (_f32(t[k]) for k in ("mu_compton", "mu_pe", "mu_pair", "stop_pow", "rad_len"))
         self.n_mat = int(mc.shape[0])
+        if "electrons_per_gram" in t:                       # input of mode 2 (Class II collisions)
+            ne = _f32(t["electrons_per_gram"])
+            self._chk(self._l.orc_set_class2(self._h, len(ne), _p(ne, C.c_float)))
         self._chk(self._l.orc_init_materials(self._h, self.n_mat, len(E), _p(E, C.c_float), _p(mc, C.c_float), _p(mp, C.c_float),
                                              _p(mpp, C.c_float), len(T), _p(T, C.c_float), _p(sp, C.c_float), _p(x0, C.c_float)))
 

@@ -148,6 +148,7 @@ struct Ctx {
     // physics
     int mode = 1;
     double photon_cut = 0.010, electron_cut = 0.200, f_E = 0.10, s_max = 1.0;
+    std::vector<double> ne;                // electrons per gram [n_mat] (mode 2: Class II, reading A31)
     int tracking = 0;                      // 0 Woodcock, 1 exact voxel-by-voxel surface tracking
     int eq1_printed = 0;                   // 1: use Eq. 1 exactly as printed
     // fixed-primary override (pencil beams for pins)
@@ -158,7 +159,7 @@ struct Ctx {
     std::vector<double> ep_sum, ep_sq, rb_sum, rb_sq, ph_sum, ph_sq, unc;
     double ledger[8] = {0};
     uint64_t counters[16] = {0};
-    double aux[4] = {0};                   // 0: electron path length [cm], 1: sum rho*s [g/cm^2]
+    double aux[4] = {0};                   // 0: electron path length [cm], 1: sum rho*s [g/cm^2], 2 / 3: Moller events in the phantom / elsewhere
     int fc_bins = 0; double fc_w0 = 0, fc_dw = 0; std::vector<double> fc_hist;
     // per-history scratch
     std::vector<std::pair<int64_t, double>> hpix, hvox;
@@ -587,6 +588,46 @@ void transport_photon(Ctx& c, Particle p, const Run& r) {
 
 // ---------------------------------------------------------------- electron / positron
 // Highland width for a step of mass thickness rho*s in material m at mid-step kinetic energy Tm.
+// ---------------------------------------------------------------- Class II collisions (mode 2; "Class II
+// condensed history"; reading A31): discrete Moller events with energy transfer W above Tc = the electron
+// cut-off, continuous loss with the restricted stopping power below it.  With eps = W / T, tau = T / m_e c^2,
+//   d sigma / d eps = (2 pi r_e^2 m_e c^2 / (beta^2 T)) [1/eps^2 + 1/(1-eps)^2 + (tau/(tau+1))^2 - (2 tau+1)/(tau+1)^2 / (eps (1-eps))]
+// per electron, eps in [Tc/T, 1/2] (the faster outgoing electron is the primary); zero for T <= 2 Tc.
+constexpr double R_E = 2.8179403262e-13;   // cm
+struct MollerXs { double sigma, hard; };    // cross section per electron [cm^2]; int W d sigma [MeV cm^2]
+MollerXs moller_xs(double T, double Tc) {
+    MollerXs r{0.0, 0.0};
+    if (!(T > 2.0 * Tc)) return r;
+    const double tau = T / MEC2, b2 = tau * (tau + 2.0) / ((tau + 1.0) * (tau + 1.0));
+    const double c1 = (tau / (tau + 1.0)) * (tau / (tau + 1.0)), c2 = (2.0 * tau + 1.0) / ((tau + 1.0) * (tau + 1.0));
+    const double a = Tc / T, K = 2.0 * PI * R_E * R_E * MEC2 / (b2 * T);
+    // antiderivatives between a and 1/2
+    r.sigma = K * (1.0 / a - 1.0 / (1.0 - a) + c1 * (0.5 - a) - c2 * std::log((1.0 - a) / a));
+    const double i1 = std::log(0.5 / a);                                              // int eps / eps^2
+    const double i2 = (2.0 + std::log(0.5)) - (1.0 / (1.0 - a) + std::log(1.0 - a));   // int eps / (1-eps)^2
+    const double i3 = c1 * (0.125 - 0.5 * a * a);                                     // int c1 eps
+    const double i4 = c2 * std::log(2.0 * (1.0 - a));                                 // int c2 / (1-eps)
+    r.hard = K * T * (i1 + i2 + i3 - i4);
+    return r;
+}
+// eps from the Moller density on [a, 1/2] by rejection from 1/eps^2 (envelope: the bracket times eps^2 without its
+// negative term is at most 2 + c1/4)
+double sample_moller_eps(Rng& rng, double T, double Tc, uint64_t* trials) {
+    const double tau = T / MEC2, a = Tc / T;
+    const double c1 = (tau / (tau + 1.0)) * (tau / (tau + 1.0)), c2 = (2.0 * tau + 1.0) / ((tau + 1.0) * (tau + 1.0));
+    const double gmax = 2.0 + 0.25 * c1;
+    for (;;) {
+        const double x1 = rng.u(), x2 = rng.u();
+        if (trials) ++*trials;
+        const double eps = a / (1.0 - x1 * (1.0 - 2.0 * a));
+        const double x = eps / (1.0 - eps);
+        const double g = 1.0 + x * x + c1 * eps * eps - c2 * x;
+        if (x2 * gmax <= g) return eps;
+    }
+}
+// scattering angles of the two outgoing electrons (energy-momentum conservation, target at rest)
+inline double moller_cos(double Tout, double Tin) { return std::sqrt(Tout * (Tin + 2.0 * MEC2) / (Tin * (Tout + 2.0 * MEC2))); }
+
 double highland_theta0(const Ctx& c, int m, double rho_s, double Tm) {
     const double t = rho_s / c.X0[m];
     if (!(t > 0)) return 0.0;
@@ -624,10 +665,21 @@ void transport_electron(Ctx& c, Particle p, const Run& r) {
             const double tl = world_exit_lateral(p.pos, p.dir);
             if (tl < tf) { tb = tl; kind = 2; } else { tb = tf; kind = 0; }
         }
-        const double S = stop_pow(c, m, p.E);
-        double s = std::min(tb, std::min(c.f_E * p.E / (rho * S), c.s_max));
+        // mode 2: restricted stopping power L = S - n_e int W d sigma and a distance to the next hard (Moller) collision,
+        // both from the cross section at the energy the step starts with (reading A31)
+        const bool class2 = c.mode == 2;
+        auto loss = [&](double T) { return stop_pow(c, m, T) - (class2 ? c.ne[m] * moller_xs(T, c.electron_cut).hard : 0.0); };
+        const double S = loss(p.E);
+        double s_hard = INF;
+        if (class2) {
+            const double Sig = c.ne[m] * moller_xs(p.E, c.electron_cut).sigma;
+            const double xh = p.rng.u();                                    // drawn every step, also when no hard collision is possible
+            if (Sig > 0) s_hard = -std::log(xh) / (rho * Sig);
+        }
+        double s = std::min(std::min(tb, s_hard), std::min(c.f_E * p.E / (rho * S), c.s_max));
         const bool on_face = (s == tb);
-        const double dE = std::min(p.E, rho * s * stop_pow(c, m, p.E - 0.5 * rho * s * S));   // midpoint rule
+        const bool hard = class2 && !on_face && s == s_hard;
+        const double dE = std::min(p.E, rho * s * loss(p.E - 0.5 * rho * s * S));   // midpoint rule
         const double Tmid = p.E - 0.5 * dE;
         const Vec3 mid = p.pos + (0.5 * s) * p.dir;
         p.pos = p.pos + s * p.dir;
@@ -669,6 +721,18 @@ void transport_electron(Ctx& c, Particle p, const Run& r) {
             }
         }
         if (deflect) p.dir = rotate(p.dir, std::cos(th), std::sin(th), phi);
+        if (hard && p.E > 2.0 * c.electron_cut) {                          // Moller event where the step ended, at the energy left
+            const double eps = sample_moller_eps(p.rng, p.E, c.electron_cut, nullptr);
+            const double W = eps * p.E, T1 = p.E - W, phi2 = 2.0 * PI * p.rng.u();
+            const double cd = moller_cos(W, p.E), cp = moller_cos(T1, p.E);
+            const Vec3 d0 = p.dir;
+            Particle dl = make_child(p, 0, ELECTRON, W, rotate(d0, cd, std::sqrt(std::max(0.0, 1.0 - cd * cd)), phi2 + PI), r.seed);
+            p.dir = rotate(d0, cp, std::sqrt(std::max(0.0, 1.0 - cp * cp)), phi2);
+            p.E = T1;
+            c.counters[9]++;
+            c.aux[p.region == PHANTOM ? 2 : 3] += 1.0;                     // hard collisions in the phantom / elsewhere (pins)
+            c.stack.push_back(dl);                                         // followed after the primary (LIFO; the order is immaterial, A27)
+        }
     }
 }
 
@@ -703,6 +767,7 @@ int check_ready(Ctx& c) {
     if (c.n[0] <= 0) { c.err = "load_phantom not called"; return -2; }
     if (c.n_layers <= 0) { c.err = "load_epid_layers not called"; return -2; }
     if (c.fu <= 0) { c.err = "load_source not called"; return -2; }
+    if (c.mode == 2 && (int)c.ne.size() != c.n_mat) { c.err = "mode 2 needs orc_set_class2 (electrons per gram)"; return -2; }
     // phantom AABB must lie inside the air part of the world box
     for (int k = 0; k < 8; ++k) {
         Vec3 p{c.org[0] + ((k & 1) ? c.n[0] * c.h[0] : 0), c.org[1] + ((k & 2) ? c.n[1] * c.h[1] : 0), c.org[2] + ((k & 4) ? c.n[2] * c.h[2] : 0)};
@@ -795,6 +860,16 @@ int orc_set_physics(orc_ctx* x, int mode, double pcut, double ecut, double fE, d
     Ctx& c = C(x); c.mode = mode; c.photon_cut = pcut; c.electron_cut = ecut; c.f_E = fE; c.s_max = smax; return 0;
 }
 // options: tracking (0 Woodcock / 1 surface), rebin factor, keep phantom sum of squares, first-collision histogram
+// mode 2 input: electrons per gram of every material
+int orc_set_class2(orc_ctx* x, int n_mat, const float* ne) { Ctx& c = C(x); c.ne.assign(ne, ne + n_mat); return 0; }
+// unit-level: Moller cross section per electron and hard-loss integral; n samples of eps
+int orc_moller_xs(double T, double Tc, double out[2]) { const MollerXs r = moller_xs(T, Tc); out[0] = r.sigma; out[1] = r.hard; return 0; }
+int orc_sample_moller(double T, double Tc, uint64_t seed, uint64_t n, double* eps) {
+    Rng rng; rng.init(seed, 0, 0);
+    for (uint64_t i = 0; i < n; ++i) eps[i] = sample_moller_eps(rng, T, Tc, nullptr);
+    return 0;
+}
+double orc_moller_cos(double Tout, double Tin) { return moller_cos(Tout, Tin); }
 int orc_set_options(orc_ctx* x, int tracking, int rebin, int want_phantom_sq, int fc_bins, double fc_w0, double fc_dw) {
     Ctx& c = C(x);
     if (rebin < 1) { c.err = "rebin < 1"; return -1; }
