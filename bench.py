@@ -98,10 +98,12 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def build_cfg(name, field=0):
+def build_cfg(name, field=0, mode=None):
     from gen import make_config
     from gen.configs import paper_table1_lut
     cfg = make_config(name, field=field)
+    if mode is not None:
+        cfg["physics"]["mode"] = int(mode)      # 2: Class II collisions (Moller delta rays, reading A31)
     if cfg.get("lut") is None:
         cfg["lut"] = paper_table1_lut()          # PAPER.md:157-162 Table 1 as the response LUT (C4 brings its own)
     return cfg
@@ -114,7 +116,7 @@ def run_reference(args):
     if rank != 0:
         return
     import oracle
-    cfg = build_cfg(args.config, args.field)
+    cfg = build_cfg(args.config, args.field, args.physics_mode)
     procs = os.cpu_count() or 1
     sample = args.ref_histories
     oracle.build()
@@ -160,7 +162,7 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    cfg = build_cfg(args.config, args.field)
+    cfg = build_cfg(args.config, args.field, args.physics_mode)
     n = int(args.histories or cfg["n_histories"])
     n_total = n * world
     seed = cfg["seed"]
@@ -251,6 +253,7 @@ def run_ours(args):
 
     def e2e_step():
         eng.init_materials(hin["E_grid"], hin["mu_compton"], hin["mu_pe"], hin["mu_pair"], hin["T_grid"], hin["stop_pow"], hin["rad_len"])
+        eng.set_class2(t["electrons_per_gram"])                          # [n_mat] floats, input of physics mode 2
         eng.load_phantom(ph["spacing"], ph["origin"], hin["density"], hin["material"])
         eng.load_epid_layers(ep["thickness"], ep["material"], ep["density"], ep["scored"], ep["sid"], ep["nu"], ep["nv"], ep["pitch"])
         eng.load_source(s["src_pos"], s["beam_axes"], hin["E_edges"], hin["E_pdf"], s["f_pitch"], s["f_plane_dist"], hin["fluence"])
@@ -303,7 +306,7 @@ def run_ours(args):
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": "%s (BASELINE.json configs[%s])%s" % (args.config, args.config[1:], " field %d" % args.field if args.config == "C4" else ""), "histories_per_gpu_per_step": n,
-                       "n_batches": eng.n_batches, "l2": "flushed between timed steps (256 MiB write)",
+                       "n_batches": eng.n_batches, "physics_mode": int(cfg["physics"]["mode"]), "l2": "flushed between timed steps (256 MiB write)",
                        "parallelism": "history-range sharding x%d, one all-reduce of tally moments per step" % world if world > 1 else "single GPU"},
             "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
@@ -322,6 +325,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3", "C4"])
+    ap.add_argument("--physics-mode", type=int, default=None, choices=[0, 1, 2], help="override the config's physics mode (2: Class II collisions)")
     ap.add_argument("--field", type=int, default=0, help="which of C4's 25 IMRT fields (seeds per reading A23)")
     ap.add_argument("--histories", type=int, default=0, help="histories per GPU per step (default: the config's)")
     ap.add_argument("--cpu-sample", type=int, default=1_000_000, help="oracle histories timed for cpu_baseline")

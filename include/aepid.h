@@ -107,8 +107,11 @@ int aepid_load_source(aepid_ctx* ctx, const float src_pos_cm[3], const float bea
                       int fu, int fv, float f_pitch_cm, float f_plane_dist_cm, const float* fluence);
 
 /* mode 0: kerma (charged-particle energy deposited at the interaction point, configs[0]);
- * mode 1: coupled (CSDA electron steps with Highland deflection).  Cutoffs PAPER.md:104
- * (defaults 0.010 / 0.200 MeV); step rule f_E = 0.10, s_max = 1 cm (reading A13). */
+ * mode 1: coupled (CSDA electron steps with Highland deflection);
+ * mode 2: coupled with Class II collisions ("Class II condensed history"; reading A31): discrete Moller events
+ * with energy transfer above the electron cut-off, each starting a delta ray, and the restricted collision stopping
+ * power below it; needs aepid_set_class2.  Cutoffs PAPER.md:104 (defaults 0.010 / 0.200 MeV); step rule f_E = 0.10,
+ * s_max = 1 cm (reading A13). */
 int aepid_set_physics(aepid_ctx* ctx, int mode, float photon_cut_MeV, float electron_cut_MeV,
                       float f_E, float s_max_cm);
 
@@ -169,6 +172,10 @@ int aepid_field_size(aepid_ctx* ctx, int printed_form, float* s_cm);
 int aepid_apply_response_lut(aepid_ctx* ctx, const float* lut, int nt, int ns,
                              float t_min, float t_max, float s_min, float s_max, float s_eff_cm,
                              const float* epid_in, float* signal_out, float* tmap_out);
+
+/* Input of physics mode 2: electrons per gram of every material, N_A sum_i w_i Z_i / A_i ([n_mat], host or device, copied).
+ * Call after aepid_init_materials (which forgets it). */
+int aepid_set_class2(aepid_ctx* ctx, const float* electrons_per_gram);
 
 /* Scheduler knob of the transport kernel: the most particles a CTA keeps alive at a time, 64 .. 65536
  * (0 = the default, 65536 = half a class queue).  Results do not depend on it (every particle has its own Philox stream);

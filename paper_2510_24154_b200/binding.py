@@ -30,7 +30,7 @@ EXPORTS = ("aepid_workspace_bytes", "aepid_create", "aepid_destroy", "aepid_last
            "aepid_set_counting", "aepid_read_counters", "aepid_sample_source", "aepid_field_size",
            "aepid_apply_response_lut", "aepid_synchronize", "aepid_set_history_offset", "aepid_read_moments",
            "aepid_finalize_moments", "aepid_upsample", "aepid_gamma_index",
-           "aepid_set_phase_space", "aepid_read_phase_space_count", "aepid_set_live_limit")
+           "aepid_set_phase_space", "aepid_read_phase_space_count", "aepid_set_live_limit", "aepid_set_class2")
 
 
 class AepidError(RuntimeError):
@@ -79,6 +79,7 @@ def load_library():
     lib.aepid_read_moments.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.aepid_finalize_moments.argtypes = [vp, vp, vp, C.c_size_t, C.c_double, C.c_double, vp, vp]
     lib.aepid_set_live_limit.argtypes = [vp, C.c_int]
+    lib.aepid_set_class2.argtypes = [vp, vp]
     lib.aepid_set_phase_space.argtypes = [vp, vp, C.c_ulonglong]
     lib.aepid_read_phase_space_count.argtypes = [vp, vp]
     lib.aepid_upsample.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int, C.c_int]
@@ -190,10 +191,15 @@ class Engine:
     def set_physics(self, mode=1, photon_cut=0.010, electron_cut=0.200, f_E=0.10, s_max=1.0, **_):
         self._chk(self._lib.aepid_set_physics(self._h, int(mode), float(photon_cut), float(electron_cut), float(f_E), float(s_max)))
 
+    def set_class2(self, electrons_per_gram):
+        self._chk(self._lib.aepid_set_class2(self._h, _ptr(np.ascontiguousarray(electrons_per_gram, dtype=np.float32))))
+
     def load_config(self, cfg):
         """Host-array convenience: load everything of a gen.make_config dictionary."""
         t, ph, ep, s = cfg["tables"], cfg["phantom"], cfg["epid"], cfg["source"]
         self.init_materials(t["E_grid"], t["mu_compton"], t["mu_pe"], t["mu_pair"], t["T_grid"], t["stop_pow"], t["rad_len"])
+        if "electrons_per_gram" in t:
+            self.set_class2(t["electrons_per_gram"])
         self.load_phantom(ph["spacing"], ph["origin"], ph["density"], ph["material"])
         self.load_epid_layers(ep["thickness"], ep["material"], ep["density"], ep["scored"], ep["sid"], ep["nu"], ep["nv"], ep["pitch"])
         self.load_source(s["src_pos"], s["beam_axes"], s["E_edges"], s["E_pdf"], s["f_pitch"], s["f_plane_dist"], s["fluence"])

@@ -40,7 +40,7 @@ Layout make_layout(const aepid_dims& d) {
     Layout L{};
     L.nvox = (size_t)d.nx * d.ny * d.nz;
     L.npix = (size_t)d.nu * d.nv;
-    L.blob_bytes = ((size_t)d.n_mat * d.n_E * 4 + d.n_E + (size_t)d.n_mat * d.n_T + d.n_mat) * 4;
+    L.blob_bytes = ((size_t)d.n_mat * d.n_E * 4 + d.n_E + (size_t)d.n_mat * d.n_T * 3 + d.n_mat) * 4;
     size_t o = 0;
     auto take = [&](size_t bytes) { const size_t at = o; o += up(bytes); return at; };
     L.vox = take(L.nvox * 4);
@@ -85,6 +85,7 @@ struct aepid_ctx {
     unsigned long long n_done = 0;                         // histories since the last reset
     unsigned long long first_history = 0;                  // global index of history 0 of this context (multi-GPU sharding)
     double hist[256] = {0};
+    std::vector<float> ne; bool have_ne = false;               // electrons per gram (aepid_set_class2)
     bool counting = false;
     int live_max = kPoolSlots / 2;
     float4* ps3 = nullptr; unsigned long long ps3_cap = 0;       // caller-owned Phase Space 3 buffer (aepid_set_phase_space)
@@ -156,14 +157,34 @@ int reset_tallies(aepid_ctx* ctx) {
     return 0;
 }
 
+// Moller cross section per electron for energy transfers above Tc, and the energy-weighted integral (reading A31):
+// d sigma / d eps = (2 pi r_e^2 m c^2 / (beta^2 T)) [1/eps^2 + 1/(1-eps)^2 + (tau/(tau+1))^2 - (2 tau+1)/(tau+1)^2 / (eps (1-eps))],
+// integrated over eps = W / T from Tc / T to 1/2.  Host side, double.
+void moller_integrals(double T, double Tc, double& sigma, double& hard) {
+    sigma = 0.0; hard = 0.0;
+    if (!(T > 2.0 * Tc)) return;
+    const double mec2 = 0.51099895, re = 2.8179403262e-13, pi = 3.14159265358979323846;
+    const double tau = T / mec2, t1 = tau + 1.0, beta2 = tau * (tau + 2.0) / (t1 * t1);
+    const double q1 = tau * tau / (t1 * t1), q2 = (2.0 * tau + 1.0) / (t1 * t1);
+    const double lo = Tc / T, pref = 2.0 * pi * re * re * mec2 / (beta2 * T);
+    sigma = pref * ((1.0 / lo - 2.0) + (2.0 - 1.0 / (1.0 - lo)) + q1 * (0.5 - lo) - q2 * std::log((1.0 - lo) / lo));
+    const double w1 = -std::log(2.0 * lo);
+    const double w2 = (2.0 - std::log(2.0)) - (1.0 / (1.0 - lo) + std::log(1.0 - lo));
+    const double w3 = 0.5 * q1 * (0.25 - lo * lo);
+    const double w4 = q2 * (std::log(1.0 - lo) + std::log(2.0));
+    hard = pref * T * (w1 + w2 + w3 - w4);
+}
+
 // ln-domain photon tables, majorant (reading A7 as corrected in DESIGN.md), ln stopping power, 1/X0.
 int build_tables(aepid_ctx* ctx) {
     const int nm = ctx->n_mat, nE = ctx->n_E, nT = ctx->n_T;
-    std::vector<float> blob((size_t)nm * nE * 4 + nE + (size_t)nm * nT + nm);
+    std::vector<float> blob((size_t)nm * nE * 4 + nE + (size_t)nm * nT * 3 + nm, 0.0f);
     float* phot = blob.data();
     float* maj = phot + (size_t)nm * nE * 4;
     float* lnS = maj + nE;
     float* invX0 = lnS + (size_t)nm * nT;
+    float* lnL = invX0 + nm;                       // mode 2: ln restricted stopping power, Moller cross section (cm^2/g)
+    float* sig = lnL + (size_t)nm * nT;
     for (int m = 0; m < nm; ++m)
         for (int j = 0; j < nE; ++j) {
             const size_t o = (size_t)m * nE + j;
@@ -186,6 +207,15 @@ int build_tables(aepid_ctx* ctx) {
         for (int j = 0; j < nT; ++j) lnS[(size_t)m * nT + j] = (float)std::log(std::max((double)ctx->S[(size_t)m * nT + j], 1e-37));
         invX0[m] = 1.0f / ctx->X0[m];
     }
+    if (ctx->have_ne)
+        for (int m = 0; m < nm; ++m)
+            for (int j = 0; j < nT; ++j) {
+                double sg, hd;
+                moller_integrals((double)ctx->Tg[j], (double)ctx->ph.ecut, sg, hd);
+                const size_t o = (size_t)m * nT + j;
+                lnL[o] = (float)std::log(std::max((double)ctx->S[o] - (double)ctx->ne[m] * hd, 1e-37));
+                sig[o] = (float)((double)ctx->ne[m] * sg);
+            }
     CU(cudaMemcpyAsync(ctx->d_blob(), blob.data(), blob.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));       // blob is a local vector
     ctx->tb.n_mat = nm; ctx->tb.n_E = nE; ctx->tb.n_T = nT;
@@ -229,6 +259,7 @@ int fill_params(aepid_ctx* ctx, TransportParams& p) {
     if (!ctx->have_phantom) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_load_phantom has not been called");
     if (!ctx->have_epid) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_load_epid_layers has not been called");
     if (!ctx->have_source) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_load_source has not been called");
+    if (ctx->ph.mode == 2 && !ctx->have_ne) return fail(ctx, AEPID_ERR_BAD_STATE, "physics mode 2 needs aepid_set_class2 (after aepid_init_materials)");
     if (int rc = check_geometry(ctx)) return rc;
     for (int l = 0; l < ctx->g.n_layers; ++l)
         if (ctx->g.lmat[l] >= ctx->n_mat) return fail(ctx, AEPID_ERR_BAD_ARG, "EPID layer material index out of range");
@@ -305,7 +336,7 @@ int aepid_init_materials(aepid_ctx* ctx, int n_mat, int n_E, const float* E, con
     for (float v : ctx->S) if (!(v > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "stopping power must be positive");
     for (float v : ctx->X0) if (!(v > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "radiation length must be positive");
     ctx->n_mat = n_mat; ctx->n_E = n_E; ctx->n_T = n_T;
-    ctx->have_mat = true; ctx->tables_dirty = true;
+    ctx->have_mat = true; ctx->tables_dirty = true; ctx->have_ne = false;
     return 0;
 }
 
@@ -432,7 +463,8 @@ int aepid_load_source(aepid_ctx* ctx, const float src[3], const float axes[9], i
 
 int aepid_set_physics(aepid_ctx* ctx, int mode, float pcut, float ecut, float fE, float smax) {
     if (!ctx) return AEPID_ERR_BAD_ARG;
-    if ((mode != 0 && mode != 1) || !(pcut > 0) || !(ecut > 0) || !(fE > 0) || !(fE <= 0.5f) || !(smax > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "physics parameters out of range");
+    if ((mode != 0 && mode != 1 && mode != 2) || !(pcut > 0) || !(ecut > 0) || !(fE > 0) || !(fE <= 0.5f) || !(smax > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "physics parameters out of range");
+    if (ecut != ctx->ph.ecut) ctx->tables_dirty = true;       // the restricted stopping power depends on the cut-off
     ctx->ph.mode = mode; ctx->ph.pcut = pcut; ctx->ph.ecut = ecut; ctx->ph.fE = fE; ctx->ph.smax = smax;
     return 0;
 }
@@ -618,6 +650,16 @@ int aepid_apply_response_lut(aepid_ctx* ctx, const float* lut, int nt, int ns, f
     if (!dev_out) if (int rc = deliver(ctx, signal_out, d_out, n * 4, &need_sync)) return rc;
     if (tmap_out) if (int rc = deliver(ctx, tmap_out, ctx->d_tmap(), n * 4, &need_sync)) return rc;
     if (need_sync) CU(cudaStreamSynchronize(ctx->stream));
+    return 0;
+}
+
+int aepid_set_class2(aepid_ctx* ctx, const float* electrons_per_gram) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    if (!ctx->have_mat) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_init_materials has not been called");
+    if (!electrons_per_gram) return fail(ctx, AEPID_ERR_BAD_ARG, "null pointer");
+    if (int rc = fetch(ctx, electrons_per_gram, (size_t)ctx->n_mat, ctx->ne)) return rc;
+    for (float v : ctx->ne) if (!(v > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "electrons per gram must be positive");
+    ctx->have_ne = true; ctx->tables_dirty = true;
     return 0;
 }
 

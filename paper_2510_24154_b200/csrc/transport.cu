@@ -144,6 +144,7 @@ struct Shared {
     const float* maj;
     const float* lnS;
     const float* invX0;
+    const float* sig;               // mode 2: Moller cross section [n_mat][n_T] (cm^2/g), linear in ln T; lnS then holds the restricted stopping power
 };
 
 struct Lane {
@@ -670,12 +671,26 @@ __device__ __forceinline__ bool epid_flight(Lane& L, const TransportParams& P, c
 
 // ---------------------------------------------------------------- K5 electron / positron step
 // Energy loss of the step (midpoint rule), deposit-independent part shared by the two step functions.
-struct StepLoss { float s, dep, Tmid; };
-__device__ __forceinline__ StepLoss step_loss(Lane& L, const TransportParams& P, const Shared& sh, int m, float rho, float tb) {
+// Class II (C2, physics mode 2, reading A31): sh.lnS holds the restricted stopping power, and the step also stops at the
+// next hard (Moller) collision, whose distance is drawn with the cross section at the energy the step starts with (draw rh).
+struct StepLoss { float s, dep, Tmid; bool hard; };
+template <bool C2>
+__device__ __forceinline__ StepLoss step_loss(Lane& L, const TransportParams& P, const Shared& sh, int m, float rho, float tb, uint32_t rh) {
     const float T = L.E;
     const float S = stop_pow(P, sh, m, T);
     StepLoss r;
     r.s = fminf(tb, fminf(__fdividef(P.ph.fE * T, rho * S), P.ph.smax));
+    r.hard = false;
+    if (C2) {
+        float f = (__logf(T) - P.tb.lnT0) * P.tb.inv_dlnT;
+        f = fminf(fmaxf(f, 0.0f), (float)(P.tb.n_T - 1));
+        const int i = min((int)f, P.tb.n_T - 2);
+        const float* q = sh.sig + m * P.tb.n_T + i;
+        const float sg = fmaf(f - (float)i, q[1] - q[0], q[0]);
+        const float sh_ = sg > 0.0f ? __fdividef(-__logf(u01(rh)), rho * sg) : kInf;
+        r.hard = sh_ < r.s;                                                // strictly inside the step: a step that ends on a face does not collide
+        r.s = fminf(r.s, sh_);
+    }
     const float S2 = stop_pow(P, sh, m, T - 0.5f * rho * r.s * S);        // midpoint rule
     const float dE = fminf(T, rho * r.s * S2);
     const float Tn = T - dE;
@@ -695,6 +710,37 @@ __device__ __forceinline__ void highland(const Shared& sh, int m, float rho_s, f
     __sincosf(th, &st, &ct);
     __sincosf(2.0f * kPi * u01(rb) - kPi, &sp, &cp);
 }
+// Hard (Moller) collision of a charged particle of kinetic energy L.E > 2 Tc where its step ended (reading A31): the energy
+// transfer W = eps E, eps in [Tc / E, 1/2], is sampled from the Moller density by rejection from 1 / eps^2 (one Philox block
+// per trial: two draws for the trial, the third for the azimuth); both outgoing directions follow from energy-momentum
+// conservation.  The delta ray is an electron queued on the lane's credit, the lane goes on with the rest.
+template <bool COUNT>
+__device__ __forceinline__ void moller_event(Lane& L, const TransportParams& P, uint32_t* cnt) {
+    const float T = L.E, tau = T * (1.0f / kMec2), a = __fdividef(P.ph.ecut, T);
+    const float t1 = rcp(tau + 1.0f), c1 = tau * tau * t1 * t1, c2 = (2.0f * tau + 1.0f) * t1 * t1;
+    const float gmax = 2.0f + 0.25f * c1;
+    float eps, phi;
+#pragma unroll 1
+    for (;;) {
+        const uint4 r = rng_block(L, P);
+        eps = __fdividef(a, 1.0f - u01(r.x) * (1.0f - 2.0f * a));
+        const float x = __fdividef(eps, 1.0f - eps);
+        const float g = 1.0f + x * x + c1 * eps * eps - c2 * x;
+        phi = 2.0f * kPi * u01(r.z) - kPi;
+        if (u01(r.y) * gmax <= g) break;
+    }
+    const float W = eps * T, T1 = T - W;
+    const float cd = sqrtf(__fdividef(W * (T + 2.0f * kMec2), T * (W + 2.0f * kMec2)));
+    const float cpm = sqrtf(__fdividef(T1 * (T + 2.0f * kMec2), T * (T1 + 2.0f * kMec2)));
+    float sphi, cphi; __sincosf(phi, &sphi, &cphi);
+    float ex = L.dx, ey = L.dy, ez = L.dz;
+    rotate(ex, ey, ez, cd, sqrtf(fmaxf(0.0f, 1.0f - cd * cd)), -cphi, -sphi);     // the delta ray: opposite azimuth
+    uint32_t f = L.flags; SET_TYPE(f, T_ELECTRON);
+    if (COUNT) { cnt[9]++; cnt[14]++; }
+    spawn_from(L, L.x, L.y, L.z, ex, ey, ez, W, f, child_id(L, 0));
+    rotate(L.dx, L.dy, L.dz, cpm, sqrtf(fmaxf(0.0f, 1.0f - cpm * cpm)), cphi, sphi);
+    L.E = T1;
+}
 // charged particle at or below its cutoff (PAPER.md:104, 200 keV): local deposit; a positron annihilates
 template <bool COUNT>
 __device__ __forceinline__ void stop_charged(Lane& L, const TransportParams& P, uint32_t* cnt) {
@@ -709,8 +755,8 @@ __device__ __forceinline__ void stop_charged(Lane& L, const TransportParams& P, 
 // to the rare exit from the grid (selects instead of per-axis branches: a face is crossed by a few lanes of nearly
 // every warp, so divergent code there is paid by all).  The particle is above its cutoff.  Invariant of class E: the
 // pending deposit of the lane belongs to the current voxel (L.pidx == L.vlin, set when the particle is loaded).
-template <bool COUNT>
-__device__ __forceinline__ void electron_step_phantom(Lane& L, const TransportParams& P, const Shared& sh, uint32_t ra, uint32_t rb, uint32_t* cnt) {
+template <bool COUNT, bool C2>
+__device__ __forceinline__ void electron_step_phantom(Lane& L, const TransportParams& P, const Shared& sh, uint32_t ra, uint32_t rb, uint32_t rh, uint32_t* cnt) {
     const Geom& g = P.g;
     const float rho = __uint_as_float(L.cw & ~31u); const int m = (int)(L.cw & 31u);
     // distance to the voxel face in the direction of travel, per axis (a vanishing component gives a huge distance)
@@ -719,7 +765,7 @@ __device__ __forceinline__ void electron_step_phantom(Lane& L, const TransportPa
     const float tz = (L.dz > 0.0f ? 1.0f - L.z : L.z) * g.hz * rcp(fabsf(L.dz) + 1e-30f);
     const float tb = fmaxf(fminf(tx, fminf(ty, tz)), 0.0f);
     const bool ax0 = tx <= ty && tx <= tz, ax1 = !ax0 && ty <= tz, ax2 = !ax0 && !ax1;
-    const StepLoss sl = step_loss(L, P, sh, m, rho, tb);
+    const StepLoss sl = step_loss<C2>(L, P, sh, m, rho, tb, rh);
     if (COUNT) { cnt[6]++; if (!(sl.s > 0.0f)) cnt[15]++; }
     L.pval += sl.dep; L.a_ph += sl.dep;
     L.x = fmaf(sl.s * g.ihx, L.dx, L.x); L.y = fmaf(sl.s * g.ihy, L.dy, L.y); L.z = fmaf(sl.s * g.ihz, L.dz, L.z);
@@ -749,10 +795,11 @@ __device__ __forceinline__ void electron_step_phantom(Lane& L, const TransportPa
         SET_REGION(L.flags, R_AIR);
     }
     rotate(L.dx, L.dy, L.dz, ct, st, cp, sp);
+    if (C2 && sl.hard && L.E > 2.0f * P.ph.ecut) moller_event<COUNT>(L, P, cnt);   // at the end of the step, with the energy left
 }
 // one step in the air or inside the EPID (the particle is above its cutoff)
-template <bool COUNT>
-__device__ __forceinline__ void electron_step_outside(Lane& L, const TransportParams& P, const Shared& sh, uint32_t ra, uint32_t rb, uint32_t* cnt) {
+template <bool COUNT, bool C2>
+__device__ __forceinline__ void electron_step_outside(Lane& L, const TransportParams& P, const Shared& sh, uint32_t ra, uint32_t rb, uint32_t rh, uint32_t* cnt) {
     const Geom& g = P.g;
     const bool in_air = F_REGION(L.flags) == R_AIR;
     float rho, tb; int m, axis = 0, kind = 0;
@@ -780,7 +827,7 @@ __device__ __forceinline__ void electron_step_outside(Lane& L, const TransportPa
         const float tl = lateral_exit(L.x, L.y, L.dx, L.dy);
         if (tl < tf) { tb = tl; kind = 2; } else { tb = tf; kind = 0; }
     }
-    const StepLoss sl = step_loss(L, P, sh, m, rho, tb);
+    const StepLoss sl = step_loss<C2>(L, P, sh, m, rho, tb, rh);
     if (COUNT && !(sl.s > 0.0f)) cnt[15]++;
     if (in_air) { if (COUNT) cnt[7]++; L.a_air += sl.dep; }
     else { if (COUNT) cnt[8]++; dep_epid(L, fmaf(0.5f * sl.s, L.dx, L.x), fmaf(0.5f * sl.s, L.dy, L.y), sl.dep); }   // pixel of the step midpoint (A24)
@@ -807,23 +854,31 @@ __device__ __forceinline__ void electron_step_outside(Lane& L, const TransportPa
         }
     }
     rotate(L.dx, L.dy, L.dz, ct, st, cp, sp);
+    if (C2 && sl.hard && L.E > 2.0f * P.ph.ecut) moller_event<COUNT>(L, P, cnt);   // at the end of the step, with the energy left
 }
 // K5 for one lane: up to kStepsE / kStepsX consecutive steps per event, one Philox block per two steps
-template <bool COUNT, bool PHANTOM>
+template <bool COUNT, bool PHANTOM, bool C2>
 __device__ __forceinline__ void charged_event(Lane& L, const TransportParams& P, const Shared& sh, uint32_t* cnt) {
     if (L.E <= P.ph.ecut) { stop_charged<COUNT>(L, P, cnt); return; }
     uint4 r = PHANTOM ? rng_block_hot(L, P) : rng_block(L, P);
 #pragma unroll 1
     for (int k = 0; k < (PHANTOM ? kStepsE : kStepsX); ++k) {
-        if (k && !(k & 1)) r = PHANTOM ? rng_block_hot(L, P) : rng_block(L, P);
-        if (PHANTOM) electron_step_phantom<COUNT>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, cnt);
-        else electron_step_outside<COUNT>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, cnt);
+        if (C2) {                                                          // a block per step: deflection (x, y), hard-collision distance (z)
+            if (k) r = PHANTOM ? rng_block_hot(L, P) : rng_block(L, P);
+            if (PHANTOM) electron_step_phantom<COUNT, true>(L, P, sh, r.x, r.y, r.z, cnt);
+            else electron_step_outside<COUNT, true>(L, P, sh, r.x, r.y, r.z, cnt);
+        } else {
+            if (k && !(k & 1)) r = PHANTOM ? rng_block_hot(L, P) : rng_block(L, P);
+            if (PHANTOM) electron_step_phantom<COUNT, false>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, 0u, cnt);
+            else electron_step_outside<COUNT, false>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, 0u, cnt);
+        }
         if (!L.alive) break;
         if (L.E <= P.ph.ecut) {                                            // cutoff reached: an electron stops here and now;
             if (F_TYPE(L.flags) == T_ELECTRON) { dep_here(L, P, L.E); L.alive = false; }   // a positron first needs a slot for its second photon
             break;
         }
         if ((F_REGION(L.flags) == R_PHANTOM) != PHANTOM) break;
+        if (C2 && L.spare == kNone) break;                                 // the credit went into a delta ray: the next step needs a new one
     }
 }
 
@@ -925,11 +980,11 @@ __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned lon
 }
 
 // One phase of class C for one warp (header comment).  On return every lane is empty and holds no slot.
-template <bool COUNT, int C>
+template <bool COUNT, int C, bool C2>
 __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, const Shared& sh, double* led, uint32_t* cnt) {
     const unsigned lane = threadIdx.x & 31u;
     const unsigned lt_mask = (1u << lane) - 1u;
-    constexpr bool kSpawns = C == C_W || C == C_P;             // classes whose events create secondaries all the time
+    constexpr bool kSpawns = C == C_W || C == C_P || (C2 && (C == C_E || C == C_X));   // classes whose events create secondaries all the time
     const int keep = *((volatile int*)&s_keep);
     bool leaving = false, park = false;
 #pragma unroll 1
@@ -1027,6 +1082,8 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
         bool on = L.alive;
         if (C == C_W || C == C_P) {
             if (on && !ensure_spare(L)) { park = true; on = false; if (COUNT && !kPhaseClock) cnt[29]++; }   // an interaction may create a secondary
+        } else if (C2 && (C == C_E || C == C_X)) {
+            if (on && !ensure_spare(L)) { park = true; on = false; if (COUNT && !kPhaseClock) cnt[29]++; }   // a step may end in a Moller event
         } else if (C == C_E || C == C_X) {
             if (on && F_TYPE(L.flags) == T_POSITRON && L.E <= P.ph.ecut && !ensure_spare(L)) { park = true; on = false; if (COUNT && !kPhaseClock) cnt[29]++; }   // annihilation needs a slot
         }
@@ -1043,8 +1100,8 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
             }
             if (hit) interact<COUNT>(L, P, sh, xsel, pe, co, cnt);
         } else if (on) {
-            if (C == C_E) charged_event<COUNT, true>(L, P, sh, cnt);
-            else if (C == C_X) charged_event<COUNT, false>(L, P, sh, cnt);
+            if (C == C_E) charged_event<COUNT, true, C2>(L, P, sh, cnt);
+            else if (C == C_X) charged_event<COUNT, false, C2>(L, P, sh, cnt);
             else if (L.E < P.ph.pcut) { if (COUNT) cnt[13]++; dep_here(L, P, L.E); L.alive = false; }   // PAPER.md:104, 10 keV
             else {
                 bool hit = false; float xsel = 0.0f, pe = 0.0f, co = 0.0f;
@@ -1071,7 +1128,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
     if (lane == 0) atomicAdd(&s_left, 1);
 }
 
-template <bool COUNT>
+template <bool COUNT, bool C2>
 __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_constant__ TransportParams P) {
     // dynamic shared memory: per-warp ledger | table blob
     double* const led_all = reinterpret_cast<double*>(smem_raw);
@@ -1082,6 +1139,8 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
     sh.maj = reinterpret_cast<const float*>(sh.phot + P.tb.n_mat * P.tb.n_E);
     sh.lnS = sh.maj + P.tb.n_E;
     sh.invX0 = sh.lnS + P.tb.n_mat * P.tb.n_T;
+    sh.sig = sh.invX0 + P.tb.n_mat + P.tb.n_mat * P.tb.n_T;
+    if (C2) sh.lnS = sh.invX0 + P.tb.n_mat;                    // the restricted stopping power takes the place of the total one
     for (int i = threadIdx.x; i < kWarps * 8; i += kThreads) led_all[i] = 0.0;
     if (threadIdx.x < kRings) { s_tail[threadIdx.x] = 0u; s_head[threadIdx.x] = 0u; s_snap[threadIdx.x] = 0u; }
     if (threadIdx.x < 2) s_flag[threadIdx.x] = 0;
@@ -1115,11 +1174,11 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
         const long long t0 = clock64();
 #endif
         switch (ph) {
-            case C_A: run_phase<COUNT, C_A>(L, P, sh, led, cnt); break;
-            case C_W: run_phase<COUNT, C_W>(L, P, sh, led, cnt); break;
-            case C_E: run_phase<COUNT, C_E>(L, P, sh, led, cnt); break;
-            case C_P: run_phase<COUNT, C_P>(L, P, sh, led, cnt); break;
-            default:  run_phase<COUNT, C_X>(L, P, sh, led, cnt); break;
+            case C_A: run_phase<COUNT, C_A, C2>(L, P, sh, led, cnt); break;
+            case C_W: run_phase<COUNT, C_W, C2>(L, P, sh, led, cnt); break;
+            case C_E: run_phase<COUNT, C_E, C2>(L, P, sh, led, cnt); break;
+            case C_P: run_phase<COUNT, C_P, C2>(L, P, sh, led, cnt); break;
+            default:  run_phase<COUNT, C_X, C2>(L, P, sh, led, cnt); break;
         }
 #ifdef AEPID_PHASE_CLOCK
         if (COUNT && lane == 0) { atomicAdd(P.counters + 10, (unsigned long long)(clock64() - t0)); atomicAdd(P.counters + 27 + ph, (unsigned long long)(clock64() - t0)); }   // busy warp-cycles
@@ -1157,20 +1216,23 @@ size_t transport_smem_bytes(const Tables& t) {      // dynamic + static shared m
     return kDynSmemFixed + (size_t)t.blob_words * 4 + sizeof(Geom) + 512;
 }
 
+template <bool COUNT, bool C2>
+static int launch_one(const TransportParams& p, unsigned blocks, size_t smem, cudaStream_t stream) {
+    const cudaError_t e = cudaFuncSetAttribute(transport_kernel<COUNT, C2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return (int)e;
+    transport_kernel<COUNT, C2><<<blocks, kThreads, smem, stream>>>(p);
+    return (int)cudaGetLastError();
+}
 int launch_transport(const TransportParams& p, bool counting, int sm_count, void* stream) {
     const size_t smem = kDynSmemFixed + (size_t)p.tb.blob_words * 4;
-    cudaError_t e;
-    if (counting) e = cudaFuncSetAttribute(transport_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    else e = cudaFuncSetAttribute(transport_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return (int)e;
-    // persistent grid: one CTA per SM (each with its own slice of the particle pool), but no more CTAs than there is work for
+    // persistent grid: one CTA per SM (each with its own class queues), but no more CTAs than there is work for
     long long blocks = sm_count < kMaxCtas ? sm_count : kMaxCtas;
     const long long need = ((long long)p.n + 255) / 256;
     if (blocks > need) blocks = need;
     if (blocks < 1) blocks = 1;
-    if (counting) transport_kernel<true><<<(unsigned)blocks, kThreads, smem, (cudaStream_t)stream>>>(p);
-    else transport_kernel<false><<<(unsigned)blocks, kThreads, smem, (cudaStream_t)stream>>>(p);
-    return (int)cudaGetLastError();
+    const bool c2 = p.ph.mode == 2;                       // Class II collisions: its own instantiation, modes 0 and 1 pay nothing for it
+    if (counting) return c2 ? launch_one<true, true>(p, (unsigned)blocks, smem, (cudaStream_t)stream) : launch_one<true, false>(p, (unsigned)blocks, smem, (cudaStream_t)stream);
+    return c2 ? launch_one<false, true>(p, (unsigned)blocks, smem, (cudaStream_t)stream) : launch_one<false, false>(p, (unsigned)blocks, smem, (cudaStream_t)stream);
 }
 // K1 alone (aepid_sample_source): out[k] = {E, dx, dy, dz, pixel, u, v, 0} for history first + k
 __global__ void sample_source_kernel(const __grid_constant__ TransportParams P, uint64_t first, uint64_t n, float* __restrict__ out) {

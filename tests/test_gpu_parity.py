@@ -157,6 +157,47 @@ def test_paper_scoring_grid_160x160_at_2p5mm():
     compare(cfg, cfg["n_histories"], 4_000_000, rebin=4, phantom_voxels=False)   # 40x40 @ 1 cm: ~90 oracle events per tested pixel
 
 
+def test_c1_class2_collisions_full_size():
+    """Physics mode 2 (Moller delta rays above the cut-off, restricted stopping power; reading A31) on the C1 workload."""
+    cfg = make_config("C1")
+    cfg["physics"]["mode"] = 2
+    compare(cfg, cfg["n_histories"], 4_000_000, rebin=8)
+
+
+def test_class2_needs_its_input_and_does_not_depend_on_the_live_limit():
+    from paper_2510_24154_b200 import AepidError
+    cfg = make_config("C1", shrink=4)
+    cfg["physics"]["mode"] = 2
+    t = cfg["tables"]
+    eng = engine_for(cfg)
+    eng.init_materials(t["E_grid"], t["mu_compton"], t["mu_pe"], t["mu_pair"], t["T_grid"], t["stop_pow"], t["rad_len"])   # forgets the electron densities
+    with pytest.raises(AepidError):
+        eng.simulate(1000, 1)
+    eng.close()
+    res = []
+    for lim in (0, 1024, 256):                              # every charged-particle step needs a credit in this mode
+        eng = engine_for(cfg)
+        eng.set_live_limit(lim)
+        eng.set_counting(True)
+        eng.simulate(300_000, 9)
+        r = eng.read_tallies()
+        check_ledger(r["ledger"], 300_000)
+        r["n_charged"] = eng.read_counters()[9]
+        res.append(r)
+        eng.close()
+    for r in res[1:]:
+        assert r["n_charged"] == res[0]["n_charged"]                     # the same delta rays
+        assert np.allclose(r["ledger"][:6], res[0]["ledger"][:6], rtol=2e-6)
+        assert np.allclose(r["phantom_mean"], res[0]["phantom_mean"], rtol=1e-3, atol=1e-9)
+    # and there are more charged particles than without the hard collisions
+    cfg["physics"]["mode"] = 1
+    eng = engine_for(cfg); eng.set_counting(True); eng.simulate(300_000, 9)
+    n1 = eng.read_counters()[9]; eng.close()
+    raw1 = oracle.run_sharded(cfg, 300_000, 9); cfg["physics"]["mode"] = 2; raw2 = oracle.run_sharded(cfg, 300_000, 9)
+    d_gpu, d_or = (res[0]["n_charged"] - n1) / 3e5, (raw2["counters"][9] - raw1["counters"][9]) / 3e5
+    assert d_or > 0.03 and abs(d_gpu - d_or) < 0.05 * d_or + 5 * np.sqrt(d_or / 3e5)   # delta rays per history
+
+
 def test_c2_heterogeneous_imrt_full_grid():
     cfg = make_config("C2")
     compare(cfg, 40_000_000, 2_000_000, rebin=32, frac_ok=0.985, phantom_voxels=False, min_tested=15)

@@ -77,10 +77,11 @@ def _hist(x, bins, w=None):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("name,shrink,n", [("C1", 1, 400_000), ("C0", 1, 300_000), ("C2", 2, 300_000)])
-def test_ps3_gpu_matches_oracle(name, shrink, n):
+@pytest.mark.parametrize("name,shrink,n,mode", [("C1", 1, 400_000, 1), ("C0", 1, 300_000, 0), ("C2", 2, 300_000, 1), ("C1", 1, 400_000, 2)])
+def test_ps3_gpu_matches_oracle(name, shrink, n, mode):
     from paper_2510_24154_b200 import Engine
     cfg = make_config(name, shrink=shrink)
+    cfg["physics"]["mode"] = mode                                        # 2: with Moller delta rays (reading A31)
     seed = cfg["seed"]
     eng = Engine.for_config(cfg); eng.load_config(cfg)
     eng.set_phase_space(n)                                               # at most ~0.5 arrivals per history
