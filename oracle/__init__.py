@@ -94,6 +94,19 @@ def sample_moller(T, Tc, seed, n):
     return eps
 
 
+def brems_xs(T, kc, X0):
+    """(Sigma of photons above kc [cm^2/g], restricted radiative stopping power [MeV cm^2/g]) of the reading-A32 model."""
+    o = (C.c_double * 2)()
+    lib().orc_brems_xs(C.c_double(T), C.c_double(kc), C.c_double(X0), o)
+    return o[0], o[1]
+
+
+def sample_brems(T, kc, seed, n):
+    k = np.empty(n)
+    lib().orc_sample_brems(C.c_double(T), C.c_double(kc), C.c_uint64(seed), C.c_uint64(n), _p(k, C.c_double))
+    return k
+
+
 def moller_cos(T_out, T_in):
     return lib().orc_moller_cos(C.c_double(T_out), C.c_double(T_in))
 

@@ -628,6 +628,28 @@ double sample_moller_eps(Rng& rng, double T, double Tc, uint64_t* trials) {
 // scattering angles of the two outgoing electrons (energy-momentum conservation, target at rest)
 inline double moller_cos(double Tout, double Tin) { return std::sqrt(Tout * (Tin + 2.0 * MEC2) / (Tin * (Tout + 2.0 * MEC2))); }
 
+// Bremsstrahlung (mode 3; reading A32): parametric, complete-screening shape normalised by the radiation length,
+//   d Sigma / d k = (1 / (X0 k)) (4/3 - 4/3 y + y^2),  y = k / T,  0 < k <= T      [cm^2/g per MeV]
+// so that the total radiative stopping power is T / X0.  Photons above kc (the photon cut-off) are discrete events,
+// the loss to photons below kc is continuous.
+struct BremsXs { double sigma, soft; };     // Sigma(k > kc) [cm^2/g]; restricted radiative stopping power [MeV cm^2/g]
+BremsXs brems_xs(double T, double kc, double X0) {
+    BremsXs r{0.0, T / X0};
+    if (!(T > kc)) return r;                                         // everything is soft
+    const double a = kc / T;
+    r.sigma = (4.0 / 3.0 * std::log(1.0 / a) - 4.0 / 3.0 * (1.0 - a) + 0.5 * (1.0 - a * a)) / X0;
+    r.soft = T * (4.0 / 3.0 * a - 2.0 / 3.0 * a * a + a * a * a / 3.0) / X0;
+    return r;
+}
+// photon energy from the density above on [kc, T]: rejection from 1/k with (4/3 - 4/3 y + y^2) / (4/3) <= 1
+double sample_brems_k(Rng& rng, double T, double kc) {
+    for (;;) {
+        const double x1 = rng.u(), x2 = rng.u();
+        const double k = kc * std::pow(T / kc, x1), y = k / T;
+        if (x2 <= 1.0 - y + 0.75 * y * y) return k;
+    }
+}
+
 double highland_theta0(const Ctx& c, int m, double rho_s, double Tm) {
     const double t = rho_s / c.X0[m];
     if (!(t > 0)) return 0.0;
@@ -667,14 +689,19 @@ void transport_electron(Ctx& c, Particle p, const Run& r) {
         }
         // mode 2: restricted stopping power L = S - n_e int W d sigma and a distance to the next hard (Moller) collision,
         // both from the cross section at the energy the step starts with (reading A31)
-        const bool class2 = c.mode == 2;
-        auto loss = [&](double T) { return stop_pow(c, m, T) - (class2 ? c.ne[m] * moller_xs(T, c.electron_cut).hard : 0.0); };
+        // mode 3 adds bremsstrahlung (reading A32): photons above the photon cut-off are discrete, the rest is continuous loss
+        const bool class2 = c.mode >= 2, brems = c.mode == 3;
+        auto loss = [&](double T) {
+            return stop_pow(c, m, T) - (class2 ? c.ne[m] * moller_xs(T, c.electron_cut).hard : 0.0)
+                   + (brems ? brems_xs(T, c.photon_cut, c.X0[m]).soft : 0.0);
+        };
         const double S = loss(p.E);
-        double s_hard = INF;
+        double s_hard = INF, sig_b = 0.0, sig_all = 0.0;
         if (class2) {
-            const double Sig = c.ne[m] * moller_xs(p.E, c.electron_cut).sigma;
+            sig_b = brems ? brems_xs(p.E, c.photon_cut, c.X0[m]).sigma : 0.0;
+            sig_all = c.ne[m] * moller_xs(p.E, c.electron_cut).sigma + sig_b;
             const double xh = p.rng.u();                                    // drawn every step, also when no hard collision is possible
-            if (Sig > 0) s_hard = -std::log(xh) / (rho * Sig);
+            if (sig_all > 0) s_hard = -std::log(xh) / (rho * sig_all);
         }
         double s = std::min(std::min(tb, s_hard), std::min(c.f_E * p.E / (rho * S), c.s_max));
         const bool on_face = (s == tb);
@@ -721,7 +748,18 @@ void transport_electron(Ctx& c, Particle p, const Run& r) {
             }
         }
         if (deflect) p.dir = rotate(p.dir, std::cos(th), std::sin(th), phi);
-        if (hard && p.E > 2.0 * c.electron_cut) {                          // Moller event where the step ended, at the energy left
+        // which kind of hard event: by the cross sections the distance was drawn with
+        const bool is_brems = hard && brems && p.rng.u() * sig_all < sig_b;
+        if (is_brems) {
+            if (p.E > c.photon_cut) {                                       // photon along the electron's direction (reading A32)
+                const double k = sample_brems_k(p.rng, p.E, c.photon_cut);
+                Particle ph = make_child(p, 0, PHOTON, k, p.dir, r.seed);
+                p.E -= k;
+                p.rng.skip_block();
+                c.counters[9]++;
+                c.stack.push_back(ph);
+            }
+        } else if (hard && p.E > 2.0 * c.electron_cut) {                   // Moller event where the step ended, at the energy left
             const double eps = sample_moller_eps(p.rng, p.E, c.electron_cut, nullptr);
             const double W = eps * p.E, T1 = p.E - W, phi2 = 2.0 * PI * p.rng.u();
             const double cd = moller_cos(W, p.E), cp = moller_cos(T1, p.E);
@@ -731,6 +769,7 @@ void transport_electron(Ctx& c, Particle p, const Run& r) {
             p.E = T1;
             c.counters[9]++;
             c.aux[p.region == PHANTOM ? 2 : 3] += 1.0;                     // hard collisions in the phantom / elsewhere (pins)
+            p.rng.skip_block();
             c.stack.push_back(dl);                                         // followed after the primary (LIFO; the order is immaterial, A27)
         }
     }
@@ -767,7 +806,7 @@ int check_ready(Ctx& c) {
     if (c.n[0] <= 0) { c.err = "load_phantom not called"; return -2; }
     if (c.n_layers <= 0) { c.err = "load_epid_layers not called"; return -2; }
     if (c.fu <= 0) { c.err = "load_source not called"; return -2; }
-    if (c.mode == 2 && (int)c.ne.size() != c.n_mat) { c.err = "mode 2 needs orc_set_class2 (electrons per gram)"; return -2; }
+    if (c.mode >= 2 && (int)c.ne.size() != c.n_mat) { c.err = "mode 2 needs orc_set_class2 (electrons per gram)"; return -2; }
     // phantom AABB must lie inside the air part of the world box
     for (int k = 0; k < 8; ++k) {
         Vec3 p{c.org[0] + ((k & 1) ? c.n[0] * c.h[0] : 0), c.org[1] + ((k & 2) ? c.n[1] * c.h[1] : 0), c.org[2] + ((k & 4) ? c.n[2] * c.h[2] : 0)};
@@ -870,6 +909,12 @@ int orc_sample_moller(double T, double Tc, uint64_t seed, uint64_t n, double* ep
     return 0;
 }
 double orc_moller_cos(double Tout, double Tin) { return moller_cos(Tout, Tin); }
+int orc_brems_xs(double T, double kc, double X0, double out[2]) { const BremsXs r = brems_xs(T, kc, X0); out[0] = r.sigma; out[1] = r.soft; return 0; }
+int orc_sample_brems(double T, double kc, uint64_t seed, uint64_t n, double* k) {
+    Rng rng; rng.init(seed, 0, 0);
+    for (uint64_t i = 0; i < n; ++i) k[i] = sample_brems_k(rng, T, kc);
+    return 0;
+}
 int orc_set_options(orc_ctx* x, int tracking, int rebin, int want_phantom_sq, int fc_bins, double fc_w0, double fc_dw) {
     Ctx& c = C(x);
     if (rebin < 1) { c.err = "rebin < 1"; return -1; }

@@ -126,3 +126,60 @@ def test_class2_full_config_ledger_and_mode1_equivalence_of_totals():
     assert res[2]["ledger"][0] == res[1]["ledger"][0]
     assert res[2]["ledger"][1] == pytest.approx(res[1]["ledger"][1], rel=0.01)
     assert res[2]["counters"][9] > res[1]["counters"][9]                 # more charged particles are born
+
+
+# ------------------------------------------------------------------------------------------------ bremsstrahlung (mode 3, A32)
+def dSigma_dk(k, T, X0):
+    y = k / T
+    return (4.0 / 3.0 - 4.0 / 3.0 * y + y * y) / (X0 * k)
+
+
+@pytest.mark.parametrize("T,kc,X0", [(0.5, 0.01, 36.3), (2.0, 0.01, 36.3), (6.0, 0.01, 13.2), (20.0, 0.1, 8.6), (0.02, 0.01, 40.8)])
+def test_brems_closed_forms_quadrature_and_radiation_length_sum_rule(T, kc, X0):
+    sig, soft = oracle.brems_xs(T, kc, X0)
+    assert sig == pytest.approx(integrate.quad(dSigma_dk, kc, T, args=(T, X0), epsrel=1e-11)[0], rel=1e-8)
+    assert soft == pytest.approx(integrate.quad(lambda k: k * dSigma_dk(k, T, X0), 0, kc, epsrel=1e-11)[0], rel=1e-8)
+    hard = integrate.quad(lambda k: k * dSigma_dk(k, T, X0), kc, T, epsrel=1e-11)[0]
+    assert soft + hard == pytest.approx(T / X0, rel=1e-8)               # total radiative stopping power = T / X0
+    assert oracle.brems_xs(0.5 * kc, kc, X0) == (0.0, pytest.approx(0.5 * kc / X0))   # below the cut-off everything is soft
+
+
+@pytest.mark.parametrize("T", [0.3, 2.0, 15.0])
+def test_brems_sampler_follows_the_density(T):
+    kc, n, X0 = 0.01, 200_000, 36.3
+    k = oracle.sample_brems(T, kc, 11, n)
+    assert k.min() >= kc and k.max() <= T
+    edges = np.exp(np.linspace(np.log(kc), np.log(T), 25))
+    obs = np.histogram(k, bins=edges)[0]
+    sig = oracle.brems_xs(T, kc, X0)[0]
+    exp = np.array([integrate.quad(dSigma_dk, a, b, args=(T, X0))[0] for a, b in zip(edges[:-1], edges[1:])]) / sig * n
+    assert ((obs - exp) ** 2 / exp).sum() < stats.chi2.ppf(0.9999, len(exp) - 1)
+
+
+def test_mode3_thin_slab_mean_loss_and_photon_yield():
+    n, T0, thick = 100_000, 6.0, 0.2
+    o3, r3, ps3 = _thin_slab(3, n, T0=T0, thick=thick)
+    L = r3["ledger"]
+    assert abs(L[1] + L[2] + L[3] + L[4] + L[5] - L[0]) < 1e-11 * L[0]
+    X0 = float(o3.cfg["tables"]["rad_len"][gt.MAT_SOFT]); assert X0 > 1e29          # the slab config switches scattering off ...
+    # ... which also switches this bremsstrahlung model off (it is normalised by X0): so give the slab its real X0 back
+    t = tables(); X0 = float(t["rad_len"][gt.MAT_SOFT])
+    t2 = tables(); t2["rad_len"][:] = 1e30; t2["rad_len"][gt.MAT_SOFT] = X0
+    cfg = slab_cfg(n=(4, 4, 1), h=(5.0, 5.0, thick), w0=100.0, mode=3, t=t2, sid=100.0 + thick + 1.0)
+    o = oracle.Oracle(cfg)
+    o.set_fixed_primary(1, T0, (0.1, 0.1, 100.0 + 1e-9), (0, 0, 1))
+    o.set_ps3(True); o.reset(); o.run(0, n, 3)
+    r, ps = o.read(), o.read_ps3()
+    el = ps[ps[:, 0] == 1]
+    prim = np.zeros(n); np.maximum.at(prim, el[:, 7].astype(np.int64), el[:, 1])
+    loss = T0 - prim[prim > 0]
+    assert (prim > 0).mean() > 0.97                                     # multiple scattering in water is back on: a few do not arrive
+    # mean loss of the primary over the slab = int (S_col + T / X0) ds (path a little longer than the slab because of scattering)
+    S = lambda T: o.stop_pow(gt.MAT_SOFT, T) + T / X0
+    sol = integrate.solve_ivp(lambda s, T: [-S(T[0])], (0, thick), [T0], rtol=1e-9)
+    expect = T0 - sol.y[0, -1]
+    assert loss.mean() == pytest.approx(expect, rel=0.03, abs=4 * loss.std() / np.sqrt(len(loss)))
+    # photons at the plane per primary ~ int rho Sigma_brems(T(s)) ds (the slab and 1 cm of air absorb next to none of them)
+    yield_exp = integrate.quad(lambda s: oracle.brems_xs(T0 - (T0 - sol.y[0, -1]) * s / thick, 0.01, X0)[0], 0, thick)[0]
+    n_ph = (ps[:, 0] == 0).sum()
+    assert n_ph / n == pytest.approx(yield_exp, rel=0.05, abs=4 * np.sqrt(n_ph) / n)
