@@ -325,7 +325,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3", "C4"])
-    ap.add_argument("--physics-mode", type=int, default=None, choices=[0, 1, 2], help="override the config's physics mode (2: Class II collisions)")
+    ap.add_argument("--physics-mode", type=int, default=None, choices=[0, 1, 2, 3], help="override the physics mode (2: Class II collisions, 3: + bremsstrahlung)")
     ap.add_argument("--field", type=int, default=0, help="which of C4's 25 IMRT fields (seeds per reading A23)")
     ap.add_argument("--histories", type=int, default=0, help="histories per GPU per step (default: the config's)")
     ap.add_argument("--cpu-sample", type=int, default=1_000_000, help="oracle histories timed for cpu_baseline")

@@ -110,7 +110,10 @@ int aepid_load_source(aepid_ctx* ctx, const float src_pos_cm[3], const float bea
  * mode 1: coupled (CSDA electron steps with Highland deflection);
  * mode 2: coupled with Class II collisions ("Class II condensed history"; reading A31): discrete Moller events
  * with energy transfer above the electron cut-off, each starting a delta ray, and the restricted collision stopping
- * power below it; needs aepid_set_class2.  Cutoffs PAPER.md:104 (defaults 0.010 / 0.200 MeV); step rule f_E = 0.10,
+ * power below it;
+ * mode 3: mode 2 plus bremsstrahlung (reading A32): photons above the photon cut-off are emitted as discrete events along the
+ * particle's direction, the loss to softer photons is continuous; the spectrum (4/3 - 4/3 y + y^2) / (X0 k), y = k / T, makes the
+ * total radiative stopping power T / X0.  Modes 2 and 3 need aepid_set_class2.  Cutoffs PAPER.md:104 (defaults 0.010 / 0.200 MeV); step rule f_E = 0.10,
  * s_max = 1 cm (reading A13). */
 int aepid_set_physics(aepid_ctx* ctx, int mode, float photon_cut_MeV, float electron_cut_MeV,
                       float f_E, float s_max_cm);

@@ -40,7 +40,7 @@ Layout make_layout(const aepid_dims& d) {
     Layout L{};
     L.nvox = (size_t)d.nx * d.ny * d.nz;
     L.npix = (size_t)d.nu * d.nv;
-    L.blob_bytes = ((size_t)d.n_mat * d.n_E * 4 + d.n_E + (size_t)d.n_mat * d.n_T * 3 + d.n_mat) * 4;
+    L.blob_bytes = ((size_t)d.n_mat * d.n_E * 4 + d.n_E + (size_t)d.n_mat * d.n_T * 4 + d.n_mat) * 4;
     size_t o = 0;
     auto take = [&](size_t bytes) { const size_t at = o; o += up(bytes); return at; };
     L.vox = take(L.nvox * 4);
@@ -178,13 +178,14 @@ void moller_integrals(double T, double Tc, double& sigma, double& hard) {
 // ln-domain photon tables, majorant (reading A7 as corrected in DESIGN.md), ln stopping power, 1/X0.
 int build_tables(aepid_ctx* ctx) {
     const int nm = ctx->n_mat, nE = ctx->n_E, nT = ctx->n_T;
-    std::vector<float> blob((size_t)nm * nE * 4 + nE + (size_t)nm * nT * 3 + nm, 0.0f);
+    std::vector<float> blob((size_t)nm * nE * 4 + nE + (size_t)nm * nT * 4 + nm, 0.0f);
     float* phot = blob.data();
     float* maj = phot + (size_t)nm * nE * 4;
     float* lnS = maj + nE;
     float* invX0 = lnS + (size_t)nm * nT;
     float* lnL = invX0 + nm;                       // mode 2: ln restricted stopping power, Moller cross section (cm^2/g)
     float* sig = lnL + (size_t)nm * nT;
+    float* sigb = sig + (size_t)nm * nT;           // mode 3: the bremsstrahlung part of sig
     for (int m = 0; m < nm; ++m)
         for (int j = 0; j < nE; ++j) {
             const size_t o = (size_t)m * nE + j;
@@ -213,8 +214,17 @@ int build_tables(aepid_ctx* ctx) {
                 double sg, hd;
                 moller_integrals((double)ctx->Tg[j], (double)ctx->ph.ecut, sg, hd);
                 const size_t o = (size_t)m * nT + j;
-                lnL[o] = (float)std::log(std::max((double)ctx->S[o] - (double)ctx->ne[m] * hd, 1e-37));
-                sig[o] = (float)((double)ctx->ne[m] * sg);
+                double bs = 0.0, bsoft = 0.0;                  // mode 3 (reading A32): photons above the photon cut-off, soft radiative loss
+                if (ctx->ph.mode == 3) {
+                    const double T = ctx->Tg[j], kc = ctx->ph.pcut, X0 = ctx->X0[m], lo = kc / T;
+                    if (T > kc) {
+                        bs = (4.0 / 3.0 * std::log(1.0 / lo) - 4.0 / 3.0 * (1.0 - lo) + 0.5 * (1.0 - lo * lo)) / X0;
+                        bsoft = T * (4.0 / 3.0 * lo - 2.0 / 3.0 * lo * lo + lo * lo * lo / 3.0) / X0;
+                    } else bsoft = T / X0;
+                }
+                lnL[o] = (float)std::log(std::max((double)ctx->S[o] - (double)ctx->ne[m] * hd + bsoft, 1e-37));
+                sig[o] = (float)((double)ctx->ne[m] * sg + bs);
+                sigb[o] = (float)bs;
             }
     CU(cudaMemcpyAsync(ctx->d_blob(), blob.data(), blob.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));       // blob is a local vector
@@ -259,7 +269,7 @@ int fill_params(aepid_ctx* ctx, TransportParams& p) {
     if (!ctx->have_phantom) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_load_phantom has not been called");
     if (!ctx->have_epid) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_load_epid_layers has not been called");
     if (!ctx->have_source) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_load_source has not been called");
-    if (ctx->ph.mode == 2 && !ctx->have_ne) return fail(ctx, AEPID_ERR_BAD_STATE, "physics mode 2 needs aepid_set_class2 (after aepid_init_materials)");
+    if (ctx->ph.mode >= 2 && !ctx->have_ne) return fail(ctx, AEPID_ERR_BAD_STATE, "physics modes 2 and 3 need aepid_set_class2 (after aepid_init_materials)");
     if (int rc = check_geometry(ctx)) return rc;
     for (int l = 0; l < ctx->g.n_layers; ++l)
         if (ctx->g.lmat[l] >= ctx->n_mat) return fail(ctx, AEPID_ERR_BAD_ARG, "EPID layer material index out of range");
@@ -463,8 +473,8 @@ int aepid_load_source(aepid_ctx* ctx, const float src[3], const float axes[9], i
 
 int aepid_set_physics(aepid_ctx* ctx, int mode, float pcut, float ecut, float fE, float smax) {
     if (!ctx) return AEPID_ERR_BAD_ARG;
-    if ((mode != 0 && mode != 1 && mode != 2) || !(pcut > 0) || !(ecut > 0) || !(fE > 0) || !(fE <= 0.5f) || !(smax > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "physics parameters out of range");
-    if (ecut != ctx->ph.ecut) ctx->tables_dirty = true;       // the restricted stopping power depends on the cut-off
+    if (mode < 0 || mode > 3 || !(pcut > 0) || !(ecut > 0) || !(fE > 0) || !(fE <= 0.5f) || !(smax > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "physics parameters out of range");
+    if (ecut != ctx->ph.ecut || pcut != ctx->ph.pcut || mode != ctx->ph.mode) ctx->tables_dirty = true;   // the restricted stopping powers depend on the cut-offs and the mode
     ctx->ph.mode = mode; ctx->ph.pcut = pcut; ctx->ph.ecut = ecut; ctx->ph.fE = fE; ctx->ph.smax = smax;
     return 0;
 }

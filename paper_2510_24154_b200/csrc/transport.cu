@@ -483,7 +483,7 @@ __device__ __forceinline__ void interact(Lane& L, const TransportParams& P, cons
     const uint32_t reg = F_REGION(L.flags);
     if (xsel < pe) {                                                       // photoelectric: electron T = E along d
         if (COUNT) cnt[3]++;
-        if (!coupled || L.E <= P.ph.ecut) { dep_here(L, P, L.E); L.alive = false; return; }
+        if (!coupled || L.E <= P.ph.ecut) { if (COUNT && coupled) { cnt[9]++; cnt[14]++; } dep_here(L, P, L.E); L.alive = false; return; }
         SET_TYPE(L.flags, T_ELECTRON);
         L.pid = child_id(L, 0); L.blk = 0;
         if (COUNT) { cnt[9]++; cnt[14]++; }
@@ -673,20 +673,22 @@ __device__ __forceinline__ bool epid_flight(Lane& L, const TransportParams& P, c
 // Energy loss of the step (midpoint rule), deposit-independent part shared by the two step functions.
 // Class II (C2, physics mode 2, reading A31): sh.lnS holds the restricted stopping power, and the step also stops at the
 // next hard (Moller) collision, whose distance is drawn with the cross section at the energy the step starts with (draw rh).
-struct StepLoss { float s, dep, Tmid; bool hard; };
-template <bool C2>
+struct StepLoss { float s, dep, Tmid, sig, sigb; bool hard; };
+template <int PH>
 __device__ __forceinline__ StepLoss step_loss(Lane& L, const TransportParams& P, const Shared& sh, int m, float rho, float tb, uint32_t rh) {
     const float T = L.E;
     const float S = stop_pow(P, sh, m, T);
     StepLoss r;
     r.s = fminf(tb, fminf(__fdividef(P.ph.fE * T, rho * S), P.ph.smax));
-    r.hard = false;
-    if (C2) {
+    r.hard = false; r.sig = 0.0f; r.sigb = 0.0f;
+    if (PH >= 2) {
         float f = (__logf(T) - P.tb.lnT0) * P.tb.inv_dlnT;
         f = fminf(fmaxf(f, 0.0f), (float)(P.tb.n_T - 1));
         const int i = min((int)f, P.tb.n_T - 2);
         const float* q = sh.sig + m * P.tb.n_T + i;
         const float sg = fmaf(f - (float)i, q[1] - q[0], q[0]);
+        r.sig = sg;
+        if (PH == 3) { const float* qb = q + P.tb.n_mat * P.tb.n_T; r.sigb = fmaf(f - (float)i, qb[1] - qb[0], qb[0]); }   // bremsstrahlung part
         const float sh_ = sg > 0.0f ? __fdividef(-__logf(u01(rh)), rho * sg) : kInf;
         r.hard = sh_ < r.s;                                                // strictly inside the step: a step that ends on a face does not collide
         r.s = fminf(r.s, sh_);
@@ -741,6 +743,33 @@ __device__ __forceinline__ void moller_event(Lane& L, const TransportParams& P, 
     rotate(L.dx, L.dy, L.dz, cpm, sqrtf(fmaxf(0.0f, 1.0f - cpm * cpm)), cphi, sphi);
     L.E = T1;
 }
+// Bremsstrahlung event of a charged particle of kinetic energy L.E > kc = the photon cut-off (physics mode 3, reading A32):
+// photon energy k in [kc, E] from (4/3 - 4/3 y + y^2) / k, y = k / E, by rejection from 1/k (one Philox block per trial);
+// the photon leaves along the particle's direction with its own stream, the particle keeps E - k.  IN_PHANTOM: the lane
+// holds voxel fractions, the photon record wants the world position.
+template <bool COUNT, bool IN_PHANTOM>
+__device__ __forceinline__ void brems_event(Lane& L, const TransportParams& P, uint32_t* cnt) {
+    const float T = L.E, lr = __logf(__fdividef(T, P.ph.pcut));
+    float k;
+#pragma unroll 1
+    for (;;) {
+        const uint4 r = rng_block(L, P);
+        k = P.ph.pcut * __expf(u01(r.x) * lr);
+        const float y = __fdividef(k, T);
+        if (u01(r.y) <= 1.0f - y + 0.75f * y * y) break;
+    }
+    k = fminf(k, T);
+    float px = L.x, py = L.y, pz = L.z;
+    if (IN_PHANTOM) {
+        px = fmaf(((float)(L.vox & 1023u) + L.x), P.g.hx, P.g.lox);
+        py = fmaf(((float)((L.vox >> 10) & 1023u) + L.y), P.g.hy, P.g.loy);
+        pz = fmaf(((float)((L.vox >> 20) & 1023u) + L.z), P.g.hz, P.g.loz);
+    }
+    uint32_t f = L.flags; SET_TYPE(f, T_PHOTON);
+    if (COUNT) cnt[9]++;
+    spawn_from(L, px, py, pz, L.dx, L.dy, L.dz, k, f, child_id(L, 0));
+    L.E = T - k;
+}
 // charged particle at or below its cutoff (PAPER.md:104, 200 keV): local deposit; a positron annihilates
 template <bool COUNT>
 __device__ __forceinline__ void stop_charged(Lane& L, const TransportParams& P, uint32_t* cnt) {
@@ -755,8 +784,9 @@ __device__ __forceinline__ void stop_charged(Lane& L, const TransportParams& P, 
 // to the rare exit from the grid (selects instead of per-axis branches: a face is crossed by a few lanes of nearly
 // every warp, so divergent code there is paid by all).  The particle is above its cutoff.  Invariant of class E: the
 // pending deposit of the lane belongs to the current voxel (L.pidx == L.vlin, set when the particle is loaded).
-template <bool COUNT, bool C2>
-__device__ __forceinline__ void electron_step_phantom(Lane& L, const TransportParams& P, const Shared& sh, uint32_t ra, uint32_t rb, uint32_t rh, uint32_t* cnt) {
+template <bool COUNT, int PH>
+__device__ __forceinline__ void electron_step_phantom(Lane& L, const TransportParams& P, const Shared& sh, uint32_t ra, uint32_t rb, uint32_t rh, uint32_t rw, uint32_t* cnt) {
+    constexpr bool C2 = PH >= 2, PHANTOM_FRAME = true;
     const Geom& g = P.g;
     const float rho = __uint_as_float(L.cw & ~31u); const int m = (int)(L.cw & 31u);
     // distance to the voxel face in the direction of travel, per axis (a vanishing component gives a huge distance)
@@ -765,7 +795,7 @@ __device__ __forceinline__ void electron_step_phantom(Lane& L, const TransportPa
     const float tz = (L.dz > 0.0f ? 1.0f - L.z : L.z) * g.hz * rcp(fabsf(L.dz) + 1e-30f);
     const float tb = fmaxf(fminf(tx, fminf(ty, tz)), 0.0f);
     const bool ax0 = tx <= ty && tx <= tz, ax1 = !ax0 && ty <= tz, ax2 = !ax0 && !ax1;
-    const StepLoss sl = step_loss<C2>(L, P, sh, m, rho, tb, rh);
+    const StepLoss sl = step_loss<PH>(L, P, sh, m, rho, tb, rh);
     if (COUNT) { cnt[6]++; if (!(sl.s > 0.0f)) cnt[15]++; }
     L.pval += sl.dep; L.a_ph += sl.dep;
     L.x = fmaf(sl.s * g.ihx, L.dx, L.x); L.y = fmaf(sl.s * g.ihy, L.dy, L.y); L.z = fmaf(sl.s * g.ihz, L.dz, L.z);
@@ -795,11 +825,16 @@ __device__ __forceinline__ void electron_step_phantom(Lane& L, const TransportPa
         SET_REGION(L.flags, R_AIR);
     }
     rotate(L.dx, L.dy, L.dz, ct, st, cp, sp);
-    if (C2 && sl.hard && L.E > 2.0f * P.ph.ecut) moller_event<COUNT>(L, P, cnt);   // at the end of the step, with the energy left
+    if (C2 && sl.hard) {                                                   // hard event at the end of the step, with the energy left;
+        if (PH == 3 && u01(rw) * sl.sig < sl.sigb) {                       // its kind by the cross sections the distance was drawn with
+            if (L.E > P.ph.pcut) brems_event<COUNT, PHANTOM_FRAME>(L, P, cnt);
+        } else if (L.E > 2.0f * P.ph.ecut) moller_event<COUNT>(L, P, cnt);
+    }
 }
 // one step in the air or inside the EPID (the particle is above its cutoff)
-template <bool COUNT, bool C2>
-__device__ __forceinline__ void electron_step_outside(Lane& L, const TransportParams& P, const Shared& sh, uint32_t ra, uint32_t rb, uint32_t rh, uint32_t* cnt) {
+template <bool COUNT, int PH>
+__device__ __forceinline__ void electron_step_outside(Lane& L, const TransportParams& P, const Shared& sh, uint32_t ra, uint32_t rb, uint32_t rh, uint32_t rw, uint32_t* cnt) {
+    constexpr bool C2 = PH >= 2, PHANTOM_FRAME = false;
     const Geom& g = P.g;
     const bool in_air = F_REGION(L.flags) == R_AIR;
     float rho, tb; int m, axis = 0, kind = 0;
@@ -827,7 +862,7 @@ __device__ __forceinline__ void electron_step_outside(Lane& L, const TransportPa
         const float tl = lateral_exit(L.x, L.y, L.dx, L.dy);
         if (tl < tf) { tb = tl; kind = 2; } else { tb = tf; kind = 0; }
     }
-    const StepLoss sl = step_loss<C2>(L, P, sh, m, rho, tb, rh);
+    const StepLoss sl = step_loss<PH>(L, P, sh, m, rho, tb, rh);
     if (COUNT && !(sl.s > 0.0f)) cnt[15]++;
     if (in_air) { if (COUNT) cnt[7]++; L.a_air += sl.dep; }
     else { if (COUNT) cnt[8]++; dep_epid(L, fmaf(0.5f * sl.s, L.dx, L.x), fmaf(0.5f * sl.s, L.dy, L.y), sl.dep); }   // pixel of the step midpoint (A24)
@@ -854,23 +889,28 @@ __device__ __forceinline__ void electron_step_outside(Lane& L, const TransportPa
         }
     }
     rotate(L.dx, L.dy, L.dz, ct, st, cp, sp);
-    if (C2 && sl.hard && L.E > 2.0f * P.ph.ecut) moller_event<COUNT>(L, P, cnt);   // at the end of the step, with the energy left
+    if (C2 && sl.hard) {                                                   // hard event at the end of the step, with the energy left;
+        if (PH == 3 && u01(rw) * sl.sig < sl.sigb) {                       // its kind by the cross sections the distance was drawn with
+            if (L.E > P.ph.pcut) brems_event<COUNT, PHANTOM_FRAME>(L, P, cnt);
+        } else if (L.E > 2.0f * P.ph.ecut) moller_event<COUNT>(L, P, cnt);
+    }
 }
 // K5 for one lane: up to kStepsE / kStepsX consecutive steps per event, one Philox block per two steps
-template <bool COUNT, bool PHANTOM, bool C2>
+template <bool COUNT, bool PHANTOM, int PH>
 __device__ __forceinline__ void charged_event(Lane& L, const TransportParams& P, const Shared& sh, uint32_t* cnt) {
+    constexpr bool C2 = PH >= 2;
     if (L.E <= P.ph.ecut) { stop_charged<COUNT>(L, P, cnt); return; }
     uint4 r = PHANTOM ? rng_block_hot(L, P) : rng_block(L, P);
 #pragma unroll 1
     for (int k = 0; k < (PHANTOM ? kStepsE : kStepsX); ++k) {
-        if (C2) {                                                          // a block per step: deflection (x, y), hard-collision distance (z)
+        if (C2) {                                                          // a block per step: deflection (x, y), hard-collision distance (z), kind (w)
             if (k) r = PHANTOM ? rng_block_hot(L, P) : rng_block(L, P);
-            if (PHANTOM) electron_step_phantom<COUNT, true>(L, P, sh, r.x, r.y, r.z, cnt);
-            else electron_step_outside<COUNT, true>(L, P, sh, r.x, r.y, r.z, cnt);
+            if (PHANTOM) electron_step_phantom<COUNT, PH>(L, P, sh, r.x, r.y, r.z, r.w, cnt);
+            else electron_step_outside<COUNT, PH>(L, P, sh, r.x, r.y, r.z, r.w, cnt);
         } else {
             if (k && !(k & 1)) r = PHANTOM ? rng_block_hot(L, P) : rng_block(L, P);
-            if (PHANTOM) electron_step_phantom<COUNT, false>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, 0u, cnt);
-            else electron_step_outside<COUNT, false>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, 0u, cnt);
+            if (PHANTOM) electron_step_phantom<COUNT, 1>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, 0u, 0u, cnt);
+            else electron_step_outside<COUNT, 1>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, 0u, 0u, cnt);
         }
         if (!L.alive) break;
         if (L.E <= P.ph.ecut) {                                            // cutoff reached: an electron stops here and now;
@@ -980,10 +1020,11 @@ __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned lon
 }
 
 // One phase of class C for one warp (header comment).  On return every lane is empty and holds no slot.
-template <bool COUNT, int C, bool C2>
+template <bool COUNT, int C, int PH>
 __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, const Shared& sh, double* led, uint32_t* cnt) {
     const unsigned lane = threadIdx.x & 31u;
     const unsigned lt_mask = (1u << lane) - 1u;
+    constexpr bool C2 = PH >= 2;
     constexpr bool kSpawns = C == C_W || C == C_P || (C2 && (C == C_E || C == C_X));   // classes whose events create secondaries all the time
     const int keep = *((volatile int*)&s_keep);
     bool leaving = false, park = false;
@@ -1100,8 +1141,8 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
             }
             if (hit) interact<COUNT>(L, P, sh, xsel, pe, co, cnt);
         } else if (on) {
-            if (C == C_E) charged_event<COUNT, true, C2>(L, P, sh, cnt);
-            else if (C == C_X) charged_event<COUNT, false, C2>(L, P, sh, cnt);
+            if (C == C_E) charged_event<COUNT, true, PH>(L, P, sh, cnt);
+            else if (C == C_X) charged_event<COUNT, false, PH>(L, P, sh, cnt);
             else if (L.E < P.ph.pcut) { if (COUNT) cnt[13]++; dep_here(L, P, L.E); L.alive = false; }   // PAPER.md:104, 10 keV
             else {
                 bool hit = false; float xsel = 0.0f, pe = 0.0f, co = 0.0f;
@@ -1128,7 +1169,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
     if (lane == 0) atomicAdd(&s_left, 1);
 }
 
-template <bool COUNT, bool C2>
+template <bool COUNT, int PH>
 __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_constant__ TransportParams P) {
     // dynamic shared memory: per-warp ledger | table blob
     double* const led_all = reinterpret_cast<double*>(smem_raw);
@@ -1140,7 +1181,7 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
     sh.lnS = sh.maj + P.tb.n_E;
     sh.invX0 = sh.lnS + P.tb.n_mat * P.tb.n_T;
     sh.sig = sh.invX0 + P.tb.n_mat + P.tb.n_mat * P.tb.n_T;
-    if (C2) sh.lnS = sh.invX0 + P.tb.n_mat;                    // the restricted stopping power takes the place of the total one
+    if (PH >= 2) sh.lnS = sh.invX0 + P.tb.n_mat;                    // the restricted stopping power takes the place of the total one
     for (int i = threadIdx.x; i < kWarps * 8; i += kThreads) led_all[i] = 0.0;
     if (threadIdx.x < kRings) { s_tail[threadIdx.x] = 0u; s_head[threadIdx.x] = 0u; s_snap[threadIdx.x] = 0u; }
     if (threadIdx.x < 2) s_flag[threadIdx.x] = 0;
@@ -1174,11 +1215,11 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
         const long long t0 = clock64();
 #endif
         switch (ph) {
-            case C_A: run_phase<COUNT, C_A, C2>(L, P, sh, led, cnt); break;
-            case C_W: run_phase<COUNT, C_W, C2>(L, P, sh, led, cnt); break;
-            case C_E: run_phase<COUNT, C_E, C2>(L, P, sh, led, cnt); break;
-            case C_P: run_phase<COUNT, C_P, C2>(L, P, sh, led, cnt); break;
-            default:  run_phase<COUNT, C_X, C2>(L, P, sh, led, cnt); break;
+            case C_A: run_phase<COUNT, C_A, PH>(L, P, sh, led, cnt); break;
+            case C_W: run_phase<COUNT, C_W, PH>(L, P, sh, led, cnt); break;
+            case C_E: run_phase<COUNT, C_E, PH>(L, P, sh, led, cnt); break;
+            case C_P: run_phase<COUNT, C_P, PH>(L, P, sh, led, cnt); break;
+            default:  run_phase<COUNT, C_X, PH>(L, P, sh, led, cnt); break;
         }
 #ifdef AEPID_PHASE_CLOCK
         if (COUNT && lane == 0) { atomicAdd(P.counters + 10, (unsigned long long)(clock64() - t0)); atomicAdd(P.counters + 27 + ph, (unsigned long long)(clock64() - t0)); }   // busy warp-cycles
@@ -1216,11 +1257,11 @@ size_t transport_smem_bytes(const Tables& t) {      // dynamic + static shared m
     return kDynSmemFixed + (size_t)t.blob_words * 4 + sizeof(Geom) + 512;
 }
 
-template <bool COUNT, bool C2>
+template <bool COUNT, int PH>
 static int launch_one(const TransportParams& p, unsigned blocks, size_t smem, cudaStream_t stream) {
-    const cudaError_t e = cudaFuncSetAttribute(transport_kernel<COUNT, C2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const cudaError_t e = cudaFuncSetAttribute(transport_kernel<COUNT, PH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return (int)e;
-    transport_kernel<COUNT, C2><<<blocks, kThreads, smem, stream>>>(p);
+    transport_kernel<COUNT, PH><<<blocks, kThreads, smem, stream>>>(p);
     return (int)cudaGetLastError();
 }
 int launch_transport(const TransportParams& p, bool counting, int sm_count, void* stream) {
@@ -1230,9 +1271,11 @@ int launch_transport(const TransportParams& p, bool counting, int sm_count, void
     const long long need = ((long long)p.n + 255) / 256;
     if (blocks > need) blocks = need;
     if (blocks < 1) blocks = 1;
-    const bool c2 = p.ph.mode == 2;                       // Class II collisions: its own instantiation, modes 0 and 1 pay nothing for it
-    if (counting) return c2 ? launch_one<true, true>(p, (unsigned)blocks, smem, (cudaStream_t)stream) : launch_one<true, false>(p, (unsigned)blocks, smem, (cudaStream_t)stream);
-    return c2 ? launch_one<false, true>(p, (unsigned)blocks, smem, (cudaStream_t)stream) : launch_one<false, false>(p, (unsigned)blocks, smem, (cudaStream_t)stream);
+    // Class II physics (mode 2: Moller delta rays, mode 3: + bremsstrahlung) has its own instantiations: modes 0 and 1 pay nothing
+    const cudaStream_t st = (cudaStream_t)stream; const unsigned nb = (unsigned)blocks;
+    if (p.ph.mode == 3) return counting ? launch_one<true, 3>(p, nb, smem, st) : launch_one<false, 3>(p, nb, smem, st);
+    if (p.ph.mode == 2) return counting ? launch_one<true, 2>(p, nb, smem, st) : launch_one<false, 2>(p, nb, smem, st);
+    return counting ? launch_one<true, 1>(p, nb, smem, st) : launch_one<false, 1>(p, nb, smem, st);
 }
 // K1 alone (aepid_sample_source): out[k] = {E, dx, dy, dz, pixel, u, v, 0} for history first + k
 __global__ void sample_source_kernel(const __grid_constant__ TransportParams P, uint64_t first, uint64_t n, float* __restrict__ out) {

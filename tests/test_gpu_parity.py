@@ -157,17 +157,26 @@ def test_paper_scoring_grid_160x160_at_2p5mm():
     compare(cfg, cfg["n_histories"], 4_000_000, rebin=4, phantom_voxels=False)   # 40x40 @ 1 cm: ~90 oracle events per tested pixel
 
 
-def test_c1_class2_collisions_full_size():
-    """Physics mode 2 (Moller delta rays above the cut-off, restricted stopping power; reading A31) on the C1 workload."""
+@pytest.mark.parametrize("mode", [2, 3])
+def test_c1_class2_physics_full_size(mode):
+    """Physics mode 2 (Moller delta rays above the cut-off, restricted stopping power; reading A31) and mode 3 (plus
+    bremsstrahlung, reading A32) on the C1 workload."""
     cfg = make_config("C1")
-    cfg["physics"]["mode"] = 2
+    cfg["physics"]["mode"] = mode
     compare(cfg, cfg["n_histories"], 4_000_000, rebin=8)
 
 
-def test_class2_needs_its_input_and_does_not_depend_on_the_live_limit():
+def test_class2_in_the_high_z_epid_stack():
+    """Mode 3 where bremsstrahlung matters most: 6 MeV photons straight onto the Cu / Gd2O2S stack through a thin phantom."""
+    cfg = slab_cfg(n=(16, 16, 4), h=(2.0, 2.0, 0.5), w0=100.0, E=6.0, mode=3, epid="C1", nu=64, nv=64, pitch=0.4, sid=150.0, field_cm=10.0)
+    compare(cfg, 4_000_000, 2_000_000, rebin=4, phantom_voxels=False, min_tested=20)
+
+
+@pytest.mark.parametrize("mode", [2, 3])
+def test_class2_needs_its_input_and_does_not_depend_on_the_live_limit(mode):
     from paper_2510_24154_b200 import AepidError
     cfg = make_config("C1", shrink=4)
-    cfg["physics"]["mode"] = 2
+    cfg["physics"]["mode"] = mode
     t = cfg["tables"]
     eng = engine_for(cfg)
     eng.init_materials(t["E_grid"], t["mu_compton"], t["mu_pe"], t["mu_pair"], t["T_grid"], t["stop_pow"], t["rad_len"])   # forgets the electron densities
@@ -193,9 +202,9 @@ def test_class2_needs_its_input_and_does_not_depend_on_the_live_limit():
     cfg["physics"]["mode"] = 1
     eng = engine_for(cfg); eng.set_counting(True); eng.simulate(300_000, 9)
     n1 = eng.read_counters()[9]; eng.close()
-    raw1 = oracle.run_sharded(cfg, 300_000, 9); cfg["physics"]["mode"] = 2; raw2 = oracle.run_sharded(cfg, 300_000, 9)
+    raw1 = oracle.run_sharded(cfg, 300_000, 9); cfg["physics"]["mode"] = mode; raw2 = oracle.run_sharded(cfg, 300_000, 9)
     d_gpu, d_or = (res[0]["n_charged"] - n1) / 3e5, (raw2["counters"][9] - raw1["counters"][9]) / 3e5
-    assert d_or > 0.03 and abs(d_gpu - d_or) < 0.05 * d_or + 5 * np.sqrt(d_or / 3e5)   # delta rays per history
+    assert d_or > 0.03 and abs(d_gpu - d_or) < 0.05 * d_or + 5 * np.sqrt(d_or / 3e5)   # delta rays (and bremsstrahlung photons) per history
 
 
 def test_c2_heterogeneous_imrt_full_grid():
@@ -370,7 +379,7 @@ def test_error_codes():
     with pytest.raises(AepidError, match="BAD_ARG"):
         eng.load_source(s["src_pos"], s["beam_axes"], s["E_edges"], s["E_pdf"], s["f_pitch"], s["f_plane_dist"], np.zeros((100, 100), np.float32))
     with pytest.raises(AepidError, match="BAD_ARG"):
-        eng.set_physics(mode=3)
+        eng.set_physics(mode=4)
     eng.load_epid_layers(ep["thickness"], ep["material"], ep["density"], ep["scored"], ep["sid"], ep["nu"], ep["nv"], ep["pitch"])
     eng.simulate(1000, 1)                                             # recovers after the errors
     check_ledger(eng.read_tallies()["ledger"], 1000)

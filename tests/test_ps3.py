@@ -77,7 +77,7 @@ def _hist(x, bins, w=None):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("name,shrink,n,mode", [("C1", 1, 400_000, 1), ("C0", 1, 300_000, 0), ("C2", 2, 300_000, 1), ("C1", 1, 400_000, 2)])
+@pytest.mark.parametrize("name,shrink,n,mode", [("C1", 1, 400_000, 1), ("C0", 1, 300_000, 0), ("C2", 2, 300_000, 1), ("C1", 1, 400_000, 2), ("C1", 1, 400_000, 3)])
 def test_ps3_gpu_matches_oracle(name, shrink, n, mode):
     from paper_2510_24154_b200 import Engine
     cfg = make_config(name, shrink=shrink)
