@@ -153,7 +153,7 @@ int aepid_read_batches(aepid_ctx* ctx, float* epid_batches, double* histories_pe
  * secondaries, -, -, KN iterations, photon cutoffs, charged tracks, zero-length steps;
  * [16..31] scheduler: [16..20] warp-level event iterations of the phases A, W, E, P, X (transport.cu), [21..25] live lanes
  * summed over those, [26] phases run (all CTAs), [27] particles stored, [28] particles loaded, [29] particles parked for
- * want of a free slot, [30] source tasks, [31] unused. */
+ * want of head room, [30] source tasks, [31] unused. */
 int aepid_set_counting(aepid_ctx* ctx, int on);
 int aepid_read_counters(aepid_ctx* ctx, unsigned long long counters[32]);
 

@@ -20,9 +20,9 @@ constexpr float kMec2 = 0.51099895f;
 constexpr int kPoolSlots = 1 << AEPID_POOL_LOG;   // particle records per CTA of the transport kernel (transport.cu)
 constexpr int kRingCount = 5;         // class queues per CTA: the five event classes
 constexpr int kRecordBytes = 48;      // three 16-byte vectors per particle
-constexpr int kMaxCtas = 160;
+constexpr int kMaxCtas = 160;         // CTAs of the transport kernel the workspace provides class queues for (one per SM)
 constexpr int kGuideLog = 12;         // the fluence search starts from a guide table indexed by the top kGuideLog bits of the draw
-constexpr int kGuideSize = 1 << kGuideLog;         // CTAs of the transport kernel the workspace provides a pool for (one per SM)
+constexpr int kGuideSize = 1 << kGuideLog;
 
 enum Region : uint32_t { R_AIR = 0, R_PHANTOM = 1, R_EPID = 2 };
 enum PType : uint32_t { T_PHOTON = 0, T_ELECTRON = 1, T_POSITRON = 2 };

@@ -9,7 +9,7 @@
 //   * Event classes: A photon in air (new histories start here), W photon in the phantom, E charged particle in the
 //     phantom, P photon inside the EPID or with a collision pending outside the phantom, X charged particle outside
 //     the phantom.  The CTA runs PHASES, one class per phase, separated by block barriers; thread 0 picks the next
-//     phase: new histories while the particle pool has room, else the class with the most waiting particles.
+//     phase: new histories while there is head room for them, else the class with the most waiting particles.
 //   * Particle records (48 B, three 16 B vectors) live in per-CTA CLASS QUEUES in global memory: one ring of kPool
 //     records per event class (L2 / HBM, written and read with .cg accesses, consecutive tickets = consecutive records,
 //     so a refill is one coalesced, prefetchable read with no index to chase).  Shared memory holds the material tables
@@ -155,7 +155,7 @@ struct Lane {
     uint32_t cw, vlin;              // packed word and linear index of the current voxel (charged particle in PHANTOM)
     int ci; float ct, mumaj;        // photon: table cell, fraction, majorant at E
     uint32_t pidx; float pval;      // pending phantom deposit (merged while the voxel does not change)
-    uint32_t slot;                  // 1: the lane holds a particle that is counted in s_live (alive, or dead and not yet released); kNone: none
+    uint32_t counted;               // 1: the lane holds a particle that is counted in s_live (alive, or dead and not yet released); kNone: none
     uint32_t spare;                 // 1: the lane holds a head-room credit for its next secondary (kNone: none)
     float a_emit, a_ph, a_eps, a_epo, a_air, a_esc;   // ledger sums since the last flush
     bool alive;
@@ -511,7 +511,7 @@ __device__ __forceinline__ void interact(Lane& L, const TransportParams& P, cons
         float d1x = L.dx, d1y = L.dy, d1z = L.dz;
         rotate(d1x, d1y, d1z, ct, st, cp, sp);
         if (coupled && T > P.ph.ecut) {
-            // electron from momentum conservation: spawned into the pool with its own stream (reading A1)
+            // electron from momentum conservation: queued with its own stream (reading A1)
             float ex = E0 * L.dx - E1 * d1x, ey = E0 * L.dy - E1 * d1y, ez = E0 * L.dz - E1 * d1z;
             const float inv = rsqrtf(ex * ex + ey * ey + ez * ez);
             float px = L.x, py = L.y, pz = L.z;
@@ -914,7 +914,7 @@ __device__ __forceinline__ void charged_event(Lane& L, const TransportParams& P,
         }
         if (!L.alive) break;
         if (L.E <= P.ph.ecut) {                                            // cutoff reached: an electron stops here and now;
-            if (F_TYPE(L.flags) == T_ELECTRON) { dep_here(L, P, L.E); L.alive = false; }   // a positron first needs a slot for its second photon
+            if (F_TYPE(L.flags) == T_ELECTRON) { dep_here(L, P, L.E); L.alive = false; }   // a positron first needs a credit for its second photon
             break;
         }
         if ((F_REGION(L.flags) == R_PHANTOM) != PHANTOM) break;
@@ -974,9 +974,9 @@ __device__ __forceinline__ void ledger_flush(Lane& L, double* led) {
 }
 
 // Thread 0, between two barriers: publish what the last phase pushed (snapshot of every tail) and pick the next
-// phase: new histories (class A) while the pool has room for a full wave of them, else the class with the most
-// waiting particles.  W and P need free slots for their secondaries, so they wait while the pool is nearly full and
-// another class can run (E and X give slots back).
+// phase: new histories (class A) while there is head room for a full wave of them, else the class with the most
+// waiting particles.  W and P need credits for their secondaries, so they wait while the head room is nearly used up
+// and another class can run (particles that die in E and X give it back).
 __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned long long* phase_count) {
     int n[kRings];
 #pragma unroll
@@ -1019,7 +1019,7 @@ __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned lon
     if (phase_count && ph >= 0) atomicAdd(phase_count, 1ull);
 }
 
-// One phase of class C for one warp (header comment).  On return every lane is empty and holds no slot.
+// One phase of class C for one warp (header comment).  On return every lane is empty and holds no credit.
 template <bool COUNT, int C, int PH>
 __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, const Shared& sh, double* led, uint32_t* cnt) {
     const unsigned lane = threadIdx.x & 31u;
@@ -1037,10 +1037,10 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
             if (L.alive) {
                 queue_particle(L.x, L.y, L.z, L.dx, L.dy, L.dz, L.E, L.vox, L.flags, L.h, L.pid, L.blk);
                 if (COUNT && !kPhaseClock) cnt[27]++;
-                L.alive = false; L.slot = kNone;
-            } else if (L.slot != kNone) {
+                L.alive = false; L.counted = kNone;
+            } else if (L.counted != kNone) {
                 if (kSpawns && !leaving && L.spare == kNone) L.spare = 1u; else atomicSub(&s_live, 1);
-                L.slot = kNone;
+                L.counted = kNone;
             }
             park = false;
         }
@@ -1066,7 +1066,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                 L.x = __uint_as_float(a.x); L.y = __uint_as_float(a.y); L.z = __uint_as_float(a.z); L.dx = __uint_as_float(a.w);
                 L.dy = __uint_as_float(b.x); L.dz = __uint_as_float(b.y); L.E = __uint_as_float(b.z); L.vox = b.w;
                 L.flags = c.x; L.h = c.y; L.pid = c.z; L.blk = c.w;
-                L.slot = 1u; L.alive = true;
+                L.counted = 1u; L.alive = true;
                 L.pval = 0.0f; L.pidx = kNone;
                 if (COUNT && !kPhaseClock) cnt[28]++;
                 if (C == C_A || C == C_W || C == C_P) set_energy(L, P, sh);
@@ -1075,13 +1075,13 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
             if (C == C_A) {
                 // K1: new histories in the lanes that are still empty (the budget of the phase is head room set aside for them)
                 empty = __ballot_sync(FULL_MASK, !L.alive);
-                const int nslots = budget_claim(__popc(empty));
-                if (nslots > 0) {
+                const int nnew = budget_claim(__popc(empty));
+                if (nnew > 0) {
                     const int rk2 = __popc(empty & lt_mask);
                     uint32_t h0 = 0;
-                    if (lane == 0) { h0 = atomicAdd(P.hist_counter, (unsigned)nslots); atomicAdd(&s_live, nslots); }
+                    if (lane == 0) { h0 = atomicAdd(P.hist_counter, (unsigned)nnew); atomicAdd(&s_live, nnew); }
                     h0 = __shfl_sync(FULL_MASK, h0, 0);
-                    if (!L.alive && rk2 < nslots) {
+                    if (!L.alive && rk2 < nnew) {
                         const uint32_t h = h0 + (uint32_t)rk2;
                         if (h >= P.n) { atomicSub(&s_live, 1); atomicExch(s_flag, 1); }
                         else {
@@ -1092,7 +1092,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                             L.dx = s.dx; L.dy = s.dy; L.dz = s.dz; L.E = s.E;
                             L.vox = 0;
                             L.flags = T_PHOTON | (R_AIR << 2) | (min(h / P.hist_per_batch, (uint32_t)P.n_batches - 1u) << 16);
-                            L.alive = true; L.slot = 1u;
+                            L.alive = true; L.counted = 1u;
                             L.pval = 0.0f; L.pidx = kNone;
                             L.a_emit += s.E;
                             set_energy(L, P, sh);
@@ -1126,7 +1126,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
         } else if (C2 && (C == C_E || C == C_X)) {
             if (on && !ensure_spare(L)) { park = true; on = false; if (COUNT && !kPhaseClock) cnt[29]++; }   // a step may end in a Moller event
         } else if (C == C_E || C == C_X) {
-            if (on && F_TYPE(L.flags) == T_POSITRON && L.E <= P.ph.ecut && !ensure_spare(L)) { park = true; on = false; if (COUNT && !kPhaseClock) cnt[29]++; }   // annihilation needs a slot
+            if (on && F_TYPE(L.flags) == T_POSITRON && L.E <= P.ph.ecut && !ensure_spare(L)) { park = true; on = false; if (COUNT && !kPhaseClock) cnt[29]++; }   // annihilation needs a credit
         }
         if (C == C_W) {
             // K3 + K4: flights against the majorant until at least kHitMin lanes have a collision to sample (or nobody flies
@@ -1202,7 +1202,7 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
     Lane L;
     L.x = L.y = L.z = 0.0f; L.dx = L.dy = 0.0f; L.dz = 1.0f; L.E = 0.0f; L.vox = 0; L.flags = 0; L.h = L.pid = L.blk = 0;
     L.cw = 0; L.vlin = 0; L.ci = 0; L.ct = 0.0f; L.mumaj = 1.0f;
-    L.pval = 0.0f; L.pidx = kNone; L.slot = kNone; L.spare = kNone; L.alive = false;
+    L.pval = 0.0f; L.pidx = kNone; L.counted = kNone; L.spare = kNone; L.alive = false;
     L.a_emit = L.a_ph = L.a_eps = L.a_epo = L.a_air = L.a_esc = 0.0f;
 
 #pragma unroll 1
