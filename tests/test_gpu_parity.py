@@ -166,6 +166,13 @@ def test_c1_class2_physics_full_size(mode):
     compare(cfg, cfg["n_histories"], 4_000_000, rebin=8)
 
 
+def test_c2_heterogeneous_phantom_class2_physics():
+    """Mode 3 on the heterogeneous thorax phantom (lung, bone, air) at half resolution, rotated beam axes."""
+    cfg = make_config("C2", shrink=2)
+    cfg["physics"]["mode"] = 3
+    compare(cfg, 20_000_000, 1_500_000, rebin=32, frac_ok=0.985, phantom_voxels=False, min_tested=15)
+
+
 def test_class2_in_the_high_z_epid_stack():
     """Mode 3 where bremsstrahlung matters most: 6 MeV photons straight onto the Cu / Gd2O2S stack through a thin phantom."""
     cfg = slab_cfg(n=(16, 16, 4), h=(2.0, 2.0, 0.5), w0=100.0, E=6.0, mode=3, epid="C1", nu=64, nv=64, pitch=0.4, sid=150.0, field_cm=10.0)
