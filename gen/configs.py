@@ -202,6 +202,21 @@ def _source(src_pos, axes, spectrum, fluence, pitch, plane=100.0):
             "f_pitch": float(pitch), "f_plane_dist": float(plane), "fluence": np.ascontiguousarray(fluence)}
 
 
+def calibration_config(t_cm, s_cm, tables=None):
+    """One point of the k(t, s) calibration of PAPER.md:114 (section 2.2): a solid-water slab of thickness t_cm centred at the
+    isocentre (30 x 30 cm, 0.5 cm voxels laterally, 1 cm along the beam), an open s_cm x s_cm field, the C1 EPID stack scored on
+    the paper's 160 x 160 grid of 2.5 mm.  t_cm = 0 ("no phantom") is a 1 cm slab of density 1e-6."""
+    t = tables if tables is not None else make_tables()
+    nz = max(int(round(t_cm)), 1)
+    ph = phantom_water((60, 60, nz), (0.5, 0.5, (t_cm if t_cm > 0 else 1.0) / nz), (-15.0, -15.0, 100.0 - 0.5 * (t_cm if t_cm > 0 else 1.0)),
+                       rho=1.0 if t_cm > 0 else 1e-6)
+    fl, p = open_field(float(s_cm))
+    return {"name": "K_t%g_s%g" % (t_cm, s_cm), "tables": t, "lut": None, "phantom": ph,
+            "epid": epid_stack("C1", 160, 160, 0.25, 150.0),
+            "source": _source((0, 0, 0), _IDENT, mv6_spectrum(), fl, p),
+            "physics": default_physics(mode=1), "n_histories": 10_000_000, "seed": 1}
+
+
 def make_config(name, field=0, shrink=1, tables=None):
     """Build config `name` in {"C0".."C4"}.
 

@@ -196,6 +196,12 @@ int aepid_set_live_limit(aepid_ctx* ctx, int max_live_per_cta);
 int aepid_set_phase_space(aepid_ctx* ctx, void* records, unsigned long long capacity);
 int aepid_read_phase_space_count(aepid_ctx* ctx, unsigned long long* n_arrived);
 
+/* Eq. 2 of the paper, k(t, s) = M(t, s) / S(t, s): S is "the average simulated dose" in the central
+ * roi_cm x roi_cm region (the paper: 1 cm x 1 cm) of the EPID image.  mean_out (HOST) = mean over the pixels whose centre
+ * lies in the closed central square (reading A33); nan if there is none.  image: DEVICE [nv][nu] with its pitch, or NULL
+ * for the current mean EPID image of the context (nu, nv, pitch_cm are then ignored).  Synchronises. */
+int aepid_roi_mean(aepid_ctx* ctx, const float* image, int nu, int nv, float pitch_cm, float roi_cm, double* mean_out);
+
 /* Analysis chain (section 2.3.3).
  * aepid_upsample: out [mv][mu] = bilinear interpolant of in [nv][nu] over the same physical area: output pixel (j, i)
  * is taken at x = (i + 0.5) nu/mu - 0.5, y = (j + 0.5) nv/mv - 0.5 in input pixels (centres at the integers), clamped to

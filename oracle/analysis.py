@@ -77,3 +77,21 @@ def gamma_index(ref, ev, pitch_cm, dose_frac, dta_cm, threshold_frac=0.10, cap=2
     gt = g[tested]
     stats = (n, int((gt <= 1.0).sum()), float(gt.mean()) if n else 0.0, float(gt.max()) if n else 0.0)
     return g, stats
+
+
+def roi_mean(img, pitch_cm, roi_cm):
+    """Mean of img [nv][nu] over the pixels whose centre lies in the central roi_cm x roi_cm square (Eq. 2:
+    "the average ... within a 1 cm x 1 cm central region of the EPID image"; reading A33).  The image is centred on
+    the beam axis: pixel (j, i) has its centre at u = (i + 0.5 - nu/2) pitch, v = (j + 0.5 - nv/2) pitch; the square is
+    closed (|u|, |v| <= roi/2).  An ROI that holds no pixel centre gives nan."""
+    a = np.asarray(img, dtype=np.float64)
+    nv, nu = a.shape
+    u = (np.arange(nu) + 0.5 - 0.5 * nu) * pitch_cm
+    v = (np.arange(nv) + 0.5 - 0.5 * nv) * pitch_cm
+    m = (np.abs(v)[:, None] <= 0.5 * roi_cm) & (np.abs(u)[None, :] <= 0.5 * roi_cm)
+    return float(a[m].mean()) if m.any() else float("nan")
+
+
+def response_factors(measured, simulated):
+    """k(t, s) = M(t, s) / S(t, s) (Eq. 2) for arrays of ROI means of the measured signal and the simulated dose."""
+    return np.asarray(measured, dtype=np.float64) / np.asarray(simulated, dtype=np.float64)

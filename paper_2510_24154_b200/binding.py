@@ -30,7 +30,7 @@ EXPORTS = ("aepid_workspace_bytes", "aepid_create", "aepid_destroy", "aepid_last
            "aepid_set_counting", "aepid_read_counters", "aepid_sample_source", "aepid_field_size",
            "aepid_apply_response_lut", "aepid_synchronize", "aepid_set_history_offset", "aepid_read_moments",
            "aepid_finalize_moments", "aepid_upsample", "aepid_gamma_index",
-           "aepid_set_phase_space", "aepid_read_phase_space_count", "aepid_set_live_limit", "aepid_set_class2")
+           "aepid_set_phase_space", "aepid_read_phase_space_count", "aepid_set_live_limit", "aepid_set_class2", "aepid_roi_mean")
 
 
 class AepidError(RuntimeError):
@@ -82,6 +82,7 @@ def load_library():
     lib.aepid_set_class2.argtypes = [vp, vp]
     lib.aepid_set_phase_space.argtypes = [vp, vp, C.c_ulonglong]
     lib.aepid_read_phase_space_count.argtypes = [vp, vp]
+    lib.aepid_roi_mean.argtypes = [vp, vp, C.c_int, C.c_int, C.c_float, C.c_float, vp]
     lib.aepid_upsample.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int, C.c_int]
     lib.aepid_gamma_index.argtypes = [vp, vp, vp, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_float, C.c_float, vp, vp]
     _lib = lib
@@ -306,6 +307,17 @@ class Engine:
         if isinstance(a, np.ndarray):
             a = torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32))
         return a.to(device=self.device, dtype=torch.float32).contiguous()
+
+    def roi_mean(self, roi_cm=1.0, image=None, pitch_cm=None):
+        """Eq. 2: mean of the current EPID image (or of `image` with its pitch) over the central ROI."""
+        m = C.c_double(0.0)
+        if image is None:
+            self._chk(self._lib.aepid_roi_mean(self._h, None, 0, 0, 0.0, float(roi_cm), C.byref(m)))
+        else:
+            a = self._device_image(image)
+            nv, nu = (int(v) for v in a.shape)
+            self._chk(self._lib.aepid_roi_mean(self._h, _ptr(a), nu, nv, float(pitch_cm), float(roi_cm), C.byref(m)))
+        return float(m.value)
 
     def upsample(self, image, mv, mu, out=None):
         """K9: bilinear up-sampling of image [nv][nu] to [mv][mu]; returns a device tensor."""

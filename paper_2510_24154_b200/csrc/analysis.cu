@@ -137,4 +137,26 @@ int launch_gamma(const float* ref, const float* ev, float* gamma, int nu, int nv
     return 0;
 }
 
+// ---- Eq. 2 (reading A33): mean of the image over the pixels whose centre lies in the central roi x roi
+// square; acc[0] += sum, acc[1] += number of pixels (doubles).  A reduction over a few hundred pixels: latency-bound.
+__global__ void roi_sum_kernel(const float* __restrict__ img, int nu, int nv, float pitch, float half_roi, double* __restrict__ acc) {
+    const size_t n = (size_t)nu * nv;
+    double s = 0.0, c = 0.0;
+    for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (size_t)gridDim.x * blockDim.x) {
+        const int j = (int)(k / nu), i = (int)(k - (size_t)j * nu);
+        const float u = ((float)i + 0.5f - 0.5f * (float)nu) * pitch, v = ((float)j + 0.5f - 0.5f * (float)nv) * pitch;
+        if (fabsf(u) <= half_roi && fabsf(v) <= half_roi) { s += (double)__ldg(img + k); c += 1.0; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { s += __shfl_xor_sync(0xffffffffu, s, o); c += __shfl_xor_sync(0xffffffffu, c, o); }
+    if ((threadIdx.x & 31) == 0 && c > 0.0) { atomicAdd(acc, s); atomicAdd(acc + 1, c); }
+}
+void launch_roi_sum(const float* img, int nu, int nv, float pitch, float roi, double* acc, void* stream) {
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaMemsetAsync(acc, 0, 2 * sizeof(double), st);
+    size_t b = ((size_t)nu * nv + 255) / 256;
+    if (b > 148 * 4) b = 148 * 4;
+    roi_sum_kernel<<<(unsigned)b, 256, 0, st>>>(img, nu, nv, pitch, 0.5f * roi, acc);
+}
+
 }  // namespace aepid

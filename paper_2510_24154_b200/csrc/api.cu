@@ -698,6 +698,32 @@ int aepid_read_phase_space_count(aepid_ctx* ctx, unsigned long long* n_arrived) 
     return 0;
 }
 
+int aepid_roi_mean(aepid_ctx* ctx, const float* image, int nu, int nv, float pitch_cm, float roi_cm, double* mean_out) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    if (!mean_out) return fail(ctx, AEPID_ERR_BAD_ARG, "null output");
+    if (!(roi_cm > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "ROI size must be positive");
+    const float* d_img = image;
+    if (!image) {                                                       // the current mean EPID image
+        if (!ctx->have_epid) return fail(ctx, AEPID_ERR_BAD_STATE, "aepid_load_epid_layers has not been called");
+        FoldParams f{};
+        f.batches = ctx->d_ep_batch(); f.n = ctx->lay.npix; f.n_batches = ctx->dims.n_batches; f.total = (double)ctx->n_done;
+        std::copy(ctx->hist, ctx->hist + 256, f.hist);
+        f.mean = ctx->d_dose_in(); f.sigma = nullptr;
+        launch_fold(f, ctx->stream);
+        d_img = ctx->d_dose_in(); nu = ctx->g.nu; nv = ctx->g.nv; pitch_cm = ctx->g.pitch;
+    } else {
+        if (nu < 1 || nv < 1 || nu > 32768 || nv > 32768 || !(pitch_cm > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "image size or pitch out of range");
+        if (classify(image) != MEM_DEVICE) return fail(ctx, AEPID_ERR_BAD_ARG, "aepid_roi_mean takes a device pointer (or NULL for the current image)");
+    }
+    launch_roi_sum(d_img, nu, nv, pitch_cm, roi_cm, ctx->d_gamma_stats(), ctx->stream);
+    CU(cudaGetLastError());
+    double h[2];
+    CU(cudaMemcpyAsync(h, ctx->d_gamma_stats(), sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    *mean_out = h[1] > 0 ? h[0] / h[1] : std::nan("");
+    return 0;
+}
+
 int aepid_upsample(aepid_ctx* ctx, const float* in, int nu, int nv, float* out, int mu, int mv) {
     if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
     if (!in || !out) return fail(ctx, AEPID_ERR_BAD_ARG, "null image pointer");

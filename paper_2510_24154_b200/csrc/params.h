@@ -123,6 +123,7 @@ void launch_apply_lut(const float* lut, int nt, int ns, float t_min, float t_max
 void launch_zero(void* ptr, size_t bytes, void* stream);
 // analysis.cu
 void launch_upsample(const float* in, int nu, int nv, float* out, int mu, int mv, void* stream);
+void launch_roi_sum(const float* img, int nu, int nv, float pitch, float roi, double* acc, void* stream);
 int launch_gamma(const float* ref, const float* ev, float* gamma, int nu, int nv, float pitch, float dose_frac, float dta,
                  float thr_frac, float cap, unsigned int* dmax_bits, double* stats, void* stream);
 

@@ -124,3 +124,25 @@ def test_gamma_brute_force_on_a_tiny_image():
                     d = np.hypot((ii - i) * p, (jj - j) * p) / dta
                     best = min(best, np.hypot(d, (e[jj, ii] - r[j, i]) / dd))
             assert abs(g[j, i] - best) < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------ ROI mean, Eq. 2 (A33)
+def test_roi_mean_hand_worked_and_symmetry():
+    a = np.arange(36, dtype=float).reshape(6, 6)            # pitch 1 cm: centres at -2.5 ... 2.5
+    assert A.roi_mean(a, 1.0, 1.0) == pytest.approx(a[2:4, 2:4].mean())        # the four pixels around the axis (|centre| = 0.5 <= 0.5)
+    assert A.roi_mean(a, 1.0, 0.9) != A.roi_mean(a, 1.0, 0.9)                 # no centre inside: nan
+    assert A.roi_mean(a, 1.0, 3.0) == pytest.approx(a[1:5, 1:5].mean())
+    assert A.roi_mean(a, 1.0, 100.0) == pytest.approx(a.mean())
+    b = np.zeros((5, 7)); b[2, 3] = 9.0                     # odd sizes: the central pixel sits on the axis
+    assert A.roi_mean(b, 0.4, 0.1) == 9.0
+    assert A.roi_mean(b, 0.4, 0.8) == pytest.approx(9.0 / 9)
+    # transposing the image changes nothing for a square ROI
+    rng = np.random.default_rng(2); c = rng.random((12, 20))
+    assert A.roi_mean(c, 0.25, 1.0) == pytest.approx(A.roi_mean(c.T.copy(), 0.25, 1.0))
+
+
+def test_response_factors_reproduce_table1_from_its_own_products():
+    from gen.configs import paper_table1_lut
+    k = paper_table1_lut()["lut"].astype(np.float64)
+    S = np.random.default_rng(4).uniform(0.5, 2.0, k.shape)
+    assert np.allclose(A.response_factors(k * S, S), k, rtol=1e-14)
