@@ -1028,6 +1028,9 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
     constexpr bool kSpawns = C == C_W || C == C_P || (C2 && (C == C_E || C == C_X));   // classes whose events create secondaries all the time
     const int keep = *((volatile int*)&s_keep);
     bool leaving = false, park = false;
+    // every lane enters a phase empty: saying so lets the compiler drop what this class never touches from the registers
+    L.a_emit = L.a_ph = L.a_eps = L.a_epo = L.a_air = L.a_esc = 0.0f;
+    L.alive = false; L.counted = kNone; L.spare = kNone; L.pval = 0.0f; L.pidx = kNone;
 #pragma unroll 1
     for (uint32_t it = 1;; ++it) {
         // ---- A: particles that left the class (or all of them, when the warp leaves) go to the queue of their class;
