@@ -310,6 +310,22 @@ def test_results_do_not_depend_on_the_live_limit(name, shrink, n):
         assert np.allclose(r["epid_mean"], res[0]["epid_mean"], rtol=1e-3, atol=1e-9)
 
 
+def test_more_histories_than_32_bits():
+    """4.5e9 histories of C0 in one aepid_simulate call (split into launches below 2^32 inside the library): every history is
+    run, the ledger closes, the float32 tallies still reproduce the double ledger (B batch buffers)."""
+    cfg = make_config("C0")
+    n = 4_500_000_000
+    eng = engine_for(cfg)
+    eng.simulate(n, 3)
+    r = eng.read_tallies()
+    check_ledger(r["ledger"], n)
+    assert abs(r["phantom_mean"].sum(dtype=np.float64) * n / r["ledger"][1] - 1) < 2e-4
+    assert abs(r["epid_mean"].sum(dtype=np.float64) * n / r["ledger"][2] - 1) < 2e-4
+    b, hist = eng.read_batches()
+    assert hist.sum() == n
+    eng.close()
+
+
 def test_moments_path_equals_read_tallies():
     cfg = make_config("C1", shrink=4)
     eng = engine_for(cfg)
