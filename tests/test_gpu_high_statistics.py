@@ -1,0 +1,45 @@
+"""Opt-in high-statistics parity run (minutes of oracle time): AEPID_LONG=1 python -m pytest tests/test_gpu_high_statistics.py -s -m gpu
+
+The regular parity tests resolve differences of a few per mille; this one runs 5e8 oracle histories against 4e9 on the GPU and
+resolves every channel of the energy budget to about 1e-4 (numbers of round 1: DESIGN.md section 7)."""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from gen import make_config
+
+pytestmark = [pytest.mark.gpu, pytest.mark.skipif(os.environ.get("AEPID_LONG") != "1", reason="set AEPID_LONG=1 (takes minutes)")]
+
+
+@pytest.mark.parametrize("name,shrink,mode,n_or,n_gpu", [("C1", 1, 1, 500_000_000, 4_000_000_000), ("C2", 2, 1, 100_000_000, 1_000_000_000),
+                                                          ("C1", 1, 3, 100_000_000, 1_000_000_000)])
+def test_energy_budget_and_depth_dose_to_1e4(name, shrink, mode, n_or, n_gpu):
+    from paper_2510_24154_b200 import Engine
+    cfg = make_config(name, shrink=shrink)
+    cfg["physics"]["mode"] = mode
+    eng = Engine.for_config(cfg); eng.load_config(cfg)
+    eng.simulate(n_gpu, 77)
+    r = eng.read_tallies(); L = r["ledger"]
+    assert L[7] == 0
+    K, per = 10, n_or // 10                                 # K independent oracle runs give the spread of every channel
+    runs = [oracle.run_sharded(cfg, per, 78, first=k * per, want_phantom_sq=False) for k in range(K)]
+    Lo = np.array([x["ledger"] for x in runs])
+    print("\n%s mode %d: gpu %.1e histories, oracle %.1e" % (name, mode, n_gpu, n_or))
+    for k, nm in ((1, "dep_phantom"), (2, "dep_epid_scored"), (3, "dep_epid_other"), (4, "dep_air"), (5, "escaped")):
+        per_run = Lo[:, k] / Lo[:, 6]
+        o, so = per_run.mean(), per_run.std(ddof=1) / np.sqrt(K)
+        g = L[k] / L[6]
+        sg = so * np.sqrt(n_or / n_gpu)                      # the same per-history spread on the GPU side
+        print("  %-16s gpu %.7f oracle %.7f  rel diff %+.2e  (sigma %.1e)" % (nm, g, o, g / o - 1, np.hypot(so, sg) / o))
+        assert abs(g - o) <= 5 * np.hypot(so, sg) + 2e-5 * o
+    ax = (0, 2) if cfg["source"]["beam_axes"].reshape(3, 3)[2][1] != 0 else (1, 2)
+    dd = np.array([x["phantom_sum"].sum(axis=ax) / per for x in runs])
+    do, sd = dd.mean(0), dd.std(0, ddof=1) / np.sqrt(K)
+    dg = r["phantom_mean"].astype(np.float64).sum(axis=ax)
+    k = do > 0.2 * do.max()
+    z = (dg[k] - do[k]) / (sd[k] * np.sqrt(1 + n_or / n_gpu))
+    print("  depth dose over %d slabs: max |gpu/oracle - 1| %.2e, z mean %+.2f std %.2f" % (k.sum(), np.abs(dg[k] / do[k] - 1).max(), z.mean(), z.std()))
+    assert np.abs(z).max() < 5.5 and abs(z.mean()) < 1.0
+    eng.close()
