@@ -11,7 +11,8 @@
 //     the phantom.  The CTA runs PHASES, one class per phase, separated by block barriers; thread 0 picks the next
 //     phase: new histories while there is head room for them, else the class with the most waiting particles.
 //   * Particle records (48 B, three 16 B vectors) live in per-CTA CLASS QUEUES in global memory: one ring of kPool
-//     records per event class (L2 / HBM, written and read with .cg accesses, consecutive tickets = consecutive records,
+//     records per event class (L2 / HBM, written and read once with streaming .cs accesses so that they do not push the
+//     voxels and tallies out of the L2; consecutive tickets = consecutive records,
 //     so a refill is one coalesced, prefetchable read with no index to chase).  Shared memory holds the material tables
 //     (ln domain, one LDS.128 per node) and the scheduler state.  Up to kLiveMax = 65536 particles for 1024 lanes
 //     make a phase many waves long, so that the phase switch (two barriers, a cold instruction cache) and the tail of
@@ -437,9 +438,9 @@ __device__ __noinline__ void queue_particle(float x, float y, float z, float dx,
                                             uint32_t vox, uint32_t flags, uint32_t h, uint32_t pid, uint32_t blk) {
     const int r = class_of(flags);
     uint4* rec = queue_rec(r, atomicAdd(s_tail + r, 1u));
-    __stcg(rec + 0, make_uint4(__float_as_uint(x), __float_as_uint(y), __float_as_uint(z), __float_as_uint(dx)));
-    __stcg(rec + 1, make_uint4(__float_as_uint(dy), __float_as_uint(dz), __float_as_uint(E), vox));
-    __stcg(rec + 2, make_uint4(flags, h, pid, blk));
+    __stcs(rec + 0, make_uint4(__float_as_uint(x), __float_as_uint(y), __float_as_uint(z), __float_as_uint(dx)));
+    __stcs(rec + 1, make_uint4(__float_as_uint(dy), __float_as_uint(dz), __float_as_uint(E), vox));
+    __stcs(rec + 2, make_uint4(flags, h, pid, blk));
 }
 // Head room: s_live counts the particles alive in the CTA plus the credits lanes hold for secondaries they may create; it
 // never exceeds kLiveMax, which is what keeps every queue from wrapping onto unread records (header comment).  A lane
@@ -1057,7 +1058,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
             if (!L.alive && rk < got) {
                 const uint32_t tk = (uint32_t)(cl >> 32) + (uint32_t)rk;
                 const uint4* rec = queue_rec(C, tk);
-                const uint4 a = __ldcg(rec), b = __ldcg(rec + 1), c = __ldcg(rec + 2);
+                const uint4 a = __ldcs(rec), b = __ldcs(rec + 1), c = __ldcs(rec + 2);
 #if AEPID_PREFETCH > 0
                 // the records a later refill will want (same queue, AEPID_PREFETCH tickets ahead, if published): into the L2
                 if ((int)(s_snap[C] - (tk + AEPID_PREFETCH)) > 0) {
