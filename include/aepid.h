@@ -44,7 +44,11 @@ enum aepid_status {
     AEPID_ERR_BAD_STATE = -2, /* call order: something required has not been loaded */
     AEPID_ERR_GEOMETRY = -3,  /* phantom / EPID / source overlap or lie outside the world box */
     AEPID_ERR_CUDA = -4,      /* a CUDA runtime call failed (message holds cudaGetErrorString) */
-    AEPID_ERR_NOMEM = -5      /* workspace smaller than aepid_workspace_bytes(dims), or an input exceeds dims */
+    AEPID_ERR_NOMEM = -5,     /* workspace smaller than aepid_workspace_bytes(dims), or an input exceeds dims */
+    AEPID_ERR_INTERNAL = -6   /* the transport kernel raised an error flag (ledger[7] != 0): a secondary was dropped for want of
+                                 head room or the scheduler stalled; the tallies of that run are incomplete.  Reported by the calls
+                                 that synchronise: aepid_read_tallies (with a ledger or a host output), aepid_read_moments (with
+                                 totals), aepid_synchronize. */
 };
 
 /* Capacities the workspace is laid out for.  Loads may use less (fewer energy bins, a smaller
@@ -57,6 +61,9 @@ typedef struct aepid_dims {
     int n_bins;               /* spectrum bins */
     int fu, fv;               /* fluence map */
     int n_batches;            /* B independent tally buffers for the batch variance estimate (2..255) */
+    int max_live_per_cta;     /* most particles one CTA of the transport kernel keeps alive, 64..65536 (0 = 65536); the workspace
+                                 holds 160 x 5 class queues of twice that many 48-byte records (rounded up to a power of two):
+                                 5.0 GB at 65536, 80 MB at 1024.  Results do not depend on it; small runs want it small. */
 } aepid_dims;
 
 /* Bytes of device memory the context needs for `dims` (0 if dims are invalid). */
@@ -118,16 +125,28 @@ int aepid_load_source(aepid_ctx* ctx, const float src_pos_cm[3], const float bea
 int aepid_set_physics(aepid_ctx* ctx, int mode, float photon_cut_MeV, float electron_cut_MeV,
                       float f_E, float s_max_cm);
 
+/* Zero the B batch buffers, the energy ledger, the counters, the history count and the history offset: the start of a new
+ * field (every IMRT field is simulated on its own; aepid_load_source "implies nothing about
+ * tallies").  Asynchronous on the stream. */
 int aepid_reset_tallies(aepid_ctx* ctx);
 
-/* Transport histories [first, first + n) where first = histories run since the last reset; history h
+/* The hot path, K1-K7 of SURVEY.md 8(a).  One history = one particle of Phase Space 2, i.e. one source photon entering the
+ * patient stage (section 2.1.1); it and all its descendants are followed through the phantom (photoelectric,
+ * Compton and pair interactions, electrons down to 200 keV, photons down to 10 keV: section 2.1.2), the air gap
+ * and the EPID layers, scoring energy into the phantom grid and the image.
+ * Transports histories [first, first + n) where first = history offset + histories run since the last reset; history h
  * draws from Philox4x32-10 keyed by `seed` with counter (h_lo, h_hi, particle, block) (reading A1).
- * Accumulates into the B batch buffers; asynchronous on the stream. */
+ * Accumulates into the B batch buffers (history k of a launch scores into batch min(k / ceil(n / B), B - 1)); asynchronous
+ * on the stream; n_histories above 2^31 is split into several launches. */
 int aepid_simulate(aepid_ctx* ctx, unsigned long long n_histories, unsigned long long seed);
 
-/* Mean energy per history and its standard error from the B batches.  Images [nv][nu], volumes
- * [nz][ny][nx]; any of the four may be NULL; host or device.  ledger (HOST, may be NULL):
- * {emitted, dep_phantom, dep_epid_scored, dep_epid_other, dep_air, escaped, n_histories, overflow flags}. */
+/* The results of the path: the three-dimensional energy deposition in the patient grid ("3-D dose") and the
+ * EPID image, each as the mean energy per history and its standard error, which is what the paper's
+ * "statistical uncertainty below 1 %" is a statement about (reading A19; estimator: DESIGN.md section 3, B
+ * independent batches).  Images [nv][nu], volumes [nz][ny][nx]; any of the four may be NULL; host or device.  ledger (HOST,
+ * may be NULL): {emitted, dep_phantom, dep_epid_scored, dep_epid_other, dep_air, escaped, n_histories, error flags of the
+ * transport kernel}.  With a ledger or any host output the call synchronises and returns AEPID_ERR_INTERNAL if the error
+ * flags are set (the outputs are still written). */
 int aepid_read_tallies(aepid_ctx* ctx, float* epid_mean, float* epid_sigma,
                        float* phantom_mean, float* phantom_sigma, double ledger[8]);
 
@@ -148,12 +167,21 @@ int aepid_finalize_moments(aepid_ctx* ctx, const double* s1, const double* s2, s
 /* Raw per-batch EPID sums [B][nv][nu] (host or device, may be NULL) and histories per batch (HOST [B]). */
 int aepid_read_batches(aepid_ctx* ctx, float* epid_batches, double* histories_per_batch);
 
-/* Event and scheduler counters since the last reset (HOST [32]), only counted while aepid_set_counting(ctx, 1):
- * [0..15] Woodcock flights, air flights, EPID flights, photoelectric, Compton, pair, electron steps in phantom / air / EPID,
- * secondaries, -, -, KN iterations, photon cutoffs, charged tracks, zero-length steps;
- * [16..31] scheduler: [16..20] warp-level event iterations of the phases A, W, E, P, X (transport.cu), [21..25] live lanes
- * summed over those, [26] phases run (all CTAs), [27] particles stored, [28] particles loaded, [29] particles parked for
- * want of head room, [30] source tasks, [31] unused. */
+/* Event and scheduler counters since the last reset (HOST [32]), only counted while aepid_set_counting(ctx, 1) (an
+ * instrumented instantiation of the transport kernel runs then).  Counter map, index name (the binding's COUNTER_NAMES):
+ *    0 woodcock_flights    1 air_flights        2 epid_flights       3 n_pe
+ *    4 n_compton           5 n_pair             6 esteps_phantom     7 esteps_air
+ *    8 esteps_epid         9 n_secondaries     10 unused10          11 unused11
+ *   12 kn_iterations      13 photon_cutoffs    14 e_tracks          15 zero_steps
+ *   16 iter_A             17 iter_W            18 iter_E            19 iter_P
+ *   20 iter_X             21 lanes_A           22 lanes_W           23 lanes_E
+ *   24 lanes_P            25 lanes_X           26 phases            27 particles_stored
+ *   28 particles_loaded   29 particles_parked  30 source_tasks      31 unused31
+ * 0-9, 12-15: events of the physics (flights per region, interactions per channel, charged-particle steps per region,
+ * secondaries created, Klein-Nishina trials, photons ended by the 10 keV cut-off, charged tracks, zero-length steps);
+ * 16-20: warp-level event iterations of the scheduler phases A, W, E, P, X (transport.cu), 21-25: live lanes summed over
+ * those iterations, 26 phases run (all CTAs), 27 / 28 particle records written to / read from the class queues, 29 lanes
+ * that parked their particle for want of head room, 30 source tasks. */
 int aepid_set_counting(aepid_ctx* ctx, int on);
 int aepid_read_counters(aepid_ctx* ctx, unsigned long long counters[32]);
 

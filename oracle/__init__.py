@@ -39,6 +39,7 @@ def lib():
         _lib.orc_create.restype = C.c_void_p
         _lib.orc_last_error.restype = C.c_char_p
         _lib.orc_ps3_count.restype = C.c_uint64
+        _lib.orc_event_log_count.restype = C.c_uint64
         _lib.orc_moller_cos.restype = C.c_double
         for f in ("orc_stop_pow", "orc_majorant", "orc_highland_theta0", "orc_field_size", "orc_lut_bilinear"):
             getattr(_lib, f).restype = C.c_double
@@ -176,6 +177,21 @@ class Oracle:
                                           C.c_double(fc_w0), C.c_double(fc_dw)))
         self._want_sq = bool(want_phantom_sq)
 
+    def set_phantom_rebin(self, rx=1, ry=1, rz=1):
+        """Also tally the phantom on blocks of rx x ry x rz voxels, history by history (takes effect at reset)."""
+        self.prb = (int(rx), int(ry), int(rz))
+        self._chk(self._l.orc_set_phantom_rebin(self._h, *self.prb))
+
+    def set_event_log(self, capacity):
+        """Pins only: keep up to `capacity` interaction / birth records (see log_event in oracle.cpp)."""
+        self._chk(self._l.orc_set_event_log(self._h, C.c_uint64(int(capacity))))
+
+    def read_event_log(self):
+        n = int(self._l.orc_event_log_count(self._h))
+        out = np.empty((n, 16))
+        self._chk(self._l.orc_read_event_log(self._h, _p(out, C.c_double)))
+        return out
+
     def set_fixed_primary(self, ptype, E=0.0, pos=(0, 0, 0), direction=(0, 0, 1)):
         p = (C.c_double * 3)(*pos); d = (C.c_double * 3)(*direction)
         self._chk(self._l.orc_set_fixed_primary(self._h, int(ptype), C.c_double(E), p, d))
@@ -214,6 +230,12 @@ class Oracle:
                                    _p(out["phantom_sum"], C.c_double), _p(out["phantom_sq"], C.c_double),
                                    _p(out["uncollided"], C.c_double), _p(out["ledger"], C.c_double),
                                    _p(out["counters"], C.c_uint64), _p(out["aux"], C.c_double), _p(out["fc_hist"], C.c_double)))
+        rx, ry, rz = getattr(self, "prb", (1, 1, 1))
+        coarse = rx * ry * rz > 1
+        out["pc_sum"] = np.zeros((nz // rz, ny // ry, nx // rx)) if coarse else None
+        out["pc_sq"] = np.zeros((nz // rz, ny // ry, nx // rx)) if coarse else None
+        out["ledger_sq"] = np.zeros(8)
+        self._chk(self._l.orc_read_extra(self._h, _p(out["pc_sum"], C.c_double), _p(out["pc_sq"], C.c_double), _p(out["ledger_sq"], C.c_double)))
         return out
 
     # ---- Phase Space 3 (reading A30)
@@ -267,8 +289,11 @@ def stats(raw):
     """Mean per history and sigma of the mean from raw sums."""
     n = float(raw["ledger"][6])
     res = {"n": n}
-    for k in ("epid", "rb", "phantom"):
-        s, q = raw[k + "_sum"], raw[k + "_sq"]
+    for k, ks, kq in (("epid", "epid_sum", "epid_sq"), ("rb", "rb_sum", "rb_sq"), ("phantom", "phantom_sum", "phantom_sq"),
+                      ("pc", "pc_sum", "pc_sq"), ("ledger", "ledger", "ledger_sq")):
+        s, q = raw.get(ks), raw.get(kq)
+        if s is None:
+            continue
         mean = s / n
         res[k + "_mean"] = mean
         if q is not None:
@@ -279,8 +304,12 @@ def stats(raw):
 
 def _worker(args):
     cfg, first, n, seed, opts = args
+    opts = dict(opts)
+    prb = opts.pop("phantom_rebin", None)
     o = Oracle(cfg)
     o.set_options(**opts)
+    if prb is not None:
+        o.set_phantom_rebin(*prb)
     o.reset()
     o.run(first, n, seed)
     return o.read()

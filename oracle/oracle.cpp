@@ -167,6 +167,12 @@ struct Ctx {
     // Phase Space 3 (reading A30): every particle arriving at the EPID top plane from the air,
     // 8 doubles per record = {type, E, u, v, du, dv, dw (beam frame), history index}
     bool ps3_on = false; uint64_t cur_h = 0; std::vector<double> ps3;
+    // coarse phantom tally (history-by-history, like the re-binned image): blocks of prb[0] x prb[1] x prb[2] voxels
+    int prb[3] = {1, 1, 1}; bool prb_on = false; std::vector<double> pc_sum, pc_sq;
+    // second moments of the ledger channels over histories (sum over histories of (per-history amount)^2)
+    double ledger_sq[8] = {0}, ledger_prev[8] = {0};
+    // event log for the pins (tests/test_oracle_pins2.py): 16 doubles per record, see log_event
+    size_t log_cap = 0; std::vector<double> evlog;
 };
 
 // ---------------------------------------------------------------- tables
@@ -191,7 +197,9 @@ void mu_partial(const Ctx& c, int m, double E, double out[3]) {   // [pe, compto
     const size_t o = (size_t)m * c.n_E + k.i;
     out[0] = lerp_loglog(c.muPE[o], c.muPE[o + 1], k.t);
     out[1] = lerp_loglog(c.muC[o], c.muC[o + 1], k.t);
-    out[2] = c.muPP[o] + k.t * (c.muPP[o + 1] - c.muPP[o]);
+    // pair: linear in ln E on mu; impossible at or below the threshold 2 m_e c^2 (reading A34: the linear
+    // interpolant across the grid cell that straddles the threshold would otherwise be > 0 just below it)
+    out[2] = E > 2.0 * MEC2 ? c.muPP[o] + k.t * (c.muPP[o + 1] - c.muPP[o]) : 0.0;
 }
 double mu_tot(const Ctx& c, int m, double E) {
     double p[3]; mu_partial(c, m, E, p); return p[0] + p[1] + p[2];
@@ -283,7 +291,20 @@ void flush_history(Ctx& c) {
             c.ph_sum[kv.first] += kv.second;
             if (c.want_phantom_sq) c.ph_sq[kv.first] += kv.second * kv.second;
         }
+        if (c.prb_on) {
+            const int64_t nx = c.n[0], ny = c.n[1], cx = c.n[0] / c.prb[0], cy = c.n[1] / c.prb[1];
+            for (auto& kv : c.hvox) {
+                const int64_t ix = kv.first % nx, iy = (kv.first / nx) % ny, iz = kv.first / (nx * ny);
+                kv.first = ((iz / c.prb[2]) * cy + iy / c.prb[1]) * cx + ix / c.prb[0];
+            }
+            merge_history(c.hvox);
+            for (auto& kv : c.hvox) { c.pc_sum[kv.first] += kv.second; c.pc_sq[kv.first] += kv.second * kv.second; }
+        }
         c.hvox.clear();
+    }
+    for (int k = 0; k < 8; ++k) {
+        const double d = c.ledger[k] - c.ledger_prev[k];
+        c.ledger_sq[k] += d * d; c.ledger_prev[k] = c.ledger[k];
     }
 }
 
@@ -386,12 +407,24 @@ void epid_to_air(const Ctx& c, Particle& p) {                       // leaving t
     p.pos = to_world(c, pb); p.dir = dir_to_world(c, p.dir); p.region = AIR;
 }
 
+// ---------------------------------------------------------------- event log (pins only; off unless orc_set_event_log)
+// record = {kind (1 interaction, 2 birth), history, particle id, particle type, its energy when the event starts,
+//           its direction xyz, [8] channel 0 PE / 1 Compton / 2 pair (kind 1) or child type (kind 2),
+//           [9] material (kind 1) or child energy (kind 2), child direction xyz, sibling, region, child id}
+void log_event(Ctx& c, int kind, const Particle& p, double a8, double a9, Vec3 cd, int sibling, uint32_t child_pid) {
+    if (c.evlog.size() / 16 >= c.log_cap) return;
+    const double rec[16] = {(double)kind, (double)c.cur_h, (double)p.rng.ctr[2], (double)p.type, p.E, p.dir.x, p.dir.y, p.dir.z,
+                            a8, a9, cd.x, cd.y, cd.z, (double)sibling, (double)p.region, (double)child_pid};
+    c.evlog.insert(c.evlog.end(), rec, rec + 16);
+}
+
 // ---------------------------------------------------------------- secondaries
-Particle make_child(const Particle& parent, int sibling, int type, double E, Vec3 dir, uint64_t seed) {
+Particle make_child(Ctx& c, const Particle& parent, int sibling, int type, double E, Vec3 dir, uint64_t seed) {
     Particle s = parent;
     s.type = type; s.E = E; s.dir = dir; s.uncollided = false;
     const uint64_t h = ((uint64_t)parent.rng.ctr[1] << 32) | parent.rng.ctr[0];
     s.rng.init(seed, h, parent.rng.child_id(sibling));
+    if (c.log_cap) log_event(c, 2, parent, (double)type, E, dir, sibling, s.rng.ctr[2]);
     return s;
 }
 struct Run { uint64_t seed; };
@@ -401,8 +434,8 @@ void annihilate(Ctx& c, Particle& p, const Run& r) {
     const double ct = 2.0 * p.rng.u() - 1.0, phi = 2.0 * PI * p.rng.u();
     const double st = std::sqrt(std::max(0.0, 1.0 - ct * ct));
     Vec3 d{st * std::cos(phi), st * std::sin(phi), ct};
-    c.stack.push_back(make_child(p, 0, PHOTON, MEC2, d, r.seed));
-    c.stack.push_back(make_child(p, 1, PHOTON, MEC2, -1.0 * d, r.seed));
+    c.stack.push_back(make_child(c, p, 0, PHOTON, MEC2, d, r.seed));
+    c.stack.push_back(make_child(c, p, 1, PHOTON, MEC2, -1.0 * d, r.seed));
     c.counters[9] += 2;
     p.rng.skip_block();
 }
@@ -443,31 +476,34 @@ bool interact(Ctx& c, Particle& p, int m, const Run& r) {
     const double x = p.rng.u() * (mu[0] + mu[1] + mu[2]);
     if (x < mu[0]) {                                               // photoelectric
         c.counters[3]++;
+        if (c.log_cap) log_event(c, 1, p, 0.0, (double)m, Vec3{0, 0, 0}, 0, 0);
         if (c.mode == 0) deposit_here(c, p, p.E);
-        else { c.stack.push_back(make_child(p, 0, ELECTRON, p.E, p.dir, r.seed)); c.counters[9]++; p.rng.skip_block(); }
+        else { c.stack.push_back(make_child(c, p, 0, ELECTRON, p.E, p.dir, r.seed)); c.counters[9]++; p.rng.skip_block(); }
         return false;
     }
     if (x < mu[0] + mu[1]) {                                       // Compton
         c.counters[4]++;
+        if (c.log_cap) log_event(c, 1, p, 1.0, (double)m, Vec3{0, 0, 0}, 0, 0);
         double E1, T; Vec3 d1, de;
         compton_scatter(p.rng, p.E, p.dir, &E1, &d1, &T, &de, &c.counters[12]);
         if (c.mode == 0) deposit_here(c, p, T);
         else {
-            c.stack.push_back(make_child(p, 0, ELECTRON, T, de, r.seed)); c.counters[9]++;
+            c.stack.push_back(make_child(c, p, 0, ELECTRON, T, de, r.seed)); c.counters[9]++;
             p.rng.skip_block();
         }
         p.E = E1; p.dir = d1;
         return true;
     }
     c.counters[5]++;                                               // pair
+    if (c.log_cap) log_event(c, 1, p, 2.0, (double)m, Vec3{0, 0, 0}, 0, 0);
     const double Ttot = p.E - 2.0 * MEC2;
     const double Tm = p.rng.u() * Ttot, Tp = Ttot - Tm;          // uniform split (reading A10)
     if (c.mode == 0) {
         deposit_here(c, p, Ttot);
         annihilate(c, p, r);                                       // 2 m_e c^2 re-emitted at the interaction point (A11)
     } else {
-        c.stack.push_back(make_child(p, 0, ELECTRON, Tm, p.dir, r.seed));
-        c.stack.push_back(make_child(p, 1, POSITRON, Tp, p.dir, r.seed));
+        c.stack.push_back(make_child(c, p, 0, ELECTRON, Tm, p.dir, r.seed));
+        c.stack.push_back(make_child(c, p, 1, POSITRON, Tp, p.dir, r.seed));
         c.counters[9] += 2;
         p.rng.skip_block();
     }
@@ -753,7 +789,7 @@ void transport_electron(Ctx& c, Particle p, const Run& r) {
         if (is_brems) {
             if (p.E > c.photon_cut) {                                       // photon along the electron's direction (reading A32)
                 const double k = sample_brems_k(p.rng, p.E, c.photon_cut);
-                Particle ph = make_child(p, 0, PHOTON, k, p.dir, r.seed);
+                Particle ph = make_child(c, p, 0, PHOTON, k, p.dir, r.seed);
                 p.E -= k;
                 p.rng.skip_block();
                 c.counters[9]++;
@@ -764,7 +800,7 @@ void transport_electron(Ctx& c, Particle p, const Run& r) {
             const double W = eps * p.E, T1 = p.E - W, phi2 = 2.0 * PI * p.rng.u();
             const double cd = moller_cos(W, p.E), cp = moller_cos(T1, p.E);
             const Vec3 d0 = p.dir;
-            Particle dl = make_child(p, 0, ELECTRON, W, rotate(d0, cd, std::sqrt(std::max(0.0, 1.0 - cd * cd)), phi2 + PI), r.seed);
+            Particle dl = make_child(c, p, 0, ELECTRON, W, rotate(d0, cd, std::sqrt(std::max(0.0, 1.0 - cd * cd)), phi2 + PI), r.seed);
             p.dir = rotate(d0, cp, std::sqrt(std::max(0.0, 1.0 - cp * cp)), phi2);
             p.E = T1;
             c.counters[9]++;
@@ -825,6 +861,10 @@ void alloc_tallies(Ctx& c) {
     c.ph_sum.assign(nvx, 0); c.ph_sq.assign(c.want_phantom_sq ? nvx : 0, 0);
     std::fill(c.ledger, c.ledger + 8, 0.0); std::fill(c.counters, c.counters + 16, (uint64_t)0);
     std::fill(c.aux, c.aux + 4, 0.0);
+    std::fill(c.ledger_sq, c.ledger_sq + 8, 0.0); std::fill(c.ledger_prev, c.ledger_prev + 8, 0.0);
+    if (c.prb_on) { const size_t nc = (size_t)(c.n[0] / c.prb[0]) * (c.n[1] / c.prb[1]) * (c.n[2] / c.prb[2]); c.pc_sum.assign(nc, 0); c.pc_sq.assign(nc, 0); }
+    else { c.pc_sum.clear(); c.pc_sq.clear(); }
+    c.evlog.clear();
     c.fc_hist.assign(std::max(c.fc_bins, 0), 0.0);
 }
 
@@ -983,6 +1023,27 @@ int orc_read(orc_ctx* x, double* ep_sum, double* ep_sq, double* rb_sum, double* 
     if (aux) std::memcpy(aux, c.aux, sizeof(c.aux));
     return 0;
 }
+
+// Coarse phantom tally: blocks of rx x ry x rz voxels (must divide the grid; 1,1,1 switches it off).  Takes effect at orc_reset.
+int orc_set_phantom_rebin(orc_ctx* x, int rx, int ry, int rz) {
+    Ctx& c = C(x);
+    if (rx < 1 || ry < 1 || rz < 1) { c.err = "phantom rebin < 1"; return -1; }
+    if (c.n[0] > 0 && (c.n[0] % rx || c.n[1] % ry || c.n[2] % rz)) { c.err = "phantom rebin must divide the grid"; return -1; }
+    c.prb[0] = rx; c.prb[1] = ry; c.prb[2] = rz; c.prb_on = rx * ry * rz > 1;
+    return 0;
+}
+// Coarse phantom sums / sums of squares [(nz/rz)][(ny/ry)][(nx/rx)] and the second moments of the ledger channels (any may be NULL).
+int orc_read_extra(orc_ctx* x, double* pc_sum, double* pc_sq, double ledger_sq[8]) {
+    Ctx& c = C(x);
+    if (pc_sum && !c.pc_sum.empty()) std::memcpy(pc_sum, c.pc_sum.data(), c.pc_sum.size() * sizeof(double));
+    if (pc_sq && !c.pc_sq.empty()) std::memcpy(pc_sq, c.pc_sq.data(), c.pc_sq.size() * sizeof(double));
+    if (ledger_sq) std::memcpy(ledger_sq, c.ledger_sq, sizeof(c.ledger_sq));
+    return 0;
+}
+// Event log for the pins: keep up to `capacity` records of 16 doubles (0 switches it off); cleared by orc_reset.
+int orc_set_event_log(orc_ctx* x, uint64_t capacity) { Ctx& c = C(x); c.log_cap = (size_t)capacity; c.evlog.clear(); return 0; }
+uint64_t orc_event_log_count(orc_ctx* x) { return C(x).evlog.size() / 16; }
+int orc_read_event_log(orc_ctx* x, double* out) { Ctx& c = C(x); if (!c.evlog.empty()) std::memcpy(out, c.evlog.data(), c.evlog.size() * sizeof(double)); return 0; }
 
 // Phase Space 3: switch the recording on / off (clears the store), number of records, copy out [n][8].
 int orc_set_ps3(orc_ctx* x, int on) { Ctx& c = C(x); c.ps3_on = on != 0; c.ps3.clear(); return 0; }

@@ -15,15 +15,16 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libaepid.so")
 _lib = None
 
-STATUS = {0: "OK", -1: "BAD_ARG", -2: "BAD_STATE", -3: "GEOMETRY", -4: "CUDA", -5: "NOMEM"}
+STATUS = {0: "OK", -1: "BAD_ARG", -2: "BAD_STATE", -3: "GEOMETRY", -4: "CUDA", -5: "NOMEM", -6: "INTERNAL"}
 LEDGER_NAMES = ("emitted", "dep_phantom", "dep_epid_scored", "dep_epid_other", "dep_air", "escaped",
                 "n_histories", "overflow")
+# the counter map of include/aepid.h (aepid_read_counters); tests/test_boundary.py checks the two against each other
 COUNTER_NAMES = ("woodcock_flights", "air_flights", "epid_flights", "n_pe", "n_compton", "n_pair",
-                 "esteps_phantom", "esteps_air", "esteps_epid", "n_secondaries", "unused",
+                 "esteps_phantom", "esteps_air", "esteps_epid", "n_secondaries", "unused10",
                  "unused11", "kn_iterations", "photon_cutoffs", "e_tracks", "zero_steps",
-                 "sched_phases", "photon_iterations", "photon_lane_iterations", "charged_iterations", "charged_lane_iterations",
-                 "source_tasks", "idle_polls", "queue_claims", "particles_loaded", "particles_stored", "secondaries_spawned",
-                 "unused27", "unused28", "unused29", "unused30", "unused31")
+                 "iter_A", "iter_W", "iter_E", "iter_P", "iter_X",
+                 "lanes_A", "lanes_W", "lanes_E", "lanes_P", "lanes_X",
+                 "phases", "particles_stored", "particles_loaded", "particles_parked", "source_tasks", "unused31")
 EXPORTS = ("aepid_workspace_bytes", "aepid_create", "aepid_destroy", "aepid_last_error", "aepid_init_materials",
            "aepid_load_phantom", "aepid_load_epid_layers", "aepid_load_source", "aepid_set_physics",
            "aepid_reset_tallies", "aepid_simulate", "aepid_read_tallies", "aepid_read_batches",
@@ -39,7 +40,7 @@ class AepidError(RuntimeError):
 
 class Dims(C.Structure):
     _fields_ = [(n, C.c_int) for n in ("n_mat", "n_E", "n_T", "nx", "ny", "nz", "n_layers", "nu", "nv",
-                                       "n_bins", "fu", "fv", "n_batches")]
+                                       "n_bins", "fu", "fv", "n_batches", "max_live_per_cta")]
 
 
 def load_library():
@@ -141,13 +142,19 @@ class Engine:
         self.n_batches = dims.n_batches
 
     @classmethod
-    def for_config(cls, cfg, n_batches=None, device=0, stream=None):
-        """Engine sized for a gen.make_config dictionary (inputs are not loaded)."""
+    def for_config(cls, cfg, n_batches=None, device=0, stream=None, max_live_per_cta=None):
+        """Engine sized for a gen.make_config dictionary (inputs are not loaded).  The class queues of the transport
+        kernel are sized for the config's history count (aepid_dims.max_live_per_cta: a CTA never has more histories
+        than n / 148 to start, times the two or three particles a history has alive at a time); 0 = the maximum."""
         t, ph, ep, s = cfg["tables"], cfg["phantom"], cfg["epid"], cfg["source"]
+        if max_live_per_cta is None:
+            want = 4 * int(cfg.get("n_histories", 1 << 30)) // 128 + 1024
+            max_live_per_cta = 0 if want >= 65536 else 1 << (want - 1).bit_length()
         d = Dims(n_mat=int(t["mu_compton"].shape[0]), n_E=len(t["E_grid"]), n_T=len(t["T_grid"]),
                  nx=int(ph["nx"]), ny=int(ph["ny"]), nz=int(ph["nz"]), n_layers=len(ep["thickness"]),
                  nu=int(ep["nu"]), nv=int(ep["nv"]), n_bins=len(s["E_pdf"]), fu=int(s["fu"]), fv=int(s["fv"]),
-                 n_batches=int(n_batches if n_batches is not None else cfg["physics"]["n_batches"]))
+                 n_batches=int(n_batches if n_batches is not None else cfg["physics"]["n_batches"]),
+                 max_live_per_cta=int(max_live_per_cta))
         return cls(d, device=device, stream=stream)
 
     def close(self):

@@ -33,7 +33,16 @@ bool dims_ok(const aepid_dims* d) {
     if (d->n_layers < 1 || d->n_layers > kMaxLayers || d->nu < 1 || d->nv < 1 || d->nu > 16384 || d->nv > 16384) return false;
     if (d->n_bins < 1 || d->n_bins > 65536 || d->fu < 1 || d->fv < 1 || d->fu > 4096 || d->fv > 4096) return false;
     if (d->n_batches < 2 || d->n_batches > 255) return false;
+    if (d->max_live_per_cta != 0 && (d->max_live_per_cta < 64 || d->max_live_per_cta > kMaxPoolSlots / 2)) return false;
     return true;
+}
+
+// records per class queue of a CTA: twice the most particles a CTA keeps alive (queue protocol in transport.cu), a power of two
+int pool_log_for(const aepid_dims& d) {
+    const int live = d.max_live_per_cta ? d.max_live_per_cta : kMaxPoolSlots / 2;
+    int lg = 7;
+    while ((1 << lg) < 2 * live) ++lg;
+    return lg;
 }
 
 Layout make_layout(const aepid_dims& d) {
@@ -57,8 +66,8 @@ Layout make_layout(const aepid_dims& d) {
     L.edges = take(((size_t)d.n_bins + 1) * 4);
     L.thrF = take(((size_t)d.fu * d.fv + 1) * 4);
     L.guideF = take(((size_t)kGuideSize + 1) * 4);
-    L.queues = take((size_t)kMaxCtas * kRingCount * kPoolSlots * kRecordBytes);   // class queues of the transport kernel (scratch)
-    L.small = take(1024);            // ledger [8] f64 @0 | chunk counter @64 | rho_max [32] f32 @128 | counters [32] u64 @256 | gamma stats [4] f64 @512, max bits @544 | PS3 count u64 @576
+    L.queues = take((size_t)kMaxCtas * kRingCount * ((size_t)1 << pool_log_for(d)) * kRecordBytes);   // class queues of the transport kernel (scratch)
+    L.small = take(1024);            // ledger [8] f64 @0 | chunk counter @64 | bad-material flag @68 | rho_max [32] f32 @128 | counters [32] u64 @256 | gamma stats [4] f64 @512, max bits @544 | PS3 count u64 @576
     L.total = o;
     return L;
 }
@@ -87,7 +96,8 @@ struct aepid_ctx {
     double hist[256] = {0};
     std::vector<float> ne; bool have_ne = false;               // electrons per gram (aepid_set_class2)
     bool counting = false;
-    int live_max = kPoolSlots / 2;
+    int pool_log = kMaxPoolLog;                                // log2 of the records per class queue of a CTA (from dims.max_live_per_cta)
+    int live_max = kMaxPoolSlots / 2;
     float4* ps3 = nullptr; unsigned long long ps3_cap = 0;       // caller-owned Phase Space 3 buffer (aepid_set_phase_space)
 
     uint32_t* d_vox() { return reinterpret_cast<uint32_t*>(ws + lay.vox); }
@@ -107,6 +117,7 @@ struct aepid_ctx {
     double* d_ledger() { return reinterpret_cast<double*>(ws + lay.small); }
     unsigned long long* d_counters() { return reinterpret_cast<unsigned long long*>(ws + lay.small + 256); }
     unsigned int* d_chunk() { return reinterpret_cast<unsigned int*>(ws + lay.small + 64); }
+    unsigned int* d_bad_mat() { return reinterpret_cast<unsigned int*>(ws + lay.small + 68); }
     float* d_rho_max() { return reinterpret_cast<float*>(ws + lay.small + 128); }
     double* d_gamma_stats() { return reinterpret_cast<double*>(ws + lay.small + 512); }
     unsigned int* d_gamma_max() { return reinterpret_cast<unsigned int*>(ws + lay.small + 544); }
@@ -142,6 +153,17 @@ int deliver(aepid_ctx* ctx, void* dst, const void* dev_src, size_t bytes, bool* 
     const MemKind k = classify(dst);
     CU(cudaMemcpyAsync(dst, dev_src, bytes, k == MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
     if (k != MEM_DEVICE) *need_sync = true;
+    return 0;
+}
+
+// The transport kernel reports what must never happen (a secondary without head room, a scheduler that found no runnable
+// phase) in ledger[7]; tallies of such a run are incomplete.  Called right after a stream synchronisation.
+int check_internal(aepid_ctx* ctx, const double* host_ledger) {
+    if (host_ledger[7] != 0.0) {
+        char buf[160];
+        std::snprintf(buf, sizeof buf, "transport kernel raised internal error flags %.0f (2: secondary dropped for want of head room, 8: scheduler stalled); tallies are incomplete", host_ledger[7]);
+        return fail(ctx, AEPID_ERR_INTERNAL, buf);
+    }
     return 0;
 }
 
@@ -280,6 +302,7 @@ int fill_params(aepid_ctx* ctx, TransportParams& p) {
     p.ledger = ctx->d_ledger(); p.counters = ctx->d_counters(); p.hist_counter = ctx->d_chunk();
     p.queues = reinterpret_cast<uint4*>(ctx->ws + ctx->lay.queues);
     p.n_batches = ctx->dims.n_batches; p.nvox = ctx->lay.nvox; p.npix = ctx->lay.npix; p.live_max = ctx->live_max;
+    p.pool_log = ctx->pool_log;
     p.ps3 = ctx->ps3; p.ps3_count = ctx->d_ps3_count(); p.ps3_cap = ctx->ps3 ? ctx->ps3_cap : 0;
     p.base = 0; set_seed(p, 0); p.n = 0; p.hist_per_batch = 1;
     return 0;
@@ -309,6 +332,7 @@ int aepid_create(aepid_ctx** out, int device, void* cuda_stream, const aepid_dim
     ctx->device = device; ctx->sm_count = prop.multiProcessorCount;
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->dims = *dims; ctx->lay = make_layout(*dims);
+    ctx->pool_log = pool_log_for(*dims); ctx->live_max = (1 << ctx->pool_log) / 2;
     if (!workspace || ((uintptr_t)workspace & (kAlign - 1))) return fail(ctx, AEPID_ERR_BAD_ARG, "workspace must be a 256-byte aligned device pointer");
     if (classify(workspace) != MEM_DEVICE) return fail(ctx, AEPID_ERR_BAD_ARG, "workspace is not device memory");
     if (workspace_bytes < ctx->lay.total) return fail(ctx, AEPID_ERR_NOMEM, "workspace smaller than aepid_workspace_bytes(dims)");
@@ -322,8 +346,10 @@ const char* aepid_last_error(const aepid_ctx* ctx) { return ctx ? ctx->err.c_str
 
 int aepid_synchronize(aepid_ctx* ctx) {
     if (!ctx) return AEPID_ERR_BAD_ARG;
+    double led[8] = {0};
+    if (ctx->ws) CU(cudaMemcpyAsync(led, ctx->d_ledger(), sizeof(led), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
-    return 0;
+    return check_internal(ctx, led);
 }
 
 int aepid_init_materials(aepid_ctx* ctx, int n_mat, int n_E, const float* E, const float* muC, const float* muPE, const float* muPP,
@@ -364,13 +390,14 @@ int aepid_load_phantom(aepid_ctx* ctx, int nx, int ny, int nz, const float sp[3]
     char* stage = reinterpret_cast<char*>(ctx->d_ph_batch());
     if (kr != MEM_DEVICE) { CU(cudaMemcpyAsync(stage, rho, n * 4, cudaMemcpyHostToDevice, ctx->stream)); d_rho = reinterpret_cast<const float*>(stage); }
     if (km != MEM_DEVICE) { CU(cudaMemcpyAsync(stage + n * 4, mat, n, cudaMemcpyHostToDevice, ctx->stream)); d_mat = reinterpret_cast<const unsigned char*>(stage + n * 4); }
-    launch_pack_voxels(d_rho, d_mat, ctx->d_vox(), n, ctx->d_rho_max(), ctx->stream);
+    launch_pack_voxels(d_rho, d_mat, ctx->d_vox(), n, ctx->d_rho_max(), ctx->n_mat, ctx->d_bad_mat(), ctx->stream);
     CU(cudaGetLastError());
     ctx->rho_max.assign(kMaxMat, 0.0f);
+    unsigned int bad = 0;
     CU(cudaMemcpyAsync(ctx->rho_max.data(), ctx->d_rho_max(), kMaxMat * 4, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaMemcpyAsync(&bad, ctx->d_bad_mat(), sizeof(bad), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
-    for (int m = ctx->n_mat; m < kMaxMat; ++m)
-        if (ctx->rho_max[m] > 0) return fail(ctx, AEPID_ERR_BAD_ARG, "material index out of range in the phantom");
+    if (bad) { ctx->have_phantom = false; return fail(ctx, AEPID_ERR_BAD_ARG, "material index out of range in the phantom (a material byte >= n_mat)"); }
     Geom& g = ctx->g;
     g.nx = nx; g.ny = ny; g.nz = nz;
     g.hx = sp[0]; g.hy = sp[1]; g.hz = sp[2];
@@ -528,13 +555,14 @@ int aepid_read_tallies(aepid_ctx* ctx, float* ep_mean, float* ep_sigma, float* p
     };
     if (int rc = fold(ctx->d_ep_batch(), ctx->lay.npix, ep_mean, ep_sigma, ctx->d_out_ep())) return rc;
     if (int rc = fold(ctx->d_ph_batch(), ctx->lay.nvox, ph_mean, ph_sigma, ctx->d_out_ph())) return rc;
-    if (ledger) {
-        CU(cudaMemcpyAsync(ledger, ctx->d_ledger(), 8 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
-        need_sync = true;
+    double led[8] = {0};
+    if (ledger) need_sync = true;
+    if (need_sync) {                                       // the call synchronises anyway: look at the kernel's error flags too
+        CU(cudaMemcpyAsync(led, ctx->d_ledger(), sizeof(led), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
     }
-    if (need_sync) CU(cudaStreamSynchronize(ctx->stream));
-    if (ledger) ledger[6] = (double)ctx->n_done;
-    return 0;
+    if (ledger) { std::copy(led, led + 8, ledger); ledger[6] = (double)ctx->n_done; }
+    return need_sync ? check_internal(ctx, led) : 0;
 }
 
 int aepid_set_history_offset(aepid_ctx* ctx, unsigned long long first_history) {
@@ -553,9 +581,13 @@ int aepid_read_moments(aepid_ctx* ctx, double* ep_s1, double* ep_s2, double* ph_
     std::copy(ctx->hist, ctx->hist + 256, f.hist);
     if (ep_s1 || ep_s2) { f.batches = ctx->d_ep_batch(); f.n = ctx->lay.npix; launch_moments(f, ep_s1, ep_s2, ctx->stream); CU(cudaGetLastError()); }
     if (ph_s1 || ph_s2) { f.batches = ctx->d_ph_batch(); f.n = ctx->lay.nvox; launch_moments(f, ph_s1, ph_s2, ctx->stream); CU(cudaGetLastError()); }
-    if (totals) {
+    if (totals) {                                          // host output: synchronise and look at the kernel's error flags
         totals[0] = (double)ctx->n_done; totals[1] = 0.0;
         for (int b = 0; b < ctx->dims.n_batches; ++b) if (ctx->hist[b] > 0) totals[1] += 1.0;
+        double led[8] = {0};
+        CU(cudaMemcpyAsync(led, ctx->d_ledger(), sizeof(led), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        return check_internal(ctx, led);
     }
     return 0;
 }
@@ -675,8 +707,9 @@ int aepid_set_class2(aepid_ctx* ctx, const float* electrons_per_gram) {
 
 int aepid_set_live_limit(aepid_ctx* ctx, int max_live_per_cta) {
     if (!ctx) return AEPID_ERR_BAD_ARG;
-    if (max_live_per_cta == 0) max_live_per_cta = kPoolSlots / 2;
-    if (max_live_per_cta < 64 || max_live_per_cta > kPoolSlots / 2) return fail(ctx, AEPID_ERR_BAD_ARG, "live limit out of range (64 .. half a class queue)");
+    const int cap = (1 << ctx->pool_log) / 2;
+    if (max_live_per_cta == 0) max_live_per_cta = cap;
+    if (max_live_per_cta < 64 || max_live_per_cta > cap) return fail(ctx, AEPID_ERR_BAD_ARG, "live limit out of range (64 .. half a class queue = dims.max_live_per_cta)");
     ctx->live_max = max_live_per_cta;
     return 0;
 }

@@ -17,7 +17,8 @@ constexpr float kMec2 = 0.51099895f;
 #ifndef AEPID_POOL_LOG
 #define AEPID_POOL_LOG 17
 #endif
-constexpr int kPoolSlots = 1 << AEPID_POOL_LOG;   // particle records per CTA of the transport kernel (transport.cu)
+constexpr int kMaxPoolLog = AEPID_POOL_LOG;       // largest class queue: 2^17 records per class per CTA (65536 particles alive per CTA)
+constexpr int kMaxPoolSlots = 1 << kMaxPoolLog;   // the size in force comes from aepid_dims.max_live_per_cta (TransportParams::pool_log)
 constexpr int kRingCount = 5;         // class queues per CTA: the five event classes
 constexpr int kRecordBytes = 48;      // three 16-byte vectors per particle
 constexpr int kMaxCtas = 160;         // CTAs of the transport kernel the workspace provides class queues for (one per SM)
@@ -80,7 +81,8 @@ struct TransportParams {
     double* ledger;                    // [8]
     unsigned long long* counters;      // [32]
     unsigned int* hist_counter;        // next history of this launch that has not been started
-    uint4* queues;                     // class queues of particle records [kMaxCtas][kRingCount][kPoolSlots][3], scratch of one launch
+    uint4* queues;                     // class queues of particle records [kMaxCtas][kRingCount][1 << pool_log][3], scratch of one launch
+    int pool_log;                      // log2 of the records per class queue of a CTA
     float4* ps3;                       // Phase Space 3 records [ps3_cap][2] (null: not recorded), see aepid_set_phase_space
     unsigned long long* ps3_count;     // arrivals at the EPID top plane so far (also beyond the capacity)
     unsigned long long ps3_cap;
@@ -90,7 +92,7 @@ struct TransportParams {
     uint32_t n;                        // histories in this launch (< 2^32)
     uint32_t hist_per_batch;           // history k of the launch scores into batch min(k / hist_per_batch, B - 1)
     int n_batches;
-    int live_max;                      // most particles alive per CTA (<= kPoolSlots / 2), aepid_set_live_limit
+    int live_max;                      // most particles alive per CTA (<= half a class queue), aepid_set_live_limit
     size_t nvox, npix;
 };
 
@@ -112,7 +114,7 @@ inline void set_seed(TransportParams& p, uint64_t seed) {
 // launchers (defined in transport.cu / postpass.cu)
 int launch_transport(const TransportParams& p, bool counting, int sm_count, void* stream);
 size_t transport_smem_bytes(const Tables& t);
-void launch_pack_voxels(const float* rho, const unsigned char* mat, uint32_t* out, size_t n, float* rho_max, void* stream);
+void launch_pack_voxels(const float* rho, const unsigned char* mat, uint32_t* out, size_t n, float* rho_max, int n_mat, unsigned int* bad, void* stream);
 void launch_fold(const FoldParams& p, void* stream);
 void launch_moments(const FoldParams& p, double* s1, double* s2, void* stream);
 void launch_finalize_moments(const double* s1, const double* s2, size_t n, double total, double batches, float* mean, float* sigma, void* stream);
@@ -120,7 +122,6 @@ void launch_sample_source(const TransportParams& p, uint64_t first, uint64_t n, 
 void launch_tmap(const Geom& g, const uint32_t* vox, float* tmap, void* stream);
 void launch_apply_lut(const float* lut, int nt, int ns, float t_min, float t_max, float s_min, float s_max,
                       float s_eff, const float* dose, const float* tmap, float* out, size_t n, void* stream);
-void launch_zero(void* ptr, size_t bytes, void* stream);
 // analysis.cu
 void launch_upsample(const float* in, int nu, int nv, float* out, int mu, int mv, void* stream);
 void launch_roi_sum(const float* img, int nu, int nv, float pitch, float roi, double* acc, void* stream);

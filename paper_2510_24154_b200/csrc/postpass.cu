@@ -16,13 +16,15 @@ static inline unsigned grid_for(size_t n, int per_block) {
 }
 
 // ---- voxel repacking: density (rounded to 19 mantissa bits) | material (5 bits); per-material max density
+// A material byte >= n_mat raises *bad (aepid_load_phantom then fails) instead of aliasing to a valid material.
 __global__ void pack_voxels_kernel(const float* __restrict__ rho, const unsigned char* __restrict__ mat, uint32_t* __restrict__ out,
-                                   size_t n, float* __restrict__ rho_max) {
+                                   size_t n, float* __restrict__ rho_max, int n_mat, unsigned int* __restrict__ bad) {
     __shared__ unsigned int s_max[kMaxMat];
     if (threadIdx.x < kMaxMat) s_max[threadIdx.x] = 0u;
     __syncthreads();
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         const float r = fmaxf(rho[i], 0.0f);
+        if ((int)mat[i] >= n_mat) atomicOr(bad, 1u);
         const uint32_t m = mat[i] & 31u;
         const uint32_t bits = (__float_as_uint(r) + 16u) & ~31u;     // round to nearest on the kept mantissa
         out[i] = bits | m;
@@ -31,9 +33,10 @@ __global__ void pack_voxels_kernel(const float* __restrict__ rho, const unsigned
     __syncthreads();
     if (threadIdx.x < kMaxMat && s_max[threadIdx.x]) atomicMax(reinterpret_cast<unsigned int*>(rho_max) + threadIdx.x, s_max[threadIdx.x]);
 }
-void launch_pack_voxels(const float* rho, const unsigned char* mat, uint32_t* out, size_t n, float* rho_max, void* stream) {
+void launch_pack_voxels(const float* rho, const unsigned char* mat, uint32_t* out, size_t n, float* rho_max, int n_mat, unsigned int* bad, void* stream) {
     cudaMemsetAsync(rho_max, 0, kMaxMat * sizeof(float), (cudaStream_t)stream);
-    pack_voxels_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)stream>>>(rho, mat, out, n, rho_max);
+    cudaMemsetAsync(bad, 0, sizeof(unsigned int), (cudaStream_t)stream);
+    pack_voxels_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)stream>>>(rho, mat, out, n, rho_max, n_mat, bad);
 }
 
 // ---- K7 fold: mean per history and standard error of the mean from B independent batch sums
@@ -177,7 +180,5 @@ void launch_apply_lut(const float* lut, int nt, int ns, float t_min, float t_max
     if (n == 0) return;
     apply_lut_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)stream>>>(lut, nt, ns, t_min, t_max, s_min, s_max, s_eff, dose, tmap, out, n);
 }
-
-void launch_zero(void* ptr, size_t bytes, void* stream) { cudaMemsetAsync(ptr, 0, bytes, (cudaStream_t)stream); }
 
 }  // namespace aepid

@@ -53,11 +53,9 @@ namespace aepid {
 #endif
 constexpr int kWarps = AEPID_WARPS;
 constexpr int kThreads = kWarps * 32;
-constexpr int kPoolLog = AEPID_POOL_LOG;
-constexpr int kPool = 1 << kPoolLog;          // records per class queue of a CTA
-static_assert(kPool == kPoolSlots, "queue size");
-constexpr int kLiveMax = kPool / 2;           // most particles alive in a CTA at any time: half a queue, see "queue protocol" in the header
-                                              // comment; the limit in force is TransportParams::live_max <= kLiveMax (s_live_max)
+// Records per class queue of a CTA: kPool = 1 << TransportParams::pool_log (from aepid_dims.max_live_per_cta, at most 2^17);
+// the most particles alive in a CTA at any time is half a queue (see "queue protocol" above), the limit in force is
+// TransportParams::live_max <= kPool / 2 (s_live_max).
 #ifndef AEPID_RESERVE_8THS
 #define AEPID_RESERVE_8THS 3
 #endif
@@ -139,7 +137,9 @@ __shared__ int s_live_max;                          // limit of s_live for this 
 __shared__ int s_live;                              // particles alive in this CTA (in the queues, in lanes) + head-room credits held by lanes
 extern __shared__ __align__(16) unsigned char smem_raw[];   // per-warp ledger | table blob
 
-__device__ __forceinline__ uint4* queue_rec(int r, uint32_t ticket) { return s_queue + ((size_t)r * kPool + (ticket & (uint32_t)(kPool - 1))) * 3; }
+__shared__ uint32_t s_pool_mask;                    // records per class queue - 1
+__shared__ int s_pool_log;
+__device__ __forceinline__ uint4* queue_rec(int r, uint32_t ticket) { return s_queue + ((((size_t)r) << s_pool_log) + (ticket & s_pool_mask)) * 3; }
 struct Shared {
     const float4* phot;
     const float* maj;
@@ -207,11 +207,13 @@ __device__ __forceinline__ uint32_t child_id(const Lane& L, uint32_t sibling) { 
 }
 
 // ---------------------------------------------------------------- tables
-__device__ __forceinline__ void mu3(const TransportParams& P, const Shared& sh, int m, int ci, float ct, float& pe, float& co, float& pp) {
+// (pe, co, pp) of material m for a photon of energy E in table cell (ci, ct).  Pair production is impossible at or below
+// 2 m_e c^2 although the linear interpolant across the cell that straddles the threshold is positive there (reading A34).
+__device__ __forceinline__ void mu3(const TransportParams& P, const Shared& sh, int m, int ci, float ct, float E, float& pe, float& co, float& pp) {
     const float4 a = sh.phot[m * P.tb.n_E + ci], b = sh.phot[m * P.tb.n_E + ci + 1];
     pe = __expf(fmaf(ct, b.x - a.x, a.x));
     co = __expf(fmaf(ct, b.y - a.y, a.y));
-    pp = fmaf(ct, b.z - a.z, a.z);
+    pp = E > 2.0f * kMec2 ? fmaf(ct, b.z - a.z, a.z) : 0.0f;
 }
 __device__ __forceinline__ void set_energy(Lane& L, const TransportParams& P, const Shared& sh) {
     float f = (__logf(L.E) - P.tb.lnE0) * P.tb.inv_dlnE;
@@ -582,7 +584,7 @@ __device__ __forceinline__ bool woodcock_flight(Lane& L, const TransportParams& 
     const uint32_t w = __ldg(P.vox + ((size_t)iz * g.ny + iy) * g.nx + ix);
     const float rho = __uint_as_float(w & ~31u);
     float pp;
-    mu3(P, sh, (int)(w & 31u), L.ci, L.ct, pe, co, pp);
+    mu3(P, sh, (int)(w & 31u), L.ci, L.ct, L.E, pe, co, pp);
     xsel = u2 * L.mumaj;
     if (xsel < rho * (pe + co + pp)) {
         xsel = __fdividef(xsel, rho);                                      // reuse the accept draw for the channel (reading A8)
@@ -605,7 +607,7 @@ __device__ __forceinline__ bool air_transit(Lane& L, const TransportParams& P, c
     const float u1 = u01(rr.x), u2 = u01(rr.y);
     float nl = -__logf(u1);
     float pp;
-    mu3(P, sh, 0, L.ci, L.ct, pe, co, pp);
+    mu3(P, sh, 0, L.ci, L.ct, L.E, pe, co, pp);
     float mt = pe + co + pp;
     const float mua = kRhoAir * mt;
     if (nl < mua * ah.t) {                                                 // collision in air
@@ -625,7 +627,7 @@ __device__ __forceinline__ bool air_transit(Lane& L, const TransportParams& P, c
     if (COUNT) cnt[2]++;
 #pragma unroll 1
     for (int l = 0; l < g.n_layers; ++l) {
-        mu3(P, sh, g.lmat[l], L.ci, L.ct, pe, co, pp);
+        mu3(P, sh, g.lmat[l], L.ci, L.ct, L.E, pe, co, pp);
         mt = pe + co + pp;
         const float mul = g.lrho[l] * mt, path = (g.zt[l + 1] - g.zt[l]) * idw;
         if (nl < mul * path) {                                             // collision in layer l
@@ -649,7 +651,7 @@ __device__ __forceinline__ bool epid_flight(Lane& L, const TransportParams& P, c
     if (COUNT) cnt[2]++;
     const int l = F_LAYER(L.flags);
     float pp;
-    mu3(P, sh, g.lmat[l], L.ci, L.ct, pe, co, pp);
+    mu3(P, sh, g.lmat[l], L.ci, L.ct, L.E, pe, co, pp);
     const float mt = pe + co + pp;
     const float s = __fdividef(-__logf(u1), g.lrho[l] * mt);
     float tf = kInf;
@@ -1157,7 +1159,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                         L.flags &= ~F_HIT;
                         const bool in_air = F_REGION(L.flags) == R_AIR;
                         float pp;
-                        mu3(P, sh, in_air ? 0 : P.g.lmat[F_LAYER(L.flags)], L.ci, L.ct, pe, co, pp);
+                        mu3(P, sh, in_air ? 0 : P.g.lmat[F_LAYER(L.flags)], L.ci, L.ct, L.E, pe, co, pp);
                         xsel = u01(rng_block(L, P).x) * (pe + co + pp);
                         hit = true;
                     } else hit = epid_flight<COUNT>(L, P, sh, xsel, pe, co, cnt);
@@ -1191,8 +1193,9 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
     if (threadIdx.x < 2) s_flag[threadIdx.x] = 0;
     if (threadIdx.x == 0) {
         s_g = P.g; s_ep_batch = P.ep_batch; s_npix = P.npix; s_nphase = 0u;
-        s_queue = P.queues + (size_t)blockIdx.x * kClasses * kPool * 3;
-        s_live = 0; s_live_max = min(max(P.live_max, 64), kLiveMax);
+        s_pool_log = P.pool_log; s_pool_mask = (1u << P.pool_log) - 1u;
+        s_queue = P.queues + (((size_t)blockIdx.x * kClasses) << P.pool_log) * 3;
+        s_live = 0; s_live_max = min(max(P.live_max, 64), (1 << P.pool_log) / 2);
     }
     __syncthreads();
 

@@ -33,6 +33,19 @@ def test_library_exports_every_declared_symbol(lib):
         assert "aepid_" + name in declared
 
 
+def test_counter_names_match_the_header():
+    hdr = open(os.path.join(ROOT, "include", "aepid.h")).read()
+    blk = hdr[hdr.index("Counter map, index name"):hdr.index("0-9, 12-15: events of the physics")]
+    pairs = dict((int(i), n) for i, n in re.findall(r"\b(\d+) ([a-z][a-z_0-9A-Z]*)", blk))
+    assert sorted(pairs) == list(range(32))
+    assert tuple(pairs[i] for i in range(32)) == tuple(pkg.COUNTER_NAMES)
+    # the oracle counts the same physics events under the same names (0-9, 12-15)
+    import oracle
+    for i in list(range(10)) + [12, 13, 14, 15]:
+        assert oracle.COUNTER_NAMES[i] == pkg.COUNTER_NAMES[i], i
+    assert "AEPID_ERR_INTERNAL = -6" in hdr and pkg.binding.STATUS[-6] == "INTERNAL"
+
+
 def test_workspace_bytes_validates_dims(lib):
     d = pkg.Dims(n_mat=8, n_E=500, n_T=200, nx=120, ny=120, nz=80, n_layers=4, nu=512, nv=384, n_bins=200, fu=100, fv=100, n_batches=32)
     n = pkg.workspace_bytes(d)
@@ -40,7 +53,11 @@ def test_workspace_bytes_validates_dims(lib):
     assert n >= 4 * vox * (1 + 32 + 2) + 4 * pix * (32 + 2 + 3)
     pool = 160 * 5 * 131072 * 48                             # class queues of particle records of the transport kernel (params.h)
     assert n < 1.1 * (4 * vox * 35 + 4 * pix * 37) + pool + (2 << 20)
-    for field, bad in (("n_batches", 1), ("n_batches", 256), ("nx", 0), ("nx", 2000), ("n_mat", 33), ("n_layers", 9), ("fu", 0)):
+    # the class queues follow dims.max_live_per_cta: twice as many 48-byte records per class and CTA, rounded up to a power of two
+    small = pkg.Dims.from_buffer_copy(d); small.max_live_per_cta = 1000
+    assert n - pkg.workspace_bytes(small) == 160 * 5 * (131072 - 2048) * 48
+    for field, bad in (("n_batches", 1), ("n_batches", 256), ("nx", 0), ("nx", 2000), ("n_mat", 33), ("n_layers", 9), ("fu", 0),
+                       ("max_live_per_cta", 63), ("max_live_per_cta", 65537)):
         e = pkg.Dims.from_buffer_copy(d)
         setattr(e, field, bad)
         assert pkg.workspace_bytes(e) == 0, field

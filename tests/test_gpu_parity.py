@@ -42,7 +42,7 @@ def gpu_rebinned(eng, r):
 
 
 def check_ledger(L, n, tol=1e-6):
-    assert L[6] == n and L[7] == 0
+    assert L[6] == n and L[7] == 0                        # (aepid_read_tallies itself fails with INTERNAL when L[7] != 0)
     assert abs(L[1] + L[2] + L[3] + L[4] + L[5] - L[0]) <= tol * L[0]
 
 
@@ -68,11 +68,12 @@ def compare(cfg, n_gpu, n_or, rebin, seed=None, frac_ok=0.99, procs=None, phanto
     raw = oracle.run_sharded(cfg, n_or, seed, rebin=rebin, procs=procs, want_phantom_sq=phantom_voxels)
     st = oracle.stats(raw)
     Lo = raw["ledger"]
-    # ledger entries per history: every channel of the energy budget agrees
-    for k in (1, 3, 4, 5):
+    # ledger entries per history: every channel of the energy budget agrees within 0.5 % + 3 combined sigma; the spread over
+    # histories is the oracle's own second moment of the channel (the same physics on both sides)
+    for k in (1, 2, 3, 4, 5):
         per_o, per_g = Lo[k] / n_or, L[k] / n_gpu
-        spread = 2.0 * max(per_o, 0.01)                                   # generous per-history standard deviation
-        assert abs(per_g - per_o) <= 0.005 * per_o + 4 * spread * np.sqrt(1.0 / n_or + 1.0 / n_gpu), (k, per_g, per_o)
+        spread = np.sqrt(max(raw["ledger_sq"][k] / n_or - per_o ** 2, 0.0))
+        assert abs(per_g - per_o) <= 0.005 * per_o + 3 * spread * np.sqrt(1.0 / n_or + 1.0 / n_gpu), (k, per_g, per_o)
     # EPID image, re-binned
     gm, gs = gpu_rebinned(eng, rebin)
     om, os_ = st["rb_mean"], st["rb_sigma"]
@@ -87,7 +88,6 @@ def compare(cfg, n_gpu, n_or, rebin, seed=None, frac_ok=0.99, procs=None, phanto
     integral_check(gm.sum(), raw["rb_sum"].sum(), max(q, (raw["rb_sum"].sum() ** 2) / n_or * 1.0001), n_or, g_tot_sigma)
     # phantom
     pm, ps = r["phantom_mean"].astype(np.float64), r["phantom_sigma"].astype(np.float64)
-    assert abs(pm.sum() - st["phantom_mean"].sum()) <= 0.005 * st["phantom_mean"].sum() + 4 * 2.0 * np.sqrt(1.0 / n_or + 1.0 / n_gpu)
     if phantom_voxels:
         om, os_ = st["phantom_mean"], st["phantom_sigma"]
         k = om > 0.2 * om.max()
@@ -215,13 +215,21 @@ def test_class2_needs_its_input_and_does_not_depend_on_the_live_limit(mode):
 
 
 def test_c2_heterogeneous_imrt_full_grid():
+    """Live oracle run on the full C2 grid (1e7 histories); the 2e8-history comparison is tests/test_gpu_full_size.py."""
     cfg = make_config("C2")
-    compare(cfg, 40_000_000, 2_000_000, rebin=32, frac_ok=0.985, phantom_voxels=False, min_tested=15)
+    compare(cfg, 100_000_000, 10_000_000, rebin=16, frac_ok=0.99, phantom_voxels=False, min_tested=100)   # 6.3 mm pixels
 
 
 def test_c3_large_patient_quarter_resolution():
-    cfg = make_config("C3", shrink=2)                   # 256x256x100 grid of the same anatomy; full grid: test_c3_full_grid_properties
-    compare(cfg, 20_000_000, 1_000_000, rebin=32, frac_ok=0.985, phantom_voxels=False, min_tested=10, procs=8)
+    cfg = make_config("C3", shrink=2)                   # 256x256x100 grid of the same anatomy, 512x384 image
+    compare(cfg, 100_000_000, 6_000_000, rebin=8, frac_ok=0.99, phantom_voxels=False, min_tested=100)   # 6.3 mm pixels
+
+
+def test_c3_full_grid_vs_oracle():
+    """The config the metric is quoted on, at its full 512 x 512 x 200 grid, against a live run of the oracle (1e7 histories);
+    the 2e8-history comparison incl. voxel blocks is tests/test_gpu_full_size.py."""
+    cfg = make_config("C3")
+    compare(cfg, 400_000_000, 10_000_000, rebin=16, frac_ok=0.99, phantom_voxels=False, min_tested=100)   # 6.3 mm pixels
 
 
 def test_c3_full_grid_properties():
@@ -407,6 +415,48 @@ def test_error_codes():
     eng.simulate(1000, 1)                                             # recovers after the errors
     check_ledger(eng.read_tallies()["ledger"], 1000)
     eng.close()
+
+
+def test_material_byte_out_of_range_is_refused_not_aliased():
+    """A material byte >= n_mat (also >= 32, which the 5-bit voxel word would alias to a valid material, and on a zero-density
+    voxel) makes aepid_load_phantom fail with BAD_ARG."""
+    from paper_2510_24154_b200 import AepidError
+    cfg = make_config("C0", shrink=4)
+    ph = cfg["phantom"]
+    eng = engine_for(cfg)
+    for bad, rho0 in ((33, None), (8, None), (200, 0.0)):
+        m = ph["material"].copy(); d = ph["density"].copy()
+        m[1, 2, 3] = bad
+        if rho0 is not None:
+            d[1, 2, 3] = rho0
+        with pytest.raises(AepidError, match="BAD_ARG"):
+            eng.load_phantom(ph["spacing"], ph["origin"], d, m)
+        with pytest.raises(AepidError, match="BAD_STATE"):
+            eng.simulate(10, 1)                                       # the refused phantom is not used
+    eng.load_phantom(ph["spacing"], ph["origin"], ph["density"], ph["material"])
+    eng.simulate(1000, 1)
+    check_ledger(eng.read_tallies()["ledger"], 1000)
+    eng.close()
+
+
+def test_no_pair_production_at_or_below_threshold():
+    """Reading A34: photons of 1.0219 MeV (below 2 m_e c^2 = 1.02199790 MeV, inside the table cell that straddles the threshold)
+    never pair-produce, 1.03 MeV photons do, at the oracle's rate."""
+    for E, expect in ((1.0219, False), (1.03, True)):
+        cfg = slab_cfg(n=(8, 8, 8), h=(4.0, 4.0, 2.5), rho=7.32, mat=5, E=E, mode=1, field_cm=2.0)
+        eng = engine_for(cfg)
+        eng.set_counting(True)
+        n = 20_000_000 if expect else 2_000_000
+        eng.simulate(n, 3)
+        check_ledger(eng.read_tallies(epid=False, phantom=False)["ledger"], n)
+        c = eng.read_counters()
+        if not expect:
+            assert c[5] == 0
+        else:
+            raw = oracle.run_sharded(cfg, 4_000_000, 3, want_phantom_sq=False)
+            po, pg = raw["counters"][5] / 4e6, c[5] / n
+            assert po > 0 and abs(pg - po) < 0.02 * po + 5 * np.sqrt(po / 4e6 + po / n)
+        eng.close()
 
 
 def test_response_post_pass_paper_table1():
