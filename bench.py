@@ -110,10 +110,12 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def build_cfg(name, field=0, mode=None):
-    from gen import make_config
+def build_cfg(name, field=0, mode=None, collimator=False):
+    from gen import make_config, head_config
     from gen.configs import paper_table1_lut
-    cfg = make_config(name, field=field)
+    if collimator and name != "C4":
+        raise SystemExit("--collimator goes with --config C4 (the field's apertures become jaws and leaves)")
+    cfg = head_config(field=field) if collimator else make_config(name, field=field)   # NEXT-3: Phase Space 1 + jaws / MLC instead of the fluence map
     if mode is not None:
         cfg["physics"]["mode"] = int(mode)      # 2: Class II collisions (Moller delta rays, reading A31)
     if cfg.get("lut") is None:
@@ -149,9 +151,9 @@ def run_reference(args):
         return
     import multiprocessing as mp
     import oracle
-    cfg = build_cfg(args.config, args.field, args.physics_mode)
+    cfg = build_cfg(args.config, args.field, args.physics_mode, args.collimator)
     procs = os.cpu_count() or 1
-    sample = args.ref_histories or {"C0": 400_000, "C1": 400_000, "C2": 200_000}.get(args.config, 60_000)
+    sample = args.ref_histories or {"C0": 8_000_000, "C1": 4_000_000, "C2": 2_000_000}.get(args.config, 1_000_000)   # a few seconds per step
     oracle.build()
     per = max(sample // procs, 1); sample = per * procs
     with mp.get_context("fork").Pool(procs, initializer=_ref_init, initargs=(cfg,)) as pool:
@@ -190,7 +192,8 @@ def workload_name(args):
     desc = {"C0": "photon-only toy", "C1": "6 MV open field on a water slab", "C2": "IMRT-like field on the heterogeneous thorax phantom",
             "C3": "9-segment IMRT field on the 512x512x200 synthetic patient, EPID 1024x768, 1e9 histories",
             "C4": "batch of 25 IMRT fields on the thorax phantom + response LUT"}[args.config]
-    return "%s (BASELINE.json configs[%s]: %s)%s" % (args.config, args.config[1:], desc, " field %d" % args.field if args.config == "C4" else "")
+    return "%s (BASELINE.json configs[%s]: %s)%s%s" % (args.config, args.config[1:], desc, " field %d" % args.field if args.config == "C4" else "",
+                                                     " through the collimation stage (one history = one Phase Space 1 particle)" if args.collimator else "")
 
 
 # ------------------------------------------------------------------------------------------------ our arm
@@ -211,7 +214,7 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    cfg = build_cfg(args.config, args.field, args.physics_mode)
+    cfg = build_cfg(args.config, args.field, args.physics_mode, args.collimator)
     n = int(args.histories or cfg["n_histories"])
     n_total = n * world
     seed = cfg["seed"]
@@ -301,6 +304,11 @@ def run_ours(args):
                "seconds_to_1pct_native": t1(un), "seconds_to_1pct_rebinned": t1(ur), "seconds_to_1pct_rebinned_divisor": t1(ud),
                "seconds_per_field": ms_per_step * 1e-3}
 
+    head = None
+    if cfg.get("ps1") is not None and world == 1:
+        hs = eng.read_head()
+        head = {"ps2_particles_per_history": hs[0] / n, "ps2_particles_per_s": hs[0] / (ms_per_step * 1e-3), "ps2_energy_per_history_MeV": hs[1] / n,
+                "absorbed_in_head_per_history_MeV": hs[2] / n, "note": "one history = one Phase Space 1 particle (synthetic, DESIGN.md A35); the paper counts Phase Space 2 particles (PAPER.md:100)"}
     # event mix of the workload: one untimed counting launch (instrumented instantiation of the same kernel)
     n_cnt = int(min(n, 20_000_000))
     eng.reset_tallies(); eng.set_history_offset(first); eng.set_counting(True)
@@ -315,6 +323,8 @@ def run_ours(args):
     hin = {k: pin(t[k]) for k in ("E_grid", "mu_compton", "mu_pe", "mu_pair", "T_grid", "stop_pow", "rad_len")}
     hin.update(density=pin(ph["density"]), material=pin(ph["material"]), E_edges=pin(s["E_edges"]), E_pdf=pin(s["E_pdf"]),
                fluence=pin(s["fluence"]), lut=pin(np.ascontiguousarray(lut["lut"], dtype=np.float32)))
+    if cfg.get("ps1") is not None:
+        hin["ps1"] = pin(cfg["ps1"]["records"])
     hout = {k: torch.empty(v.shape, dtype=torch.float32).pin_memory() for k, v in outs.items()}
     hsig = torch.empty((eng.nv, eng.nu), dtype=torch.float32).pin_memory()
     h2d = sum(v.numel() * v.element_size() for v in hin.values())
@@ -326,6 +336,9 @@ def run_ours(args):
         eng.load_phantom(ph["spacing"], ph["origin"], hin["density"], hin["material"])
         eng.load_epid_layers(ep["thickness"], ep["material"], ep["density"], ep["scored"], ep["sid"], ep["nu"], ep["nv"], ep["pitch"])
         eng.load_source(s["src_pos"], s["beam_axes"], hin["E_edges"], hin["E_pdf"], s["f_pitch"], s["f_plane_dist"], hin["fluence"])
+        if cfg.get("ps1") is not None:                                   # collimation stage: Phase Space 1 table and the jaws / leaves
+            eng.load_phase_space_source(hin["ps1"], cfg["ps1"]["plane"])
+            eng.load_collimator(cfg["collimator"])
         eng.set_history_offset(first)
         eng.simulate(n, seed)
         eng.read_tallies(out=hout)                                       # host outputs: synchronises and checks the kernel's error flags
@@ -373,13 +386,12 @@ def run_ours(args):
     import oracle
     procs = os.cpu_count() or 1
     oracle.build()
-    slow = args.config in ("C3", "C4")
-    ns = 10_000 if args.profile else (args.cpu_sample or (300_000 if slow else 1_000_000))
+    ns = 10_000 if args.profile else (args.cpu_sample or {"C0": 60_000_000, "C1": 40_000_000, "C2": 20_000_000}.get(args.config, 8_000_000))   # 10-30 s
     wk = _OraclePool(cfg, procs)
     wk.run(procs * 50, seed, 0)                                          # page-in warm-up
     t0 = time.perf_counter(); wk.run(ns, seed, 0); dt = time.perf_counter() - t0
     wk.close()
-    n1 = max(ns // (2 * procs), 1000)
+    n1 = max(ns // (4 * procs), 1000)
     w1 = _OraclePool(cfg, 1); w1.run(100, seed, 0)
     t0 = time.perf_counter(); w1.run(n1, seed, 0); dt1 = time.perf_counter() - t0
     w1.close()
@@ -397,7 +409,7 @@ def run_ours(args):
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": float(e2e_ms[0])},
             "gpu_launches": launches_per_step * args.steps,
-            "uncertainty": unc, "wall_s_timed_region": t_wall,
+            "uncertainty": unc, "collimation_stage": head, "wall_s_timed_region": t_wall,
             "context": {"paper": "~90 s per 1e9-history IMRT field on 1x RTX 3090 (PAPER.md:127, 202), ~1.1e7 histories/s, fuller physics"}}
     print(json.dumps(line))
     if world > 1: dist.destroy_process_group()
@@ -429,8 +441,9 @@ def main():
     ap.add_argument("--config", default="C3", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--physics-mode", type=int, default=None, choices=[0, 1, 2, 3], help="override the physics mode (2: Class II collisions, 3: + bremsstrahlung)")
     ap.add_argument("--field", type=int, default=0, help="which of C4's 25 IMRT fields (seeds per reading A23)")
+    ap.add_argument("--collimator", action="store_true", help="C4 only: collimation stage (synthetic Phase Space 1, jaws, MLC) in place of the fluence map")
     ap.add_argument("--histories", type=int, default=0, help="histories per GPU per step (default: the config's)")
-    ap.add_argument("--cpu-sample", type=int, default=0, help="oracle histories timed for cpu_baseline (default: 1e6, 3e5 for C3 / C4)")
+    ap.add_argument("--cpu-sample", type=int, default=0, help="oracle histories timed for cpu_baseline (default: by config, 10-30 s of host time)")
     ap.add_argument("--ref-histories", type=int, default=0, help="oracle histories per step of --impl reference (default: by config)")
     ap.add_argument("--skip-ref-postpass", action="store_true", help="--impl reference: do not time the oracle's K8 post-pass")
     ap.add_argument("--profile", action="store_true", help="short run for ncu: one e2e step, tiny cpu_baseline sample (numbers are not bench values)")

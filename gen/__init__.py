@@ -9,4 +9,4 @@ method's arithmetic (no interpolation, no sampling, no tracking); the oracle
 implement that on their own and neither is imported here.
 """
 from .tables import make_tables, MATERIALS, ELEMENTS  # noqa: F401
-from .configs import make_config, CONFIG_NAMES  # noqa: F401
+from .configs import make_config, head_config, CONFIG_NAMES  # noqa: F401

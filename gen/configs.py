@@ -16,7 +16,7 @@ from __future__ import annotations
 import numpy as np
 
 from .tables import (make_tables, MATERIALS, MAT_AIR, MAT_LUNG, MAT_SOFT, MAT_BONE,
-                     MAT_CU, MAT_GOS, MAT_GLASS, MAT_PMMA)
+                     MAT_CU, MAT_GOS, MAT_GLASS, MAT_PMMA, TUNGSTEN, MAT_W)
 
 CONFIG_NAMES = ("C0", "C1", "C2", "C3", "C4")
 
@@ -215,6 +215,80 @@ def calibration_config(t_cm, s_cm, tables=None):
             "epid": epid_stack("C1", 160, 160, 0.25, 150.0),
             "source": _source((0, 0, 0), _IDENT, mv6_spectrum(), fl, p),
             "physics": default_physics(mode=1), "n_histories": 10_000_000, "seed": 1}
+
+
+# ---------------------------------------------------------------- collimation stage
+# The paper samples a pre-computed, patient-independent Phase Space 1 of the Varian VitalBeam head and transports it through jaws
+# and MLC built from the RTPLAN.  Neither the head model nor any plan is in the container and they are not recreated: the records
+# below are SYNTHETIC (a Gaussian focal spot radiating into the maximum field with the Schiff-shaped stand-in spectrum), and the
+# jaws / leaves are plain tungsten slabs with straight (unfocused) edges at invented but plausible distances from the target.
+HEAD_W = {"ps1": 20.0, "jaw_y": (28.0, 35.8), "jaw_x": (36.7, 44.5), "mlc": (48.2, 54.9), "ps2": 56.0}   # cm from the source
+
+
+def phase_space_1(seed=7, n=1_000_000, field_half_cm=14.0, spot_sigma_cm=0.05, plane=HEAD_W["ps1"], spectrum=None):
+    """Synthetic Phase Space 1: n records [x, y, du, dv, dw, E, 0, 0] (float32, beam frame) on the plane w = `plane`.
+
+    Each photon leaves a Gaussian focal spot on w = 0 towards a point drawn uniformly (planar fluence) in the square of
+    half-size field_half_cm on the isocentre plane w = 100; its energy is drawn from the histogram spectrum.  The record is
+    the crossing of the plane w = `plane`."""
+    rng = np.random.default_rng(seed)
+    edges, pdf = spectrum if spectrum is not None else mv6_spectrum()
+    sx, sy = rng.normal(0.0, spot_sigma_cm, n), rng.normal(0.0, spot_sigma_cm, n)
+    tx, ty = rng.uniform(-field_half_cm, field_half_cm, n), rng.uniform(-field_half_cm, field_half_cm, n)
+    d = np.stack([tx - sx, ty - sy, np.full(n, 100.0)], axis=1)
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    t = plane / d[:, 2]
+    k = rng.choice(len(pdf), size=n, p=np.asarray(pdf, dtype=np.float64) / np.sum(pdf, dtype=np.float64))
+    E = edges[k] + rng.uniform(0.0, 1.0, n) * (edges[k + 1] - edges[k])
+    rec = np.zeros((n, 8), dtype=np.float32)
+    rec[:, 0] = sx + t * d[:, 0]; rec[:, 1] = sy + t * d[:, 1]
+    rec[:, 2:5] = d; rec[:, 5] = E
+    return {"records": rec, "plane": float(plane), "n": int(n)}
+
+
+def _slab(w, axis, row0, pitch, lo, hi):
+    return {"w0": float(w[0]), "w1": float(w[1]), "axis": int(axis), "row0": float(row0), "pitch": float(pitch),
+            "lo": np.asarray(lo, dtype=np.float32), "hi": np.asarray(hi, dtype=np.float32)}
+
+
+def collimator_for_fluence(fluence, f_pitch=0.1, leaf_cm=0.5, margin_cm=0.5):
+    """Jaws and MLC whose openings follow the envelope of a fluence map given on the isocentre plane (w = 100 cm).
+
+    A slab opens, per row, the interval [lo, hi] of the coordinate across the rows; everything else inside its w-range is
+    tungsten.  axis = 0: rows are stacked along v (leaf direction u, the MLC and the x-jaws), axis = 1: one row stacked along u
+    (the y-jaws, opening in v).  Openings are given at the slab itself: isocentre size x (slab mid-plane / 100), straight edges.
+    MLC: one leaf pair per leaf_cm at the isocentre; leaf row k opens from the first to the last non-zero fluence pixel of its
+    rows (closed pairs park at lo = hi = 0 under the x-jaws); the jaws frame the bounding box plus margin_cm."""
+    f = np.asarray(fluence)
+    fv, fu = f.shape
+    px = int(round(leaf_cm / f_pitch))
+    n_leaf = fv // px
+    u = (np.arange(fu + 1) - fu / 2) * f_pitch                     # pixel edges at the isocentre
+    lo, hi = np.zeros(n_leaf), np.zeros(n_leaf)
+    for k in range(n_leaf):
+        cols = np.nonzero(f[k * px:(k + 1) * px].sum(axis=0) > 0)[0]
+        if len(cols):
+            lo[k], hi[k] = u[cols[0]], u[cols[-1] + 1]
+    rows = np.nonzero(hi > lo)[0]
+    v_lo, v_hi = (rows[0] * px - fv / 2) * f_pitch, ((rows[-1] + 1) * px - fv / 2) * f_pitch
+    u_lo, u_hi = lo[rows].min(), hi[rows].max()
+    sc = lambda w: 0.5 * (w[0] + w[1]) / 100.0
+    jy, jx, ml = HEAD_W["jaw_y"], HEAD_W["jaw_x"], HEAD_W["mlc"]
+    slabs = [_slab(jy, 1, -100.0, 200.0, [(v_lo - margin_cm) * sc(jy)], [(v_hi + margin_cm) * sc(jy)]),
+             _slab(jx, 0, -100.0, 200.0, [(u_lo - margin_cm) * sc(jx)], [(u_hi + margin_cm) * sc(jx)]),
+             _slab(ml, 0, -0.5 * n_leaf * leaf_cm * sc(ml), leaf_cm * sc(ml), lo * sc(ml), hi * sc(ml))]
+    return {"slabs": slabs, "material": MAT_W, "density": float(TUNGSTEN[2]), "w_ps2": HEAD_W["ps2"]}
+
+
+def head_config(field=0, shrink=1, n_ps1=1_000_000, seed_ps1=7):
+    """C4 field `field` with the collimation stage in place of the fluence-map source: the same phantom, EPID, spectrum and
+    aperture envelope, tables with tungsten as material 8, a synthetic Phase Space 1 and jaws / MLC from the field's map."""
+    t = make_tables(extra=(TUNGSTEN,))
+    cfg = make_config("C4", field=field, shrink=shrink, tables=t)
+    cfg["name"] = "C4H"
+    cfg["collimator"] = collimator_for_fluence(cfg["source"]["fluence"], cfg["source"]["f_pitch"])
+    cfg["ps1"] = phase_space_1(seed_ps1, n_ps1)
+    return cfg
 
 
 def make_config(name, field=0, shrink=1, tables=None):

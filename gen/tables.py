@@ -27,7 +27,7 @@ ELEMENTS = {
     "O": (8, 15.999, 95.0), "Na": (11, 22.990, 149.0), "Mg": (12, 24.305, 156.0),
     "Si": (14, 28.085, 173.0), "P": (15, 30.974, 173.0), "S": (16, 32.06, 180.0),
     "Ar": (18, 39.948, 188.0), "Ca": (20, 40.078, 191.0), "Cu": (29, 63.546, 322.0),
-    "Gd": (64, 157.25, 591.0),
+    "Gd": (64, 157.25, 591.0), "W": (74, 183.84, 727.0),
 }
 
 _WATER = {"H": 0.111894, "O": 0.888106}
@@ -45,6 +45,10 @@ MATERIALS = [
 ]
 MAT_AIR, MAT_LUNG, MAT_SOFT, MAT_BONE, MAT_CU, MAT_GOS, MAT_GLASS, MAT_PMMA = range(8)
 RHO_AIR = 1.205e-3
+# Jaws and MLC leaves of the collimation stage: tungsten.  Not part of MATERIALS, so that the tables of
+# C0-C4 keep their eight materials; make_tables(extra=(TUNGSTEN,)) appends it as material 8.
+TUNGSTEN = ("W", {"W": 1.0}, 19.3)
+MAT_W = 8
 
 
 def sigma_kn(E):
@@ -105,14 +109,15 @@ def radiation_length(comp):
     return 1.0 / inv
 
 
-def make_tables(n_E=500, E_min=1e-3, E_max=20.0, n_T=200, T_min=0.01, T_max=20.0):
-    """All material tables, float32, in the layout of `aepid_init_materials`."""
+def make_tables(n_E=500, E_min=1e-3, E_max=20.0, n_T=200, T_min=0.01, T_max=20.0, extra=()):
+    """All material tables, float32, in the layout of `aepid_init_materials`; `extra` appends materials to MATERIALS."""
     E = np.exp(np.linspace(np.log(E_min), np.log(E_max), n_E))
     T = np.exp(np.linspace(np.log(T_min), np.log(T_max), n_T))
-    n_mat = len(MATERIALS)
+    mats = list(MATERIALS) + list(extra)
+    n_mat = len(mats)
     mc = np.empty((n_mat, n_E)); mp = np.empty((n_mat, n_E)); mpp = np.empty((n_mat, n_E))
     sp = np.empty((n_mat, n_T)); x0 = np.empty(n_mat); ne = np.empty(n_mat)
-    for m, (_, comp, _) in enumerate(MATERIALS):
+    for m, (_, comp, _) in enumerate(mats):
         mc[m] = mu_compton(comp, E)
         mp[m] = mu_photoelectric(comp, E)
         mpp[m] = mu_pair(comp, E)
@@ -121,7 +126,7 @@ def make_tables(n_E=500, E_min=1e-3, E_max=20.0, n_T=200, T_min=0.01, T_max=20.0
         ne[m] = N_A * sum(w * ELEMENTS[el][0] / ELEMENTS[el][1] for el, w in _fractions(comp).items())
     f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
     return {
-        "n_mat": n_mat, "names": [m[0] for m in MATERIALS],
+        "n_mat": n_mat, "names": [m[0] for m in mats],
         "E_grid": f32(E), "mu_compton": f32(mc), "mu_pe": f32(mp), "mu_pair": f32(mpp),
         "T_grid": f32(T), "stop_pow": f32(sp), "rad_len": f32(x0),
         "electrons_per_gram": f32(ne),      # N_A sum_i w_i Z_i / A_i: input of the Class II (Moller) mode

@@ -61,6 +61,7 @@ typedef struct aepid_dims {
     int n_bins;               /* spectrum bins */
     int fu, fv;               /* fluence map */
     int n_batches;            /* B independent tally buffers for the batch variance estimate (2..255) */
+    int n_ps1;                /* capacity for Phase Space 1 records (aepid_load_phase_space_source), 0 if not used */
     int max_live_per_cta;     /* most particles one CTA of the transport kernel keeps alive, 64..65536 (0 = 65536); the workspace
                                  holds 160 x 5 class queues of twice that many 48-byte records (rounded up to a power of two):
                                  5.0 GB at 65536, 80 MB at 1024.  Results do not depend on it; small runs want it small. */
@@ -207,6 +208,30 @@ int aepid_apply_response_lut(aepid_ctx* ctx, const float* lut, int nt, int ns,
 /* Input of physics mode 2: electrons per gram of every material, N_A sum_i w_i Z_i / A_i ([n_mat], host or device, copied).
  * Call after aepid_init_materials (which forgets it). */
 int aepid_set_class2(aepid_ctx* ctx, const float* electrons_per_gram);
+
+/* Collimation stage (section 2.1.1: "particles are sampled from Phase Space 1 and transported through the
+ * jaws and MLC ... the resulting phase space (Phase Space 2) is ... streamed directly into the next simulation stage";
+ * SURVEY.md 8(f) NEXT-3; readings A35-A37 in DESIGN.md).
+ * aepid_load_phase_space_source: n_records x 8 floats = {u, v, du, dv, dw, E, -, -} (host or device, copied): position on the
+ * plane w = w_plane_cm of the beam frame (the frame of aepid_load_source: source position and axes), direction, energy.  While
+ * a table is loaded, history h starts from record floor(xi n_records), xi = the first draw of its Philox block 0, instead of
+ * the fluence-map sampler (one history = one Phase Space 1 particle; aepid_read_head counts the Phase Space 2 particles).
+ * n_records = 0 goes back to the fluence-map source.  n_records <= dims.n_ps1.
+ * aepid_load_collimator: n_slabs (<= 4) tungsten slabs sorted along w between the Phase Space 1 plane and w_ps2_cm.  Slab k spans
+ * [w0[k], w1[k]); its rows are stacked along v (axis[k] = 0: the MLC and the x-jaws, openings in u) or along u (axis[k] = 1: the
+ * y-jaws, openings in v), row r covering [row0[k] + r pitch[k], row0[k] + (r+1) pitch[k]); row r is open on [lo, hi) (lo, hi:
+ * concatenated over the slabs, n_rows[k] entries each, at most 1024 in all; a closed leaf pair has lo = hi), all in cm at the slab
+ * itself (straight, unfocused edges).  Everything else inside a slab's w-range is `material` at `density`.  All pointers HOST.
+ * Photons are followed through the stage with the photon physics of the path; charged particles are not (their energy stays in
+ * the head and is booked in ledger[4]), annihilation quanta born in the head are dropped, photons that turn upstream escape.
+ * n_slabs = 0 removes the collimator.
+ * aepid_read_head (synchronises): {Phase Space 2 particles, their energy [MeV], energy absorbed in the stage [MeV], 0} since the
+ * last aepid_reset_tallies. */
+int aepid_load_phase_space_source(aepid_ctx* ctx, unsigned long long n_records, const float* records, float w_plane_cm);
+int aepid_load_collimator(aepid_ctx* ctx, int n_slabs, const float* w0_cm, const float* w1_cm, const int* axis, const int* n_rows,
+                          const float* row0_cm, const float* pitch_cm, const float* lo_cm, const float* hi_cm,
+                          int material, float density_g_cm3, float w_ps2_cm);
+int aepid_read_head(aepid_ctx* ctx, double out[4]);
 
 /* Scheduler knob of the transport kernel: the most particles a CTA keeps alive at a time, 64 .. 65536
  * (0 = the default, 65536 = half a class queue).  Results do not depend on it (every particle has its own Philox stream);

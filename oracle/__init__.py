@@ -40,6 +40,7 @@ def lib():
         _lib.orc_last_error.restype = C.c_char_p
         _lib.orc_ps3_count.restype = C.c_uint64
         _lib.orc_event_log_count.restype = C.c_uint64
+        _lib.orc_ps2_count.restype = C.c_uint64
         _lib.orc_moller_cos.restype = C.c_double
         for f in ("orc_stop_pow", "orc_majorant", "orc_highland_theta0", "orc_field_size", "orc_lut_bilinear"):
             getattr(_lib, f).restype = C.c_double
@@ -196,12 +197,50 @@ class Oracle:
         p = (C.c_double * 3)(*pos); d = (C.c_double * 3)(*direction)
         self._chk(self._l.orc_set_fixed_primary(self._h, int(ptype), C.c_double(E), p, d))
 
+    # ---- collimation stage: Phase Space 1 source, jaws / MLC slabs, Phase Space 2 dump
+    def load_phase_space_source(self, ps1):
+        rec = _f32(ps1["records"]) if ps1 is not None else np.zeros((0, 8), np.float32)
+        self._chk(self._l.orc_load_phase_space_source(self._h, C.c_uint64(len(rec)), _p(rec, C.c_float), C.c_double(ps1["plane"] if ps1 is not None else 0.0)))
+
+    def load_collimator(self, col):
+        if col is None:
+            self._chk(self._l.orc_load_collimator(self._h, 0, None, None, None, None, None, None, None, None, 0, C.c_double(1.0), C.c_double(0.0)))
+            return
+        sl = col["slabs"]
+        w0, w1 = _f32([s["w0"] for s in sl]), _f32([s["w1"] for s in sl])
+        axis = np.ascontiguousarray([s["axis"] for s in sl], dtype=np.int32); nr = np.ascontiguousarray([len(s["lo"]) for s in sl], dtype=np.int32)
+        row0, pitch = _f32([s["row0"] for s in sl]), _f32([s["pitch"] for s in sl])
+        lo, hi = _f32(np.concatenate([s["lo"] for s in sl])), _f32(np.concatenate([s["hi"] for s in sl]))
+        self._chk(self._l.orc_load_collimator(self._h, len(sl), _p(w0, C.c_float), _p(w1, C.c_float), _p(axis, C.c_int), _p(nr, C.c_int),
+                                              _p(row0, C.c_float), _p(pitch, C.c_float), _p(lo, C.c_float), _p(hi, C.c_float),
+                                              int(col["material"]), C.c_double(col["density"]), C.c_double(col["w_ps2"])))
+
+    def set_ps2(self, on=True):
+        self._chk(self._l.orc_set_ps2(self._h, int(bool(on))))
+
+    def read_ps2(self):
+        """Records [n][8] = {E, u, v, du, dv, dw, history, uncollided} of every photon that reached the Phase Space 2 plane."""
+        n = int(self._l.orc_ps2_count(self._h))
+        out = np.empty((n, 8))
+        self._chk(self._l.orc_read_ps2(self._h, _p(out, C.c_double)))
+        return out
+
+    def read_head(self):
+        """{PS2 particles, their energy, energy absorbed in the stage, interactions in the stage}."""
+        out = np.zeros(4)
+        self._chk(self._l.orc_read_head(self._h, _p(out, C.c_double)))
+        return out
+
     def load(self, cfg):
         self.cfg = cfg
         self.init_materials(cfg["tables"])
         self.load_phantom(cfg["phantom"])
         self.load_epid_layers(cfg["epid"])
         self.load_source(cfg["source"])
+        if cfg.get("ps1") is not None:
+            self.load_phase_space_source(cfg["ps1"])
+        if cfg.get("collimator") is not None:
+            self.load_collimator(cfg["collimator"])
         self.set_physics(cfg["physics"])
         self.set_options()
 
@@ -236,6 +275,7 @@ class Oracle:
         out["pc_sq"] = np.zeros((nz // rz, ny // ry, nx // rx)) if coarse else None
         out["ledger_sq"] = np.zeros(8)
         self._chk(self._l.orc_read_extra(self._h, _p(out["pc_sum"], C.c_double), _p(out["pc_sq"], C.c_double), _p(out["ledger_sq"], C.c_double)))
+        out["head"] = self.read_head()
         return out
 
     # ---- Phase Space 3 (reading A30)
@@ -302,8 +342,13 @@ def stats(raw):
     return res
 
 
+_SHARED_CFG = None          # inherited by forked workers (copy-on-write): the config is not pickled per job
+
+
 def _worker(args):
     cfg, first, n, seed, opts = args
+    if cfg is None:
+        cfg = _SHARED_CFG
     opts = dict(opts)
     prb = opts.pop("phantom_rebin", None)
     o = Oracle(cfg)
@@ -319,23 +364,30 @@ def run_sharded(cfg, n, seed, first=0, procs=None, **opts):
     """Run histories [first, first+n) split over `procs` processes (legal: the RNG is keyed by
     the global history index) and add the raw accumulators."""
     import multiprocessing as mp
+    global _SHARED_CFG
     procs = procs or min(os.cpu_count() or 1, 32)
     procs = max(1, min(procs, int(n)))
     if procs == 1:
         return _worker((cfg, first, n, seed, opts))
     build()
     bounds = np.linspace(first, first + n, procs + 1).astype(np.uint64)
-    jobs = [(cfg, int(bounds[i]), int(bounds[i + 1] - bounds[i]), seed, opts) for i in range(procs)]
-    with mp.get_context("fork").Pool(procs) as pool:
-        parts = pool.map(_worker, jobs)
-    tot = parts[0]
-    for p in parts[1:]:
-        for k, v in p.items():
-            if v is None:
-                continue
-            if k == "counters":
-                mx = max(int(tot[k][11]), int(v[11]))
-                tot[k] = tot[k] + v; tot[k][11] = mx
-            else:
-                tot[k] = tot[k] + v
+    jobs = [(None, int(bounds[i]), int(bounds[i + 1] - bounds[i]), seed, opts) for i in range(procs)]
+    _SHARED_CFG = cfg
+    try:
+        with mp.get_context("fork").Pool(procs) as pool:
+            tot = None
+            for p in pool.imap_unordered(_worker, jobs):       # add as they arrive: one worker's arrays in flight at a time
+                if tot is None:
+                    tot = p
+                    continue
+                for k, v in p.items():
+                    if v is None:
+                        continue
+                    if k == "counters":
+                        mx = max(int(tot[k][11]), int(v[11]))
+                        tot[k] = tot[k] + v; tot[k][11] = mx
+                    else:
+                        tot[k] += v
+    finally:
+        _SHARED_CFG = None
     return tot

@@ -171,8 +171,15 @@ struct Ctx {
     int prb[3] = {1, 1, 1}; bool prb_on = false; std::vector<double> pc_sum, pc_sq;
     // second moments of the ledger channels over histories (sum over histories of (per-history amount)^2)
     double ledger_sq[8] = {0}, ledger_prev[8] = {0};
-    // event log for the pins (tests/test_oracle_pins2.py): 16 doubles per record, see log_event
+    // event log for the pins (tests/test_oracle_pins_events.py): 16 doubles per record, see log_event
     size_t log_cap = 0; std::vector<double> evlog;
+    // collimation stage (readings A35-A37): Phase Space 1 records on the plane
+    // w = w_ps1 (beam frame) and tungsten slabs with per-row openings between it and the Phase Space 2 plane w = w_ps2
+    struct Slab { double w0, w1; int axis; double row0, pitch; std::vector<double> lo, hi; };
+    std::vector<Slab> slabs; int col_mat = 0; double col_rho = 0, w_ps2 = 0; bool have_col = false;
+    std::vector<float> ps1; size_t n_ps1 = 0; double w_ps1 = 0;
+    double head[4] = {0};                  // PS2 particles, their energy, energy absorbed in the stage, interactions in the stage
+    bool ps2_on = false; std::vector<double> ps2;   // Phase Space 2 dump: {E, u, v, du, dv, dw, history, uncollided}
 };
 
 // ---------------------------------------------------------------- tables
@@ -811,6 +818,56 @@ void transport_electron(Ctx& c, Particle p, const Run& r) {
     }
 }
 
+// ---------------------------------------------------------------- collimation stage (section 2.1.1)
+// "Particles are sampled from Phase Space 1 and transported through the jaws and MLC ... The resulting phase space (Phase Space
+// 2) is ... streamed directly into the next simulation stage."  Readings (A35-A37): the stage lies between the planes
+// w = w_ps1 and w = w_ps2 of the beam frame; inside the w-range of a slab every point outside the opening of its row is tungsten,
+// every other point of the stage is air.  Photons are tracked by Woodcock flights against the tungsten coefficient (exact for
+// any arrangement of openings); charged particles are not followed (their energy stays where the photon interacted, pair
+// production included: annihilation quanta born in the head are dropped); a photon that turns upstream (dw <= 0) or leaves
+// the world sideways has left the stage (escaped).  Energy absorbed in the stage is booked in the ledger's air channel.
+int head_material(const Ctx& c, Vec3 q) {
+    for (const Ctx::Slab& sl : c.slabs) {
+        if (q.z < sl.w0 || q.z >= sl.w1) continue;
+        const double across = sl.axis == 0 ? q.y : q.x, along = sl.axis == 0 ? q.x : q.y;
+        const double fr = std::floor((across - sl.row0) / sl.pitch);
+        if (fr < 0 || fr >= (double)sl.lo.size()) return c.col_mat;
+        const size_t r = (size_t)fr;
+        return (along >= sl.lo[r] && along < sl.hi[r]) ? MAT_AIR : c.col_mat;
+    }
+    return MAT_AIR;
+}
+// p.pos / p.dir in the BEAM frame, on or below the Phase Space 1 plane.  Returns true with p on the Phase Space 2 plane.
+bool head_stage(Ctx& c, Particle& p) {
+    auto absorb = [&](double e) { dep_air(c, e); c.head[2] += e; };
+    for (;;) {
+        if (p.E < c.photon_cut) { absorb(p.E); return false; }
+        const double mm = std::max(c.col_rho * mu_tot(c, c.col_mat, p.E), RHO_AIR * mu_tot(c, MAT_AIR, p.E)) * (1.0 + 1e-6);
+        const double s = -std::log(p.rng.u()) / mm;
+        const Vec3 q = p.pos + s * p.dir;
+        if (q.z >= c.w_ps2) {                                              // reaches the Phase Space 2 plane first
+            const double t = (c.w_ps2 - p.pos.z) / p.dir.z;
+            p.pos = p.pos + t * p.dir; p.pos.z = c.w_ps2;
+            if (std::fabs(p.pos.x) >= WORLD_HALF || std::fabs(p.pos.y) >= WORLD_HALF) { escape(c, p.E); return false; }
+            return true;
+        }
+        if (std::fabs(q.x) >= WORLD_HALF || std::fabs(q.y) >= WORLD_HALF) { escape(c, p.E); return false; }
+        p.pos = q;
+        const int m = head_material(c, q);
+        const double rho = m == MAT_AIR ? RHO_AIR : c.col_rho;
+        double mu[3]; mu_partial(c, m, p.E, mu);
+        if (!(p.rng.u() * mm < rho * (mu[0] + mu[1] + mu[2]))) continue;   // virtual collision
+        p.uncollided = false; c.head[3] += 1.0;
+        const double x = p.rng.u() * (mu[0] + mu[1] + mu[2]);
+        if (x < mu[0] || !(x < mu[0] + mu[1])) { absorb(p.E); return false; }   // photoelectric, or pair (all of E stays, reading A36)
+        double E1, T; Vec3 d1, de;
+        compton_scatter(p.rng, p.E, p.dir, &E1, &d1, &T, &de, nullptr);
+        absorb(T);
+        p.E = E1; p.dir = d1;
+        if (!(p.dir.z > 0.0)) { escape(c, p.E); return false; }           // turned upstream: out of the stage
+    }
+}
+
 // ---------------------------------------------------------------- source
 struct SourceSample { double E; Vec3 dir_world; Vec3 dir_beam; int pixel; double u, v; };
 SourceSample sample_source(const Ctx& c, Rng& rng) {
@@ -842,6 +899,7 @@ int check_ready(Ctx& c) {
     if (c.n[0] <= 0) { c.err = "load_phantom not called"; return -2; }
     if (c.n_layers <= 0) { c.err = "load_epid_layers not called"; return -2; }
     if (c.fu <= 0) { c.err = "load_source not called"; return -2; }
+    if (c.have_col && c.n_ps1 == 0) { c.err = "a collimator needs a phase-space source"; return -2; }
     if (c.mode >= 2 && (int)c.ne.size() != c.n_mat) { c.err = "mode 2 needs orc_set_class2 (electrons per gram)"; return -2; }
     // phantom AABB must lie inside the air part of the world box
     for (int k = 0; k < 8; ++k) {
@@ -860,7 +918,7 @@ void alloc_tallies(Ctx& c) {
     c.rb_sum.assign(nr, 0); c.rb_sq.assign(nr, 0);
     c.ph_sum.assign(nvx, 0); c.ph_sq.assign(c.want_phantom_sq ? nvx : 0, 0);
     std::fill(c.ledger, c.ledger + 8, 0.0); std::fill(c.counters, c.counters + 16, (uint64_t)0);
-    std::fill(c.aux, c.aux + 4, 0.0);
+    std::fill(c.aux, c.aux + 4, 0.0); std::fill(c.head, c.head + 4, 0.0); c.ps2.clear();
     std::fill(c.ledger_sq, c.ledger_sq + 8, 0.0); std::fill(c.ledger_prev, c.ledger_prev + 8, 0.0);
     if (c.prb_on) { const size_t nc = (size_t)(c.n[0] / c.prb[0]) * (c.n[1] / c.prb[1]) * (c.n[2] / c.prb[2]); c.pc_sum.assign(nc, 0); c.pc_sq.assign(nc, 0); }
     else { c.pc_sum.clear(); c.pc_sq.clear(); }
@@ -985,6 +1043,31 @@ int orc_run(orc_ctx* x, uint64_t first, uint64_t n, uint64_t seed) {
         Particle p{};
         c.cur_h = h;
         p.rng.init(seed, h, 0);
+        bool through = true;
+        if (c.n_ps1 > 0) {
+            // Phase Space 1 source (reading A35): record floor(xi0 n) of the table, xi0 = first draw of block 0; the other
+            // three draws of the block are not used
+            const double x0 = p.rng.u(); p.rng.skip_block();
+            const size_t j = std::min((size_t)(x0 * (double)c.n_ps1), c.n_ps1 - 1);
+            const float* q = c.ps1.data() + 8 * j;
+            p.type = PHOTON; p.E = q[5]; p.region = AIR; p.uncollided = true;
+            p.pos = {q[0], q[1], c.w_ps1}; p.dir = normalize(Vec3{q[2], q[3], q[4]});
+            c.ledger[0] += p.E; c.ledger[6] += 1.0;
+            if (c.have_col) through = head_stage(c, p);
+            if (through) {
+                c.head[0] += 1.0; c.head[1] += p.E;
+                if (c.ps2_on) { const double rec[8] = {p.E, p.pos.x, p.pos.y, p.dir.x, p.dir.y, p.dir.z, (double)h, p.uncollided ? 1.0 : 0.0}; c.ps2.insert(c.ps2.end(), rec, rec + 8); }
+                p.pos = to_world(c, p.pos); p.dir = dir_to_world(c, p.dir);
+            }
+            c.stack.clear();
+            if (through) c.stack.push_back(p);
+            while (!c.stack.empty()) {
+                Particle q2 = c.stack.back(); c.stack.pop_back();
+                if (q2.type == PHOTON) transport_photon(c, q2, r); else transport_electron(c, q2, r);
+            }
+            flush_history(c);
+            continue;
+        }
         const SourceSample s = sample_source(c, p.rng);             // block 0 of particle 0 (reading A1)
         p.type = PHOTON; p.E = s.E; p.pos = c.src; p.dir = s.dir_world; p.region = AIR; p.uncollided = true;
         if (c.fixed) {
@@ -1044,6 +1127,38 @@ int orc_read_extra(orc_ctx* x, double* pc_sum, double* pc_sq, double ledger_sq[8
 int orc_set_event_log(orc_ctx* x, uint64_t capacity) { Ctx& c = C(x); c.log_cap = (size_t)capacity; c.evlog.clear(); return 0; }
 uint64_t orc_event_log_count(orc_ctx* x) { return C(x).evlog.size() / 16; }
 int orc_read_event_log(orc_ctx* x, double* out) { Ctx& c = C(x); if (!c.evlog.empty()) std::memcpy(out, c.evlog.data(), c.evlog.size() * sizeof(double)); return 0; }
+
+// Collimation stage.  Slab k spans w in [w0[k], w1[k]) of the beam frame, its rows are stacked along v (axis 0: openings in u) or
+// along u (axis 1: openings in v) from row0[k] with pitch[k]; row r opens [lo, hi) (concatenated arrays, n_rows[k] entries per
+// slab); outside the rows and outside the openings the slab is material `mat` at `rho`.  n_slabs = 0 removes the collimator.
+int orc_load_collimator(orc_ctx* x, int n_slabs, const float* w0, const float* w1, const int* axis, const int* n_rows, const float* row0,
+                        const float* pitch, const float* lo, const float* hi, int mat, double rho, double w_ps2) {
+    Ctx& c = C(x);
+    c.slabs.clear(); c.have_col = false;
+    if (n_slabs == 0) return 0;
+    if (mat < 0 || mat >= c.n_mat || !(rho > 0)) { c.err = "bad collimator material"; return -1; }
+    size_t o = 0; double prev = -INF;
+    for (int k = 0; k < n_slabs; ++k) {
+        if (!(w1[k] > w0[k]) || !(w0[k] >= prev) || n_rows[k] < 1 || !(pitch[k] > 0)) { c.err = "bad collimator slab"; return -1; }
+        Ctx::Slab sl{w0[k], w1[k], axis[k], row0[k], pitch[k], {}, {}};
+        for (int r = 0; r < n_rows[k]; ++r, ++o) { sl.lo.push_back(lo[o]); sl.hi.push_back(hi[o]); }
+        c.slabs.push_back(sl); prev = w1[k];
+    }
+    if (!(w_ps2 >= prev)) { c.err = "Phase Space 2 plane above the last slab"; return -1; }
+    c.col_mat = mat; c.col_rho = rho; c.w_ps2 = w_ps2; c.have_col = true;
+    return 0;
+}
+// Phase Space 1 records [n][8] = {u, v, du, dv, dw, E, -, -} on the plane w = w_plane of the beam frame; n = 0 goes back to the
+// fluence-map source.  The beam frame is the one of orc_load_source (source position and axes).
+int orc_load_phase_space_source(orc_ctx* x, uint64_t n, const float* rec, double w_plane) {
+    Ctx& c = C(x);
+    c.ps1.assign(rec, rec + 8 * n); c.n_ps1 = (size_t)n; c.w_ps1 = w_plane;
+    return 0;
+}
+int orc_read_head(orc_ctx* x, double out[4]) { std::memcpy(out, C(x).head, 4 * sizeof(double)); return 0; }
+int orc_set_ps2(orc_ctx* x, int on) { Ctx& c = C(x); c.ps2_on = on != 0; c.ps2.clear(); return 0; }
+uint64_t orc_ps2_count(orc_ctx* x) { return C(x).ps2.size() / 8; }
+int orc_read_ps2(orc_ctx* x, double* out) { Ctx& c = C(x); if (!c.ps2.empty()) std::memcpy(out, c.ps2.data(), c.ps2.size() * sizeof(double)); return 0; }
 
 // Phase Space 3: switch the recording on / off (clears the store), number of records, copy out [n][8].
 int orc_set_ps3(orc_ctx* x, int on) { Ctx& c = C(x); c.ps3_on = on != 0; c.ps3.clear(); return 0; }

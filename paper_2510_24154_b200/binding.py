@@ -31,7 +31,8 @@ EXPORTS = ("aepid_workspace_bytes", "aepid_create", "aepid_destroy", "aepid_last
            "aepid_set_counting", "aepid_read_counters", "aepid_sample_source", "aepid_field_size",
            "aepid_apply_response_lut", "aepid_synchronize", "aepid_set_history_offset", "aepid_read_moments",
            "aepid_finalize_moments", "aepid_upsample", "aepid_gamma_index",
-           "aepid_set_phase_space", "aepid_read_phase_space_count", "aepid_set_live_limit", "aepid_set_class2", "aepid_roi_mean")
+           "aepid_set_phase_space", "aepid_read_phase_space_count", "aepid_set_live_limit", "aepid_set_class2", "aepid_roi_mean",
+           "aepid_load_phase_space_source", "aepid_load_collimator", "aepid_read_head")
 
 
 class AepidError(RuntimeError):
@@ -40,7 +41,7 @@ class AepidError(RuntimeError):
 
 class Dims(C.Structure):
     _fields_ = [(n, C.c_int) for n in ("n_mat", "n_E", "n_T", "nx", "ny", "nz", "n_layers", "nu", "nv",
-                                       "n_bins", "fu", "fv", "n_batches", "max_live_per_cta")]
+                                       "n_bins", "fu", "fv", "n_batches", "n_ps1", "max_live_per_cta")]
 
 
 def load_library():
@@ -84,6 +85,9 @@ def load_library():
     lib.aepid_set_phase_space.argtypes = [vp, vp, C.c_ulonglong]
     lib.aepid_read_phase_space_count.argtypes = [vp, vp]
     lib.aepid_roi_mean.argtypes = [vp, vp, C.c_int, C.c_int, C.c_float, C.c_float, vp]
+    lib.aepid_load_phase_space_source.argtypes = [vp, C.c_ulonglong, vp, C.c_float]
+    lib.aepid_load_collimator.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, vp, vp, vp, C.c_int, C.c_float, C.c_float]
+    lib.aepid_read_head.argtypes = [vp, vp]
     lib.aepid_upsample.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int, C.c_int]
     lib.aepid_gamma_index.argtypes = [vp, vp, vp, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_float, C.c_float, vp, vp]
     _lib = lib
@@ -154,7 +158,7 @@ class Engine:
                  nx=int(ph["nx"]), ny=int(ph["ny"]), nz=int(ph["nz"]), n_layers=len(ep["thickness"]),
                  nu=int(ep["nu"]), nv=int(ep["nv"]), n_bins=len(s["E_pdf"]), fu=int(s["fu"]), fv=int(s["fv"]),
                  n_batches=int(n_batches if n_batches is not None else cfg["physics"]["n_batches"]),
-                 max_live_per_cta=int(max_live_per_cta))
+                 n_ps1=int(cfg["ps1"]["n"]) if cfg.get("ps1") is not None else 0, max_live_per_cta=int(max_live_per_cta))
         return cls(d, device=device, stream=stream)
 
     def close(self):
@@ -211,6 +215,10 @@ class Engine:
         self.load_phantom(ph["spacing"], ph["origin"], ph["density"], ph["material"])
         self.load_epid_layers(ep["thickness"], ep["material"], ep["density"], ep["scored"], ep["sid"], ep["nu"], ep["nv"], ep["pitch"])
         self.load_source(s["src_pos"], s["beam_axes"], s["E_edges"], s["E_pdf"], s["f_pitch"], s["f_plane_dist"], s["fluence"])
+        if cfg.get("ps1") is not None:
+            self.load_phase_space_source(cfg["ps1"]["records"], cfg["ps1"]["plane"])
+        if cfg.get("collimator") is not None:
+            self.load_collimator(cfg["collimator"])
         self.set_physics(**cfg["physics"])
 
     # ---- running
@@ -283,6 +291,32 @@ class Engine:
         s = C.c_float()
         self._chk(self._lib.aepid_field_size(self._h, int(bool(printed_form)), C.byref(s)))
         return float(s.value)
+
+    # ---- collimation stage
+    def load_phase_space_source(self, records, w_plane):
+        """Phase Space 1 records [n][8] float32 (numpy or torch, host or device); None or empty: back to the fluence-map source."""
+        n = 0 if records is None else int(records.shape[0])
+        self._chk(self._lib.aepid_load_phase_space_source(self._h, n, _ptr(records) if n else None, float(w_plane)))
+
+    def load_collimator(self, col):
+        """col: {"slabs": [{w0, w1, axis, row0, pitch, lo[], hi[]}, ...], "material", "density", "w_ps2"} or None."""
+        if col is None:
+            self._chk(self._lib.aepid_load_collimator(self._h, 0, None, None, None, None, None, None, None, None, 0, 1.0, 0.0))
+            return
+        sl = col["slabs"]
+        f = lambda k: _host_f32([s[k] for s in sl])
+        i = lambda v: np.ascontiguousarray(v, dtype=np.int32)
+        w0, w1, row0, pitch = f("w0"), f("w1"), f("row0"), f("pitch")
+        axis, nr = i([s["axis"] for s in sl]), i([len(s["lo"]) for s in sl])
+        lo, hi = _host_f32(np.concatenate([s["lo"] for s in sl])), _host_f32(np.concatenate([s["hi"] for s in sl]))
+        self._chk(self._lib.aepid_load_collimator(self._h, len(sl), _ptr(w0), _ptr(w1), _ptr(axis), _ptr(nr), _ptr(row0), _ptr(pitch),
+                                                  _ptr(lo), _ptr(hi), int(col["material"]), float(col["density"]), float(col["w_ps2"])))
+
+    def read_head(self):
+        """{Phase Space 2 particles, their energy, energy absorbed in the collimation stage, 0} since the last reset."""
+        out = np.zeros(4, dtype=np.float64)
+        self._chk(self._lib.aepid_read_head(self._h, _ptr(out)))
+        return out
 
     def set_live_limit(self, max_live_per_cta=0):
         self._chk(self._lib.aepid_set_live_limit(self._h, int(max_live_per_cta)))

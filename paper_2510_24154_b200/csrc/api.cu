@@ -22,7 +22,7 @@ constexpr size_t kMaxLut = 65536;
 inline size_t up(size_t x) { return (x + kAlign - 1) & ~(kAlign - 1); }
 
 struct Layout {
-    size_t vox, ph_batch, ep_batch, out_ph, out_ep, tmap, signal, dose_in, lut, blob, thrE, edges, thrF, guideF, queues, small, total;
+    size_t vox, ph_batch, ep_batch, out_ph, out_ep, tmap, signal, dose_in, lut, blob, thrE, edges, thrF, guideF, queues, small, ps1, head_rows, total;
     size_t nvox, npix, blob_bytes;
 };
 
@@ -34,6 +34,7 @@ bool dims_ok(const aepid_dims* d) {
     if (d->n_bins < 1 || d->n_bins > 65536 || d->fu < 1 || d->fv < 1 || d->fu > 4096 || d->fv > 4096) return false;
     if (d->n_batches < 2 || d->n_batches > 255) return false;
     if (d->max_live_per_cta != 0 && (d->max_live_per_cta < 64 || d->max_live_per_cta > kMaxPoolSlots / 2)) return false;
+    if (d->n_ps1 < 0) return false;
     return true;
 }
 
@@ -68,6 +69,8 @@ Layout make_layout(const aepid_dims& d) {
     L.guideF = take(((size_t)kGuideSize + 1) * 4);
     L.queues = take((size_t)kMaxCtas * kRingCount * ((size_t)1 << pool_log_for(d)) * kRecordBytes);   // class queues of the transport kernel (scratch)
     L.small = take(1024);            // ledger [8] f64 @0 | chunk counter @64 | bad-material flag @68 | rho_max [32] f32 @128 | counters [32] u64 @256 | gamma stats [4] f64 @512, max bits @544 | PS3 count u64 @576
+    L.ps1 = take((size_t)d.n_ps1 * 32);                 // Phase Space 1 records (collimation stage), 0 if not used
+    L.head_rows = take((size_t)kMaxHeadRows * 8);        // openings lo[] | hi[] of the collimator rows
     L.total = o;
     return L;
 }
@@ -99,6 +102,7 @@ struct aepid_ctx {
     int pool_log = kMaxPoolLog;                                // log2 of the records per class queue of a CTA (from dims.max_live_per_cta)
     int live_max = kMaxPoolSlots / 2;
     float4* ps3 = nullptr; unsigned long long ps3_cap = 0;       // caller-owned Phase Space 3 buffer (aepid_set_phase_space)
+    Head hd{};                                                   // collimation stage (aepid_load_phase_space_source, aepid_load_collimator)
 
     uint32_t* d_vox() { return reinterpret_cast<uint32_t*>(ws + lay.vox); }
     float* d_ph_batch() { return reinterpret_cast<float*>(ws + lay.ph_batch); }
@@ -122,6 +126,9 @@ struct aepid_ctx {
     double* d_gamma_stats() { return reinterpret_cast<double*>(ws + lay.small + 512); }
     unsigned int* d_gamma_max() { return reinterpret_cast<unsigned int*>(ws + lay.small + 544); }
     unsigned long long* d_ps3_count() { return reinterpret_cast<unsigned long long*>(ws + lay.small + 576); }
+    double* d_head_stats() { return reinterpret_cast<double*>(ws + lay.small + 640); }      // [4]
+    float4* d_ps1() { return reinterpret_cast<float4*>(ws + lay.ps1); }
+    float* d_head_rows() { return reinterpret_cast<float*>(ws + lay.head_rows); }
 };
 
 namespace {
@@ -174,6 +181,7 @@ int reset_tallies(aepid_ctx* ctx) {
     CU(cudaMemsetAsync(ctx->ws + ctx->lay.small, 0, 128, ctx->stream));
     CU(cudaMemsetAsync(ctx->ws + ctx->lay.small + 256, 0, 256, ctx->stream));
     CU(cudaMemsetAsync(ctx->d_ps3_count(), 0, 8, ctx->stream));
+    CU(cudaMemsetAsync(ctx->d_head_stats(), 0, 32, ctx->stream));
     ctx->n_done = 0; ctx->first_history = 0;
     std::fill(ctx->hist, ctx->hist + 256, 0.0);
     return 0;
@@ -303,6 +311,12 @@ int fill_params(aepid_ctx* ctx, TransportParams& p) {
     p.queues = reinterpret_cast<uint4*>(ctx->ws + ctx->lay.queues);
     p.n_batches = ctx->dims.n_batches; p.nvox = ctx->lay.nvox; p.npix = ctx->lay.npix; p.live_max = ctx->live_max;
     p.pool_log = ctx->pool_log;
+    p.hd = ctx->hd; p.hd.stats = ctx->d_head_stats(); p.hd.ps1 = ctx->d_ps1();
+    p.hd.lo = ctx->d_head_rows(); p.hd.hi = ctx->d_head_rows() + kMaxHeadRows;
+    if (p.hd.n_slabs > 0 && p.hd.n_ps1 == 0) return fail(ctx, AEPID_ERR_BAD_STATE, "a collimator needs a phase-space source (aepid_load_phase_space_source)");
+    if (p.hd.n_slabs > 0 && p.hd.mat >= ctx->n_mat) return fail(ctx, AEPID_ERR_BAD_ARG, "collimator material index out of range");
+    if (p.hd.n_slabs == 0) p.hd.w_ps2 = p.hd.w_ps1;
+    if (p.hd.n_ps1 != 0 && !(p.hd.w_ps2 < ctx->g.sid)) return fail(ctx, AEPID_ERR_GEOMETRY, "Phase Space 2 plane below the EPID");
     p.ps3 = ctx->ps3; p.ps3_count = ctx->d_ps3_count(); p.ps3_cap = ctx->ps3 ? ctx->ps3_cap : 0;
     p.base = 0; set_seed(p, 0); p.n = 0; p.hist_per_batch = 1;
     return 0;
@@ -702,6 +716,54 @@ int aepid_set_class2(aepid_ctx* ctx, const float* electrons_per_gram) {
     if (int rc = fetch(ctx, electrons_per_gram, (size_t)ctx->n_mat, ctx->ne)) return rc;
     for (float v : ctx->ne) if (!(v > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "electrons per gram must be positive");
     ctx->have_ne = true; ctx->tables_dirty = true;
+    return 0;
+}
+
+int aepid_load_phase_space_source(aepid_ctx* ctx, unsigned long long n_records, const float* records, float w_plane_cm) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    if (n_records == 0) { ctx->hd.n_ps1 = 0; return 0; }                  // back to the fluence-map source
+    if (!records) return fail(ctx, AEPID_ERR_BAD_ARG, "null records");
+    if (n_records > (unsigned long long)ctx->dims.n_ps1) return fail(ctx, AEPID_ERR_NOMEM, "phase-space records exceed dims.n_ps1");
+    if (!(w_plane_cm > kWorldWMin)) return fail(ctx, AEPID_ERR_GEOMETRY, "Phase Space 1 plane outside the world");
+    CU(cudaMemcpyAsync(ctx->d_ps1(), records, (size_t)n_records * 32, classify(records) == MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->hd.n_ps1 = (uint32_t)n_records; ctx->hd.w_ps1 = w_plane_cm;
+    return 0;
+}
+
+int aepid_load_collimator(aepid_ctx* ctx, int n_slabs, const float* w0, const float* w1, const int* axis, const int* n_rows,
+                          const float* row0, const float* pitch, const float* lo, const float* hi, int material, float density, float w_ps2) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    Head& H = ctx->hd;
+    if (n_slabs == 0) { H.n_slabs = 0; return 0; }
+    if (n_slabs < 0 || n_slabs > kMaxSlabs) return fail(ctx, AEPID_ERR_BAD_ARG, "at most 4 collimator slabs");
+    if (!w0 || !w1 || !axis || !n_rows || !row0 || !pitch || !lo || !hi) return fail(ctx, AEPID_ERR_BAD_ARG, "null collimator pointer");
+    if (material < 0 || material >= kMaxMat || !(density > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "bad collimator material or density");
+    int total = 0; float prev = -1e30f;
+    for (int k = 0; k < n_slabs; ++k) {
+        if (!(w1[k] > w0[k]) || !(w0[k] >= prev) || n_rows[k] < 1 || !(pitch[k] > 0) || (axis[k] != 0 && axis[k] != 1))
+            return fail(ctx, AEPID_ERR_BAD_ARG, "collimator slabs must be sorted along w, non-overlapping, with positive thickness and pitch");
+        total += n_rows[k]; prev = w1[k];
+    }
+    if (total > kMaxHeadRows) return fail(ctx, AEPID_ERR_NOMEM, "more than 1024 collimator rows");
+    if (!(w_ps2 >= prev)) return fail(ctx, AEPID_ERR_GEOMETRY, "Phase Space 2 plane above the last slab");
+    CU(cudaMemcpyAsync(ctx->d_head_rows(), lo, (size_t)total * 4, cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->d_head_rows() + kMaxHeadRows, hi, (size_t)total * 4, cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    int off = 0;
+    for (int k = 0; k < n_slabs; ++k) {
+        H.w0[k] = w0[k]; H.w1[k] = w1[k]; H.axis[k] = axis[k]; H.n_rows[k] = n_rows[k]; H.row0[k] = row0[k]; H.inv_pitch[k] = 1.0f / pitch[k];
+        H.off[k] = off; off += n_rows[k];
+    }
+    H.n_slabs = n_slabs; H.mat = material; H.rho = density; H.w_ps2 = w_ps2;
+    return 0;
+}
+
+int aepid_read_head(aepid_ctx* ctx, double out[4]) {
+    if (!ctx || !ctx->ws) return AEPID_ERR_BAD_STATE;
+    if (!out) return fail(ctx, AEPID_ERR_BAD_ARG, "null output");
+    CU(cudaMemcpyAsync(out, ctx->d_head_stats(), 4 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
     return 0;
 }
 

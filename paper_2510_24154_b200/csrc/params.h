@@ -70,8 +70,25 @@ struct Source {
     const uint32_t* guideF;            // [kGuideSize+1] bracket of the search in thrF per top-bits bucket of the draw
 };
 
+// Collimation stage: Phase Space 1 records and tungsten slabs with per-row openings
+// between the planes w = w_ps1 and w = w_ps2 of the beam frame (include/aepid.h: aepid_load_phase_space_source, aepid_load_collimator).
+constexpr int kMaxSlabs = 4;
+constexpr int kMaxHeadRows = 1024;     // rows (leaf pairs, jaw openings) over all slabs
+struct Head {
+    uint32_t n_ps1;                    // 0: fluence-map source
+    float w_ps1;
+    const float4* ps1;                 // [n_ps1][2] = {u, v, du, dv} {dw, E, -, -}
+    int n_slabs, mat;                  // slabs sorted by w; material index and density of the jaws / leaves
+    float rho, w_ps2;
+    float w0[kMaxSlabs], w1[kMaxSlabs], row0[kMaxSlabs], inv_pitch[kMaxSlabs];
+    int axis[kMaxSlabs], n_rows[kMaxSlabs], off[kMaxSlabs];
+    const float* lo; const float* hi;  // openings of all rows, slab after slab
+    double* stats;                     // [4]: Phase Space 2 particles, their energy, energy absorbed in the stage, unused
+};
+
 struct TransportParams {
     Geom g;
+    Head hd;
     Physics ph;
     Tables tb;
     Source so;

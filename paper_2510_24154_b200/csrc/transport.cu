@@ -128,6 +128,7 @@ __shared__ unsigned int s_head[kRings];             // tickets handed to poppers
 __shared__ unsigned int s_snap[kRings];             // tail at the last barrier: pops stay below it
 __shared__ int s_flag[2];                           // [0] no histories left, [1] error bits
 __shared__ int s_phase, s_keep, s_budget, s_left;   // class of the phase (-1: done), soft-end threshold, new histories allowed, warps gone
+__shared__ int s_did;                               // set by any warp whose lanes ran an event in the current phase (choose_phase: progress check)
 __shared__ unsigned int s_nphase;
 __shared__ Geom s_g;
 __shared__ float* s_ep_batch;
@@ -480,6 +481,23 @@ __device__ __forceinline__ void annihilate(Lane& L, const TransportParams& P) {
 }
 
 // ---------------------------------------------------------------- K4 interaction
+// Klein-Nishina by epsilon-mixture rejection for a photon of energy L.E: eps = E'/E, t = 1 - cos(theta), x4 = a spare uniform for
+// the azimuth; one Philox block per trial.
+template <bool COUNT>
+__device__ __forceinline__ void sample_kn(Lane& L, const TransportParams& P, float& eps, float& t, float& x4, uint32_t* cnt) {
+    const float k = L.E * (1.0f / kMec2), e0 = rcp(1.0f + 2.0f * k), e02 = e0 * e0;
+    const float a1 = -__logf(e0), a2 = 0.5f * (1.0f - e02);
+#pragma unroll 1
+    for (;;) {
+        const uint4 r = rng_block_hot(L, P);                               // one block per trial
+        const float x1 = u01(r.x), x2 = u01(r.y), x3 = u01(r.z); x4 = u01(r.w);
+        if (COUNT) cnt[12]++;
+        eps = (x1 * (a1 + a2) < a1) ? __expf(-x2 * a1) : sqrtf(fmaf(1.0f - e02, x2, e02));
+        t = __fdividef(1.0f - eps, k * eps);
+        const float g = 1.0f - __fdividef(eps * t * (2.0f - t), 1.0f + eps * eps);
+        if (g >= x3) break;
+    }
+}
 template <bool COUNT>
 __device__ __forceinline__ void interact(Lane& L, const TransportParams& P, const Shared& sh, float xsel, float pe, float co, uint32_t* cnt) {
     const bool coupled = P.ph.mode != 0;
@@ -495,19 +513,8 @@ __device__ __forceinline__ void interact(Lane& L, const TransportParams& P, cons
     }
     if (xsel < pe + co) {                                                  // Compton: Klein-Nishina by epsilon-mixture rejection
         if (COUNT) cnt[4]++;
-        const float k = L.E * (1.0f / kMec2), e0 = rcp(1.0f + 2.0f * k), e02 = e0 * e0;
-        const float a1 = -__logf(e0), a2 = 0.5f * (1.0f - e02);
         float eps, t, x4;
-#pragma unroll 1
-        for (;;) {
-            const uint4 r = rng_block_hot(L, P);                           // one block per trial
-            const float x1 = u01(r.x), x2 = u01(r.y), x3 = u01(r.z); x4 = u01(r.w);
-            if (COUNT) cnt[12]++;
-            eps = (x1 * (a1 + a2) < a1) ? __expf(-x2 * a1) : sqrtf(fmaf(1.0f - e02, x2, e02));
-            t = __fdividef(1.0f - eps, k * eps);
-            const float g = 1.0f - __fdividef(eps * t * (2.0f - t), 1.0f + eps * eps);
-            if (g >= x3) break;
-        }
+        sample_kn<COUNT>(L, P, eps, t, x4, cnt);
         const float ct = 1.0f - t, st = sqrtf(fmaxf(0.0f, t * (2.0f - t)));
         float sp, cp; __sincosf(2.0f * kPi * x4 - kPi, &sp, &cp);
         const float E0 = L.E, E1 = eps * E0, T = E0 - E1;
@@ -925,6 +932,100 @@ __device__ __forceinline__ void charged_event(Lane& L, const TransportParams& P,
     }
 }
 
+// ---------------------------------------------------------------- collimation stage
+// A photon sampled from Phase Space 1 is followed through the jaws and the MLC down to the Phase Space 2 plane (readings
+// A35-A37): inside the w-range of a slab every point outside the opening of its row is tungsten, everything else is air;
+// charged particles are not followed (their energy stays in the head: the ledger's air channel), annihilation quanta born in
+// the head are dropped, a photon that turns upstream or leaves the world sideways has escaped.  The oracle tracks the whole
+// stage by Woodcock flights against the tungsten coefficient; the same distribution costs less here: air gaps and slab
+// crossings that provably stay inside the openings are one exponential flight in air, and only a slab whose tungsten the ray
+// may touch is tracked by Woodcock flights (exact for any arrangement of openings), ended at the slab's faces.
+__device__ __forceinline__ bool head_blocked(const Head& H, int k, float x, float y) {
+    const float across = H.axis[k] == 0 ? y : x, along = H.axis[k] == 0 ? x : y;
+    const float fr = floorf((across - H.row0[k]) * H.inv_pitch[k]);
+    if (!(fr >= 0.0f && fr < (float)H.n_rows[k])) return true;
+    const int r = H.off[k] + (int)fr;
+    return !(along >= __ldg(H.lo + r) && along < __ldg(H.hi + r));
+}
+// does the straight path from (x, y, w) to the bottom face of slab k stay inside the openings of every row it passes?
+__device__ __forceinline__ bool head_clear(const Head& H, int k, float x, float y, float w, float dx, float dy, float dz) {
+    const float t = (H.w1[k] - w) / dz;
+    const float x1 = fmaf(t, dx, x), y1 = fmaf(t, dy, y);
+    const bool ax0 = H.axis[k] == 0;
+    const float a0 = ax0 ? y : x, a1 = ax0 ? y1 : x1, l0 = ax0 ? x : y, l1 = ax0 ? x1 : y1;
+    const float f0 = floorf((fminf(a0, a1) - H.row0[k]) * H.inv_pitch[k]), f1 = floorf((fmaxf(a0, a1) - H.row0[k]) * H.inv_pitch[k]);
+    if (!(f0 >= 0.0f && f1 < (float)H.n_rows[k])) return false;
+    const float lmin = fminf(l0, l1), lmax = fmaxf(l0, l1);
+    for (int r = (int)f0; r <= (int)f1; ++r)
+        if (!(lmin >= __ldg(H.lo + H.off[k] + r) && lmax < __ldg(H.hi + H.off[k] + r))) return false;
+    return true;
+}
+// The lane's photon: (L.x, L.y, L.z) = (u, v, w) and direction in the BEAM frame, dw > 0.  Returns true with the photon on the
+// Phase Space 2 plane; false if it ended in the stage (energy booked).  dep sums what the stage absorbed.
+template <bool COUNT>
+__device__ __noinline__ bool head_stage(Lane& L, const TransportParams& P, const Shared& sh, float& dep, uint32_t* cnt) {
+    const Head& H = P.hd;
+    int k = 0;
+#pragma unroll 1
+    for (;;) {
+        if (L.E < P.ph.pcut) { dep += L.E; L.a_air += L.E; return false; }
+        set_energy(L, P, sh);
+        while (k < H.n_slabs && L.z >= H.w1[k]) ++k;
+        const bool in_slab = k < H.n_slabs && L.z >= H.w0[k];
+        const float w_end = in_slab ? H.w1[k] : (k < H.n_slabs ? H.w0[k] : H.w_ps2);
+        if (!in_slab && k >= H.n_slabs && L.z >= H.w_ps2) return true;
+        const float t_end = fmaxf((w_end - L.z) / L.dz, 0.0f);
+        const uint4 rr = rng_block(L, P);
+        const float nl = -__logf(u01(rr.x)), u2 = u01(rr.y);
+        float pe, co, pp;
+        mu3(P, sh, 0, L.ci, L.ct, L.E, pe, co, pp);
+        const float mta = pe + co + pp, mua = kRhoAir * mta;
+        float xsel;
+        bool tungsten = false;
+        if (!(in_slab && !head_clear(H, k, L.x, L.y, L.z, L.dx, L.dy, L.dz))) {
+            // air gap, or a slab crossed inside its openings: one exponential flight in air up to the next plane
+            if (!(nl < mua * t_end)) {
+                L.x = fmaf(t_end, L.dx, L.x); L.y = fmaf(t_end, L.dy, L.y); L.z = w_end;
+                if (!(fabsf(L.x) < kWorldHalf && fabsf(L.y) < kWorldHalf)) { L.a_esc += L.E; return false; }
+                if (in_slab) ++k;
+                continue;
+            }
+            const float s = __fdividef(nl, mua);
+            L.x = fmaf(s, L.dx, L.x); L.y = fmaf(s, L.dy, L.y); L.z = fminf(fmaf(s, L.dz, L.z), w_end);
+            xsel = u2 * mta;
+        } else {
+            // Woodcock flight inside slab k against the tungsten coefficient
+            float pw, cw, ppw;
+            mu3(P, sh, H.mat, L.ci, L.ct, L.E, pw, cw, ppw);
+            const float mtw = pw + cw + ppw, muw = H.rho * mtw, mm = fmaxf(muw, mua) * 1.0001f;
+            if (!(nl < mm * t_end)) {
+                L.x = fmaf(t_end, L.dx, L.x); L.y = fmaf(t_end, L.dy, L.y); L.z = w_end; ++k;
+                if (!(fabsf(L.x) < kWorldHalf && fabsf(L.y) < kWorldHalf)) { L.a_esc += L.E; return false; }
+                continue;
+            }
+            const float s = __fdividef(nl, mm);
+            L.x = fmaf(s, L.dx, L.x); L.y = fmaf(s, L.dy, L.y); L.z = fminf(fmaf(s, L.dz, L.z), w_end);
+            tungsten = head_blocked(H, k, L.x, L.y);
+            const float acc = u2 * mm;
+            if (!(acc < (tungsten ? muw : mua))) continue;                 // virtual collision
+            xsel = tungsten ? __fdividef(acc, H.rho) : __fdividef(acc, kRhoAir);   // reuse the accept draw for the channel (reading A8)
+            if (tungsten) { pe = pw; co = cw; }
+        }
+        if (!(fabsf(L.x) < kWorldHalf && fabsf(L.y) < kWorldHalf)) { L.a_esc += L.E; return false; }
+        if (COUNT) cnt[11]++;
+        if (xsel < pe || !(xsel < pe + co)) { dep += L.E; L.a_air += L.E; return false; }   // photoelectric, or pair: all of E stays (A36)
+        float eps, t, x4;
+        sample_kn<COUNT>(L, P, eps, t, x4, cnt);
+        const float ct = 1.0f - t, st = sqrtf(fmaxf(0.0f, t * (2.0f - t)));
+        float sp, cp; __sincosf(2.0f * kPi * x4 - kPi, &sp, &cp);
+        const float E1 = eps * L.E, T = L.E - E1;
+        dep += T; L.a_air += T;
+        L.E = E1;
+        rotate(L.dx, L.dy, L.dz, ct, st, cp, sp);
+        if (!(L.dz > 0.0f)) { L.a_esc += L.E; return false; }              // turned upstream: out of the stage
+    }
+}
+
 // ---------------------------------------------------------------- K1 source
 __device__ __forceinline__ uint32_t upper_bound_u32(const uint32_t* a, uint32_t n, uint32_t key) {   // #{k in [0,n): a[k] <= key}
     uint32_t lo = 0, hi = n;
@@ -964,11 +1065,11 @@ __device__ __forceinline__ SourceSample sample_source(const TransportParams& P, 
 
 // ---------------------------------------------------------------- the kernel
 // Add the warp's sum of v to *dst (lane 0); all lanes must call.
-__device__ __noinline__ void ledger_add(float v, double* dst) {
+__device__ __noinline__ void ledger_add(float v, double* dst, bool atomic = false) {
     if (__ballot_sync(FULL_MASK, v != 0.0f) == 0u) return;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL_MASK, v, o);
-    if ((threadIdx.x & 31u) == 0) *dst += (double)v;
+    if ((threadIdx.x & 31u) == 0) { if (atomic) atomicAdd(dst, (double)v); else *dst += (double)v; }
 }
 __device__ __forceinline__ void ledger_flush(Lane& L, double* led) {
     ledger_add(L.a_emit, led + 0); ledger_add(L.a_ph, led + 1); ledger_add(L.a_eps, led + 2);
@@ -988,6 +1089,16 @@ __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned lon
 #pragma unroll
     for (int c = 0; c < kClasses; ++c) n_live += n[c];
     s_live = n_live;                                           // between phases every particle sits in a queue and no lane holds a credit
+    // Progress check: the last phase ran no event although particles wait.  Every lane that could have run one parked its
+    // particle for want of a head-room credit, and if no other class can run, nothing will ever give one back (possible with
+    // a small aepid_set_live_limit and many pair / annihilation / bremsstrahlung photons).  The limit set by the caller is a
+    // soft one: raise it, up to the hard bound the queue protocol needs (half a class queue); beyond that the error is flagged.
+    if (s_nphase > 0u && s_did == 0 && n_live > 0) {
+        const int hard = (1 << P.pool_log) / 2;
+        if (s_live_max < hard) s_live_max = min(2 * s_live_max, hard);
+        else if (n[C_E] + n[C_X] + n[C_A] == 0) { raise_error(8); for (int r = 0; r < kRings; ++r) n[r] = 0; s_flag[0] = 1; }
+    }
+    s_did = 0;
     const int nf = s_live_max - n_live;
     bool more = s_flag[0] == 0;
     int budget = 0;
@@ -1030,7 +1141,8 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
     constexpr bool C2 = PH >= 2;
     constexpr bool kSpawns = C == C_W || C == C_P || (C2 && (C == C_E || C == C_X));   // classes whose events create secondaries all the time
     const int keep = *((volatile int*)&s_keep);
-    bool leaving = false, park = false;
+    bool leaving = false, park = false, did = false;
+    float h_n = 0.0f, h_E = 0.0f, h_dep = 0.0f;                 // collimation stage (class A only): Phase Space 2 particles, their energy, absorbed
     // every lane enters a phase empty: saying so lets the compiler drop what this class never touches from the registers
     L.a_emit = L.a_ph = L.a_eps = L.a_epo = L.a_air = L.a_esc = 0.0f;
     L.alive = false; L.counted = kNone; L.spare = kNone; L.pval = 0.0f; L.pidx = kNone;
@@ -1093,15 +1205,36 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                         else {
                             L.h = h; L.pid = 0; L.blk = 0;
                             const uint4 r = rng_block(L, P);               // block 0 of particle 0: E, pixel, u, v (reading A1)
-                            const SourceSample s = sample_source(P, r.x, r.y, r.z, r.w);
-                            L.x = P.g.src[0]; L.y = P.g.src[1]; L.z = P.g.src[2];
-                            L.dx = s.dx; L.dy = s.dy; L.dz = s.dz; L.E = s.E;
                             L.vox = 0;
                             L.flags = T_PHOTON | (R_AIR << 2) | (min(h / P.hist_per_batch, (uint32_t)P.n_batches - 1u) << 16);
                             L.alive = true; L.counted = 1u;
                             L.pval = 0.0f; L.pidx = kNone;
-                            L.a_emit += s.E;
-                            set_energy(L, P, sh);
+                            if (P.hd.n_ps1 == 0u) {
+                                const SourceSample s = sample_source(P, r.x, r.y, r.z, r.w);
+                                L.x = P.g.src[0]; L.y = P.g.src[1]; L.z = P.g.src[2];
+                                L.dx = s.dx; L.dy = s.dy; L.dz = s.dz; L.E = s.E;
+                                L.a_emit += s.E;
+                                set_energy(L, P, sh);
+                            } else {
+                                // Phase Space 1 source (reading A35): record floor(xi0 n), xi0 = (r + 0.5) 2^-32 = the first draw of block 0
+                                const uint32_t j = (uint32_t)((((unsigned long long)r.x * 2ull + 1ull) * (unsigned long long)P.hd.n_ps1) >> 33);
+                                const float4 qa = __ldg(P.hd.ps1 + 2 * (size_t)j), qb = __ldg(P.hd.ps1 + 2 * (size_t)j + 1);
+                                const float inv = rsqrtf(qa.z * qa.z + qa.w * qa.w + qb.x * qb.x);
+                                L.x = qa.x; L.y = qa.y; L.z = P.hd.w_ps1;
+                                L.dx = qa.z * inv; L.dy = qa.w * inv; L.dz = qb.x * inv; L.E = qb.y;
+                                L.a_emit += L.E;
+                                const bool through = P.hd.n_slabs > 0 ? head_stage<COUNT>(L, P, sh, h_dep, cnt) : true;
+                                if (through) {
+                                    h_n += 1.0f; h_E += L.E;
+                                    if (COUNT) cnt[10]++;
+                                    float x, y, z;                         // beam frame -> world frame
+                                    dir_to_world(P.g, L.x, L.y, L.z, x, y, z);
+                                    L.x = x + P.g.src[0]; L.y = y + P.g.src[1]; L.z = z + P.g.src[2];
+                                    dir_to_world(P.g, L.dx, L.dy, L.dz, x, y, z);
+                                    L.dx = x; L.dy = y; L.dz = z;
+                                    set_energy(L, P, sh);
+                                } else L.alive = false;                    // ended in the head: the lane's count goes back in section A
+                            }
                         }
                     }
                     if (COUNT && !kPhaseClock && lane == 0) cnt[30]++;
@@ -1134,6 +1267,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
         } else if (C == C_E || C == C_X) {
             if (on && F_TYPE(L.flags) == T_POSITRON && L.E <= P.ph.ecut && !ensure_spare(L)) { park = true; on = false; if (COUNT && !kPhaseClock) cnt[29]++; }   // annihilation needs a credit
         }
+        did |= on;
         if (C == C_W) {
             // K3 + K4: flights against the majorant until at least kHitMin lanes have a collision to sample (or nobody flies
             // any more), then the interactions together: keeps both halves of the event well filled when few flights collide
@@ -1172,6 +1306,10 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
     }
     if (L.spare != kNone) { atomicSub(&s_live, 1); L.spare = kNone; }
     ledger_flush(L, led);
+    if (C == C_A && P.hd.n_ps1 != 0u) {
+        ledger_add(h_n, P.hd.stats + 0, true); ledger_add(h_E, P.hd.stats + 1, true); ledger_add(h_dep, P.hd.stats + 2, true);
+    }
+    if (__any_sync(FULL_MASK, did) && lane == 0) s_did = 1;
     if (lane == 0) atomicAdd(&s_left, 1);
 }
 
@@ -1195,7 +1333,7 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
         s_g = P.g; s_ep_batch = P.ep_batch; s_npix = P.npix; s_nphase = 0u;
         s_pool_log = P.pool_log; s_pool_mask = (1u << P.pool_log) - 1u;
         s_queue = P.queues + (((size_t)blockIdx.x * kClasses) << P.pool_log) * 3;
-        s_live = 0; s_live_max = min(max(P.live_max, 64), (1 << P.pool_log) / 2);
+        s_live = 0; s_live_max = min(max(P.live_max, 64), (1 << P.pool_log) / 2); s_did = 0;
     }
     __syncthreads();
 

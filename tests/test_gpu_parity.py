@@ -318,6 +318,27 @@ def test_results_do_not_depend_on_the_live_limit(name, shrink, n):
         assert np.allclose(r["epid_mean"], res[0]["epid_mean"], rtol=1e-3, atol=1e-9)
 
 
+@pytest.mark.parametrize("mode", [1, 3])
+def test_tiny_live_limit_with_pair_and_bremsstrahlung_photons(mode):
+    """with room for only 64 live particles per CTA and a workload that multiplies photons (10 MeV photons on
+    Gd2O2S: pair production, annihilation, in mode 3 bremsstrahlung) every lane can end up parked for want of a credit.  The
+    scheduler notices a phase without progress and raises the (soft) limit; the results are those of the default limit and
+    no error flag is raised."""
+    cfg = slab_cfg(n=(8, 8, 8), h=(4.0, 4.0, 2.5), rho=7.32, mat=5, E=10.0, mode=mode, epid="C1", field_cm=2.0)
+    res = []
+    for lim in (0, 64, 100):
+        eng = engine_for(cfg)
+        eng.set_live_limit(lim)
+        eng.simulate(300_000, 11)
+        r = eng.read_tallies()                              # AepidError INTERNAL if the kernel had flagged a stall
+        check_ledger(r["ledger"], 300_000)
+        res.append(r)
+        eng.close()
+    for r in res[1:]:
+        assert np.allclose(r["ledger"][:6], res[0]["ledger"][:6], rtol=2e-6)
+        assert np.allclose(r["phantom_mean"], res[0]["phantom_mean"], rtol=1e-3, atol=1e-9)
+
+
 def test_more_histories_than_32_bits():
     """4.5e9 histories of C0 in one aepid_simulate call (split into launches below 2^32 inside the library): every history is
     run, the ledger closes, the float32 tallies still reproduce the double ledger (B batch buffers)."""
