@@ -121,7 +121,11 @@ int aepid_load_source(aepid_ctx* ctx, const float src_pos_cm[3], const float bea
  * power below it;
  * mode 3: mode 2 plus bremsstrahlung (reading A32): photons above the photon cut-off are emitted as discrete events along the
  * particle's direction, the loss to softer photons is continuous; the spectrum (4/3 - 4/3 y + y^2) / (X0 k), y = k / T, makes the
- * total radiative stopping power T / X0.  Modes 2 and 3 need aepid_set_class2.  Cutoffs PAPER.md:104 (defaults 0.010 / 0.200 MeV); step rule f_E = 0.10,
+ * total radiative stopping power T / X0.  Modes 2 and 3 need aepid_set_class2;
+ * mode 4: the physics of mode 1 with DPM-style steps ("developed based on DPM"; reading A38): a step loses f_E T in two
+ * legs split at a uniformly drawn hinge where the Highland deflection of the whole step is applied; voxel, layer and region faces
+ * end straight segments (each deposits rho S ds of its own medium), not steps; s_max is not used.  The class queues hold half as
+ * many (64-byte) records in this mode.  Cutoffs PAPER.md:104 (defaults 0.010 / 0.200 MeV); step rule f_E = 0.10,
  * s_max = 1 cm (reading A13). */
 int aepid_set_physics(aepid_ctx* ctx, int mode, float photon_cut_MeV, float electron_cut_MeV,
                       float f_E, float s_max_cm);

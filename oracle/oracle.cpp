@@ -818,6 +818,102 @@ void transport_electron(Ctx& c, Particle p, const Run& r) {
     }
 }
 
+// ---------------------------------------------------------------- mode 4: multi-voxel condensed-history steps with a random hinge
+// the patient transport "was developed based on DPM", a Class II condensed-history code whose electron steps cross
+// voxel boundaries and are split at a random hinge.  The paper says no more; reading A38 in the notation of SURVEY 8(c)
+// step 4, with the physics of mode 1 (CSDA loss, Highland deflection, no discrete events):
+//   * a STEP is an energy loss dE_k = f_E T_k (T_k = energy at its start); faces do not end it;
+//   * at its start one Philox block gives xi (hinge position) and (xi_a, xi_b) (deflection): the step is travelled in two LEGS,
+//     losing xi dE_k before and (1 - xi) dE_k after the HINGE, where the direction is rotated by the polar angle
+//     min(pi, theta0 sqrt(-2 ln xi_a)) and the azimuth 2 pi xi_b;
+//   * theta0 is Highland's width for the whole step in the medium m where the hinge lies (the medium of the segment that ends
+//     the first leg): mass thickness dE_k / S_m(T_k - dE_k / 2) (density cancels), mid-step energy T_k - dE_k / 2;
+//   * a leg is a chain of straight SEGMENTS, each ending on a voxel / layer / region face or where the leg's energy budget R is
+//     used up: ds = R / (rho S_m(T - R/2)) if that is nearer than the face (the segment then loses exactly R), else the distance
+//     to the face with the midpoint-rule loss of mode 1; every segment deposits its loss in the voxel / pixel (mid-point, A24) /
+//     scalar it lies in; crossing a face changes the voxel index / layer / region exactly as in mode 1;
+//   * T <= T_cut ends the track as in mode 1; s_max is not used.
+void transport_electron_hinge(Ctx& c, Particle p, const Run& r) {
+    c.counters[14]++;
+    double R = 0.0, R_after = 0.0, dEk = 0.0, Tm = 0.0, xa = 0.5, xb = 0.0;   // budget of the current leg and of the leg after the hinge; the step's loss, mid energy and deflection draws
+    bool before_hinge = false;
+    for (;;) {
+        if (p.E <= c.electron_cut) {                                // PAPER.md:104 (200 keV): local deposit
+            deposit_here(c, p, p.E);
+            if (p.type == POSITRON) annihilate(c, p, r);
+            return;
+        }
+        double rho; int m; double tb = INF; int kind = -1, axis = -1; AirHit hb{INF, 0, -1};
+        if (p.region == AIR) {
+            rho = RHO_AIR; m = MAT_AIR; hb = air_boundary(c, p); tb = hb.t;
+        } else if (p.region == PHANTOM) {
+            const size_t vi = vox_index(c, p.iv); rho = c.rho[vi]; m = c.mat[vi];
+            for (int a = 0; a < 3; ++a) {
+                const double da = comp(p.dir, a);
+                double t = INF;
+                if (da > 0) t = (c.org[a] + (p.iv[a] + 1) * c.h[a] - comp(p.pos, a)) / da;
+                else if (da < 0) t = (c.org[a] + p.iv[a] * c.h[a] - comp(p.pos, a)) / da;
+                if (t < tb) { tb = t; axis = a; }
+            }
+            if (tb < 0) tb = 0;
+        } else {
+            const int l = p.layer; rho = c.lrho[l]; m = c.lmat[l];
+            double tf = INF;
+            if (p.dir.z > 0) tf = (c.ztop[l + 1] - p.pos.z) / p.dir.z;
+            else if (p.dir.z < 0) tf = (c.ztop[l] - p.pos.z) / p.dir.z;
+            if (tf < 0) tf = 0;
+            const double tl = world_exit_lateral(p.pos, p.dir);
+            if (tl < tf) { tb = tl; kind = 2; } else { tb = tf; kind = 0; }
+        }
+        if (!(R > 0.0) && !before_hinge) {                          // a new step starts here, in this medium
+            dEk = c.f_E * p.E; Tm = p.E - 0.5 * dEk;
+            const double xi = p.rng.u(); xa = p.rng.u(); xb = p.rng.u();
+            p.rng.skip_block();                                     // one block per step
+            R = xi * dEk; R_after = dEk - R; before_hinge = true;
+            c.counters[15]++;                                       // (mode 4: counter 15 counts steps, counters 6-8 segments)
+        }
+        // one segment: to the face, or to where the leg's budget is used up
+        const double s_R = R / (rho * stop_pow(c, m, p.E - 0.5 * R));
+        const bool on_face = !(s_R < tb);
+        const double s = on_face ? tb : s_R;
+        const double dE = on_face ? std::min(p.E, rho * s * stop_pow(c, m, p.E - 0.5 * rho * s * stop_pow(c, m, p.E))) : R;
+        const Vec3 mid = p.pos + (0.5 * s) * p.dir;
+        p.pos = p.pos + s * p.dir;
+        if (p.region == AIR) { dep_air(c, dE); c.counters[7]++; }
+        else if (p.region == PHANTOM) { dep_phantom(c, p.iv, dE); c.counters[6]++; }
+        else { dep_epid(c, p.layer, mid.x, mid.y, dE); c.counters[8]++; }
+        p.E -= dE; R -= dE;
+        c.aux[0] += s; c.aux[1] += rho * s;
+        if (on_face) {
+            const double e_out = p.E + (p.type == POSITRON ? 2.0 * MEC2 : 0.0);
+            if (p.region == AIR) {
+                if (hb.kind == 0) enter_phantom(c, p, 0.0, hb.axis);
+                else if (hb.kind == 1) enter_epid(c, p, 0.0);
+                else { escape(c, e_out); return; }
+            } else if (p.region == PHANTOM) {
+                const bool up = comp(p.dir, axis) > 0;
+                setcomp(p.pos, axis, c.org[axis] + (p.iv[axis] + (up ? 1 : 0)) * c.h[axis]);
+                p.iv[axis] += up ? 1 : -1;
+                if (p.iv[axis] < 0 || p.iv[axis] >= c.n[axis]) {
+                    p.iv[axis] = std::min(std::max(p.iv[axis], 0), c.n[axis] - 1);
+                    p.region = AIR;
+                }
+            } else {
+                if (kind == 2) { escape(c, e_out); return; }
+                const int l = p.layer;
+                if (p.dir.z > 0) { p.pos.z = c.ztop[l + 1]; p.layer = l + 1; if (p.layer >= c.n_layers) { escape(c, e_out); return; } }
+                else { p.pos.z = c.ztop[l]; p.layer = l - 1; if (p.layer < 0) epid_to_air(c, p); }
+            }
+        }
+        if (!(R > 0.0) && before_hinge) {                           // the hinge: deflect (medium m of the segment just travelled), then the second leg
+            const double th0 = highland_theta0(c, m, dEk / stop_pow(c, m, Tm), Tm);
+            const double th = std::min(PI, th0 * std::sqrt(-2.0 * std::log(xa))), phi = 2.0 * PI * xb;
+            p.dir = rotate(p.dir, std::cos(th), std::sin(th), phi);
+            R = R_after; before_hinge = false;
+        }
+    }
+}
+
 // ---------------------------------------------------------------- collimation stage (section 2.1.1)
 // "Particles are sampled from Phase Space 1 and transported through the jaws and MLC ... The resulting phase space (Phase Space
 // 2) is ... streamed directly into the next simulation stage."  Readings (A35-A37): the stage lies between the planes
@@ -900,7 +996,7 @@ int check_ready(Ctx& c) {
     if (c.n_layers <= 0) { c.err = "load_epid_layers not called"; return -2; }
     if (c.fu <= 0) { c.err = "load_source not called"; return -2; }
     if (c.have_col && c.n_ps1 == 0) { c.err = "a collimator needs a phase-space source"; return -2; }
-    if (c.mode >= 2 && (int)c.ne.size() != c.n_mat) { c.err = "mode 2 needs orc_set_class2 (electrons per gram)"; return -2; }
+    if ((c.mode == 2 || c.mode == 3) && (int)c.ne.size() != c.n_mat) { c.err = "modes 2 and 3 need orc_set_class2 (electrons per gram)"; return -2; }
     // phantom AABB must lie inside the air part of the world box
     for (int k = 0; k < 8; ++k) {
         Vec3 p{c.org[0] + ((k & 1) ? c.n[0] * c.h[0] : 0), c.org[1] + ((k & 2) ? c.n[1] * c.h[1] : 0), c.org[2] + ((k & 4) ? c.n[2] * c.h[2] : 0)};
@@ -1063,7 +1159,7 @@ int orc_run(orc_ctx* x, uint64_t first, uint64_t n, uint64_t seed) {
             if (through) c.stack.push_back(p);
             while (!c.stack.empty()) {
                 Particle q2 = c.stack.back(); c.stack.pop_back();
-                if (q2.type == PHOTON) transport_photon(c, q2, r); else transport_electron(c, q2, r);
+                if (q2.type == PHOTON) transport_photon(c, q2, r); else if (c.mode == 4) transport_electron_hinge(c, q2, r); else transport_electron(c, q2, r);
             }
             flush_history(c);
             continue;
@@ -1088,7 +1184,7 @@ int orc_run(orc_ctx* x, uint64_t first, uint64_t n, uint64_t seed) {
         while (!c.stack.empty()) {                                  // LIFO
             c.counters[11] = std::max<uint64_t>(c.counters[11], c.stack.size());
             Particle q = c.stack.back(); c.stack.pop_back();
-            if (q.type == PHOTON) transport_photon(c, q, r); else transport_electron(c, q, r);
+            if (q.type == PHOTON) transport_photon(c, q, r); else if (c.mode == 4) transport_electron_hinge(c, q, r); else transport_electron(c, q, r);
         }
         flush_history(c);
     }

@@ -310,7 +310,9 @@ int fill_params(aepid_ctx* ctx, TransportParams& p) {
     p.ledger = ctx->d_ledger(); p.counters = ctx->d_counters(); p.hist_counter = ctx->d_chunk();
     p.queues = reinterpret_cast<uint4*>(ctx->ws + ctx->lay.queues);
     p.n_batches = ctx->dims.n_batches; p.nvox = ctx->lay.nvox; p.npix = ctx->lay.npix; p.live_max = ctx->live_max;
-    p.pool_log = ctx->pool_log;
+    // physics mode 4 carries 64-byte records (the leg's energy budget): half as many fit the class queues
+    p.pool_log = ctx->ph.mode == 4 ? ctx->pool_log - 1 : ctx->pool_log;
+    if (ctx->ph.mode == 4) p.live_max = std::min(p.live_max, (1 << p.pool_log) / 2);
     p.hd = ctx->hd; p.hd.stats = ctx->d_head_stats(); p.hd.ps1 = ctx->d_ps1();
     p.hd.lo = ctx->d_head_rows(); p.hd.hi = ctx->d_head_rows() + kMaxHeadRows;
     if (p.hd.n_slabs > 0 && p.hd.n_ps1 == 0) return fail(ctx, AEPID_ERR_BAD_STATE, "a collimator needs a phase-space source (aepid_load_phase_space_source)");
@@ -514,7 +516,7 @@ int aepid_load_source(aepid_ctx* ctx, const float src[3], const float axes[9], i
 
 int aepid_set_physics(aepid_ctx* ctx, int mode, float pcut, float ecut, float fE, float smax) {
     if (!ctx) return AEPID_ERR_BAD_ARG;
-    if (mode < 0 || mode > 3 || !(pcut > 0) || !(ecut > 0) || !(fE > 0) || !(fE <= 0.5f) || !(smax > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "physics parameters out of range");
+    if (mode < 0 || mode > 4 || !(pcut > 0) || !(ecut > 0) || !(fE > 0) || !(fE <= 0.5f) || !(smax > 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "physics parameters out of range");
     if (ecut != ctx->ph.ecut || pcut != ctx->ph.pcut || mode != ctx->ph.mode) ctx->tables_dirty = true;   // the restricted stopping powers depend on the cut-offs and the mode
     ctx->ph.mode = mode; ctx->ph.pcut = pcut; ctx->ph.ecut = ecut; ctx->ph.fE = fE; ctx->ph.smax = smax;
     return 0;

@@ -109,6 +109,7 @@ enum : int { C_A = 0, C_W = 1, C_E = 2, C_P = 3, C_X = 4, kClasses = 5, kRings =
 #define F_REGION(f) (((f) >> 2) & 3u)
 #define F_LAYER(f) (((f) >> 4) & 7u)
 #define F_HIT (1u << 7)
+#define F_LEGA (1u << 8)      // physics mode 4: a charged particle on the first leg of its step (before the hinge)
 #define F_BATCH(f) (((f) >> 16) & 255u)
 #define SET_TYPE(f, t) ((f) = ((f) & ~3u) | (t))
 #define SET_REGION(f, r) ((f) = ((f) & ~(3u << 2)) | ((r) << 2))
@@ -128,7 +129,9 @@ __shared__ unsigned int s_head[kRings];             // tickets handed to poppers
 __shared__ unsigned int s_snap[kRings];             // tail at the last barrier: pops stay below it
 __shared__ int s_flag[2];                           // [0] no histories left, [1] error bits
 __shared__ int s_phase, s_keep, s_budget, s_left;   // class of the phase (-1: done), soft-end threshold, new histories allowed, warps gone
-__shared__ int s_did;                               // set by any warp whose lanes ran an event in the current phase (choose_phase: progress check)
+__shared__ int s_stuck;                             // bit c: class c was stuck in its last phase (choose_phase: progress check)
+__shared__ int s_did, s_parked;                     // set by any warp whose lanes ran an event / parked a particle for want of a credit in the
+                                                    // current phase (choose_phase: progress check)
 __shared__ unsigned int s_nphase;
 __shared__ Geom s_g;
 __shared__ float* s_ep_batch;
@@ -140,7 +143,8 @@ extern __shared__ __align__(16) unsigned char smem_raw[];   // per-warp ledger |
 
 __shared__ uint32_t s_pool_mask;                    // records per class queue - 1
 __shared__ int s_pool_log;
-__device__ __forceinline__ uint4* queue_rec(int r, uint32_t ticket) { return s_queue + ((((size_t)r) << s_pool_log) + (ticket & s_pool_mask)) * 3; }
+__shared__ uint32_t s_rec_vec;                      // 16-byte vectors per particle record: 3, or 4 in physics mode 4 (the leg's energy budget)
+__device__ __forceinline__ uint4* queue_rec(int r, uint32_t ticket) { return s_queue + ((((size_t)r) << s_pool_log) + (ticket & s_pool_mask)) * s_rec_vec; }
 struct Shared {
     const float4* phot;
     const float* maj;
@@ -157,6 +161,7 @@ struct Lane {
     uint32_t cw, vlin;              // packed word and linear index of the current voxel (charged particle in PHANTOM)
     int ci; float ct, mumaj;        // photon: table cell, fraction, majorant at E
     uint32_t pidx; float pval;      // pending phantom deposit (merged while the voxel does not change)
+    float R;                        // physics mode 4: energy the particle still loses on the current leg of its step
     uint32_t counted;               // 1: the lane holds a particle that is counted in s_live (alive, or dead and not yet released); kNone: none
     uint32_t spare;                 // 1: the lane holds a head-room credit for its next secondary (kNone: none)
     float a_emit, a_ph, a_eps, a_epo, a_air, a_esc;   // ledger sums since the last flush
@@ -438,12 +443,13 @@ __device__ __noinline__ int budget_claim(int want) {
 
 // Append a particle record to the queue of its class (one lane, divergent code); visible to poppers after the next barrier.
 __device__ __noinline__ void queue_particle(float x, float y, float z, float dx, float dy, float dz, float E,
-                                            uint32_t vox, uint32_t flags, uint32_t h, uint32_t pid, uint32_t blk) {
+                                            uint32_t vox, uint32_t flags, uint32_t h, uint32_t pid, uint32_t blk, float R = 0.0f) {
     const int r = class_of(flags);
     uint4* rec = queue_rec(r, atomicAdd(s_tail + r, 1u));
     __stcs(rec + 0, make_uint4(__float_as_uint(x), __float_as_uint(y), __float_as_uint(z), __float_as_uint(dx)));
     __stcs(rec + 1, make_uint4(__float_as_uint(dy), __float_as_uint(dz), __float_as_uint(E), vox));
     __stcs(rec + 2, make_uint4(flags, h, pid, blk));
+    if (s_rec_vec == 4u) __stcs(rec + 3, make_uint4(__float_as_uint(R), 0u, 0u, 0u));
 }
 // Head room: s_live counts the particles alive in the CTA plus the credits lanes hold for secondaries they may create; it
 // never exceeds kLiveMax, which is what keeps every queue from wrapping onto unread records (header comment).  A lane
@@ -473,7 +479,7 @@ __device__ __forceinline__ void annihilate(Lane& L, const TransportParams& P) {
     const float ct = 2.0f * u01(r.x) - 1.0f, st = sqrtf(fmaxf(0.0f, 1.0f - ct * ct));
     float sp, cp; __sincosf(2.0f * kPi * u01(r.y) - kPi, &sp, &cp);
     const float dx = st * cp, dy = st * sp, dz = ct;
-    uint32_t f = L.flags; SET_TYPE(f, T_PHOTON);
+    uint32_t f = L.flags & ~F_LEGA; SET_TYPE(f, T_PHOTON);
     spawn_from(L, L.x, L.y, L.z, -dx, -dy, -dz, kMec2, f, child_id(L, 1));
     L.pid = child_id(L, 0); L.blk = 0;
     L.flags = f;
@@ -506,7 +512,7 @@ __device__ __forceinline__ void interact(Lane& L, const TransportParams& P, cons
         if (COUNT) cnt[3]++;
         if (!coupled || L.E <= P.ph.ecut) { if (COUNT && coupled) { cnt[9]++; cnt[14]++; } dep_here(L, P, L.E); L.alive = false; return; }
         SET_TYPE(L.flags, T_ELECTRON);
-        L.pid = child_id(L, 0); L.blk = 0;
+        L.pid = child_id(L, 0); L.blk = 0; L.R = 0.0f;
         if (COUNT) { cnt[9]++; cnt[14]++; }
         if (reg == R_PHANTOM) { world_to_frac(P.g, L.vox, L.x, L.y, L.z); }
         return;
@@ -557,7 +563,7 @@ __device__ __forceinline__ void interact(Lane& L, const TransportParams& P, cons
     if (reg == R_PHANTOM) world_to_frac(P.g, L.vox, L.x, L.y, L.z);
     spawn_from(L, L.x, L.y, L.z, L.dx, L.dy, L.dz, Tp, fpos, id1);
     SET_TYPE(L.flags, T_ELECTRON);
-    L.pid = id0; L.blk = 0;
+    L.pid = id0; L.blk = 0; L.R = 0.0f;
     L.E = Tm;
 }
 
@@ -691,7 +697,7 @@ __device__ __forceinline__ StepLoss step_loss(Lane& L, const TransportParams& P,
     StepLoss r;
     r.s = fminf(tb, fminf(__fdividef(P.ph.fE * T, rho * S), P.ph.smax));
     r.hard = false; r.sig = 0.0f; r.sigb = 0.0f;
-    if (PH >= 2) {
+    if (PH == 2 || PH == 3) {
         float f = (__logf(T) - P.tb.lnT0) * P.tb.inv_dlnT;
         f = fminf(fmaxf(f, 0.0f), (float)(P.tb.n_T - 1));
         const int i = min((int)f, P.tb.n_T - 2);
@@ -796,7 +802,7 @@ __device__ __forceinline__ void stop_charged(Lane& L, const TransportParams& P, 
 // pending deposit of the lane belongs to the current voxel (L.pidx == L.vlin, set when the particle is loaded).
 template <bool COUNT, int PH>
 __device__ __forceinline__ void electron_step_phantom(Lane& L, const TransportParams& P, const Shared& sh, uint32_t ra, uint32_t rb, uint32_t rh, uint32_t rw, uint32_t* cnt) {
-    constexpr bool C2 = PH >= 2, PHANTOM_FRAME = true;
+    constexpr bool C2 = PH == 2 || PH == 3, PHANTOM_FRAME = true;
     const Geom& g = P.g;
     const float rho = __uint_as_float(L.cw & ~31u); const int m = (int)(L.cw & 31u);
     // distance to the voxel face in the direction of travel, per axis (a vanishing component gives a huge distance)
@@ -844,7 +850,7 @@ __device__ __forceinline__ void electron_step_phantom(Lane& L, const TransportPa
 // one step in the air or inside the EPID (the particle is above its cutoff)
 template <bool COUNT, int PH>
 __device__ __forceinline__ void electron_step_outside(Lane& L, const TransportParams& P, const Shared& sh, uint32_t ra, uint32_t rb, uint32_t rh, uint32_t rw, uint32_t* cnt) {
-    constexpr bool C2 = PH >= 2, PHANTOM_FRAME = false;
+    constexpr bool C2 = PH == 2 || PH == 3, PHANTOM_FRAME = false;
     const Geom& g = P.g;
     const bool in_air = F_REGION(L.flags) == R_AIR;
     float rho, tb; int m, axis = 0, kind = 0;
@@ -905,11 +911,144 @@ __device__ __forceinline__ void electron_step_outside(Lane& L, const TransportPa
         } else if (L.E > 2.0f * P.ph.ecut) moller_event<COUNT>(L, P, cnt);
     }
 }
+// ---------------------------------------------------------------- physics mode 4 (reading A38): multi-voxel steps with a random hinge
+// A step loses dE_k = f_E T_k in two legs, xi dE_k before the hinge and the rest after it; faces end SEGMENTS, not steps.  The
+// lane carries the budget of its leg (L.R) and the leg bit (F_LEGA); everything else about the step is recomputed at the hinge
+// from the step's own Philox block (the last one the particle drew): xi gives T_k = T / (1 - xi f_E), (xi_a, xi_b) the deflection.
+__device__ __forceinline__ void hinge_begin_step(Lane& L, const TransportParams& P) {
+    const uint4 r = rng_block_hot(L, P);
+    L.R = u01(r.x) * P.ph.fE * L.E;
+    L.flags |= F_LEGA;
+}
+__device__ __forceinline__ void hinge_deflect(Lane& L, const TransportParams& P, const Shared& sh, int m) {
+    L.blk--;                                                               // the step's block again: (xi, xi_a, xi_b)
+    const uint4 r = rng_block_hot(L, P);
+    const float xi = u01(r.x);
+    const float Tk = __fdividef(L.E, 1.0f - xi * P.ph.fE), dEk = P.ph.fE * Tk, Tm = Tk - 0.5f * dEk;
+    float ct, st, cp, sp;
+    highland(sh, m, __fdividef(dEk, stop_pow(P, sh, m, Tm)), Tm, r.y, r.z, ct, st, cp, sp);
+    rotate(L.dx, L.dy, L.dz, ct, st, cp, sp);
+    L.R = (1.0f - xi) * dEk;
+    L.flags &= ~F_LEGA;
+}
+// length and loss of one segment in medium (rho, m): to the face at tb, or to where the leg's budget is used up
+struct Segment { float s, dE; bool on_face; };
+__device__ __forceinline__ Segment hinge_segment(Lane& L, const TransportParams& P, const Shared& sh, int m, float rho, float tb) {
+    Segment g;
+    const float T = L.E;
+    const float sR = __fdividef(L.R, rho * stop_pow(P, sh, m, T - 0.5f * L.R));
+    g.on_face = !(sR < tb);
+    if (g.on_face) {
+        const float S = stop_pow(P, sh, m, T);
+        g.s = tb;
+        g.dE = fminf(T, rho * tb * stop_pow(P, sh, m, T - 0.5f * rho * tb * S));   // midpoint rule, as in mode 1
+        L.R -= g.dE;
+    } else { g.s = sR; g.dE = fminf(L.R, T); L.R = 0.0f; }
+    const float Tn = T - g.dE;
+    g.dE = T - Tn;                                                         // exactly what the particle loses (ledger closes)
+    L.E = Tn;
+    return g;
+}
+template <bool COUNT>
+__device__ __forceinline__ void hinge_segment_phantom(Lane& L, const TransportParams& P, const Shared& sh, uint32_t* cnt) {
+    const Geom& g = P.g;
+    const float rho = __uint_as_float(L.cw & ~31u); const int m = (int)(L.cw & 31u);
+    if (!(L.R > 0.0f) && !(L.flags & F_LEGA)) { hinge_begin_step(L, P); if (COUNT) cnt[15]++; }
+    const float tx = (L.dx > 0.0f ? 1.0f - L.x : L.x) * g.hx * rcp(fabsf(L.dx) + 1e-30f);
+    const float ty = (L.dy > 0.0f ? 1.0f - L.y : L.y) * g.hy * rcp(fabsf(L.dy) + 1e-30f);
+    const float tz = (L.dz > 0.0f ? 1.0f - L.z : L.z) * g.hz * rcp(fabsf(L.dz) + 1e-30f);
+    const float tb = fmaxf(fminf(tx, fminf(ty, tz)), 0.0f);
+    const bool ax0 = tx <= ty && tx <= tz, ax1 = !ax0 && ty <= tz, ax2 = !ax0 && !ax1;
+    const Segment sg = hinge_segment(L, P, sh, m, rho, tb);
+    if (COUNT) cnt[6]++;
+    L.pval += sg.dE; L.a_ph += sg.dE;
+    L.x = fmaf(sg.s * g.ihx, L.dx, L.x); L.y = fmaf(sg.s * g.ihy, L.dy, L.y); L.z = fmaf(sg.s * g.ihz, L.dz, L.z);
+    if (sg.on_face) {
+        const bool up = (ax0 ? L.dx : (ax1 ? L.dy : L.dz)) > 0.0f;
+        const float nf = up ? 0.0f : 1.0f;
+        const int sh10 = ax0 ? 0 : (ax1 ? 10 : 20);
+        const int nmax = ax0 ? g.nx : (ax1 ? g.ny : g.nz);
+        const int stride = ax0 ? 1 : (ax1 ? g.nx : g.nx * g.ny);
+        const int ni = (int)((L.vox >> sh10) & 1023u) + (up ? 1 : -1);
+        L.x = ax0 ? nf : L.x; L.y = ax1 ? nf : L.y; L.z = ax2 ? nf : L.z;
+        if (ni >= 0 && ni < nmax) {
+            if (L.pval != 0.0f) atomicAdd(P.ph_batch + (size_t)F_BATCH(L.flags) * P.nvox + L.vlin, L.pval);
+            L.pval = 0.0f;
+            L.vox = (L.vox & ~(1023u << sh10)) | ((uint32_t)ni << sh10);
+            L.vlin += (uint32_t)(up ? stride : -stride);
+            L.pidx = L.vlin;
+            L.cw = __ldg(P.vox + L.vlin);
+        } else {                                                           // leaves the grid
+            frac_to_world(L, g);
+            if (ax0) L.x = up ? g.hix : g.lox; else if (ax1) L.y = up ? g.hiy : g.loy; else L.z = up ? g.hiz : g.loz;
+            SET_REGION(L.flags, R_AIR);
+        }
+    }
+    if (!(L.R > 0.0f) && (L.flags & F_LEGA)) hinge_deflect(L, P, sh, m);  // the hinge, in the medium of the segment that ended the leg
+}
+template <bool COUNT>
+__device__ __forceinline__ void hinge_segment_outside(Lane& L, const TransportParams& P, const Shared& sh, uint32_t* cnt) {
+    const Geom& g = P.g;
+    const bool in_air = F_REGION(L.flags) == R_AIR;
+    float rho, tb; int m, axis = 0, kind = 0;
+    if (in_air) {
+        rho = kRhoAir; m = 0;
+        const AirHit ah = air_boundary(L.x, L.y, L.z, L.dx, L.dy, L.dz);
+        tb = ah.t; kind = ah.code & 3; axis = ah.code >> 2;
+    } else {
+        const int l = F_LAYER(L.flags);
+        rho = g.lrho[l]; m = g.lmat[l];
+        float tf = kInf;
+        if (L.dz > 0.0f) tf = (g.zt[l + 1] - L.z) / L.dz; else if (L.dz < 0.0f) tf = (g.zt[l] - L.z) / L.dz;
+        tf = fmaxf(tf, 0.0f);
+        const float tl = lateral_exit(L.x, L.y, L.dx, L.dy);
+        if (tl < tf) { tb = tl; kind = 2; } else { tb = tf; kind = 0; }
+    }
+    if (!(L.R > 0.0f) && !(L.flags & F_LEGA)) { hinge_begin_step(L, P); if (COUNT) cnt[15]++; }
+    const Segment sg = hinge_segment(L, P, sh, m, rho, tb);
+    if (in_air) { if (COUNT) cnt[7]++; L.a_air += sg.dE; }
+    else { if (COUNT) cnt[8]++; dep_epid(L, fmaf(0.5f * sg.s, L.dx, L.x), fmaf(0.5f * sg.s, L.dy, L.y), sg.dE); }   // pixel of the segment's mid-point (A24)
+    L.x = fmaf(sg.s, L.dx, L.x); L.y = fmaf(sg.s, L.dy, L.y); L.z = fmaf(sg.s, L.dz, L.z);
+    if (sg.on_face) {
+        const float e_out = L.E + (F_TYPE(L.flags) == T_POSITRON ? 2.0f * kMec2 : 0.0f);
+        if (in_air) {
+            if (kind == 0) enter_phantom(L, P, axis);
+            else if (kind == 1) enter_epid_ps3(L, P);
+            else { L.a_esc += e_out; L.alive = false; return; }
+        } else {
+            const int l = F_LAYER(L.flags);
+            if (kind == 2) { L.a_esc += e_out; L.alive = false; return; }
+            if (L.dz > 0.0f) {
+                L.z = g.zt[l + 1];
+                if (l + 1 >= g.n_layers) { L.a_esc += e_out; L.alive = false; return; }
+                SET_LAYER(L.flags, l + 1);
+            } else {
+                L.z = g.zt[l];
+                if (l == 0) epid_to_air(L, g); else SET_LAYER(L.flags, l - 1);
+            }
+        }
+    }
+    if (!(L.R > 0.0f) && (L.flags & F_LEGA)) hinge_deflect(L, P, sh, m);
+}
+
 // K5 for one lane: up to kStepsE / kStepsX consecutive steps per event, one Philox block per two steps
 template <bool COUNT, bool PHANTOM, int PH>
 __device__ __forceinline__ void charged_event(Lane& L, const TransportParams& P, const Shared& sh, uint32_t* cnt) {
-    constexpr bool C2 = PH >= 2;
+    constexpr bool C2 = PH == 2 || PH == 3;
     if (L.E <= P.ph.ecut) { stop_charged<COUNT>(L, P, cnt); return; }
+    if (PH == 4) {
+#pragma unroll 1
+        for (int k = 0; k < (PHANTOM ? kStepsE : kStepsX); ++k) {
+            if (PHANTOM) hinge_segment_phantom<COUNT>(L, P, sh, cnt); else hinge_segment_outside<COUNT>(L, P, sh, cnt);
+            if (!L.alive) break;
+            if (L.E <= P.ph.ecut) {
+                if (F_TYPE(L.flags) == T_ELECTRON) { dep_here(L, P, L.E); L.alive = false; }
+                break;
+            }
+            if ((F_REGION(L.flags) == R_PHANTOM) != PHANTOM) break;
+        }
+        return;
+    }
     uint4 r = PHANTOM ? rng_block_hot(L, P) : rng_block(L, P);
 #pragma unroll 1
     for (int k = 0; k < (PHANTOM ? kStepsE : kStepsX); ++k) {
@@ -963,7 +1102,7 @@ __device__ __forceinline__ bool head_clear(const Head& H, int k, float x, float 
 // The lane's photon: (L.x, L.y, L.z) = (u, v, w) and direction in the BEAM frame, dw > 0.  Returns true with the photon on the
 // Phase Space 2 plane; false if it ended in the stage (energy booked).  dep sums what the stage absorbed.
 template <bool COUNT>
-__device__ __noinline__ bool head_stage(Lane& L, const TransportParams& P, const Shared& sh, float& dep, uint32_t* cnt) {
+__device__ __forceinline__ bool head_stage(Lane& L, const TransportParams& P, const Shared& sh, float& dep, uint32_t* cnt) {
     const Head& H = P.hd;
     int k = 0;
 #pragma unroll 1
@@ -1089,16 +1228,25 @@ __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned lon
 #pragma unroll
     for (int c = 0; c < kClasses; ++c) n_live += n[c];
     s_live = n_live;                                           // between phases every particle sits in a queue and no lane holds a credit
-    // Progress check: the last phase ran no event although particles wait.  Every lane that could have run one parked its
-    // particle for want of a head-room credit, and if no other class can run, nothing will ever give one back (possible with
-    // a small aepid_set_live_limit and many pair / annihilation / bremsstrahlung photons).  The limit set by the caller is a
-    // soft one: raise it, up to the hard bound the queue protocol needs (half a class queue); beyond that the error is flagged.
-    if (s_nphase > 0u && s_did == 0 && n_live > 0) {
-        const int hard = (1 << P.pool_log) / 2;
-        if (s_live_max < hard) s_live_max = min(2 * s_live_max, hard);
-        else if (n[C_E] + n[C_X] + n[C_A] == 0) { raise_error(8); for (int r = 0; r < kRings; ++r) n[r] = 0; s_flag[0] = 1; }
+    // Progress check.  A phase in which every lane that could have run an event parked its particle for want of a head-room
+    // credit is STUCK (possible with a small aepid_set_live_limit, or in physics modes 2 and 3 where every charged step needs a
+    // credit, when pair / annihilation / bremsstrahlung photons multiply).  A stuck class is passed over until some phase makes
+    // progress again (a particle that dies gives its count back); if every class that has particles is stuck, the limit set by
+    // the caller, which is a soft one, is raised, up to the hard bound the queue protocol needs (half a class queue); beyond
+    // that the run cannot go on and the error is flagged.
+    if (s_did != 0) s_stuck = 0;
+    else if (s_nphase > 0u && s_parked != 0 && s_phase >= 0) s_stuck |= 1 << s_phase;
+    s_did = 0; s_parked = 0;
+    if (s_stuck != 0) {
+        bool any_free = false;
+#pragma unroll
+        for (int c = 0; c < kClasses; ++c) any_free |= n[c] > 0 && !((s_stuck >> c) & 1);
+        if (!any_free) {
+            const int hard = (1 << P.pool_log) / 2;
+            if (s_live_max < hard) { s_live_max = min(2 * s_live_max, hard); s_stuck = 0; }
+            else { raise_error(8); for (int r = 0; r < kRings; ++r) n[r] = 0; s_flag[0] = 1; }
+        }
     }
-    s_did = 0;
     const int nf = s_live_max - n_live;
     bool more = s_flag[0] == 0;
     int budget = 0;
@@ -1118,7 +1266,14 @@ __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned lon
 #pragma unroll
         for (int c = 0; c < kClasses; ++c) {
             if (starved && (c == C_W || c == C_P)) continue;
+            if ((s_stuck >> c) & 1) continue;                  // its lanes could only park last time: let another class free head room first
             if (n[c] > nb) { nb = n[c]; ph = c; }
+        }
+        if (ph < 0 && n_live > 0) {                            // whatever waits must run: first a class that is not stuck, else any
+#pragma unroll
+            for (int c = 0; c < kClasses; ++c) if (!((s_stuck >> c) & 1) && n[c] > nb) { nb = n[c]; ph = c; }
+#pragma unroll
+            for (int c = 0; c < kClasses; ++c) if (ph < 0 && n[c] > nb) { nb = n[c]; ph = c; }
         }
         if (ph >= 0) budget = 0;
         else if (more && budget > 0) ph = C_A;                 // fewer histories left than lanes
@@ -1134,14 +1289,14 @@ __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned lon
 }
 
 // One phase of class C for one warp (header comment).  On return every lane is empty and holds no credit.
-template <bool COUNT, int C, int PH>
+template <bool COUNT, int C, int PH, bool HEAD>
 __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, const Shared& sh, double* led, uint32_t* cnt) {
     const unsigned lane = threadIdx.x & 31u;
     const unsigned lt_mask = (1u << lane) - 1u;
-    constexpr bool C2 = PH >= 2;
+    constexpr bool C2 = PH == 2 || PH == 3;
     constexpr bool kSpawns = C == C_W || C == C_P || (C2 && (C == C_E || C == C_X));   // classes whose events create secondaries all the time
     const int keep = *((volatile int*)&s_keep);
-    bool leaving = false, park = false, did = false;
+    bool leaving = false, park = false, did = false, parked = false;
     float h_n = 0.0f, h_E = 0.0f, h_dep = 0.0f;                 // collimation stage (class A only): Phase Space 2 particles, their energy, absorbed
     // every lane enters a phase empty: saying so lets the compiler drop what this class never touches from the registers
     L.a_emit = L.a_ph = L.a_eps = L.a_epo = L.a_air = L.a_esc = 0.0f;
@@ -1153,7 +1308,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
         if (!(L.alive && !leaving && !park && class_of(L.flags) == C)) {
             flush_pending(L, P);
             if (L.alive) {
-                queue_particle(L.x, L.y, L.z, L.dx, L.dy, L.dz, L.E, L.vox, L.flags, L.h, L.pid, L.blk);
+                queue_particle(L.x, L.y, L.z, L.dx, L.dy, L.dz, L.E, L.vox, L.flags, L.h, L.pid, L.blk, PH == 4 ? L.R : 0.0f);
                 if (COUNT && !kPhaseClock) cnt[27]++;
                 L.alive = false; L.counted = kNone;
             } else if (L.counted != kNone) {
@@ -1173,6 +1328,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                 const uint32_t tk = (uint32_t)(cl >> 32) + (uint32_t)rk;
                 const uint4* rec = queue_rec(C, tk);
                 const uint4 a = __ldcs(rec), b = __ldcs(rec + 1), c = __ldcs(rec + 2);
+                if (PH == 4) L.R = __uint_as_float(__ldcs(rec + 3).x);
 #if AEPID_PREFETCH > 0
                 // the records a later refill will want (same queue, AEPID_PREFETCH tickets ahead, if published): into the L2
                 if ((int)(s_snap[C] - (tk + AEPID_PREFETCH)) > 0) {
@@ -1208,8 +1364,8 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                             L.vox = 0;
                             L.flags = T_PHOTON | (R_AIR << 2) | (min(h / P.hist_per_batch, (uint32_t)P.n_batches - 1u) << 16);
                             L.alive = true; L.counted = 1u;
-                            L.pval = 0.0f; L.pidx = kNone;
-                            if (P.hd.n_ps1 == 0u) {
+                            L.pval = 0.0f; L.pidx = kNone; L.R = 0.0f;
+                            if (!HEAD) {                                   // HEAD: the instantiation with the collimation stage (launch_transport)
                                 const SourceSample s = sample_source(P, r.x, r.y, r.z, r.w);
                                 L.x = P.g.src[0]; L.y = P.g.src[1]; L.z = P.g.src[2];
                                 L.dx = s.dx; L.dy = s.dy; L.dz = s.dz; L.E = s.E;
@@ -1267,7 +1423,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
         } else if (C == C_E || C == C_X) {
             if (on && F_TYPE(L.flags) == T_POSITRON && L.E <= P.ph.ecut && !ensure_spare(L)) { park = true; on = false; if (COUNT && !kPhaseClock) cnt[29]++; }   // annihilation needs a credit
         }
-        did |= on;
+        did |= on; parked |= park;
         if (C == C_W) {
             // K3 + K4: flights against the majorant until at least kHitMin lanes have a collision to sample (or nobody flies
             // any more), then the interactions together: keeps both halves of the event well filled when few flights collide
@@ -1306,14 +1462,15 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
     }
     if (L.spare != kNone) { atomicSub(&s_live, 1); L.spare = kNone; }
     ledger_flush(L, led);
-    if (C == C_A && P.hd.n_ps1 != 0u) {
+    if (C == C_A && HEAD) {
         ledger_add(h_n, P.hd.stats + 0, true); ledger_add(h_E, P.hd.stats + 1, true); ledger_add(h_dep, P.hd.stats + 2, true);
     }
     if (__any_sync(FULL_MASK, did) && lane == 0) s_did = 1;
+    if (__any_sync(FULL_MASK, parked) && lane == 0) s_parked = 1;
     if (lane == 0) atomicAdd(&s_left, 1);
 }
 
-template <bool COUNT, int PH>
+template <bool COUNT, int PH, bool HEAD>
 __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_constant__ TransportParams P) {
     // dynamic shared memory: per-warp ledger | table blob
     double* const led_all = reinterpret_cast<double*>(smem_raw);
@@ -1325,15 +1482,15 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
     sh.lnS = sh.maj + P.tb.n_E;
     sh.invX0 = sh.lnS + P.tb.n_mat * P.tb.n_T;
     sh.sig = sh.invX0 + P.tb.n_mat + P.tb.n_mat * P.tb.n_T;
-    if (PH >= 2) sh.lnS = sh.invX0 + P.tb.n_mat;                    // the restricted stopping power takes the place of the total one
+    if (PH == 2 || PH == 3) sh.lnS = sh.invX0 + P.tb.n_mat;                    // the restricted stopping power takes the place of the total one
     for (int i = threadIdx.x; i < kWarps * 8; i += kThreads) led_all[i] = 0.0;
     if (threadIdx.x < kRings) { s_tail[threadIdx.x] = 0u; s_head[threadIdx.x] = 0u; s_snap[threadIdx.x] = 0u; }
     if (threadIdx.x < 2) s_flag[threadIdx.x] = 0;
     if (threadIdx.x == 0) {
         s_g = P.g; s_ep_batch = P.ep_batch; s_npix = P.npix; s_nphase = 0u;
-        s_pool_log = P.pool_log; s_pool_mask = (1u << P.pool_log) - 1u;
-        s_queue = P.queues + (((size_t)blockIdx.x * kClasses) << P.pool_log) * 3;
-        s_live = 0; s_live_max = min(max(P.live_max, 64), (1 << P.pool_log) / 2); s_did = 0;
+        s_pool_log = P.pool_log; s_pool_mask = (1u << P.pool_log) - 1u; s_rec_vec = PH == 4 ? 4u : 3u;
+        s_queue = P.queues + (((size_t)blockIdx.x * kClasses) << P.pool_log) * (PH == 4 ? 4 : 3);
+        s_live = 0; s_live_max = min(max(P.live_max, 64), (1 << P.pool_log) / 2); s_did = 0; s_parked = 0; s_stuck = 0; s_phase = -1;
     }
     __syncthreads();
 
@@ -1347,7 +1504,7 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
     Lane L;
     L.x = L.y = L.z = 0.0f; L.dx = L.dy = 0.0f; L.dz = 1.0f; L.E = 0.0f; L.vox = 0; L.flags = 0; L.h = L.pid = L.blk = 0;
     L.cw = 0; L.vlin = 0; L.ci = 0; L.ct = 0.0f; L.mumaj = 1.0f;
-    L.pval = 0.0f; L.pidx = kNone; L.counted = kNone; L.spare = kNone; L.alive = false;
+    L.pval = 0.0f; L.pidx = kNone; L.counted = kNone; L.spare = kNone; L.alive = false; L.R = 0.0f;
     L.a_emit = L.a_ph = L.a_eps = L.a_epo = L.a_air = L.a_esc = 0.0f;
 
 #pragma unroll 1
@@ -1360,11 +1517,11 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
         const long long t0 = clock64();
 #endif
         switch (ph) {
-            case C_A: run_phase<COUNT, C_A, PH>(L, P, sh, led, cnt); break;
-            case C_W: run_phase<COUNT, C_W, PH>(L, P, sh, led, cnt); break;
-            case C_E: run_phase<COUNT, C_E, PH>(L, P, sh, led, cnt); break;
-            case C_P: run_phase<COUNT, C_P, PH>(L, P, sh, led, cnt); break;
-            default:  run_phase<COUNT, C_X, PH>(L, P, sh, led, cnt); break;
+            case C_A: run_phase<COUNT, C_A, PH, HEAD>(L, P, sh, led, cnt); break;
+            case C_W: run_phase<COUNT, C_W, PH, HEAD>(L, P, sh, led, cnt); break;
+            case C_E: run_phase<COUNT, C_E, PH, HEAD>(L, P, sh, led, cnt); break;
+            case C_P: run_phase<COUNT, C_P, PH, HEAD>(L, P, sh, led, cnt); break;
+            default:  run_phase<COUNT, C_X, PH, HEAD>(L, P, sh, led, cnt); break;
         }
 #ifdef AEPID_PHASE_CLOCK
         if (COUNT && lane == 0) { atomicAdd(P.counters + 10, (unsigned long long)(clock64() - t0)); atomicAdd(P.counters + 27 + ph, (unsigned long long)(clock64() - t0)); }   // busy warp-cycles
@@ -1402,12 +1559,17 @@ size_t transport_smem_bytes(const Tables& t) {      // dynamic + static shared m
     return kDynSmemFixed + (size_t)t.blob_words * 4 + sizeof(Geom) + 512;
 }
 
+template <bool COUNT, int PH, bool HEAD>
+static int launch_inst(const TransportParams& p, unsigned blocks, size_t smem, cudaStream_t stream) {
+    const cudaError_t e = cudaFuncSetAttribute(transport_kernel<COUNT, PH, HEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return (int)e;
+    transport_kernel<COUNT, PH, HEAD><<<blocks, kThreads, smem, stream>>>(p);
+    return (int)cudaGetLastError();
+}
+// The collimation stage (Phase Space 1 source + jaws / MLC) has its own instantiations: the fluence-map source pays nothing for it
 template <bool COUNT, int PH>
 static int launch_one(const TransportParams& p, unsigned blocks, size_t smem, cudaStream_t stream) {
-    const cudaError_t e = cudaFuncSetAttribute(transport_kernel<COUNT, PH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return (int)e;
-    transport_kernel<COUNT, PH><<<blocks, kThreads, smem, stream>>>(p);
-    return (int)cudaGetLastError();
+    return p.hd.n_ps1 != 0u ? launch_inst<COUNT, PH, true>(p, blocks, smem, stream) : launch_inst<COUNT, PH, false>(p, blocks, smem, stream);
 }
 int launch_transport(const TransportParams& p, bool counting, int sm_count, void* stream) {
     const size_t smem = kDynSmemFixed + (size_t)p.tb.blob_words * 4;
@@ -1418,6 +1580,7 @@ int launch_transport(const TransportParams& p, bool counting, int sm_count, void
     if (blocks < 1) blocks = 1;
     // Class II physics (mode 2: Moller delta rays, mode 3: + bremsstrahlung) has its own instantiations: modes 0 and 1 pay nothing
     const cudaStream_t st = (cudaStream_t)stream; const unsigned nb = (unsigned)blocks;
+    if (p.ph.mode == 4) return counting ? launch_one<true, 4>(p, nb, smem, st) : launch_one<false, 4>(p, nb, smem, st);
     if (p.ph.mode == 3) return counting ? launch_one<true, 3>(p, nb, smem, st) : launch_one<false, 3>(p, nb, smem, st);
     if (p.ph.mode == 2) return counting ? launch_one<true, 2>(p, nb, smem, st) : launch_one<false, 2>(p, nb, smem, st);
     return counting ? launch_one<true, 1>(p, nb, smem, st) : launch_one<false, 1>(p, nb, smem, st);

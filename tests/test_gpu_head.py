@@ -56,7 +56,7 @@ def test_c4_field_through_jaws_and_mlc():
     and depth dose downstream, GPU against oracle."""
     cfg = head_config(field=7, shrink=2, n_ps1=1_000_000)
     head_stats_agree(cfg, 100_000_000, 20_000_000, seed=cfg["seed"])
-    compare(cfg, 1_000_000_000, 60_000_000, rebin=8, frac_ok=0.98, phantom_voxels=False, min_tested=40)
+    compare(cfg, 2_000_000_000, 200_000_000, rebin=4, frac_ok=0.98, phantom_voxels=False, min_tested=100)   # 3.1 mm pixels
 
 
 def test_head_api_errors():

@@ -23,6 +23,7 @@ pytestmark = pytest.mark.gpu
 
 def engine_for(cfg, **kw):
     from paper_2510_24154_b200 import Engine
+    kw.setdefault("max_live_per_cta", 0)                    # tests run other history counts than the config's: the full-size queues
     eng = Engine.for_config(cfg, **kw)
     eng.load_config(cfg)
     return eng
@@ -80,6 +81,8 @@ def compare(cfg, n_gpu, n_or, rebin, seed=None, frac_ok=0.99, procs=None, phanto
     k = om > 0.2 * om.max()
     assert k.sum() >= min_tested
     z = (gm[k] - om[k]) / np.sqrt(gs[k] ** 2 + os_[k] ** 2)
+    print("%s EPID re-binned x%d: %d pixels tested, within 3 sigma %.4f, z mean %+.3f std %.3f, effective oracle events per pixel min %.0f; integral gpu/oracle - 1 = %+.2e"
+          % (cfg["name"], rebin, k.sum(), np.mean(np.abs(z) < 3), z.mean(), z.std(), ((om[k] / os_[k]) ** 2).min(), gm.sum() / om.sum() - 1))
     assert np.mean(np.abs(z) < 3) >= frac_ok, (np.mean(np.abs(z) < 3), z.mean(), z.std())
     assert abs(z.mean()) < 0.35 and 0.7 < z.std() < 1.3, (z.mean(), z.std())
     # integral EPID scored energy
@@ -164,6 +167,43 @@ def test_c1_class2_physics_full_size(mode):
     cfg = make_config("C1")
     cfg["physics"]["mode"] = mode
     compare(cfg, cfg["n_histories"], 4_000_000, rebin=8)
+
+
+def test_c1_and_c2_mode4_random_hinge():
+    """Physics mode 4 (DPM-style multi-voxel steps with a random hinge, reading A38) with steps of 20 %: C1 at full size, the
+    heterogeneous thorax phantom at half resolution (steps cross lung / tissue / bone voxels), GPU against the oracle's mode 4."""
+    cfg = make_config("C1")
+    cfg["physics"]["mode"], cfg["physics"]["f_E"] = 4, 0.2
+    compare(cfg, cfg["n_histories"], 4_000_000, rebin=8)
+    cfg = make_config("C2", shrink=2)
+    cfg["physics"]["mode"], cfg["physics"]["f_E"] = 4, 0.2
+    compare(cfg, 40_000_000, 4_000_000, rebin=16, frac_ok=0.985, phantom_voxels=False, min_tested=40)
+
+
+def test_mode4_steps_and_schedule_independence():
+    """Mode 4: half as many deflections as mode 1 has steps (the counters both sides keep), the air gap crossed in a few segments,
+    and the same particles followed whatever the live limit (64-byte records carry the leg's budget through the queues)."""
+    cfg = make_config("C1", shrink=2)
+    cfg["physics"]["mode"], cfg["physics"]["f_E"] = 4, 0.2
+    res = []
+    for lim in (0, 1024, 256):
+        eng = engine_for(cfg)
+        eng.set_live_limit(lim); eng.set_counting(True)
+        eng.simulate(400_000, 9)
+        r = eng.read_tallies(); check_ledger(r["ledger"], 400_000)
+        r["c"] = eng.read_counters()
+        res.append(r); eng.close()
+    for r in res[1:]:
+        assert np.array_equal(r["c"][:16], res[0]["c"][:16])
+        assert np.allclose(r["ledger"][:6], res[0]["ledger"][:6], rtol=2e-6)
+        assert np.allclose(r["phantom_mean"], res[0]["phantom_mean"], rtol=1e-3, atol=1e-9)
+    raw = oracle.run_sharded(cfg, 400_000, 9, want_phantom_sq=False)
+    cg, co = res[0]["c"].astype(float) / 4e5, raw["counters"].astype(float) / 4e5
+    for k in (6, 7, 8, 15, 14):                                  # segments per region, steps, charged tracks: per history, both sides
+        assert abs(cg[k] - co[k]) < 0.01 * co[k] + 5 * np.sqrt(co[k] / 4e5), (k, cg[k], co[k])
+    cfg["physics"]["mode"], cfg["physics"]["f_E"] = 1, 0.1
+    eng = engine_for(cfg); eng.set_counting(True); eng.simulate(400_000, 9); c1 = eng.read_counters().astype(float) / 4e5; eng.close()
+    assert cg[15] < 0.55 * (c1[6] + c1[7] + c1[8]) and cg[7] < 0.2 * c1[7]
 
 
 def test_c2_heterogeneous_phantom_class2_physics():
@@ -318,25 +358,51 @@ def test_results_do_not_depend_on_the_live_limit(name, shrink, n):
         assert np.allclose(r["epid_mean"], res[0]["epid_mean"], rtol=1e-3, atol=1e-9)
 
 
-@pytest.mark.parametrize("mode", [1, 3])
-def test_tiny_live_limit_with_pair_and_bremsstrahlung_photons(mode):
+def test_tiny_live_limit_with_photon_multiplication():
     """with room for only 64 live particles per CTA and a workload that multiplies photons (10 MeV photons on
-    Gd2O2S: pair production, annihilation, in mode 3 bremsstrahlung) every lane can end up parked for want of a credit.  The
-    scheduler notices a phase without progress and raises the (soft) limit; the results are those of the default limit and
-    no error flag is raised."""
-    cfg = slab_cfg(n=(8, 8, 8), h=(4.0, 4.0, 2.5), rho=7.32, mat=5, E=10.0, mode=mode, epid="C1", field_cm=2.0)
-    res = []
-    for lim in (0, 64, 100):
-        eng = engine_for(cfg)
-        eng.set_live_limit(lim)
-        eng.simulate(300_000, 11)
-        r = eng.read_tallies()                              # AepidError INTERNAL if the kernel had flagged a stall
-        check_ledger(r["ledger"], 300_000)
-        res.append(r)
-        eng.close()
-    for r in res[1:]:
-        assert np.allclose(r["ledger"][:6], res[0]["ledger"][:6], rtol=2e-6)
-        assert np.allclose(r["phantom_mean"], res[0]["phantom_mean"], rtol=1e-3, atol=1e-9)
+    Gd2O2S: pair production and annihilation) every lane of a phase can end up parked for want of a head-room credit.  The
+    scheduler notices the phase without progress, passes the stuck class over and, if all are stuck, raises the (soft) limit; the
+    results are those of the default limit and no error flag is raised.  Same with the 6 MV beam in physics mode 3, where every
+    charged step needs a credit as well."""
+    cases = [(slab_cfg(n=(8, 8, 8), h=(4.0, 4.0, 2.5), rho=7.32, mat=5, E=10.0, mode=1, epid="C1", field_cm=2.0), 300_000)]
+    c1 = make_config("C1", shrink=4); c1["physics"]["mode"] = 3
+    cases.append((c1, 300_000))
+    for cfg, n in cases:
+        res = []
+        for lim in (0, 64, 100):
+            eng = engine_for(cfg, max_live_per_cta=4096)
+            eng.set_live_limit(lim)
+            eng.simulate(n, 11)
+            r = eng.read_tallies()                          # AepidError INTERNAL if the kernel had flagged a stall
+            check_ledger(r["ledger"], n)
+            res.append(r)
+            eng.close()
+        for r in res[1:]:
+            assert np.allclose(r["ledger"][:6], res[0]["ledger"][:6], rtol=2e-6)
+            assert np.allclose(r["phantom_mean"], res[0]["phantom_mean"], rtol=1e-3, atol=1e-9)
+
+
+def test_running_out_of_head_room_fails_loudly():
+    """Physics modes 2 and 3 need head room for the particles a history has alive at a time (every charged step holds a credit);
+    a shower-heavy workload (10 MeV photons on Gd2O2S, mode 3) in class queues sized for 2048 particles per CTA cannot finish.
+    The library must say so (AEPID_ERR_INTERNAL from the calls that synchronise) instead of returning partial tallies; with the
+    default queue size the same run completes."""
+    from paper_2510_24154_b200 import AepidError
+    cfg = slab_cfg(n=(8, 8, 8), h=(4.0, 4.0, 2.5), rho=7.32, mat=5, E=10.0, mode=3, epid="C1", field_cm=2.0)
+    eng = engine_for(cfg, max_live_per_cta=2048)
+    eng.simulate(600_000, 11)
+    with pytest.raises(AepidError, match="INTERNAL"):
+        eng.read_tallies()
+    with pytest.raises(AepidError, match="INTERNAL"):
+        eng.synchronize()
+    eng.reset_tallies(); eng.set_physics(**dict(cfg["physics"], mode=1))
+    eng.simulate(100_000, 11)
+    check_ledger(eng.read_tallies()["ledger"], 100_000)     # the context recovers
+    eng.close()
+    eng = engine_for(cfg, max_live_per_cta=0)                # 65536 per CTA
+    eng.simulate(600_000, 11)
+    check_ledger(eng.read_tallies()["ledger"], 600_000)
+    eng.close()
 
 
 def test_more_histories_than_32_bits():
@@ -431,7 +497,7 @@ def test_error_codes():
     with pytest.raises(AepidError, match="BAD_ARG"):
         eng.load_source(s["src_pos"], s["beam_axes"], s["E_edges"], s["E_pdf"], s["f_pitch"], s["f_plane_dist"], np.zeros((100, 100), np.float32))
     with pytest.raises(AepidError, match="BAD_ARG"):
-        eng.set_physics(mode=4)
+        eng.set_physics(mode=5)
     eng.load_epid_layers(ep["thickness"], ep["material"], ep["density"], ep["scored"], ep["sid"], ep["nu"], ep["nv"], ep["pitch"])
     eng.simulate(1000, 1)                                             # recovers after the errors
     check_ledger(eng.read_tallies()["ledger"], 1000)
