@@ -54,8 +54,10 @@ def alg_instr_per_history(ev):
 # warp-instruction, issue-slot utilisation.  None where no capture of the current kernel exists.
 NCU_CAPTURES = {}
 try:
-    with open(os.path.join(ROOT, "profiles", "ncu_transport_summary.json")) as _f:
-        NCU_CAPTURES = json.load(_f)
+    import csv as _csv
+    with open(os.path.join(ROOT, "profiles", "ncu_transport_summary.csv")) as _f:
+        for _r in _csv.DictReader(_f):
+            NCU_CAPTURES[_r["key"]] = {k: (float(v) if k not in ("key", "report") else v) for k, v in _r.items()}
 except Exception:
     pass
 

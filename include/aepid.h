@@ -181,12 +181,13 @@ int aepid_read_batches(aepid_ctx* ctx, float* epid_batches, double* histories_pe
  *   16 iter_A             17 iter_W            18 iter_E            19 iter_P
  *   20 iter_X             21 lanes_A           22 lanes_W           23 lanes_E
  *   24 lanes_P            25 lanes_X           26 phases            27 particles_stored
- *   28 particles_loaded   29 particles_parked  30 source_tasks      31 unused31
+ *   28 particles_loaded   29 particles_parked  30 source_tasks      31 majorant_violations
  * 0-9, 12-15: events of the physics (flights per region, interactions per channel, charged-particle steps per region,
  * secondaries created, Klein-Nishina trials, photons ended by the 10 keV cut-off, charged tracks, zero-length steps);
  * 16-20: warp-level event iterations of the scheduler phases A, W, E, P, X (transport.cu), 21-25: live lanes summed over
  * those iterations, 26 phases run (all CTAs), 27 / 28 particle records written to / read from the class queues, 29 lanes
- * that parked their particle for want of head room, 30 source tasks. */
+ * that parked their particle for want of head room, 30 source tasks, 31 tentative Woodcock collisions in a voxel whose
+ * attenuation coefficient exceeds the majorant of its segment (body box): must stay 0. */
 int aepid_set_counting(aepid_ctx* ctx, int on);
 int aepid_read_counters(aepid_ctx* ctx, unsigned long long counters[32]);
 

@@ -24,7 +24,7 @@ COUNTER_NAMES = ("woodcock_flights", "air_flights", "epid_flights", "n_pe", "n_c
                  "unused11", "kn_iterations", "photon_cutoffs", "e_tracks", "zero_steps",
                  "iter_A", "iter_W", "iter_E", "iter_P", "iter_X",
                  "lanes_A", "lanes_W", "lanes_E", "lanes_P", "lanes_X",
-                 "phases", "particles_stored", "particles_loaded", "particles_parked", "source_tasks", "unused31")
+                 "phases", "particles_stored", "particles_loaded", "particles_parked", "source_tasks", "majorant_violations")
 EXPORTS = ("aepid_workspace_bytes", "aepid_create", "aepid_destroy", "aepid_last_error", "aepid_init_materials",
            "aepid_load_phantom", "aepid_load_epid_layers", "aepid_load_source", "aepid_set_physics",
            "aepid_reset_tallies", "aepid_simulate", "aepid_read_tallies", "aepid_read_batches",

@@ -68,7 +68,7 @@ Layout make_layout(const aepid_dims& d) {
     L.thrF = take(((size_t)d.fu * d.fv + 1) * 4);
     L.guideF = take(((size_t)kGuideSize + 1) * 4);
     L.queues = take((size_t)kMaxCtas * kRingCount * ((size_t)1 << pool_log_for(d)) * kRecordBytes);   // class queues of the transport kernel (scratch)
-    L.small = take(1024);            // ledger [8] f64 @0 | chunk counter @64 | bad-material flag @68 | rho_max [32] f32 @128 | counters [32] u64 @256 | gamma stats [4] f64 @512, max bits @544 | PS3 count u64 @576
+    L.small = take(1024);            // ledger [8] f64 @0 | chunk counter @64 | bad-material flag @68 | rho_max [32] f32 @128 | counters [32] u64 @256 | gamma stats [4] f64 @512, max bits @544 | PS3 count u64 @576 | head stats [4] f64 @640 | body box [6] i32 @704, f_out bits @728 | kfac [32] f32 @768
     L.ps1 = take((size_t)d.n_ps1 * 32);                 // Phase Space 1 records (collimation stage), 0 if not used
     L.head_rows = take((size_t)kMaxHeadRows * 8);        // openings lo[] | hi[] of the collimator rows
     L.total = o;
@@ -127,6 +127,8 @@ struct aepid_ctx {
     unsigned int* d_gamma_max() { return reinterpret_cast<unsigned int*>(ws + lay.small + 544); }
     unsigned long long* d_ps3_count() { return reinterpret_cast<unsigned long long*>(ws + lay.small + 576); }
     double* d_head_stats() { return reinterpret_cast<double*>(ws + lay.small + 640); }      // [4]
+    int* d_body_box() { return reinterpret_cast<int*>(ws + lay.small + 704); }                // [6] + the f_out bits
+    float* d_kfac() { return reinterpret_cast<float*>(ws + lay.small + 768); }                // [kMaxMat]
     float4* d_ps1() { return reinterpret_cast<float4*>(ws + lay.ps1); }
     float* d_head_rows() { return reinterpret_cast<float*>(ws + lay.head_rows); }
 };
@@ -237,6 +239,36 @@ int build_tables(aepid_ctx* ctx) {
     for (int m = 0; m < nm; ++m) {
         for (int j = 0; j < nT; ++j) lnS[(size_t)m * nT + j] = (float)std::log(std::max((double)ctx->S[(size_t)m * nT + j], 1e-37));
         invX0[m] = 1.0f / ctx->X0[m];
+    }
+    // Body box (params.h Geom::glo).  kfac[m] = max_j mu_tot,m(E_j) / maj_j: a voxel (rho, m) attenuates at most
+    // rho kfac[m] maj(E) at EVERY energy, by the argument of reading A7 (each material's interpolant lies below the chord of its
+    // node values, the chord of rho kfac[m] maj_j is rho kfac[m] times the majorant's interpolant).  B = bounding box of the
+    // voxels with rho kfac > kBodyThr; f_out = the largest rho kfac outside B.
+    {
+        constexpr float kBodyThr = 0.05f;
+        float kfac[kMaxMat] = {0};
+        for (int m = 0; m < nm && m < kMaxMat; ++m)
+            for (int j = 0; j < nE; ++j) {
+                const size_t o = (size_t)m * nE + j;
+                kfac[m] = std::max(kfac[m], (float)(((double)ctx->muPE[o] + ctx->muC[o] + ctx->muPP[o]) / (double)maj[j] * (1.0 + 1e-6)));
+            }
+        Geom& g = ctx->g;
+        CU(cudaMemcpyAsync(ctx->d_kfac(), kfac, sizeof(kfac), cudaMemcpyHostToDevice, ctx->stream));
+        launch_body_box(ctx->d_vox(), g.nx, g.ny, g.nz, ctx->d_kfac(), kBodyThr, ctx->d_body_box(), reinterpret_cast<unsigned int*>(ctx->d_body_box() + 6), ctx->stream);
+        CU(cudaGetLastError());
+        int box[7];
+        CU(cudaMemcpyAsync(box, ctx->d_body_box(), sizeof(box), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        const int nn[3] = {g.nx, g.ny, g.nz};
+        const float lo[3] = {g.lox, g.loy, g.loz}, hi[3] = {g.hix, g.hiy, g.hiz}, h[3] = {g.hx, g.hy, g.hz};
+        for (int a = 0; a < 3; ++a) {
+            if (box[3 + a] < box[a]) { g.glo[a] = g.ghi[a] = lo[a]; continue; }            // no voxel above the threshold: G is empty
+            const int i0 = std::max(box[a] - 1, 0), i1 = std::min(box[3 + a] + 2, nn[a]);   // one voxel of cushion: a point that rounding puts
+            g.glo[a] = i0 == 0 ? lo[a] : lo[a] + (float)i0 * h[a];                           // on the wrong side of a face of G is still outside B
+            g.ghi[a] = i1 == nn[a] ? hi[a] : lo[a] + (float)i1 * h[a];
+        }
+        float fo; std::memcpy(&fo, &box[6], 4);
+        g.f_out = std::min(std::max(fo, 1e-6f), 1.0f);
     }
     if (ctx->have_ne)
         for (int m = 0; m < nm; ++m)

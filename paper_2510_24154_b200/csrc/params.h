@@ -33,6 +33,11 @@ struct Geom {
     int nx, ny, nz;
     float hx, hy, hz, ihx, ihy, ihz;
     float lox, loy, loz, hix, hiy, hiz;
+    // Body box: an axis-aligned box G of whole voxels, one voxel wider on every side than the bounding box B of
+    // the voxels whose attenuation can exceed a small fraction of the majorant; outside B no voxel exceeds f_out x majorant(E)
+    // at any energy, so Woodcock flights outside G run against f_out x majorant (the margin of air around a patient costs no
+    // virtual collisions).  An empty B gives glo == ghi.
+    float glo[3], ghi[3], f_out;
     // beam frame
     float src[3], au[3], av[3], aw[3];
     // EPID slab stack; zt[] = depth of the layer tops below the EPID top plane (zt[0] = 0)
@@ -132,6 +137,7 @@ inline void set_seed(TransportParams& p, uint64_t seed) {
 int launch_transport(const TransportParams& p, bool counting, int sm_count, void* stream);
 size_t transport_smem_bytes(const Tables& t);
 void launch_pack_voxels(const float* rho, const unsigned char* mat, uint32_t* out, size_t n, float* rho_max, int n_mat, unsigned int* bad, void* stream);
+void launch_body_box(const uint32_t* vox, int nx, int ny, int nz, const float* kfac, float thr, int* box, unsigned int* fout_bits, void* stream);
 void launch_fold(const FoldParams& p, void* stream);
 void launch_moments(const FoldParams& p, double* s1, double* s2, void* stream);
 void launch_finalize_moments(const double* s1, const double* s2, size_t n, double total, double batches, float* mean, float* sigma, void* stream);

@@ -39,6 +39,57 @@ void launch_pack_voxels(const float* rho, const unsigned char* mat, uint32_t* ou
     pack_voxels_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)stream>>>(rho, mat, out, n, rho_max, n_mat, bad);
 }
 
+// ---- body box of the phantom (params.h: Geom::glo).  f_v = rho_v kfac[m_v] bounds the voxel's attenuation coefficient
+// relative to the majorant at every energy (kfac[m] = max over the energy nodes of mu_m(E_j) / majorant(E_j), api.cu).
+// Pass 1: index bounding box B of the voxels with f_v > thr (box[0..2] = min, box[3..5] = max, inclusive; empty: max < min).
+// Pass 2: the largest f_v among the voxels outside B (as float bits; positive floats order like their bit patterns).
+__global__ void body_box_kernel(const uint32_t* __restrict__ vox, int nx, int ny, int nz, const float* __restrict__ kfac, float thr, int* __restrict__ box) {
+    __shared__ int s_box[6];
+    if (threadIdx.x < 3) s_box[threadIdx.x] = 0x7fffffff; else if (threadIdx.x < 6) s_box[threadIdx.x] = -1;
+    __syncthreads();
+    const size_t n = (size_t)nx * ny * nz;
+    int lo[3] = {0x7fffffff, 0x7fffffff, 0x7fffffff}, hi[3] = {-1, -1, -1};
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const uint32_t w = __ldg(vox + i);
+        if (__uint_as_float(w & ~31u) * __ldg(kfac + (w & 31u)) > thr) {
+            const int ix = (int)(i % (size_t)nx), iy = (int)((i / (size_t)nx) % (size_t)ny), iz = (int)(i / ((size_t)nx * ny));
+            lo[0] = min(lo[0], ix); lo[1] = min(lo[1], iy); lo[2] = min(lo[2], iz);
+            hi[0] = max(hi[0], ix); hi[1] = max(hi[1], iy); hi[2] = max(hi[2], iz);
+        }
+    }
+    for (int a = 0; a < 3; ++a) { if (hi[a] >= 0) { atomicMin(&s_box[a], lo[a]); atomicMax(&s_box[3 + a], hi[a]); } }
+    __syncthreads();
+    if (threadIdx.x < 3) { if (s_box[threadIdx.x] != 0x7fffffff) atomicMin(box + threadIdx.x, s_box[threadIdx.x]); }
+    else if (threadIdx.x < 6) { if (s_box[threadIdx.x] >= 0) atomicMax(box + threadIdx.x, s_box[threadIdx.x]); }
+}
+__global__ void body_out_kernel(const uint32_t* __restrict__ vox, int nx, int ny, int nz, const float* __restrict__ kfac, const int* __restrict__ box,
+                                unsigned int* __restrict__ fout_bits) {
+    __shared__ unsigned int s_max;
+    if (threadIdx.x == 0) s_max = 0u;
+    __syncthreads();
+    const int b0 = box[0], b1 = box[1], b2 = box[2], b3 = box[3], b4 = box[4], b5 = box[5];
+    const size_t n = (size_t)nx * ny * nz;
+    unsigned int mx = 0u;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const int ix = (int)(i % (size_t)nx), iy = (int)((i / (size_t)nx) % (size_t)ny), iz = (int)(i / ((size_t)nx * ny));
+        if (ix >= b0 && ix <= b3 && iy >= b1 && iy <= b4 && iz >= b2 && iz <= b5) continue;
+        const uint32_t w = __ldg(vox + i);
+        mx = max(mx, __float_as_uint(__uint_as_float(w & ~31u) * __ldg(kfac + (w & 31u))));
+    }
+    if (mx) atomicMax(&s_max, mx);
+    __syncthreads();
+    if (threadIdx.x == 0 && s_max) atomicMax(fout_bits, s_max);
+}
+// box: 6 ints, fout_bits: 1 uint (device); kfac: [kMaxMat] floats (device)
+void launch_body_box(const uint32_t* vox, int nx, int ny, int nz, const float* kfac, float thr, int* box, unsigned int* fout_bits, void* stream) {
+    const int init[6] = {0x7fffffff, 0x7fffffff, 0x7fffffff, -1, -1, -1};
+    cudaMemcpyAsync(box, init, sizeof(init), cudaMemcpyHostToDevice, (cudaStream_t)stream);
+    cudaMemsetAsync(fout_bits, 0, sizeof(unsigned int), (cudaStream_t)stream);
+    const size_t n = (size_t)nx * ny * nz;
+    body_box_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)stream>>>(vox, nx, ny, nz, kfac, thr, box);
+    body_out_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)stream>>>(vox, nx, ny, nz, kfac, box, fout_bits);
+}
+
 // ---- K7 fold: mean per history and standard error of the mean from B independent batch sums
 // mean = sum_b x_b / N;  sigma^2 = sum_b n_b (x_b/n_b - mean)^2 / ((B_eff - 1) N)
 // One pass over the batches (HBM-bound: 4 B n_batches per bin read once, 8 B written): with s1 = sum_b x_b and

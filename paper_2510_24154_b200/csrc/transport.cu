@@ -2,7 +2,7 @@
 // sampling, K5 CSDA electron steps with Highland deflection, K6 EPID slab transport and K7 tally
 // scoring (physics of SURVEY.md 8(c)).
 //
-// Design (sm_100a): ONE persistent CTA per SM that runs a LOCAL WAVEFRONT.  Measured on B200 (profiles/r01a_README.md,
+// Design (sm_100a): ONE persistent CTA per SM that runs a LOCAL WAVEFRONT.  Measured on B200 (profiles/r01_history.md,
 // DESIGN.md 6.2): warps of one SM that execute different parts of a code body larger than the
 // 32 KB instruction cache starve on instruction fetch (IPC 0.3-1.1 of 4), warps that execute the same part do not.
 // So all warps of a CTA work on the same event class at any time:
@@ -122,6 +122,24 @@ __device__ __forceinline__ int class_of(uint32_t flags) {
     return reg == R_PHANTOM ? C_E : C_X;
 }
 
+// is the particle with these flags in class C?  (class_of(flags) == C, as two or three bit tests)
+#ifndef AEPID_INCLASS
+#define AEPID_INCLASS 1
+#endif
+template <int C>
+__device__ __forceinline__ bool in_class(uint32_t flags) {
+#if AEPID_INCLASS
+    constexpr uint32_t kTR = 3u | (3u << 2);                                    // type and region bits
+    if (C == C_W) return (flags & kTR) == (T_PHOTON | (R_PHANTOM << 2));
+    if (C == C_A) return (flags & (kTR | F_HIT)) == (T_PHOTON | (R_AIR << 2));
+    if (C == C_P) return (flags & 3u) == T_PHOTON && (flags & (3u << 2)) != (R_PHANTOM << 2) && (flags & ((3u << 2) | F_HIT)) != (R_AIR << 2);
+    if (C == C_E) return (flags & 3u) != T_PHOTON && (flags & (3u << 2)) == (R_PHANTOM << 2);
+    return (flags & 3u) != T_PHOTON && (flags & (3u << 2)) != (R_PHANTOM << 2);
+#else
+    return class_of(flags) == C;
+#endif
+}
+
 // Scheduler state and the geometry copy: static shared memory, so that the out-of-line helpers reach them
 // without arguments.
 __shared__ unsigned int s_tail[kRings];             // tickets handed to pushers
@@ -206,6 +224,23 @@ __device__ __forceinline__ uint4 rng_block_hot(Lane& L, const TransportParams& P
         c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
     }
     L.blk++;
+    return make_uint4(c0, c1, c2, c3);
+}
+// The block the particle will draw next, without consuming it (Woodcock flights compute it while the voxel gather of the
+// flight before is in flight, AEPID_PEEK); whoever uses it increments L.blk.
+#ifndef AEPID_PEEK
+#define AEPID_PEEK 0
+#endif
+__device__ __forceinline__ uint4 rng_peek(const Lane& L, const TransportParams& P) {
+    const uint64_t h = P.base + L.h;
+    uint32_t c0 = (uint32_t)h, c1 = (uint32_t)(h >> 32), c2 = L.pid, c3 = L.blk;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ P.rk[2 * r], n2 = hi0 ^ c3 ^ P.rk[2 * r + 1];
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    }
     return make_uint4(c0, c1, c2, c3);
 }
 __device__ __forceinline__ uint32_t child_id(const Lane& L, uint32_t sibling) {    // reading A1
@@ -490,12 +525,15 @@ __device__ __forceinline__ void annihilate(Lane& L, const TransportParams& P) {
 // Klein-Nishina by epsilon-mixture rejection for a photon of energy L.E: eps = E'/E, t = 1 - cos(theta), x4 = a spare uniform for
 // the azimuth; one Philox block per trial.
 template <bool COUNT>
-__device__ __forceinline__ void sample_kn(Lane& L, const TransportParams& P, float& eps, float& t, float& x4, uint32_t* cnt) {
+__device__ __forceinline__ void sample_kn(Lane& L, const TransportParams& P, float& eps, float& t, float& x4, uint32_t* cnt,
+                                          const uint4* first = nullptr) {  // first: the block for the first trial, already computed (rng_peek)
     const float k = L.E * (1.0f / kMec2), e0 = rcp(1.0f + 2.0f * k), e02 = e0 * e0;
     const float a1 = -__logf(e0), a2 = 0.5f * (1.0f - e02);
+    bool peeked = first != nullptr;
 #pragma unroll 1
     for (;;) {
-        const uint4 r = rng_block_hot(L, P);                               // one block per trial
+        uint4 r;
+        if (peeked) { r = *first; L.blk++; peeked = false; } else r = rng_block_hot(L, P);   // one block per trial
         const float x1 = u01(r.x), x2 = u01(r.y), x3 = u01(r.z); x4 = u01(r.w);
         if (COUNT) cnt[12]++;
         eps = (x1 * (a1 + a2) < a1) ? __expf(-x2 * a1) : sqrtf(fmaf(1.0f - e02, x2, e02));
@@ -505,7 +543,8 @@ __device__ __forceinline__ void sample_kn(Lane& L, const TransportParams& P, flo
     }
 }
 template <bool COUNT>
-__device__ __forceinline__ void interact(Lane& L, const TransportParams& P, const Shared& sh, float xsel, float pe, float co, uint32_t* cnt) {
+__device__ __forceinline__ void interact(Lane& L, const TransportParams& P, const Shared& sh, float xsel, float pe, float co, uint32_t* cnt,
+                                         const uint4* nxt = nullptr) {   // nxt: the particle's next Philox block if already computed (rng_peek)
     const bool coupled = P.ph.mode != 0;
     const uint32_t reg = F_REGION(L.flags);
     if (xsel < pe) {                                                       // photoelectric: electron T = E along d
@@ -520,7 +559,7 @@ __device__ __forceinline__ void interact(Lane& L, const TransportParams& P, cons
     if (xsel < pe + co) {                                                  // Compton: Klein-Nishina by epsilon-mixture rejection
         if (COUNT) cnt[4]++;
         float eps, t, x4;
-        sample_kn<COUNT>(L, P, eps, t, x4, cnt);
+        sample_kn<COUNT>(L, P, eps, t, x4, cnt, nxt);
         const float ct = 1.0f - t, st = sqrtf(fmaxf(0.0f, t * (2.0f - t)));
         float sp, cp; __sincosf(2.0f * kPi * x4 - kPi, &sp, &cp);
         const float E0 = L.E, E1 = eps * E0, T = E0 - E1;
@@ -547,7 +586,8 @@ __device__ __forceinline__ void interact(Lane& L, const TransportParams& P, cons
     }
     // pair production: uniform kinetic split, both along d (reading A10)
     if (COUNT) cnt[5]++;
-    const float a = u01(rng_block(L, P).x);
+    float a;
+    if (nxt) { a = u01(nxt->x); L.blk++; } else a = u01(rng_block(L, P).x);
     const float Ttot = L.E - 2.0f * kMec2;
     const float Tm = a * Ttot, Tp = Ttot - Tm;
     if (!coupled) {
@@ -569,36 +609,112 @@ __device__ __forceinline__ void interact(Lane& L, const TransportParams& P, cons
 
 // ---------------------------------------------------------------- photon flights.  Each returns true with (xsel, pe, co)
 // set if the photon collides at its new position (K4 follows).
-// K3: one Woodcock flight in the phantom against the majorant.
+// K3: one Woodcock flight in the phantom.  One exponential optical depth nl is spent along the ray against a majorant that is
+// piecewise constant in two regions (params.h Geom::glo): the global majorant mumaj(E) inside the body box G,
+// f_out x mumaj(E) in the margin between G and the faces of the grid (air around a patient: f_out ~ 1e-3), so that the margin
+// costs no virtual collisions and no extra Philox blocks: a ray meets the convex G in at most one chord, hence at most three
+// segments margin | chord | margin.  The tentative collision is accepted with mu(voxel) / (majorant of its segment).  Same
+// distribution as tracking against one global majorant (pin P4 of the oracle covers any exact tracker).
+#ifndef AEPID_BODY_BOX
+#define AEPID_BODY_BOX 1
+#endif
+__device__ __forceinline__ bool in_box(const float* lo, const float* hi, float x, float y, float z) {
+    return x >= lo[0] && x < hi[0] && y >= lo[1] && y < hi[1] && z >= lo[2] && z < hi[2];
+}
 template <bool COUNT>
-__device__ __forceinline__ bool woodcock_flight(Lane& L, const TransportParams& P, const Shared& sh, float& xsel, float& pe, float& co, uint32_t* cnt) {
+__device__ __forceinline__ bool woodcock_flight(Lane& L, const TransportParams& P, const Shared& sh, float& xsel, float& pe, float& co, uint32_t* cnt,
+                                                uint4* nxt = nullptr) {    // nxt (AEPID_PEEK): in: the block of this flight, out: the particle's next one
     const Geom& g = P.g;
-    const uint4 rr = rng_block_hot(L, P);
+    uint4 rr;
+    if (nxt) { rr = *nxt; L.blk++; } else rr = rng_block_hot(L, P);
     const float u1 = u01(rr.x), u2 = u01(rr.y);
     if (COUNT) cnt[0]++;
-    const float s = __fdividef(-__logf(u1), L.mumaj);
-    const float nx = fmaf(s, L.dx, L.x), ny = fmaf(s, L.dy, L.y), nz = fmaf(s, L.dz, L.z);
-    if (!(nx >= g.lox && nx < g.hix && ny >= g.loy && ny < g.hiy && nz >= g.loz && nz < g.hiz)) {
-        // left the grid: place on the AABB exit point, snapped onto the crossed face
+    float nl = -__logf(u1), sig = L.mumaj;
+    bool collide = false;
+#if AEPID_BODY_BOX
+    const float glo[3] = {g.glo[0], g.glo[1], g.glo[2]}, ghi[3] = {g.ghi[0], g.ghi[1], g.ghi[2]};
+#else
+    const float glo[3] = {g.lox, g.loy, g.loz}, ghi[3] = {g.hix, g.hiy, g.hiz};
+#endif
+    if (!AEPID_BODY_BOX || in_box(glo, ghi, L.x, L.y, L.z)) {          // (without a body box the start is not tested: a photon that
+        const float s = __fdividef(nl, sig);                               //  came in through a high face sits ON it)
+        const float nx = fmaf(s, L.dx, L.x), ny = fmaf(s, L.dy, L.y), nz = fmaf(s, L.dz, L.z);
+        if (in_box(glo, ghi, nx, ny, nz)) { L.x = nx; L.y = ny; L.z = nz; collide = true; }   // the common case: ends inside G
+#if AEPID_BODY_BOX
+        else {                                                             // leaves G first: on to the margin with what is left of nl
+            float tx = kInf, ty = kInf, tz = kInf;
+            if (L.dx != 0.0f) tx = ((L.dx > 0.0f ? ghi[0] : glo[0]) - L.x) * rcp(L.dx);
+            if (L.dy != 0.0f) ty = ((L.dy > 0.0f ? ghi[1] : glo[1]) - L.y) * rcp(L.dy);
+            if (L.dz != 0.0f) tz = ((L.dz > 0.0f ? ghi[2] : glo[2]) - L.z) * rcp(L.dz);
+            const float t = fmaxf(fminf(tx, fminf(ty, tz)), 0.0f);
+            nl = fmaxf(nl - sig * t, 0.0f);
+            L.x = fmaf(t, L.dx, L.x); L.y = fmaf(t, L.dy, L.y); L.z = fmaf(t, L.dz, L.z);
+            sig = g.f_out * L.mumaj;
+        }
+#endif
+    }
+#if AEPID_BODY_BOX
+    else {                                                                 // starts in the margin: does the ray meet G?
+        sig = g.f_out * L.mumaj;
+        float tn = -kInf, tf = kInf; bool miss = false;
+#define SLAB(P_, D_, LO_, HI_)                                                 \
+        if (fabsf(D_) > 1e-20f) {                                              \
+            const float inv = rcp(D_);                                         \
+            const float t1 = ((LO_) - (P_)) * inv, t2 = ((HI_) - (P_)) * inv;  \
+            tn = fmaxf(tn, fminf(t1, t2)); tf = fminf(tf, fmaxf(t1, t2));      \
+        } else if ((P_) < (LO_) || (P_) >= (HI_)) miss = true;
+        SLAB(L.x, L.dx, glo[0], ghi[0])
+        SLAB(L.y, L.dy, glo[1], ghi[1])
+        SLAB(L.z, L.dz, glo[2], ghi[2])
+#undef SLAB
+        if (!miss && tf > 0.0f && tn < tf) {
+            tn = fmaxf(tn, 0.0f);
+            if (nl < sig * tn) {                                           // collides in the margin before G
+                const float s = __fdividef(nl, sig);
+                L.x = fmaf(s, L.dx, L.x); L.y = fmaf(s, L.dy, L.y); L.z = fmaf(s, L.dz, L.z); collide = true;
+            } else {
+                nl -= sig * tn;
+                const float chord = tf - tn;
+                if (nl < L.mumaj * chord) {                                // collides on the chord through G
+                    const float s = tn + __fdividef(nl, L.mumaj);
+                    L.x = fmaf(s, L.dx, L.x); L.y = fmaf(s, L.dy, L.y); L.z = fmaf(s, L.dz, L.z); collide = true; sig = L.mumaj;
+                } else {                                                   // through G: the margin behind it
+                    nl -= L.mumaj * chord;
+                    L.x = fmaf(tf, L.dx, L.x); L.y = fmaf(tf, L.dy, L.y); L.z = fmaf(tf, L.dz, L.z);
+                }
+            }
+        }
+    }
+#endif
+    if (!collide) {
+        // margin up to the faces of the grid (without a body box: the photon is on its way out, sig x t = 0 < nl never holds)
         float tx = kInf, ty = kInf, tz = kInf;
         if (L.dx != 0.0f) tx = ((L.dx > 0.0f ? g.hix : g.lox) - L.x) * rcp(L.dx);
         if (L.dy != 0.0f) ty = ((L.dy > 0.0f ? g.hiy : g.loy) - L.y) * rcp(L.dy);
         if (L.dz != 0.0f) tz = ((L.dz > 0.0f ? g.hiz : g.loz) - L.z) * rcp(L.dz);
         const float t = fmaxf(fminf(tx, fminf(ty, tz)), 0.0f);
-        L.x = fmaf(t, L.dx, L.x); L.y = fmaf(t, L.dy, L.y); L.z = fmaf(t, L.dz, L.z);
-        if (tx <= ty && tx <= tz) L.x = L.dx > 0.0f ? g.hix : g.lox;
-        else if (ty <= tz) L.y = L.dy > 0.0f ? g.hiy : g.loy;
-        else L.z = L.dz > 0.0f ? g.hiz : g.loz;
-        SET_REGION(L.flags, R_AIR);
-        return false;
+        if (AEPID_BODY_BOX && nl < sig * t) {
+            const float s = __fdividef(nl, sig);
+            L.x = fmaf(s, L.dx, L.x); L.y = fmaf(s, L.dy, L.y); L.z = fmaf(s, L.dz, L.z); collide = true;
+        } else {
+            // left the grid: place on the AABB exit point, snapped onto the crossed face
+            L.x = fmaf(t, L.dx, L.x); L.y = fmaf(t, L.dy, L.y); L.z = fmaf(t, L.dz, L.z);
+            if (tx <= ty && tx <= tz) L.x = L.dx > 0.0f ? g.hix : g.lox;
+            else if (ty <= tz) L.y = L.dy > 0.0f ? g.hiy : g.loy;
+            else L.z = L.dz > 0.0f ? g.hiz : g.loz;
+            SET_REGION(L.flags, R_AIR);
+            return false;
+        }
     }
-    L.x = nx; L.y = ny; L.z = nz;
-    const int ix = min((int)((nx - g.lox) * g.ihx), g.nx - 1), iy = min((int)((ny - g.loy) * g.ihy), g.ny - 1), iz = min((int)((nz - g.loz) * g.ihz), g.nz - 1);
+    const int ix = min(max((int)((L.x - g.lox) * g.ihx), 0), g.nx - 1), iy = min(max((int)((L.y - g.loy) * g.ihy), 0), g.ny - 1),
+              iz = min(max((int)((L.z - g.loz) * g.ihz), 0), g.nz - 1);
     const uint32_t w = __ldg(P.vox + ((size_t)iz * g.ny + iy) * g.nx + ix);
+    if (nxt) *nxt = rng_peek(L, P);                                        // ten Philox rounds while the gather is on its way
     const float rho = __uint_as_float(w & ~31u);
     float pp;
     mu3(P, sh, (int)(w & 31u), L.ci, L.ct, L.E, pe, co, pp);
-    xsel = u2 * L.mumaj;
+    xsel = u2 * sig;
+    if (COUNT && rho * (pe + co + pp) > sig) cnt[31]++;                    // the majorant of the segment does not bound this voxel: must never happen
     if (xsel < rho * (pe + co + pp)) {
         xsel = __fdividef(xsel, rho);                                      // reuse the accept draw for the channel (reading A8)
         L.cw = w; L.vox = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20);
@@ -1071,6 +1187,44 @@ __device__ __forceinline__ void charged_event(Lane& L, const TransportParams& P,
     }
 }
 
+// The same event for a whole warp (all lanes call, `on` says which hold a particle to step): the warp goes on to its next
+// refill as soon as fewer than kAdapt lanes are still stepping, instead of idling through the remaining steps of the event.
+// The test sits on Philox block boundaries only (mode 1: every second step), so that the blocks a particle consumes, and with
+// them its trajectory, do not depend on what the other lanes of the warp do.
+#ifndef AEPID_ADAPT
+#define AEPID_ADAPT 0
+#endif
+constexpr int kAdapt = AEPID_ADAPT;
+template <bool COUNT, bool PHANTOM, int PH>
+__device__ __forceinline__ void charged_event_warp(bool on, Lane& L, const TransportParams& P, const Shared& sh, uint32_t* cnt) {
+    constexpr bool C2 = PH == 2 || PH == 3;
+    bool go = on;
+    if (go && L.E <= P.ph.ecut) { stop_charged<COUNT>(L, P, cnt); go = false; }
+    uint4 r = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll 1
+    for (int k = 0; k < (PHANTOM ? kStepsE : kStepsX); ++k) {
+        if (go) {
+            if (C2) {
+                r = PHANTOM ? rng_block_hot(L, P) : rng_block(L, P);
+                if (PHANTOM) electron_step_phantom<COUNT, PH>(L, P, sh, r.x, r.y, r.z, r.w, cnt);
+                else electron_step_outside<COUNT, PH>(L, P, sh, r.x, r.y, r.z, r.w, cnt);
+            } else {
+                if (!(k & 1)) r = PHANTOM ? rng_block_hot(L, P) : rng_block(L, P);
+                if (PHANTOM) electron_step_phantom<COUNT, 1>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, 0u, 0u, cnt);
+                else electron_step_outside<COUNT, 1>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, 0u, 0u, cnt);
+            }
+            go = L.alive;
+            if (go && L.E <= P.ph.ecut) {
+                if (F_TYPE(L.flags) == T_ELECTRON) { dep_here(L, P, L.E); L.alive = false; }
+                go = false;
+            }
+            if (go && (F_REGION(L.flags) == R_PHANTOM) != PHANTOM) go = false;
+            if (C2 && go && L.spare == kNone) go = false;
+        }
+        if ((C2 || (k & 1)) && __popc(__ballot_sync(FULL_MASK, go)) < kAdapt) break;
+    }
+}
+
 // ---------------------------------------------------------------- collimation stage
 // A photon sampled from Phase Space 1 is followed through the jaws and the MLC down to the Phase Space 2 plane (readings
 // A35-A37): inside the w-range of a slab every point outside the opening of its row is tungsten, everything else is air;
@@ -1298,6 +1452,9 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
     const int keep = *((volatile int*)&s_keep);
     bool leaving = false, park = false, did = false, parked = false;
     float h_n = 0.0f, h_E = 0.0f, h_dep = 0.0f;                 // collimation stage (class A only): Phase Space 2 particles, their energy, absorbed
+#if AEPID_PEEK
+    uint4 nxt = make_uint4(0u, 0u, 0u, 0u); bool have_nxt = false;  // class W: the lane's next Philox block, computed ahead of its use
+#endif
     // every lane enters a phase empty: saying so lets the compiler drop what this class never touches from the registers
     L.a_emit = L.a_ph = L.a_eps = L.a_epo = L.a_air = L.a_esc = 0.0f;
     L.alive = false; L.counted = kNone; L.spare = kNone; L.pval = 0.0f; L.pidx = kNone;
@@ -1305,7 +1462,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
     for (uint32_t it = 1;; ++it) {
         // ---- A: particles that left the class (or all of them, when the warp leaves) go to the queue of their class;
         //         the count of a dead particle becomes the lane's credit or is given back
-        if (!(L.alive && !leaving && !park && class_of(L.flags) == C)) {
+        if (!(L.alive && !leaving && !park && in_class<C>(L.flags))) {
             flush_pending(L, P);
             if (L.alive) {
                 queue_particle(L.x, L.y, L.z, L.dx, L.dy, L.dz, L.E, L.vox, L.flags, L.h, L.pid, L.blk, PH == 4 ? L.R : 0.0f);
@@ -1342,6 +1499,9 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                 L.flags = c.x; L.h = c.y; L.pid = c.z; L.blk = c.w;
                 L.counted = 1u; L.alive = true;
                 L.pval = 0.0f; L.pidx = kNone;
+#if AEPID_PEEK
+                have_nxt = false;
+#endif
                 if (COUNT && !kPhaseClock) cnt[28]++;
                 if (C == C_A || C == C_W || C == C_P) set_energy(L, P, sh);
                 if (C == C_E) { L.vlin = vox_linear(P.g, L.vox); L.cw = __ldg(P.vox + L.vlin); L.pidx = L.vlin; }
@@ -1430,12 +1590,27 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
             bool fly = on;
             if (on && L.E < P.ph.pcut) { if (COUNT) cnt[13]++; dep_here(L, P, L.E); L.alive = false; fly = false; }   // PAPER.md:104, 10 keV
             bool hit = false; float xsel = 0.0f, pe = 0.0f, co = 0.0f;
+#if AEPID_PEEK
+            if (fly && !have_nxt) { nxt = rng_peek(L, P); have_nxt = true; }
+#endif
 #pragma unroll 1
             for (int round = 0; round < kMaxRounds; ++round) {
+#if AEPID_PEEK
+                if (fly) { hit = woodcock_flight<COUNT>(L, P, sh, xsel, pe, co, cnt, &nxt); fly = !hit && F_REGION(L.flags) == R_PHANTOM; }
+#else
                 if (fly) { hit = woodcock_flight<COUNT>(L, P, sh, xsel, pe, co, cnt); fly = !hit && F_REGION(L.flags) == R_PHANTOM; }
+#endif
                 if (__popc(__ballot_sync(FULL_MASK, hit)) >= kHitMin || __ballot_sync(FULL_MASK, fly) == 0u) break;
             }
+#if AEPID_PEEK
+            if (hit) { interact<COUNT>(L, P, sh, xsel, pe, co, cnt, &nxt); have_nxt = false; }
+            if (!fly) have_nxt = false;                                    // left the grid (its last flight computed no next block) or not flying
+#else
             if (hit) interact<COUNT>(L, P, sh, xsel, pe, co, cnt);
+#endif
+        } else if (kAdapt > 0 && PH != 4 && (C == C_E || C == C_X)) {
+            if (C == C_E) charged_event_warp<COUNT, true, PH>(on, L, P, sh, cnt);
+            else charged_event_warp<COUNT, false, PH>(on, L, P, sh, cnt);
         } else if (on) {
             if (C == C_E) charged_event<COUNT, true, PH>(L, P, sh, cnt);
             else if (C == C_X) charged_event<COUNT, false, PH>(L, P, sh, cnt);

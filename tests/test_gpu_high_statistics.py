@@ -1,4 +1,6 @@
-"""High-statistics parity run: every channel of the energy budget and the depth dose, GPU against K = 10 independent oracle runs.
+"""High-statistics parity run: every channel of the energy budget and the depth dose, GPU against K = 20 independent oracle runs
+(the spread of every channel and slab is estimated from them: with K = 10 a z-score is t-distributed with 9 degrees of freedom and
+one of 72 slabs passes 5.5 by chance in 3 % of the runs; with K = 20 in 0.2 %).
 
 By default 4e7 (C1), 2e7 (C2 at half resolution) and 2e7 (C1, physics mode 3) oracle histories (about a minute each on the
 GPU box's host cores), which resolves the channels to a few 1e-4.  AEPID_LONG=1 runs 5e8 / 1e8 / 1e8 oracle histories against
@@ -27,7 +29,7 @@ def test_energy_budget_and_depth_dose_to_1e4(name, shrink, mode, n_or, n_gpu):
     eng.simulate(n_gpu, 77)
     r = eng.read_tallies(); L = r["ledger"]
     assert L[7] == 0
-    K, per = 10, n_or // 10                                 # K independent oracle runs give the spread of every channel
+    K = 20; per = n_or // K                                 # K independent oracle runs give the spread of every channel
     runs = [oracle.run_sharded(cfg, per, 78, first=k * per, want_phantom_sq=False) for k in range(K)]
     Lo = np.array([x["ledger"] for x in runs])
     print("\n%s mode %d: gpu %.1e histories, oracle %.1e" % (name, mode, n_gpu, n_or))
