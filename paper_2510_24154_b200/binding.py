@@ -12,7 +12,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libaepid.so")
+# AEPID_LIBRARY: another build of the same library (the checked build of build.build_checked, tests/test_gpu_checked_build.py)
+LIB_PATH = os.environ.get("AEPID_LIBRARY") or os.path.join(_HERE, "libaepid.so")
 _lib = None
 
 STATUS = {0: "OK", -1: "BAD_ARG", -2: "BAD_STATE", -3: "GEOMETRY", -4: "CUDA", -5: "NOMEM", -6: "INTERNAL"}

@@ -51,5 +51,24 @@ def build(force=False, verbose=False):
     return LIB
 
 
+LIB_CHECKED = os.path.join(HERE, "libaepid_checked.so")
+
+
+def build_checked(force=False):
+    """The same library with the transport kernel compiled -DAEPID_CHECKED (index and queue-protocol checks inside the kernel,
+    csrc/transport.cu); used by tests/test_gpu_checked_build.py through the AEPID_LIBRARY environment variable."""
+    build(force=force)
+    src = os.path.join(CSRC, "transport.cu")
+    if not force and os.path.exists(LIB_CHECKED) and all(os.path.getmtime(d) <= os.path.getmtime(LIB_CHECKED) for d in [src, LIB] + HEADERS):
+        return LIB_CHECKED
+    o = os.path.join(CSRC, "transport_checked.o")
+    subprocess.check_call([nvcc()] + NVCC_FLAGS + EXTRA_FLAGS["transport.cu"] + ["-DAEPID_CHECKED", "-c", src, "-o", o])
+    objs = [o] + [os.path.join(CSRC, s.replace(".cu", ".o")) for s in SOURCES if s != "transport.cu"]
+    subprocess.check_call([nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB_CHECKED] + objs + ["-lcudart_static", "-ldl", "-lrt", "-lpthread"])
+    return LIB_CHECKED
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--checked" in sys.argv:
+        print(build_checked(force="--force" in sys.argv))

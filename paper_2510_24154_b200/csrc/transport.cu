@@ -123,21 +123,14 @@ __device__ __forceinline__ int class_of(uint32_t flags) {
 }
 
 // is the particle with these flags in class C?  (class_of(flags) == C, as two or three bit tests)
-#ifndef AEPID_INCLASS
-#define AEPID_INCLASS 1
-#endif
 template <int C>
 __device__ __forceinline__ bool in_class(uint32_t flags) {
-#if AEPID_INCLASS
     constexpr uint32_t kTR = 3u | (3u << 2);                                    // type and region bits
     if (C == C_W) return (flags & kTR) == (T_PHOTON | (R_PHANTOM << 2));
     if (C == C_A) return (flags & (kTR | F_HIT)) == (T_PHOTON | (R_AIR << 2));
     if (C == C_P) return (flags & 3u) == T_PHOTON && (flags & (3u << 2)) != (R_PHANTOM << 2) && (flags & ((3u << 2) | F_HIT)) != (R_AIR << 2);
     if (C == C_E) return (flags & 3u) != T_PHOTON && (flags & (3u << 2)) == (R_PHANTOM << 2);
     return (flags & 3u) != T_PHOTON && (flags & (3u << 2)) != (R_PHANTOM << 2);
-#else
-    return class_of(flags) == C;
-#endif
 }
 
 // Scheduler state and the geometry copy: static shared memory, so that the out-of-line helpers reach them
@@ -159,10 +152,33 @@ __shared__ int s_live_max;                          // limit of s_live for this 
 __shared__ int s_live;                              // particles alive in this CTA (in the queues, in lanes) + head-room credits held by lanes
 extern __shared__ __align__(16) unsigned char smem_raw[];   // per-warp ledger | table blob
 
+// error bits (summed over CTAs into ledger[7]): 2 no head room for a secondary, 8 scheduler found no
+// runnable phase or ran out of phases
+__device__ __forceinline__ void raise_error(int bit) { atomicOr(s_flag + 1, bit); }
+// Checked build (-DAEPID_CHECKED, tests/test_gpu_checked_build.py): every index that reaches global memory (voxel words, tally
+// bins, queue records) and the invariants of the queue protocol are tested in the kernel; a violation raises error bit 16,
+// which aepid_read_tallies / aepid_synchronize return as AEPID_ERR_INTERNAL.  (compute-sanitizer is closed on the GPU pool
+// this was developed on; the checks cost about 4 % and are compiled out of the product build.)
+#ifdef AEPID_CHECKED
+#define AEPID_CHECK(cond) do { if (!(cond)) raise_error(16); } while (0)
+__shared__ unsigned int s_head0[kRings];            // head of every queue when the phase began (queue protocol: tail - head0 <= kPool)
+#else
+#define AEPID_CHECK(cond) do { } while (0)
+#endif
+
+
 __shared__ uint32_t s_pool_mask;                    // records per class queue - 1
 __shared__ int s_pool_log;
 __shared__ uint32_t s_rec_vec;                      // 16-byte vectors per particle record: 3, or 4 in physics mode 4 (the leg's energy budget)
+#ifndef AEPID_RING_BASE
+#define AEPID_RING_BASE 1
+#endif
+__shared__ uint4* s_ring_base[kRings];              // first record of every class queue of this CTA
+#if AEPID_RING_BASE
+__device__ __forceinline__ uint4* queue_rec(int r, uint32_t ticket) { return s_ring_base[r] + (ticket & s_pool_mask) * s_rec_vec; }
+#else
 __device__ __forceinline__ uint4* queue_rec(int r, uint32_t ticket) { return s_queue + ((((size_t)r) << s_pool_log) + (ticket & s_pool_mask)) * s_rec_vec; }
+#endif
 struct Shared {
     const float4* phot;
     const float* maj;
@@ -226,23 +242,6 @@ __device__ __forceinline__ uint4 rng_block_hot(Lane& L, const TransportParams& P
     L.blk++;
     return make_uint4(c0, c1, c2, c3);
 }
-// The block the particle will draw next, without consuming it (Woodcock flights compute it while the voxel gather of the
-// flight before is in flight, AEPID_PEEK); whoever uses it increments L.blk.
-#ifndef AEPID_PEEK
-#define AEPID_PEEK 0
-#endif
-__device__ __forceinline__ uint4 rng_peek(const Lane& L, const TransportParams& P) {
-    const uint64_t h = P.base + L.h;
-    uint32_t c0 = (uint32_t)h, c1 = (uint32_t)(h >> 32), c2 = L.pid, c3 = L.blk;
-#pragma unroll
-    for (int r = 0; r < 10; ++r) {
-        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-        const uint32_t n0 = hi1 ^ c1 ^ P.rk[2 * r], n2 = hi0 ^ c3 ^ P.rk[2 * r + 1];
-        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
-    }
-    return make_uint4(c0, c1, c2, c3);
-}
 __device__ __forceinline__ uint32_t child_id(const Lane& L, uint32_t sibling) {    // reading A1
     return L.pid * 0x9E3779B1u + L.blk * 2u + sibling + 1u;
 }
@@ -303,10 +302,43 @@ __device__ __forceinline__ void rotate(float& dx, float& dy, float& dz, float ct
     dx = nx * inv; dy = ny * inv; dz = nz * inv;
 }
 
+// voxel word through the read-only path; -DAEPID_VOX_EVICT_LAST=1 asks the L2 to keep voxel lines in preference to the streaming
+// queue records and tallies (measured: profiles/r02_README.md)
+#ifndef AEPID_VOX_EVICT_LAST
+#define AEPID_VOX_EVICT_LAST 0
+#endif
+__device__ __forceinline__ uint32_t ld_vox(const uint32_t* p) {
+#if AEPID_VOX_EVICT_LAST
+    uint64_t pol; uint32_t v;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("ld.global.nc.L2::cache_hint.u32 %0, [%1], %2;" : "=r"(v) : "l"(p), "l"(pol));
+    return v;
+#else
+    return __ldg(p);
+#endif
+}
 // ---------------------------------------------------------------- tallies
+// One RED per deposit.  -DAEPID_MATCH_TALLY=1 is the measured alternative north_star names (warp-aggregated atomics): the lanes
+// of the warp that score into the same bin are found with match.any, their values are summed by shuffles and the lowest lane
+// issues one RED (profiles/r02_README.md has both timings).
+#ifndef AEPID_MATCH_TALLY
+#define AEPID_MATCH_TALLY 0
+#endif
+__device__ __forceinline__ void tally_add(float* addr, float v) {
+#if AEPID_MATCH_TALLY
+    const unsigned act = __activemask();
+    const unsigned peers = __match_any_sync(act, (unsigned long long)addr);
+    float sum = 0.0f;
+    for (unsigned m = peers; m; m &= m - 1u) sum += __shfl_sync(peers, v, __ffs(m) - 1);
+    if ((threadIdx.x & 31u) == (unsigned)(__ffs(peers) - 1)) atomicAdd(addr, sum);
+#else
+    atomicAdd(addr, v);
+#endif
+}
 __device__ __forceinline__ void flush_pending(Lane& L, const TransportParams& P) {
     if (L.pval != 0.0f) {
-        atomicAdd(P.ph_batch + (size_t)F_BATCH(L.flags) * P.nvox + L.pidx, L.pval);
+        AEPID_CHECK(L.pidx < P.nvox && F_BATCH(L.flags) < (uint32_t)P.n_batches);
+        tally_add(P.ph_batch + (size_t)F_BATCH(L.flags) * P.nvox + L.pidx, L.pval);
         L.pval = 0.0f;
     }
 }
@@ -324,7 +356,8 @@ __device__ __noinline__ bool score_epid(uint32_t flags, float u, float v, float 
     if (!s_g.lscored[F_LAYER(flags)]) return false;
     const float fu = floorf((u + s_g.half_u) * s_g.inv_pitch), fv = floorf((v + s_g.half_v) * s_g.inv_pitch);
     if (!(fu >= 0.0f && fu < (float)s_g.nu && fv >= 0.0f && fv < (float)s_g.nv)) return false;
-    atomicAdd(s_ep_batch + (size_t)F_BATCH(flags) * s_npix + (size_t)fv * s_g.nu + (size_t)fu, e);
+    AEPID_CHECK((size_t)fv * s_g.nu + (size_t)fu < s_npix);
+    tally_add(s_ep_batch + (size_t)F_BATCH(flags) * s_npix + (size_t)fv * s_g.nu + (size_t)fu, e);
     return true;
 }
 __device__ __forceinline__ void dep_epid(Lane& L, float u, float v, float e) {
@@ -395,7 +428,8 @@ __device__ __forceinline__ void enter_phantom(Lane& L, const TransportParams& P,
         L.x = fx; L.y = fy; L.z = fz;
         L.vox = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20);
         L.vlin = vox_linear(g, L.vox);
-        L.cw = __ldg(P.vox + L.vlin);
+        AEPID_CHECK(L.vlin < P.nvox);
+        L.cw = ld_vox(P.vox + L.vlin);
     }
 }
 __device__ __forceinline__ void enter_epid(Lane& L, const Geom& g) {       // position already on the top plane
@@ -449,9 +483,6 @@ __device__ __forceinline__ void world_to_frac(const Geom& g, uint32_t vox, float
 }
 
 // ---------------------------------------------------------------- class queues (protocol in the header comment)
-// error bits (summed over CTAs into ledger[7]): 2 no head room for a secondary, 8 scheduler found no
-// runnable phase or ran out of phases
-__device__ __forceinline__ void raise_error(int bit) { atomicOr(s_flag + 1, bit); }
 
 // lane 0 claims up to `want` entries of ring r; returns count | first ticket << 32 (warp-uniform, all lanes call)
 __device__ __noinline__ unsigned long long ring_claim(int r, int want) {
@@ -480,7 +511,12 @@ __device__ __noinline__ int budget_claim(int want) {
 __device__ __noinline__ void queue_particle(float x, float y, float z, float dx, float dy, float dz, float E,
                                             uint32_t vox, uint32_t flags, uint32_t h, uint32_t pid, uint32_t blk, float R = 0.0f) {
     const int r = class_of(flags);
-    uint4* rec = queue_rec(r, atomicAdd(s_tail + r, 1u));
+    const uint32_t tk = atomicAdd(s_tail + r, 1u);
+    // the record written must not be one a pop of this phase may still read: tickets in flight fit one queue (header comment)
+#ifdef AEPID_CHECKED
+    AEPID_CHECK(r >= 0 && r < kClasses && tk - s_head0[r] <= s_pool_mask);
+#endif
+    uint4* rec = queue_rec(r, tk);
     __stcs(rec + 0, make_uint4(__float_as_uint(x), __float_as_uint(y), __float_as_uint(z), __float_as_uint(dx)));
     __stcs(rec + 1, make_uint4(__float_as_uint(dy), __float_as_uint(dz), __float_as_uint(E), vox));
     __stcs(rec + 2, make_uint4(flags, h, pid, blk));
@@ -525,15 +561,12 @@ __device__ __forceinline__ void annihilate(Lane& L, const TransportParams& P) {
 // Klein-Nishina by epsilon-mixture rejection for a photon of energy L.E: eps = E'/E, t = 1 - cos(theta), x4 = a spare uniform for
 // the azimuth; one Philox block per trial.
 template <bool COUNT>
-__device__ __forceinline__ void sample_kn(Lane& L, const TransportParams& P, float& eps, float& t, float& x4, uint32_t* cnt,
-                                          const uint4* first = nullptr) {  // first: the block for the first trial, already computed (rng_peek)
+__device__ __forceinline__ void sample_kn(Lane& L, const TransportParams& P, float& eps, float& t, float& x4, uint32_t* cnt) {
     const float k = L.E * (1.0f / kMec2), e0 = rcp(1.0f + 2.0f * k), e02 = e0 * e0;
     const float a1 = -__logf(e0), a2 = 0.5f * (1.0f - e02);
-    bool peeked = first != nullptr;
 #pragma unroll 1
     for (;;) {
-        uint4 r;
-        if (peeked) { r = *first; L.blk++; peeked = false; } else r = rng_block_hot(L, P);   // one block per trial
+        const uint4 r = rng_block_hot(L, P);                               // one block per trial
         const float x1 = u01(r.x), x2 = u01(r.y), x3 = u01(r.z); x4 = u01(r.w);
         if (COUNT) cnt[12]++;
         eps = (x1 * (a1 + a2) < a1) ? __expf(-x2 * a1) : sqrtf(fmaf(1.0f - e02, x2, e02));
@@ -543,8 +576,7 @@ __device__ __forceinline__ void sample_kn(Lane& L, const TransportParams& P, flo
     }
 }
 template <bool COUNT>
-__device__ __forceinline__ void interact(Lane& L, const TransportParams& P, const Shared& sh, float xsel, float pe, float co, uint32_t* cnt,
-                                         const uint4* nxt = nullptr) {   // nxt: the particle's next Philox block if already computed (rng_peek)
+__device__ __forceinline__ void interact(Lane& L, const TransportParams& P, const Shared& sh, float xsel, float pe, float co, uint32_t* cnt) {
     const bool coupled = P.ph.mode != 0;
     const uint32_t reg = F_REGION(L.flags);
     if (xsel < pe) {                                                       // photoelectric: electron T = E along d
@@ -559,7 +591,7 @@ __device__ __forceinline__ void interact(Lane& L, const TransportParams& P, cons
     if (xsel < pe + co) {                                                  // Compton: Klein-Nishina by epsilon-mixture rejection
         if (COUNT) cnt[4]++;
         float eps, t, x4;
-        sample_kn<COUNT>(L, P, eps, t, x4, cnt, nxt);
+        sample_kn<COUNT>(L, P, eps, t, x4, cnt);
         const float ct = 1.0f - t, st = sqrtf(fmaxf(0.0f, t * (2.0f - t)));
         float sp, cp; __sincosf(2.0f * kPi * x4 - kPi, &sp, &cp);
         const float E0 = L.E, E1 = eps * E0, T = E0 - E1;
@@ -586,8 +618,7 @@ __device__ __forceinline__ void interact(Lane& L, const TransportParams& P, cons
     }
     // pair production: uniform kinetic split, both along d (reading A10)
     if (COUNT) cnt[5]++;
-    float a;
-    if (nxt) { a = u01(nxt->x); L.blk++; } else a = u01(rng_block(L, P).x);
+    const float a = u01(rng_block(L, P).x);
     const float Ttot = L.E - 2.0f * kMec2;
     const float Tm = a * Ttot, Tp = Ttot - Tm;
     if (!coupled) {
@@ -622,11 +653,9 @@ __device__ __forceinline__ bool in_box(const float* lo, const float* hi, float x
     return x >= lo[0] && x < hi[0] && y >= lo[1] && y < hi[1] && z >= lo[2] && z < hi[2];
 }
 template <bool COUNT>
-__device__ __forceinline__ bool woodcock_flight(Lane& L, const TransportParams& P, const Shared& sh, float& xsel, float& pe, float& co, uint32_t* cnt,
-                                                uint4* nxt = nullptr) {    // nxt (AEPID_PEEK): in: the block of this flight, out: the particle's next one
+__device__ __forceinline__ bool woodcock_flight(Lane& L, const TransportParams& P, const Shared& sh, float& xsel, float& pe, float& co, uint32_t* cnt) {
     const Geom& g = P.g;
-    uint4 rr;
-    if (nxt) { rr = *nxt; L.blk++; } else rr = rng_block_hot(L, P);
+    const uint4 rr = rng_block_hot(L, P);
     const float u1 = u01(rr.x), u2 = u01(rr.y);
     if (COUNT) cnt[0]++;
     float nl = -__logf(u1), sig = L.mumaj;
@@ -708,8 +737,8 @@ __device__ __forceinline__ bool woodcock_flight(Lane& L, const TransportParams& 
     }
     const int ix = min(max((int)((L.x - g.lox) * g.ihx), 0), g.nx - 1), iy = min(max((int)((L.y - g.loy) * g.ihy), 0), g.ny - 1),
               iz = min(max((int)((L.z - g.loz) * g.ihz), 0), g.nz - 1);
-    const uint32_t w = __ldg(P.vox + ((size_t)iz * g.ny + iy) * g.nx + ix);
-    if (nxt) *nxt = rng_peek(L, P);                                        // ten Philox rounds while the gather is on its way
+    AEPID_CHECK(ix >= 0 && iy >= 0 && iz >= 0 && ((size_t)iz * g.ny + iy) * g.nx + ix < P.nvox);
+    const uint32_t w = ld_vox(P.vox + ((size_t)iz * g.ny + iy) * g.nx + ix);
     const float rho = __uint_as_float(w & ~31u);
     float pp;
     mu3(P, sh, (int)(w & 31u), L.ci, L.ct, L.E, pe, co, pp);
@@ -944,12 +973,13 @@ __device__ __forceinline__ void electron_step_phantom(Lane& L, const TransportPa
     const bool inside = ni >= 0 && ni < nmax;
     L.x = (cross && ax0) ? nf : L.x; L.y = (cross && ax1) ? nf : L.y; L.z = (cross && ax2) ? nf : L.z;
     if (cross && inside) {
-        if (L.pval != 0.0f) atomicAdd(P.ph_batch + (size_t)F_BATCH(L.flags) * P.nvox + L.vlin, L.pval);
+        if (L.pval != 0.0f) tally_add(P.ph_batch + (size_t)F_BATCH(L.flags) * P.nvox + L.vlin, L.pval);
         L.pval = 0.0f;
         L.vox = (L.vox & ~(1023u << sh10)) | ((uint32_t)ni << sh10);
         L.vlin += (uint32_t)(up ? stride : -stride);
         L.pidx = L.vlin;
-        L.cw = __ldg(P.vox + L.vlin);
+        AEPID_CHECK(L.vlin < P.nvox && L.vlin == vox_linear(g, L.vox));
+        L.cw = ld_vox(P.vox + L.vlin);
     }
     if (cross && !inside) {                                                // rare: leaves the grid
         frac_to_world(L, g);                                               // uses the old index; then snap the crossed axis
@@ -1088,12 +1118,13 @@ __device__ __forceinline__ void hinge_segment_phantom(Lane& L, const TransportPa
         const int ni = (int)((L.vox >> sh10) & 1023u) + (up ? 1 : -1);
         L.x = ax0 ? nf : L.x; L.y = ax1 ? nf : L.y; L.z = ax2 ? nf : L.z;
         if (ni >= 0 && ni < nmax) {
-            if (L.pval != 0.0f) atomicAdd(P.ph_batch + (size_t)F_BATCH(L.flags) * P.nvox + L.vlin, L.pval);
+            if (L.pval != 0.0f) tally_add(P.ph_batch + (size_t)F_BATCH(L.flags) * P.nvox + L.vlin, L.pval);
             L.pval = 0.0f;
             L.vox = (L.vox & ~(1023u << sh10)) | ((uint32_t)ni << sh10);
             L.vlin += (uint32_t)(up ? stride : -stride);
             L.pidx = L.vlin;
-            L.cw = __ldg(P.vox + L.vlin);
+            AEPID_CHECK(L.vlin < P.nvox && L.vlin == vox_linear(g, L.vox));
+            L.cw = ld_vox(P.vox + L.vlin);
         } else {                                                           // leaves the grid
             frac_to_world(L, g);
             if (ax0) L.x = up ? g.hix : g.lox; else if (ax1) L.y = up ? g.hiy : g.loy; else L.z = up ? g.hiz : g.loz;
@@ -1184,44 +1215,6 @@ __device__ __forceinline__ void charged_event(Lane& L, const TransportParams& P,
         }
         if ((F_REGION(L.flags) == R_PHANTOM) != PHANTOM) break;
         if (C2 && L.spare == kNone) break;                                 // the credit went into a delta ray: the next step needs a new one
-    }
-}
-
-// The same event for a whole warp (all lanes call, `on` says which hold a particle to step): the warp goes on to its next
-// refill as soon as fewer than kAdapt lanes are still stepping, instead of idling through the remaining steps of the event.
-// The test sits on Philox block boundaries only (mode 1: every second step), so that the blocks a particle consumes, and with
-// them its trajectory, do not depend on what the other lanes of the warp do.
-#ifndef AEPID_ADAPT
-#define AEPID_ADAPT 0
-#endif
-constexpr int kAdapt = AEPID_ADAPT;
-template <bool COUNT, bool PHANTOM, int PH>
-__device__ __forceinline__ void charged_event_warp(bool on, Lane& L, const TransportParams& P, const Shared& sh, uint32_t* cnt) {
-    constexpr bool C2 = PH == 2 || PH == 3;
-    bool go = on;
-    if (go && L.E <= P.ph.ecut) { stop_charged<COUNT>(L, P, cnt); go = false; }
-    uint4 r = make_uint4(0u, 0u, 0u, 0u);
-#pragma unroll 1
-    for (int k = 0; k < (PHANTOM ? kStepsE : kStepsX); ++k) {
-        if (go) {
-            if (C2) {
-                r = PHANTOM ? rng_block_hot(L, P) : rng_block(L, P);
-                if (PHANTOM) electron_step_phantom<COUNT, PH>(L, P, sh, r.x, r.y, r.z, r.w, cnt);
-                else electron_step_outside<COUNT, PH>(L, P, sh, r.x, r.y, r.z, r.w, cnt);
-            } else {
-                if (!(k & 1)) r = PHANTOM ? rng_block_hot(L, P) : rng_block(L, P);
-                if (PHANTOM) electron_step_phantom<COUNT, 1>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, 0u, 0u, cnt);
-                else electron_step_outside<COUNT, 1>(L, P, sh, (k & 1) ? r.z : r.x, (k & 1) ? r.w : r.y, 0u, 0u, cnt);
-            }
-            go = L.alive;
-            if (go && L.E <= P.ph.ecut) {
-                if (F_TYPE(L.flags) == T_ELECTRON) { dep_here(L, P, L.E); L.alive = false; }
-                go = false;
-            }
-            if (go && (F_REGION(L.flags) == R_PHANTOM) != PHANTOM) go = false;
-            if (C2 && go && L.spare == kNone) go = false;
-        }
-        if ((C2 || (k & 1)) && __popc(__ballot_sync(FULL_MASK, go)) < kAdapt) break;
     }
 }
 
@@ -1378,9 +1371,13 @@ __device__ __noinline__ void choose_phase(const TransportParams& P, unsigned lon
     int n[kRings];
 #pragma unroll
     for (int r = 0; r < kRings; ++r) { s_snap[r] = s_tail[r]; n[r] = (int)(s_snap[r] - s_head[r]); }
+#ifdef AEPID_CHECKED
+    for (int r = 0; r < kRings; ++r) { s_head0[r] = s_head[r]; AEPID_CHECK(n[r] >= 0 && n[r] <= s_live_max); }
+#endif
     int n_live = 0;
 #pragma unroll
     for (int c = 0; c < kClasses; ++c) n_live += n[c];
+    AEPID_CHECK(s_nphase == 0u || s_live == n_live);           // every credit was given back, every death was counted
     s_live = n_live;                                           // between phases every particle sits in a queue and no lane holds a credit
     // Progress check.  A phase in which every lane that could have run an event parked its particle for want of a head-room
     // credit is STUCK (possible with a small aepid_set_live_limit, or in physics modes 2 and 3 where every charged step needs a
@@ -1452,9 +1449,6 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
     const int keep = *((volatile int*)&s_keep);
     bool leaving = false, park = false, did = false, parked = false;
     float h_n = 0.0f, h_E = 0.0f, h_dep = 0.0f;                 // collimation stage (class A only): Phase Space 2 particles, their energy, absorbed
-#if AEPID_PEEK
-    uint4 nxt = make_uint4(0u, 0u, 0u, 0u); bool have_nxt = false;  // class W: the lane's next Philox block, computed ahead of its use
-#endif
     // every lane enters a phase empty: saying so lets the compiler drop what this class never touches from the registers
     L.a_emit = L.a_ph = L.a_eps = L.a_epo = L.a_air = L.a_esc = 0.0f;
     L.alive = false; L.counted = kNone; L.spare = kNone; L.pval = 0.0f; L.pidx = kNone;
@@ -1483,6 +1477,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
             const int rk = __popc(empty & lt_mask);
             if (!L.alive && rk < got) {
                 const uint32_t tk = (uint32_t)(cl >> 32) + (uint32_t)rk;
+                AEPID_CHECK((int)(s_snap[C] - tk) > 0 && (int)(*((volatile unsigned int*)(s_tail + C)) - tk) <= (int)(s_pool_mask + 1u));   // published, not yet overwritten
                 const uint4* rec = queue_rec(C, tk);
                 const uint4 a = __ldcs(rec), b = __ldcs(rec + 1), c = __ldcs(rec + 2);
                 if (PH == 4) L.R = __uint_as_float(__ldcs(rec + 3).x);
@@ -1499,12 +1494,9 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
                 L.flags = c.x; L.h = c.y; L.pid = c.z; L.blk = c.w;
                 L.counted = 1u; L.alive = true;
                 L.pval = 0.0f; L.pidx = kNone;
-#if AEPID_PEEK
-                have_nxt = false;
-#endif
                 if (COUNT && !kPhaseClock) cnt[28]++;
                 if (C == C_A || C == C_W || C == C_P) set_energy(L, P, sh);
-                if (C == C_E) { L.vlin = vox_linear(P.g, L.vox); L.cw = __ldg(P.vox + L.vlin); L.pidx = L.vlin; }
+                if (C == C_E) { L.vlin = vox_linear(P.g, L.vox); AEPID_CHECK(L.vlin < P.nvox); L.cw = ld_vox(P.vox + L.vlin); L.pidx = L.vlin; }
             }
             if (C == C_A) {
                 // K1: new histories in the lanes that are still empty (the budget of the phase is head room set aside for them)
@@ -1590,27 +1582,12 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
             bool fly = on;
             if (on && L.E < P.ph.pcut) { if (COUNT) cnt[13]++; dep_here(L, P, L.E); L.alive = false; fly = false; }   // PAPER.md:104, 10 keV
             bool hit = false; float xsel = 0.0f, pe = 0.0f, co = 0.0f;
-#if AEPID_PEEK
-            if (fly && !have_nxt) { nxt = rng_peek(L, P); have_nxt = true; }
-#endif
 #pragma unroll 1
             for (int round = 0; round < kMaxRounds; ++round) {
-#if AEPID_PEEK
-                if (fly) { hit = woodcock_flight<COUNT>(L, P, sh, xsel, pe, co, cnt, &nxt); fly = !hit && F_REGION(L.flags) == R_PHANTOM; }
-#else
                 if (fly) { hit = woodcock_flight<COUNT>(L, P, sh, xsel, pe, co, cnt); fly = !hit && F_REGION(L.flags) == R_PHANTOM; }
-#endif
                 if (__popc(__ballot_sync(FULL_MASK, hit)) >= kHitMin || __ballot_sync(FULL_MASK, fly) == 0u) break;
             }
-#if AEPID_PEEK
-            if (hit) { interact<COUNT>(L, P, sh, xsel, pe, co, cnt, &nxt); have_nxt = false; }
-            if (!fly) have_nxt = false;                                    // left the grid (its last flight computed no next block) or not flying
-#else
             if (hit) interact<COUNT>(L, P, sh, xsel, pe, co, cnt);
-#endif
-        } else if (kAdapt > 0 && PH != 4 && (C == C_E || C == C_X)) {
-            if (C == C_E) charged_event_warp<COUNT, true, PH>(on, L, P, sh, cnt);
-            else charged_event_warp<COUNT, false, PH>(on, L, P, sh, cnt);
         } else if (on) {
             if (C == C_E) charged_event<COUNT, true, PH>(L, P, sh, cnt);
             else if (C == C_X) charged_event<COUNT, false, PH>(L, P, sh, cnt);
@@ -1636,6 +1613,7 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
         if ((it & 63u) == 0u) ledger_flush(L, led);
     }
     if (L.spare != kNone) { atomicSub(&s_live, 1); L.spare = kNone; }
+    if (L.counted != kNone) { atomicSub(&s_live, 1); L.counted = kNone; }   // a history that ended in the collimation stage right before the warp left
     ledger_flush(L, led);
     if (C == C_A && HEAD) {
         ledger_add(h_n, P.hd.stats + 0, true); ledger_add(h_E, P.hd.stats + 1, true); ledger_add(h_dep, P.hd.stats + 2, true);
@@ -1665,6 +1643,7 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
         s_g = P.g; s_ep_batch = P.ep_batch; s_npix = P.npix; s_nphase = 0u;
         s_pool_log = P.pool_log; s_pool_mask = (1u << P.pool_log) - 1u; s_rec_vec = PH == 4 ? 4u : 3u;
         s_queue = P.queues + (((size_t)blockIdx.x * kClasses) << P.pool_log) * (PH == 4 ? 4 : 3);
+        for (int r = 0; r < kRings; ++r) s_ring_base[r] = s_queue + (((size_t)r) << P.pool_log) * (PH == 4 ? 4 : 3);
         s_live = 0; s_live_max = min(max(P.live_max, 64), (1 << P.pool_log) / 2); s_did = 0; s_parked = 0; s_stuck = 0; s_phase = -1;
     }
     __syncthreads();

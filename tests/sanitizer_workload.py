@@ -1,8 +1,11 @@
 #!/usr/bin/env python
-"""Small runs of the CUDA path for compute-sanitizer (memcheck / racecheck on C0-sized runs):
+"""Small runs of the CUDA path for the checked build and for compute-sanitizer:
 
+    AEPID_LIBRARY=paper_2510_24154_b200/libaepid_checked.so python tests/sanitizer_workload.py   (tests/test_gpu_checked_build.py)
     compute-sanitizer --tool memcheck  python tests/sanitizer_workload.py
     compute-sanitizer --tool racecheck python tests/sanitizer_workload.py
+
+(compute-sanitizer is closed on the GPU pool this was developed on, profiles/r02_README.md; the checked build is what ran.)
 
 A C0-shaped photon-only run, a small coupled run with room for only 256 live particles per CTA (the parking / head-room-credit
 paths of the scheduler), modes 3 and 4, the collimation stage, the fold, the response post-pass and the analysis kernels.  No
