@@ -109,9 +109,11 @@ def radiation_length(comp):
     return 1.0 / inv
 
 
-def make_tables(n_E=500, E_min=1e-3, E_max=20.0, n_T=200, T_min=0.01, T_max=20.0, extra=()):
-    """All material tables, float32, in the layout of `aepid_init_materials`; `extra` appends materials to MATERIALS."""
-    E = np.exp(np.linspace(np.log(E_min), np.log(E_max), n_E))
+def make_tables(n_E=500, E_min=1e-3, E_max=20.0, n_T=200, T_min=0.01, T_max=20.0, extra=(), E_grid=None):
+    """All material tables, float32, in the layout of `aepid_init_materials`; `extra` appends materials to MATERIALS.
+    `E_grid`: an explicit (increasing, not necessarily log-uniform) photon energy grid instead of the n_E-point log grid."""
+    E = np.exp(np.linspace(np.log(E_min), np.log(E_max), n_E)) if E_grid is None else np.asarray(E_grid, dtype=np.float64)
+    n_E = len(E)
     T = np.exp(np.linspace(np.log(T_min), np.log(T_max), n_T))
     mats = list(MATERIALS) + list(extra)
     n_mat = len(mats)
@@ -131,3 +133,26 @@ def make_tables(n_E=500, E_min=1e-3, E_max=20.0, n_T=200, T_min=0.01, T_max=20.0
         "T_grid": f32(T), "stop_pow": f32(sp), "rad_len": f32(x0),
         "electrons_per_gram": f32(ne),      # N_A sum_i w_i Z_i / A_i: input of the Class II (Moller) mode
     }
+
+
+GD_K_EDGE = 0.050239          # MeV, K absorption edge of gadolinium
+
+
+def edge_resolving_tables(n_coarse=90, jump=5.2, seed=5):
+    """Tables on a NON-UNIFORM photon grid of the kind real tabulations come on (SURVEY 8(f) NEXT-2 "drop-in NIST/DPM-format
+    cross-section files"): a coarse, irregularly spaced grid (seeded jitter) that is refined around an absorption edge and
+    carries the edge as two grid points a relative 2e-6 apart.  The edge itself is synthetic (the parametric Z^4/E^3
+    photoelectric formula has none): the photoelectric coefficient of Gd2O2S is multiplied by `jump` at and above the Gd K edge.
+    Inputs only: the consumer interpolates as it sees fit."""
+    rng = np.random.default_rng(seed)
+    ln = np.linspace(np.log(1e-3), np.log(20.0), n_coarse)
+    ln[1:-1] += rng.uniform(-0.3, 0.3, n_coarse - 2) * (ln[1] - ln[0])
+    E = np.exp(ln)
+    near = GD_K_EDGE * np.exp(np.array([-0.2, -0.1, -0.05, -0.02, -0.005, 0.005, 0.02, 0.05, 0.1, 0.2]))
+    E = np.sort(np.concatenate([E[np.abs(np.log(E / GD_K_EDGE)) > 0.25], near, [GD_K_EDGE * (1 - 1e-6), GD_K_EDGE * (1 + 1e-6)]]))
+    t = make_tables(E_grid=E)
+    Ef = t["E_grid"].astype(np.float64)
+    assert np.all(np.diff(Ef) > 0)
+    t["mu_pe"][MAT_GOS, Ef > GD_K_EDGE] *= np.float32(jump)
+    t["edge"] = {"material": MAT_GOS, "E": GD_K_EDGE, "jump": jump}
+    return t

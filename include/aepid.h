@@ -80,8 +80,10 @@ void aepid_destroy(aepid_ctx* ctx);
 const char* aepid_last_error(const aepid_ctx* ctx);   /* NUL-terminated, owned by the context */
 
 /* Material tables (SURVEY.md 8(c) "Cross-section / stopping-power tables"; physics list PAPER.md:104).
- * All arrays host or device, float32.  E_grid_MeV [n_E] and T_grid_MeV [n_T] must be log-uniform and
- * increasing.  mu_* [n_mat][n_E] are mass coefficients in cm^2/g: Compton and photoelectric are
+ * All arrays host or device, float32.  E_grid_MeV [n_E]: positive and strictly increasing, otherwise free (a tabulation
+ * refined around absorption edges; an edge is two grid points a hair apart): a log-uniform grid is indexed directly, any other
+ * through a guide table of 1024 buckets in ln E (AEPID_ERR_BAD_ARG if not increasing).  T_grid_MeV [n_T] must be log-uniform
+ * and increasing (stopping powers are smooth; the charged-particle step looks it up twice per step).  mu_* [n_mat][n_E] are mass coefficients in cm^2/g: Compton and photoelectric are
  * interpolated linearly in (ln E, ln mu), pair linearly in (ln E, mu).  stop_pow [n_mat][n_T] in
  * MeV cm^2/g (log-log interpolation), rad_len_g_cm2 [n_mat].  Material 0 is the air that fills the world. */
 int aepid_init_materials(aepid_ctx* ctx, int n_mat,

@@ -50,7 +50,7 @@ Layout make_layout(const aepid_dims& d) {
     Layout L{};
     L.nvox = (size_t)d.nx * d.ny * d.nz;
     L.npix = (size_t)d.nu * d.nv;
-    L.blob_bytes = ((size_t)d.n_mat * d.n_E * 4 + d.n_E + (size_t)d.n_mat * d.n_T * 4 + d.n_mat) * 4;
+    L.blob_bytes = ((size_t)d.n_mat * d.n_E * 4 + d.n_E + (size_t)d.n_mat * d.n_T * 4 + d.n_mat + d.n_E + kEGuide + 1) * 4;
     size_t o = 0;
     auto take = [&](size_t bytes) { const size_t at = o; o += up(bytes); return at; };
     L.vox = take(L.nvox * 4);
@@ -207,10 +207,21 @@ void moller_integrals(double T, double Tc, double& sigma, double& hard) {
     hard = pref * T * (w1 + w2 + w3 - w4);
 }
 
+bool log_uniform(const std::vector<float>& g) {
+    const int n = (int)g.size();
+    if (!(g[0] > 0)) return false;
+    const double l0 = std::log((double)g[0]), d = (std::log((double)g[n - 1]) - l0) / (n - 1);
+    if (!(d > 0)) return false;
+    for (int i = 0; i < n; ++i) if (std::fabs(std::log((double)g[i]) - (l0 + i * d)) > 1e-3 * d) return false;
+    return true;
+}
+
 // ln-domain photon tables, majorant (reading A7 as corrected in DESIGN.md), ln stopping power, 1/X0.
 int build_tables(aepid_ctx* ctx) {
     const int nm = ctx->n_mat, nE = ctx->n_E, nT = ctx->n_T;
-    std::vector<float> blob((size_t)nm * nE * 4 + nE + (size_t)nm * nT * 4 + nm, 0.0f);
+    const bool nonuni = !log_uniform(ctx->Eg);
+    const size_t base_words = (size_t)nm * nE * 4 + nE + (size_t)nm * nT * 4 + nm;
+    std::vector<float> blob(base_words + (nonuni ? (size_t)nE + kEGuide + 1 : 0), 0.0f);
     float* phot = blob.data();
     float* maj = phot + (size_t)nm * nE * 4;
     float* lnS = maj + nE;
@@ -288,6 +299,22 @@ int build_tables(aepid_ctx* ctx) {
                 sig[o] = (float)((double)ctx->ne[m] * sg + bs);
                 sigb[o] = (float)bs;
             }
+    // A photon grid that is not log-uniform (a real tabulation: irregular spacing, refined around absorption edges): the kernel
+    // finds the cell from a guide table that is uniform in ln E, then interpolates exactly as on a uniform grid.
+    ctx->tb.nonuni_E = nonuni ? 1 : 0; ctx->tb.inv_dg = 0.0f; ctx->tb.lnEg_off = (int)base_words;
+    if (nonuni) {
+        float* lnEg = blob.data() + base_words;
+        uint32_t* guide = reinterpret_cast<uint32_t*>(lnEg + nE);
+        for (int j = 0; j < nE; ++j) lnEg[j] = (float)std::log((double)ctx->Eg[j]);
+        const double l0 = lnEg[0], span = (double)lnEg[nE - 1] - l0;
+        ctx->tb.inv_dg = (float)(kEGuide / span);
+        int i = 0;
+        for (int k = 0; k <= kEGuide; ++k) {       // the cell of the bucket's left edge, taken a hair to the left so that float rounding
+            const float x = (float)(l0 + (k - 1e-3) * span / kEGuide);   // of the bucket index never starts the search past the cell
+            while (i < nE - 2 && lnEg[i + 1] <= x) ++i;
+            guide[k] = (uint32_t)i;
+        }
+    }
     CU(cudaMemcpyAsync(ctx->d_blob(), blob.data(), blob.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));       // blob is a local vector
     ctx->tb.n_mat = nm; ctx->tb.n_E = nE; ctx->tb.n_T = nT;
@@ -299,15 +326,6 @@ int build_tables(aepid_ctx* ctx) {
     ctx->tb.blob_words = (int)blob.size();
     ctx->tables_dirty = false;
     return 0;
-}
-
-bool log_uniform(const std::vector<float>& g) {
-    const int n = (int)g.size();
-    if (!(g[0] > 0)) return false;
-    const double l0 = std::log((double)g[0]), d = (std::log((double)g[n - 1]) - l0) / (n - 1);
-    if (!(d > 0)) return false;
-    for (int i = 0; i < n; ++i) if (std::fabs(std::log((double)g[i]) - (l0 + i * d)) > 1e-3 * d) return false;
-    return true;
 }
 
 int check_geometry(aepid_ctx* ctx) {
@@ -413,7 +431,8 @@ int aepid_init_materials(aepid_ctx* ctx, int n_mat, int n_E, const float* E, con
     if (int rc = fetch(ctx, muPP, (size_t)n_mat * n_E, ctx->muPP)) return rc;
     if (int rc = fetch(ctx, S, (size_t)n_mat * n_T, ctx->S)) return rc;
     if (int rc = fetch(ctx, X0, (size_t)n_mat, ctx->X0)) return rc;
-    if (!log_uniform(ctx->Eg) || !log_uniform(ctx->Tg)) return fail(ctx, AEPID_ERR_BAD_ARG, "energy grids must be increasing and log-uniform");
+    for (int j = 0; j < n_E; ++j) if (!(ctx->Eg[j] > 0) || (j && !(ctx->Eg[j] > ctx->Eg[j - 1]))) return fail(ctx, AEPID_ERR_BAD_ARG, "photon energy grid must be positive and strictly increasing");
+    if (!log_uniform(ctx->Tg)) return fail(ctx, AEPID_ERR_BAD_ARG, "the electron energy grid must be increasing and log-uniform (the photon grid may be any increasing grid)");
     for (float v : ctx->muC) if (!(v >= 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "negative or NaN cross section");
     for (float v : ctx->muPE) if (!(v >= 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "negative or NaN cross section");
     for (float v : ctx->muPP) if (!(v >= 0)) return fail(ctx, AEPID_ERR_BAD_ARG, "negative or NaN cross section");

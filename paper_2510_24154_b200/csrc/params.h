@@ -59,9 +59,16 @@ struct Physics {
 //   float  maj[n_E]          majorant node values, safety margin included
 //   float  lnS[n_mat][n_T]   ln stopping power
 //   float  invX0[n_mat]
+//   -- only if the photon grid is not log-uniform (nonuni_E) --
+//   float  lnEg[n_E]         ln of the photon grid points
+//   uint32 guide[kEGuide+1]  guide[k] = cell of the photon grid that holds ln E = lnE0 + k / inv_dg (start of the search)
+constexpr int kEGuide = 1024;
 struct Tables {
     int n_mat, n_E, n_T;
     float lnE0, inv_dlnE, lnT0, inv_dlnT;
+    int nonuni_E;                      // the photon grid is an arbitrary increasing one: cell found through the guide table
+    float inv_dg;                      // guide buckets per unit of ln E
+    int lnEg_off;                      // word offset of lnEg in the blob (guide follows it)
     const uint32_t* blob;
     int blob_words;
 };

@@ -185,6 +185,8 @@ struct Shared {
     const float* lnS;
     const float* invX0;
     const float* sig;               // mode 2: Moller cross section [n_mat][n_T] (cm^2/g), linear in ln T; lnS then holds the restricted stopping power
+    const float* lnEg;              // photon grid that is not log-uniform: ln E_j, and the guide table of the cell search (params.h)
+    const uint32_t* guide;
 };
 
 struct Lane {
@@ -256,11 +258,21 @@ __device__ __forceinline__ void mu3(const TransportParams& P, const Shared& sh, 
     pp = E > 2.0f * kMec2 ? fmaf(ct, b.z - a.z, a.z) : 0.0f;
 }
 __device__ __forceinline__ void set_energy(Lane& L, const TransportParams& P, const Shared& sh) {
-    float f = (__logf(L.E) - P.tb.lnE0) * P.tb.inv_dlnE;
-    f = fminf(fmaxf(f, 0.0f), (float)(P.tb.n_E - 1));
-    const int i = min((int)f, P.tb.n_E - 2);
-    L.ci = i; L.ct = f - (float)i;
-    L.mumaj = fmaf(L.ct, sh.maj[i + 1] - sh.maj[i], sh.maj[i]);
+    const float lnE = __logf(L.E);
+    int i; float t;
+    if (P.tb.nonuni_E) {            // any increasing grid (a tabulation with absorption edges): guide bucket, then a short walk
+        const float gk = fminf(fmaxf((lnE - P.tb.lnE0) * P.tb.inv_dg, 0.0f), (float)kEGuide);
+        i = (int)sh.guide[(int)gk];
+        while (i < P.tb.n_E - 2 && sh.lnEg[i + 1] <= lnE) ++i;
+        t = fminf(fmaxf(__fdividef(lnE - sh.lnEg[i], sh.lnEg[i + 1] - sh.lnEg[i]), 0.0f), 1.0f);
+    } else {
+        float f = (lnE - P.tb.lnE0) * P.tb.inv_dlnE;
+        f = fminf(fmaxf(f, 0.0f), (float)(P.tb.n_E - 1));
+        i = min((int)f, P.tb.n_E - 2);
+        t = f - (float)i;
+    }
+    L.ci = i; L.ct = t;
+    L.mumaj = fmaf(t, sh.maj[i + 1] - sh.maj[i], sh.maj[i]);
 }
 __device__ __forceinline__ float stop_pow(const TransportParams& P, const Shared& sh, int m, float T) {
     float f = (__logf(T) - P.tb.lnT0) * P.tb.inv_dlnT;
@@ -1635,6 +1647,8 @@ __global__ void __launch_bounds__(kThreads, 1) transport_kernel(const __grid_con
     sh.lnS = sh.maj + P.tb.n_E;
     sh.invX0 = sh.lnS + P.tb.n_mat * P.tb.n_T;
     sh.sig = sh.invX0 + P.tb.n_mat + P.tb.n_mat * P.tb.n_T;
+    sh.lnEg = reinterpret_cast<const float*>(blob) + P.tb.lnEg_off;
+    sh.guide = reinterpret_cast<const uint32_t*>(sh.lnEg + P.tb.n_E);
     if (PH == 2 || PH == 3) sh.lnS = sh.invX0 + P.tb.n_mat;                    // the restricted stopping power takes the place of the total one
     for (int i = threadIdx.x; i < kWarps * 8; i += kThreads) led_all[i] = 0.0;
     if (threadIdx.x < kRings) { s_tail[threadIdx.x] = 0u; s_head[threadIdx.x] = 0u; s_snap[threadIdx.x] = 0u; }
