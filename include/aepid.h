@@ -62,9 +62,10 @@ typedef struct aepid_dims {
     int fu, fv;               /* fluence map */
     int n_batches;            /* B independent tally buffers for the batch variance estimate (2..255) */
     int n_ps1;                /* capacity for Phase Space 1 records (aepid_load_phase_space_source), 0 if not used */
-    int max_live_per_cta;     /* most particles one CTA of the transport kernel keeps alive, 64..65536 (0 = 65536); the workspace
+    int max_live_per_cta;     /* most particles one CTA of the transport kernel keeps alive, 64..262144 (0 = 65536); the workspace
                                  holds 160 x 5 class queues of twice that many 48-byte records (rounded up to a power of two):
-                                 5.0 GB at 65536, 80 MB at 1024.  Results do not depend on it; small runs want it small. */
+                                 20 GB at 262144, 5.0 GB at 65536, 80 MB at 1024.  Results do not depend on it; small runs want it
+                                 small, runs of 1e9 histories are 8 % faster at 262144 than at 65536 (profiles/r02_README.md). */
 } aepid_dims;
 
 /* Bytes of device memory the context needs for `dims` (0 if dims are invalid). */
@@ -240,8 +241,8 @@ int aepid_load_collimator(aepid_ctx* ctx, int n_slabs, const float* w0_cm, const
                           int material, float density_g_cm3, float w_ps2_cm);
 int aepid_read_head(aepid_ctx* ctx, double out[4]);
 
-/* Scheduler knob of the transport kernel: the most particles a CTA keeps alive at a time, 64 .. 65536
- * (0 = the default, 65536 = half a class queue).  Results do not depend on it (every particle has its own Philox stream);
+/* Scheduler knob of the transport kernel: the most particles a CTA keeps alive at a time, 64 .. what the
+ * context was created for (0 = that: dims.max_live_per_cta, half a class queue).  Results do not depend on it (every particle has its own Philox stream);
  * small values make lanes wait for head room and exist to test exactly that path. */
 int aepid_set_live_limit(aepid_ctx* ctx, int max_live_per_cta);
 

@@ -40,7 +40,7 @@ bool dims_ok(const aepid_dims* d) {
 
 // records per class queue of a CTA: twice the most particles a CTA keeps alive (queue protocol in transport.cu), a power of two
 int pool_log_for(const aepid_dims& d) {
-    const int live = d.max_live_per_cta ? d.max_live_per_cta : kMaxPoolSlots / 2;
+    const int live = d.max_live_per_cta ? d.max_live_per_cta : kDefaultLive;
     int lg = 7;
     while ((1 << lg) < 2 * live) ++lg;
     return lg;

@@ -15,9 +15,10 @@ constexpr float kWorldHalf = 100.0f;  // |u|, |v| <= 100 cm
 constexpr float kWorldWMin = -1.0f;   // -1 <= w
 constexpr float kMec2 = 0.51099895f;
 #ifndef AEPID_POOL_LOG
-#define AEPID_POOL_LOG 17
+#define AEPID_POOL_LOG 19
 #endif
-constexpr int kMaxPoolLog = AEPID_POOL_LOG;       // largest class queue: 2^17 records per class per CTA (65536 particles alive per CTA)
+constexpr int kMaxPoolLog = AEPID_POOL_LOG;       // largest class queue: 2^19 records per class per CTA (262144 particles alive per CTA)
+constexpr int kDefaultLive = 65536;               // aepid_dims.max_live_per_cta = 0
 constexpr int kMaxPoolSlots = 1 << kMaxPoolLog;   // the size in force comes from aepid_dims.max_live_per_cta (TransportParams::pool_log)
 constexpr int kRingCount = 5;         // class queues per CTA: the five event classes
 constexpr int kRecordBytes = 48;      // three 16-byte vectors per particle

@@ -53,7 +53,7 @@ namespace aepid {
 #endif
 constexpr int kWarps = AEPID_WARPS;
 constexpr int kThreads = kWarps * 32;
-// Records per class queue of a CTA: kPool = 1 << TransportParams::pool_log (from aepid_dims.max_live_per_cta, at most 2^17);
+// Records per class queue of a CTA: kPool = 1 << TransportParams::pool_log (from aepid_dims.max_live_per_cta, at most 2^19);
 // the most particles alive in a CTA at any time is half a queue (see "queue protocol" above), the limit in force is
 // TransportParams::live_max <= kPool / 2 (s_live_max).
 #ifndef AEPID_RESERVE_8THS

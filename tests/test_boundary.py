@@ -56,8 +56,10 @@ def test_workspace_bytes_validates_dims(lib):
     # the class queues follow dims.max_live_per_cta: twice as many 48-byte records per class and CTA, rounded up to a power of two
     small = pkg.Dims.from_buffer_copy(d); small.max_live_per_cta = 1000
     assert n - pkg.workspace_bytes(small) == 160 * 5 * (131072 - 2048) * 48
+    big = pkg.Dims.from_buffer_copy(d); big.max_live_per_cta = 262144          # the largest: what Engine.for_config takes from 4e8 histories on
+    assert pkg.workspace_bytes(big) - n == 160 * 5 * (524288 - 131072) * 48
     for field, bad in (("n_batches", 1), ("n_batches", 256), ("nx", 0), ("nx", 2000), ("n_mat", 33), ("n_layers", 9), ("fu", 0),
-                       ("max_live_per_cta", 63), ("max_live_per_cta", 65537)):
+                       ("max_live_per_cta", 63), ("max_live_per_cta", 262145)):
         e = pkg.Dims.from_buffer_copy(d)
         setattr(e, field, bad)
         assert pkg.workspace_bytes(e) == 0, field

@@ -507,9 +507,12 @@ def test_error_codes():
     t, ph, ep, s = cfg["tables"], cfg["phantom"], cfg["epid"], cfg["source"]
     with pytest.raises(AepidError, match="BAD_STATE"):
         eng.load_phantom(ph["spacing"], ph["origin"], ph["density"], ph["material"])   # materials first
-    bad = t["E_grid"].copy(); bad[10] *= 1.01
+    bad = t["E_grid"].copy(); bad[10] = bad[9]                            # the photon grid may be irregular (A39) but must increase
     with pytest.raises(AepidError, match="BAD_ARG"):
         eng.init_materials(bad, t["mu_compton"], t["mu_pe"], t["mu_pair"], t["T_grid"], t["stop_pow"], t["rad_len"])
+    bad = t["T_grid"].copy(); bad[10] *= 1.01                             # the electron grid must be log-uniform
+    with pytest.raises(AepidError, match="BAD_ARG"):
+        eng.init_materials(t["E_grid"], t["mu_compton"], t["mu_pe"], t["mu_pair"], bad, t["stop_pow"], t["rad_len"])
     eng.init_materials(t["E_grid"], t["mu_compton"], t["mu_pe"], t["mu_pair"], t["T_grid"], t["stop_pow"], t["rad_len"])
     with pytest.raises(AepidError, match="NOMEM"):
         eng.load_phantom(ph["spacing"], ph["origin"], np.ones((3, 3, 3), np.float32), np.zeros((3, 3, 3), np.uint8))
