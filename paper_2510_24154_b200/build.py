@@ -68,6 +68,21 @@ def build_checked(force=False):
     return LIB_CHECKED
 
 
+def build_variant(name, flags, force=False):
+    """libaepid_<name>.so: the library with transport.cu compiled with extra flags (e.g. the analysis build -DAEPID_PHASE_CLOCK of
+    phase_clocks.py); the other objects are shared with the product build."""
+    build()
+    lib = os.path.join(HERE, "libaepid_%s.so" % name)
+    src = os.path.join(CSRC, "transport.cu")
+    if not force and os.path.exists(lib) and all(os.path.getmtime(d) <= os.path.getmtime(lib) for d in [src, LIB] + HEADERS):
+        return lib
+    o = os.path.join(CSRC, "transport_%s.o" % name)
+    subprocess.check_call([nvcc()] + NVCC_FLAGS + EXTRA_FLAGS["transport.cu"] + list(flags) + ["-c", src, "-o", o])
+    objs = [o] + [os.path.join(CSRC, s.replace(".cu", ".o")) for s in SOURCES if s != "transport.cu"]
+    subprocess.check_call([nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", lib] + objs + ["-lcudart_static", "-ldl", "-lrt", "-lpthread"])
+    return lib
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
     if "--checked" in sys.argv:
