@@ -520,7 +520,8 @@ __device__ __noinline__ int budget_claim(int want) {
 }
 
 // Append a particle record to the queue of its class (one lane, divergent code); visible to poppers after the next barrier.
-__device__ __noinline__ void queue_particle(float x, float y, float z, float dx, float dy, float dz, float E,
+// Inlined, like take_credit: out of line the two cost 3.9 % of the kernel time on C3 in call overhead (profiles/r02_README.md).
+__device__ __forceinline__ void queue_particle(float x, float y, float z, float dx, float dy, float dz, float E,
                                             uint32_t vox, uint32_t flags, uint32_t h, uint32_t pid, uint32_t blk, float R = 0.0f) {
     const int r = class_of(flags);
     const uint32_t tk = atomicAdd(s_tail + r, 1u);
@@ -538,7 +539,7 @@ __device__ __noinline__ void queue_particle(float x, float y, float z, float dx,
 // never exceeds kLiveMax, which is what keeps every queue from wrapping onto unread records (header comment).  A lane
 // keeps at most one credit (its own, when its particle died, else a fresh one) and only runs an event that can create a
 // secondary while it holds one.
-__device__ __noinline__ uint32_t take_credit() {
+__device__ __forceinline__ uint32_t take_credit() {
     if (*((volatile int*)&s_live) >= s_live_max) return kNone;
     if (atomicAdd(&s_live, 1) >= s_live_max) { atomicSub(&s_live, 1); return kNone; }
     return 1u;
