@@ -1564,14 +1564,13 @@ __device__ __forceinline__ void run_phase(Lane& L, const TransportParams& P, con
             // ---- C: leave the phase?
             const int n_live = __popc(__ballot_sync(FULL_MASK, L.alive));
             int go = 0;                                                        // 0 carry on, 1 nothing to do right now, 2 write back and leave, 3 leave
-            if (lane == 0) {
+            {   // every lane reads the same shared words (one broadcast load each): the decision is uniform without a shuffle
                 bool dry = (int)(s_snap[C] - *((volatile unsigned int*)(s_head + C))) <= 0;
                 if (C == C_A && *((volatile int*)&s_budget) > 0 && *((volatile int*)s_flag) == 0) dry = false;
                 if (n_live == 0) go = dry ? 3 : 1;
                 else if (it >= kIterLimit) go = 2;
                 else if (dry && 32 - n_live >= kRefillMin && (keep == 1 || (keep == 2 && it >= kMinIter))) go = 2;    // cannot keep its lanes full any more
             }
-            go = __shfl_sync(FULL_MASK, go, 0);
             if (go == 3) break;
             if (go == 2) { leaving = true; continue; }
             if (go == 1) continue;
