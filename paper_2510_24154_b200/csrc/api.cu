@@ -169,8 +169,8 @@ int deliver(aepid_ctx* ctx, void* dst, const void* dev_src, size_t bytes, bool* 
 // phase) in ledger[7]; tallies of such a run are incomplete.  Called right after a stream synchronisation.
 int check_internal(aepid_ctx* ctx, const double* host_ledger) {
     if (host_ledger[7] != 0.0) {
-        char buf[160];
-        std::snprintf(buf, sizeof buf, "transport kernel raised internal error flags %.0f (2: secondary dropped for want of head room, 8: scheduler stalled); tallies are incomplete", host_ledger[7]);
+        char buf[320];
+        std::snprintf(buf, sizeof buf, "transport kernel raised internal error flags %.0f (2: secondary dropped for want of head room, 8: scheduler stalled, 16: index or queue-protocol check of the checked build failed); tallies are incomplete", host_ledger[7]);
         return fail(ctx, AEPID_ERR_INTERNAL, buf);
     }
     return 0;
