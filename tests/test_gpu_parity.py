@@ -387,6 +387,22 @@ def test_results_do_not_depend_on_the_live_limit(name, shrink, n):
         assert np.allclose(r["epid_mean"], res[0]["epid_mean"], rtol=1e-3, atol=1e-9)
 
 
+def test_largest_class_queues_give_the_same_results():
+    """aepid_dims.max_live_per_cta = 262144 (20 GB of class queues; what Engine.for_config takes for runs of 4e8 histories and more,
+    the bench of C3 among them): the same particles are followed with the same Philox streams as with the default 65536."""
+    cfg = make_config("C2", shrink=4)
+    res = []
+    for live in (0, 262144):
+        eng = engine_for(cfg, max_live_per_cta=live); eng.set_counting(True)
+        eng.simulate(30_000_000, 6)
+        r = eng.read_tallies(); check_ledger(r["ledger"], 30_000_000); r["c"] = eng.read_counters()
+        res.append(r); eng.close()
+    assert np.array_equal(res[1]["c"][:16], res[0]["c"][:16])
+    assert np.allclose(res[1]["ledger"][:6], res[0]["ledger"][:6], rtol=2e-6)
+    assert np.allclose(res[1]["phantom_mean"], res[0]["phantom_mean"], rtol=1e-3, atol=1e-9)
+    assert np.allclose(res[1]["epid_mean"], res[0]["epid_mean"], rtol=1e-3, atol=1e-9)
+
+
 def test_tiny_live_limit_with_photon_multiplication():
     """with room for only 64 live particles per CTA and a workload that multiplies photons (10 MeV photons on
     Gd2O2S: pair production and annihilation) every lane of a phase can end up parked for want of a head-room credit.  The
