@@ -388,7 +388,7 @@ def run_ours(args):
     import oracle
     procs = os.cpu_count() or 1
     oracle.build()
-    ns = 10_000 if args.profile else (args.cpu_sample or {"C0": 60_000_000, "C1": 40_000_000, "C2": 20_000_000}.get(args.config, 8_000_000))   # 10-30 s
+    ns = 10_000 if args.profile else (args.cpu_sample or {"C0": 120_000_000, "C1": 60_000_000, "C2": 40_000_000, "C4": 40_000_000}.get(args.config, 30_000_000))   # 10-30 s of host time
     wk = _OraclePool(cfg, procs)
     wk.run(procs * 50, seed, 0)                                          # page-in warm-up
     t0 = time.perf_counter(); wk.run(ns, seed, 0); dt = time.perf_counter() - t0
