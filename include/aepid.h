@@ -281,6 +281,29 @@ int aepid_gamma_index(aepid_ctx* ctx, const float* ref, const float* eval, int n
 /* Block until everything queued on the context's stream has finished. */
 int aepid_synchronize(aepid_ctx* ctx);
 
+/* The analysis chain of PAPER.md:141 (up-sample the predicted image to the grid of the measured one, reading A28, then the
+ * global gamma index of it against the measured image, reading A29) for callers that cannot allocate device memory: code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  No context, no workspace: the call
+ * allocates NOTHING (no cudaMalloc / cudaFree, no allocating library routine).  Its scratch (the up-sampled image, the image
+ * maximum, the gamma statistics) is a file-scope `static __device__` array of the library, AEPID_STATIC_MAX_PIXELS floats +
+ * 256 bytes = 6.25 MiB, which every GPU that loads the library holds until the process exits.
+ *   predicted [nv][nu], measured [mv][mu] (the reference; non-negative; pixel pitch pitch_cm), gamma_out [mv][mu]: DEVICE,
+ *   caller-owned.  stats_out: DEVICE [4] doubles or NULL = {tested pixels, pixels with gamma <= 1, mean gamma, max gamma}.
+ *   The criteria are those of aepid_gamma_index; gamma_out = gamma of the up-sampled predicted image (evaluated) against
+ *   `measured` (reference), identical to aepid_upsample followed by aepid_gamma_index(measured, up-sampled, ...).
+ * Asynchronous on cuda_stream of CUDA device `device` (made current for the call, the previous one restored).  The first
+ * call per device resolves the array's device address (cudaGetSymbolAddress): make one call before a graph capture.
+ * Every call shares the one array: it keeps the last call's contents (what must start at zero is cleared on the stream by
+ * every call), and two calls that OVERLAP on the GPU (different streams, no ordering) race: order them.
+ * Errors: AEPID_ERR_NOMEM if mu * mv > AEPID_STATIC_MAX_PIXELS (use aepid_upsample + aepid_gamma_index with caller memory)
+ * or if the search window does not fit in shared memory; AEPID_ERR_BAD_ARG; AEPID_ERR_CUDA.  error_text (HOST, may be NULL)
+ * receives a NUL-terminated message of at most error_text_bytes bytes. */
+#define AEPID_STATIC_MAX_PIXELS (1280 * 1280)
+int aepid_gamma_of_upsampled_static(int device, void* cuda_stream, const float* predicted, int nu, int nv,
+                                    const float* measured, int mu, int mv, float pitch_cm, float dose_frac, float dta_cm,
+                                    float threshold_frac, float gamma_cap, float* gamma_out, double* stats_out,
+                                    char* error_text, size_t error_text_bytes);
+
 #ifdef __cplusplus
 }
 #endif

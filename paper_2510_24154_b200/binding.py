@@ -33,7 +33,8 @@ EXPORTS = ("aepid_workspace_bytes", "aepid_create", "aepid_destroy", "aepid_last
            "aepid_apply_response_lut", "aepid_synchronize", "aepid_set_history_offset", "aepid_read_moments",
            "aepid_finalize_moments", "aepid_upsample", "aepid_gamma_index",
            "aepid_set_phase_space", "aepid_read_phase_space_count", "aepid_set_live_limit", "aepid_set_class2", "aepid_roi_mean",
-           "aepid_load_phase_space_source", "aepid_load_collimator", "aepid_read_head")
+           "aepid_load_phase_space_source", "aepid_load_collimator", "aepid_read_head", "aepid_gamma_of_upsampled_static")
+STATIC_MAX_PIXELS = 1280 * 1280            # AEPID_STATIC_MAX_PIXELS of include/aepid.h
 
 
 class AepidError(RuntimeError):
@@ -401,3 +402,35 @@ class Engine:
         self._chk(self._lib.aepid_apply_response_lut(self._h, _ptr(lut), nt, ns, float(t_min), float(t_max), float(s_min), float(s_max),
                                                      float(s_eff), _ptr(epid_in), _ptr(signal_out), _ptr(tmap_out)))
         return signal_out, tmap_out
+
+
+def gamma_of_upsampled_static(predicted, measured, pitch_cm, dose_frac=0.03, dta_cm=0.3, threshold_frac=0.10, cap=2.0,
+                              out=None, stats_out=None, stream=None):
+    """aepid_gamma_of_upsampled_static (include/aepid.h): K9 + K10 without a context or a workspace; the library's static device
+    array is the scratch, nothing is allocated by the call.  predicted, measured: 2-D float32 CUDA tensors on the same device;
+    out [mv][mu] float32 and stats_out [4] float64 are CUDA tensors of the caller (created here only if not given).  Returns
+    (out, stats_out); asynchronous on `stream` (default: torch's current stream)."""
+    import torch
+    lib = load_library()
+    if not (predicted.is_cuda and measured.is_cuda and predicted.dtype == torch.float32 and measured.dtype == torch.float32):
+        raise ValueError("predicted and measured must be float32 CUDA tensors")
+    predicted, measured = predicted.contiguous(), measured.contiguous()
+    nv, nu = (int(v) for v in predicted.shape)
+    mv, mu = (int(v) for v in measured.shape)
+    dev = measured.device
+    if out is None:
+        out = torch.empty((mv, mu), dtype=torch.float32, device=dev)
+    if stats_out is None:
+        stats_out = torch.empty(4, dtype=torch.float64, device=dev)
+    st = torch.cuda.current_stream(dev).cuda_stream if stream is None else int(stream)
+    err = C.create_string_buffer(512)
+    lib.aepid_gamma_of_upsampled_static.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int, C.c_int,
+                                                    C.c_float, C.c_float, C.c_float, C.c_float, C.c_float, C.c_void_p, C.c_void_p,
+                                                    C.c_char_p, C.c_size_t]
+    rc = lib.aepid_gamma_of_upsampled_static(dev.index or 0, C.c_void_p(st), C.c_void_p(predicted.data_ptr()), nu, nv,
+                                             C.c_void_p(measured.data_ptr()), mu, mv, float(pitch_cm), float(dose_frac), float(dta_cm),
+                                             float(threshold_frac), float(cap), C.c_void_p(out.data_ptr()), C.c_void_p(stats_out.data_ptr()),
+                                             err, len(err))
+    if rc != 0:
+        raise AepidError("aepid %s: %s" % (STATUS.get(rc, rc), err.value.decode()))
+    return out, stats_out

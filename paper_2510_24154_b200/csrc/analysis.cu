@@ -5,6 +5,9 @@
 // grid), staged once per tile in shared memory, so it is bound by shared-memory reads and FMAs, not by HBM.
 #include <cuda_runtime.h>
 #include <cstdint>
+#include <cstdio>
+#include <mutex>
+#include "../../include/aepid.h"
 #include "params.h"
 
 namespace aepid {
@@ -159,4 +162,91 @@ void launch_roi_sum(const float* img, int nu, int nv, float pitch, float roi, do
     roi_sum_kernel<<<(unsigned)b, 256, 0, st>>>(img, nu, nv, pitch, 0.5f * roi, acc);
 }
 
+// ---------------------------------------------------------------- the entry point that allocates nothing (include/aepid.h:
+// aepid_gamma_of_upsampled_static).  K9 + K10 in one call with NO context and NO workspace: the up-sampled image (the
+// intermediate of the chain), the image maximum and the gamma statistics live in this file-scope device array, which every GPU
+// that loads the library holds until the process exits (6.25 MiB + 256 B).  All calls share it: it keeps the last call's
+// contents, what must start at zero is cleared on the stream at the start of every call, and calls that overlap on the GPU race.
+constexpr size_t kStaticMaxPixels = (size_t)AEPID_STATIC_MAX_PIXELS;                 // 1280 x 1280: the paper's 1190 x 1190 fits
+constexpr size_t kStaticStatsOff = kStaticMaxPixels * sizeof(float);                 // double stats[4] | uint32 dmax bits
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticStatsOff + 256];
+
+// device code names the array directly: {tested, passing, mean gamma, max gamma} from the raw accumulators
+__global__ void static_stats_kernel(double* __restrict__ out) {
+    const double* st = reinterpret_cast<const double*>(g_static_scratch + kStaticStatsOff);
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        out[0] = st[0]; out[1] = st[1]; out[2] = st[0] > 0.0 ? st[2] / st[0] : 0.0; out[3] = st[3];
+    }
+}
+
+// In host code `g_static_scratch` is a host-side stand-in, not a device address: the address a kernel can use comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+constexpr int kStaticMaxDevices = 64;
+static std::mutex g_static_mutex;
+static void* g_static_addr[kStaticMaxDevices] = {nullptr};
+static cudaError_t static_scratch_address(int device, unsigned char** out) {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[device]) {
+        void* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);              // the current device is `device` (caller)
+        if (e != cudaSuccess) return e;
+        g_static_addr[device] = p;
+    }
+    *out = static_cast<unsigned char*>(g_static_addr[device]);
+    return cudaSuccess;
+}
+static bool is_device_pointer(const void* p) {
+    cudaPointerAttributes a{};
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
 }  // namespace aepid
+
+extern "C" int aepid_gamma_of_upsampled_static(int device, void* cuda_stream, const float* predicted, int nu, int nv,
+                                               const float* measured, int mu, int mv, float pitch_cm, float dose_frac, float dta_cm,
+                                               float threshold_frac, float gamma_cap, float* gamma_out, double* stats_out,
+                                               char* error_text, size_t error_text_bytes) {
+    using namespace aepid;
+    auto fail = [&](int code, const char* what) {
+        if (error_text && error_text_bytes) std::snprintf(error_text, error_text_bytes, "%s", what);
+        return code;
+    };
+    if (error_text && error_text_bytes) error_text[0] = 0;
+    if (device < 0 || device >= kStaticMaxDevices) return fail(AEPID_ERR_BAD_ARG, "device index out of range (0..63)");
+    if (!predicted || !measured || !gamma_out) return fail(AEPID_ERR_BAD_ARG, "null image pointer");
+    if (nu < 1 || nv < 1 || mu < 1 || mv < 1 || nu > 32768 || nv > 32768) return fail(AEPID_ERR_BAD_ARG, "image size out of range");
+    if ((size_t)mu * (size_t)mv > kStaticMaxPixels) {
+        char buf[320];
+        std::snprintf(buf, sizeof buf, "measured grid of %d x %d pixels exceeds the static scratch of aepid_gamma_of_upsampled_static "
+                      "(AEPID_STATIC_MAX_PIXELS = %zu, e.g. 1280 x 1280): use aepid_upsample + aepid_gamma_index", mu, mv, kStaticMaxPixels);
+        return fail(AEPID_ERR_NOMEM, buf);
+    }
+    if (!(pitch_cm > 0) || !(dose_frac > 0) || !(dta_cm > 0) || !(threshold_frac >= 0) || !(gamma_cap >= 1))
+        return fail(AEPID_ERR_BAD_ARG, "gamma criteria out of range (pitch, dose fraction, DTA > 0; threshold >= 0; cap >= 1)");
+    int prev = -1;
+    if (cudaGetDevice(&prev) != cudaSuccess) return fail(AEPID_ERR_CUDA, "cudaGetDevice failed");
+    if (prev != device && cudaSetDevice(device) != cudaSuccess) return fail(AEPID_ERR_CUDA, "cudaSetDevice failed");
+    int rc = 0;
+    do {
+        if (!is_device_pointer(predicted) || !is_device_pointer(measured) || !is_device_pointer(gamma_out) || (stats_out && !is_device_pointer(stats_out))) {
+            rc = fail(AEPID_ERR_BAD_ARG, "aepid_gamma_of_upsampled_static takes device pointers (images, gamma_out, stats_out)"); break;
+        }
+        unsigned char* scratch = nullptr;
+        const cudaError_t e = static_scratch_address(device, &scratch);
+        if (e != cudaSuccess) { rc = fail(AEPID_ERR_CUDA, cudaGetErrorString(e)); break; }
+        float* up = reinterpret_cast<float*>(scratch);
+        double* stats = reinterpret_cast<double*>(scratch + kStaticStatsOff);
+        unsigned int* dmax = reinterpret_cast<unsigned int*>(scratch + kStaticStatsOff + 4 * sizeof(double));
+        launch_upsample(predicted, nu, nv, up, mu, mv, cuda_stream);                   // K9 into the static scratch (fully overwritten)
+        // K10: launch_gamma clears dmax and stats on the stream before it uses them
+        if (launch_gamma(measured, up, gamma_out, mu, mv, pitch_cm, dose_frac, dta_cm, threshold_frac, gamma_cap, dmax, stats, cuda_stream) != 0) {
+            rc = fail(AEPID_ERR_NOMEM, "search window (cap x DTA / pitch pixels) does not fit in shared memory"); break;
+        }
+        if (stats_out) static_stats_kernel<<<1, 32, 0, (cudaStream_t)cuda_stream>>>(stats_out);
+        const cudaError_t le = cudaGetLastError();
+        if (le != cudaSuccess) { rc = fail(AEPID_ERR_CUDA, cudaGetErrorString(le)); break; }
+    } while (false);
+    if (prev != device) cudaSetDevice(prev);
+    return rc;
+}
