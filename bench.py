@@ -379,7 +379,11 @@ def run_ours(args):
                 "events_per_history": evmix, "events_from": "aepid_read_counters after an untimed counting launch of %d histories of this workload" % n_cnt,
                 "how": "frac = sum_k alg_unit_cost[k] * events_per_history[k] * histories / kernel time / peak; peak = %s sm_max_mhz x %d SMs x 4 schedulers x 32 lanes" % (which, sm_count),
                 "ncu": cap, "hbm_gbs_peak": peaks.get("hbm_gbs"),
-                "hbm_frac": (cap["dram_bytes_per_history"] * n / (k_ms * 1e-3) / 1e9 / float(peaks.get("hbm_gbs", 6549.4))) if cap else None}
+                "hbm_frac": (cap["dram_bytes_per_history"] * n / (k_ms * 1e-3) / 1e9 / float(peaks.get("hbm_gbs", 6549.4))) if cap else None,
+                # north_star's second candidate, "the instruction count at the SM issue peak", with the EXECUTED count of the ncu
+                # capture (warp-instructions per history x active lanes) at this run's rate: what the kernel issues, not what the method needs
+                "executed_thread_instr_per_history": (cap["warp_instr_per_history"] * cap["lanes_per_warp_instr"]) if cap else None,
+                "executed_frac": (cap["warp_instr_per_history"] * cap["lanes_per_warp_instr"] * n / (k_ms * 1e-3) / 1e9 / peak_ginstr) if cap else None}
     per_kernel = {"transport_ms": k_ms, "fold_ms": float(tot[2]) / args.steps, "tmap_and_lut_ms": float(tot[3]) / args.steps,
                   "note": "CUDA events on the launching stream; fold = the two fold_kernel launches of aepid_read_tallies (EPID, phantom), "
                           "tmap_and_lut = tmap_kernel + apply_lut_kernel of aepid_apply_response_lut"}
