@@ -120,6 +120,8 @@ def build_cfg(name, field=0, mode=None, collimator=False):
     cfg = head_config(field=field) if collimator else make_config(name, field=field)   # NEXT-3: Phase Space 1 + jaws / MLC instead of the fluence map
     if mode is not None:
         cfg["physics"]["mode"] = int(mode)      # 2: Class II collisions (Moller delta rays, reading A31)
+        if int(mode) == 4:
+            cfg["physics"]["f_E"] = 0.2         # reading A38: the multi-voxel step loses 20 % of the energy (as in the parity tests)
     if cfg.get("lut") is None:
         cfg["lut"] = paper_table1_lut()          # PAPER.md:157-162 Table 1 as the response LUT (C4 brings its own)
     return cfg
@@ -445,7 +447,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C3", choices=["C0", "C1", "C2", "C3", "C4"])
-    ap.add_argument("--physics-mode", type=int, default=None, choices=[0, 1, 2, 3], help="override the physics mode (2: Class II collisions, 3: + bremsstrahlung)")
+    ap.add_argument("--physics-mode", type=int, default=None, choices=[0, 1, 2, 3, 4], help="override the physics mode (2: Class II collisions, 3: + bremsstrahlung, 4: multi-voxel steps with a random hinge)")
     ap.add_argument("--field", type=int, default=0, help="which of C4's 25 IMRT fields (seeds per reading A23)")
     ap.add_argument("--collimator", action="store_true", help="C4 only: collimation stage (synthetic Phase Space 1, jaws, MLC) in place of the fluence map")
     ap.add_argument("--histories", type=int, default=0, help="histories per GPU per step (default: the config's)")
